@@ -1,0 +1,74 @@
+"""The seeded input generators (lst_inputs): shapes, determinism, and the BASELINE.json recipes."""
+import numpy as np
+
+from lst_inputs import build_connection_map, make_config_event, make_config_geometry, make_geometry
+from lst_inputs.events import concat_events
+
+
+def test_geometry_sizes_follow_the_configs():
+    g = make_geometry("barrel_z60")
+    assert g.barrel_nphi.tolist() == [15, 23, 33, 43, 56, 68]  # ceil(2 pi r / 10 cm)
+    assert g.n_modules == 238 * 12 == 2856
+    g = make_geometry("barrel_z120_endcap")
+    assert g.n_modules == 238 * 24 + 10 * int(g.endcap_nphi.sum()) == 9512
+    assert (g.subdet == 0).sum() == 5712 and (g.subdet == 1).sum() == 3800
+
+
+def test_connection_map_is_valid_csr_and_layer_forward():
+    for cfg in ("C1", "C3"):
+        g, off, tgt = make_config_geometry(cfg)
+        assert off[0] == 0 and off[-1] == len(tgt) and np.all(np.diff(off) >= 0)
+        assert tgt.min() >= 0 and tgt.max() < g.n_modules
+        src = np.repeat(np.arange(g.n_modules), np.diff(off))
+        bb = (g.subdet[src] == 0) & (g.subdet[tgt] == 0)
+        assert np.all(g.layer[tgt][bb] == g.layer[src][bb] + 1)  # barrel -> next barrel layer only
+        ee = (g.subdet[src] == 1) & (g.subdet[tgt] == 1)
+        assert np.all(g.side[tgt][ee] == g.side[src][ee]) and np.all(g.layer[tgt][ee] == g.layer[src][ee] + 1)
+        assert not np.any((g.subdet[src] == 1) & (g.subdet[tgt] == 0))  # never endcap -> barrel
+        for m in (0, g.n_modules // 2):
+            row = tgt[off[m]:off[m + 1]]
+            assert np.all(np.diff(row) > 0)  # sorted, unique
+
+
+def test_connection_map_deterministic_without_cache():
+    g = make_geometry("barrel_z60")
+    a = build_connection_map(g, n_samples=20000, seed=5, cache=False)
+    b = build_connection_map(g, n_samples=20000, seed=5, cache=False)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_events_are_seeded_and_shaped_like_the_configs():
+    e1 = make_config_event("C1")
+    e1b = make_config_event("C1")
+    assert np.array_equal(e1.x, e1b.x) and np.array_equal(e1.sensor, e1b.sensor)
+    assert e1.x.dtype == np.float32 and e1.sensor.dtype == np.int32
+    assert 150 < e1.n_hits < 260 and np.all(e1.truth >= 0) and e1.n_pls == 0
+    e2 = make_config_event("C2")
+    assert 6000 < e2.n_hits < 7500 and (e2.truth < 0).sum() == 2000
+    e4 = make_config_event("C4")
+    assert 500 < e4.n_pls < 650 and (e4.pls["truth"] < 0).sum() > 30 and len(e4.trk["pt"]) == 550
+    g, _, _ = make_config_geometry("C1")
+    assert e2.sensor.min() >= 0 and e2.sensor.max() < g.n_sensors
+
+
+def test_hits_lie_on_their_sensor_surfaces():
+    g, _, _ = make_config_geometry("C3")
+    ev = make_config_event("C3")
+    assert 0.9e5 < ev.n_hits < 1.6e5
+    m = ev.sensor // 2
+    s = ev.sensor % 2
+    r = np.hypot(ev.x.astype(np.float64), ev.y.astype(np.float64))
+    bar = g.subdet[m] == 0
+    from lst_inputs.geometry import BARREL_R, ENDCAP_Z
+    assert np.allclose(r[bar], BARREL_R[g.layer[m[bar]] - 1] + 0.26 * s[bar], atol=1e-4)
+    end = ~bar
+    assert np.allclose(np.abs(ev.z[end]), ENDCAP_Z[g.layer[m[end]] - 1] + 0.4 * s[end], atol=1e-4)
+    assert np.all(np.sign(ev.z[end]) == g.side[m[end]])
+
+
+def test_concat_events_offsets():
+    evs = [make_config_event("C5", pu=50, index=i, seeds=True) for i in range(3)]
+    b = concat_events(evs)
+    assert b["hit_offsets"].tolist() == np.concatenate([[0], np.cumsum([e.n_hits for e in evs])]).tolist()
+    assert b["pls_offsets"][-1] == sum(e.n_pls for e in evs) == len(b["pls"]["pt"])
+    assert len(b["x"]) == b["hit_offsets"][-1]
