@@ -1,0 +1,195 @@
+/* lst.h -- C ABI of the B200-native Line Segment Tracking (LST) object-building chain.
+ *
+ * What it computes (arxiv 2407.18231, PAPER.md):
+ *   outer-tracker hits --[two sensors of a module]--> Mini-Doublets (MD)
+ *   MD x MD on modules joined by the precomputed connection map --> Line Segments
+ *   LS x LS sharing an MD --> T3;  T3 x T3 sharing an MD --> T5
+ *   inner-tracker seeds (pLS) x T3 / T5 --> pT3 / pT5
+ *   duplicate removal + selection of {pT5, pT3, T5, unlinked pLS} track candidates
+ * The numeric selections (deferred by PAPER.md:29 to its Refs. [4], [5]) are the documented
+ * stand-in of CUTS.md; all cut arithmetic is binary32, fixed order, no FMA.
+ *
+ * Conventions
+ *   - All functions return 0 (LST_OK) or a negative lst_status; no exception crosses the ABI.
+ *   - "host" / "device" is stated per pointer.  Inputs are caller-owned and never retained past the
+ *     call that takes them (lst_ctx_run: past the following lst_ctx_sync).  Outputs are library-owned
+ *     until lst_free.
+ *   - Indices in outputs: hit indices refer to the caller's INPUT hit order within the event
+ *     (0-based, event-local); object indices (md, ls, t3, t5, pls) are event-local positions in the
+ *     returned arrays of that event.
+ *   - Overflow of a preallocated object array returns LST_ERR_CAPACITY; nothing is ever truncated.
+ *   - One lst_ctx per CUDA stream; a lst_geometry is immutable and may be shared by many contexts.
+ */
+#ifndef LST_H
+#define LST_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum lst_status {
+  LST_OK = 0,
+  LST_ERR_ARG = -1,      /* NULL / negative size / sensor id or event offsets out of range */
+  LST_ERR_CUDA = -2,     /* CUDA runtime error (no device, out of memory, launch failure) */
+  LST_ERR_CAPACITY = -3, /* an object array of the context is too small for this batch */
+  LST_ERR_GEOMETRY = -4  /* malformed module table or connection map */
+} lst_status;
+
+/* Static string for a status code. */
+const char* lst_strerror(int status);
+
+/* One module = one tile of a layer with its two sensors; sensor ids are 2*m (lower)
+ * and 2*m+1 (upper).  Only `subdet` enters the arithmetic (CUTS.md 3, 4); the rest is carried. */
+typedef struct lst_module {
+  int32_t subdet; /* 0 = barrel, 1 = endcap */
+  int32_t layer;  /* 1..6 barrel layer, 1..5 endcap disk */
+  int32_t side;   /* 0 barrel, -1 / +1 endcap side */
+  int32_t ring;   /* barrel z-tile / endcap ring */
+} lst_module;
+
+/* Cut constants of CUTS.md section 1 (same order) and the stage mask of CUTS.md section 9. */
+typedef struct lst_params {
+  float b_field, pt_min, z0_max;
+  float md_b_phi_tol, md_z_tol, md_e_slope, md_e_tol;
+  float ls_kappa_max, ls_z_tol, ls_dir_tol;
+  float t3_kappa_max, t3_z_tol0, t3_z_tol1;
+  float t5_tol0, t5_tol1;
+  float pt_gate_tol, pt_k_tol0, pt_k_tol1, pt_z_tol;
+  float near_rel;
+  int32_t stage_mask; /* bit0 MD, 1 LS, 2 T3, 3 T5, 4 pT3/pT5, 5 duplicate removal + TC */
+} lst_params;
+
+/* Fills *p with the defaults of CUTS.md section 1 (stage_mask = 0x3f). */
+void lst_default_params(lst_params* p);
+
+/* Capacities of one context (object counts summed over the events of a batch). */
+typedef struct lst_caps {
+  int32_t max_events;
+  int32_t max_hits, max_pls;
+  int32_t max_md, max_ls, max_t3, max_t5, max_pt3, max_pt5, max_tc;
+} lst_caps;
+
+/* Defaults sized for 16 PU250-like events (a few hundred MB; the B200 has 180 GB). */
+void lst_default_caps(lst_caps* c);
+/* Device bytes a context with these capacities allocates for a geometry of n_modules. */
+size_t lst_workspace_bytes(const lst_caps* c, int32_t n_modules);
+
+/* Outer-tracker hits of a batch, structure of arrays.  x, y, z in cm. */
+typedef struct lst_hits {
+  const float* x;
+  const float* y;
+  const float* z;
+  const int32_t* sensor;        /* 2*module + {0,1} */
+  int32_t n;                    /* hits in the batch */
+  const int32_t* event_offsets; /* HOST pointer, n_events+1 entries, [0] = 0, [n_events] = n;
+                                   NULL = one event */
+  int32_t on_device;            /* 0: x, y, z, sensor are host pointers; 1: device pointers */
+} lst_hits;
+
+/* Inner-tracker seeds (pLS) of a batch (reading S6 of DESIGN.md). */
+typedef struct lst_pls {
+  const float* pt;  /* GeV */
+  const int32_t* q; /* +-1 */
+  const float *x0, *y0, *z0; /* inner pixel hit */
+  const float *x1, *y1, *z1; /* outer pixel hit */
+  int32_t n;
+  const int32_t* event_offsets; /* HOST pointer, n_events+1 entries; NULL = one event */
+  int32_t on_device;
+} lst_pls;
+
+typedef struct lst_geometry lst_geometry;
+typedef struct lst_ctx lst_ctx;
+
+enum { LST_ST_MD = 0, LST_ST_LS, LST_ST_T3, LST_ST_T5, LST_ST_PT3, LST_ST_PT5, LST_N_STAGES };
+
+/* Result of one event, host memory, library-owned (lst_free).  Layouts as in CUTS.md. */
+typedef struct lst_event_out {
+  uint64_t magic;
+  int32_t n_md, n_ls, n_t3, n_t5, n_pt3, n_pt5, n_tc;
+  int64_t near[LST_N_STAGES];    /* near-threshold candidates per stage (CUTS.md section 0) */
+  int64_t n_tests[LST_N_STAGES]; /* candidates evaluated per stage */
+  int32_t* md_hits;   /* [n_md][2]  h_lo, h_hi (input hit indices) */
+  int32_t* md_module; /* [n_md] */
+  float* md_f;        /* [n_md][6]  anchor x, y, z, r and unit direction ux, uy */
+  int32_t* ls_md;     /* [n_ls][2]  md_in, md_out */
+  float* ls_kappa;    /* [n_ls] */
+  int32_t* t3_ls;     /* [n_t3][2] */
+  int32_t* t3_md;     /* [n_t3][3] */
+  float* t3_k;        /* [n_t3] */
+  int32_t* t5_t3;     /* [n_t5][2] */
+  int32_t* t5_md;     /* [n_t5][5] */
+  float* t5_score;    /* [n_t5] */
+  int32_t* pt3;       /* [n_pt3][2] pls, t3 */
+  float* pt3_score;
+  int32_t* pt5;       /* [n_pt5][2] pls, t5 */
+  float* pt5_score;
+  int32_t* tc;        /* [n_tc][16] type, pls, t5, t3, hit_idx[12]; classes in order pT5, pT3, T5, pLS */
+} lst_event_out;
+
+/* Totals of the last batch of a context (host struct filled by lst_ctx_sync). */
+typedef struct lst_batch_summary {
+  int32_t n_events;
+  int32_t n_hits, n_pls;
+  int32_t n_md, n_ls, n_t3, n_t5, n_pt3, n_pt5, n_tc;
+  int64_t near[LST_N_STAGES];
+  int64_t n_tests[LST_N_STAGES];
+} lst_batch_summary;
+
+/* ---- the three calls of north_star ---------------------------------------------------------- */
+
+/* Copies the module table and the CSR connection map to the device.
+ * modules: host, n_modules records.  conn_offsets: host, n_modules+1, [0] = 0, non-decreasing.
+ * conn_targets: host, conn_offsets[n_modules] module indices.  params: host or NULL (defaults).
+ * *out: library-owned, immutable; release with lst_free. */
+int lst_load_geometry(const lst_module* modules, int32_t n_modules, const int32_t* conn_offsets,
+                      const int32_t* conn_targets, const lst_params* params, lst_geometry** out);
+
+/* Runs the whole chain on ONE event, synchronously, on an internal context (default capacities,
+ * default stream) and returns every object array on the host.  seeds may be NULL.
+ * hits->event_offsets / seeds->event_offsets must be NULL.  *out: release with lst_free. */
+int lst_run_event(lst_geometry* g, const lst_hits* hits, const lst_pls* seeds, lst_event_out** out);
+
+/* Releases a lst_geometry, lst_ctx or lst_event_out (NULL is a no-op). */
+void lst_free(void* geometry_ctx_or_event_out);
+
+/* ---- batch / stream helpers (same chain, many events per launch sequence) ------------------- */
+
+/* Creates a context: preallocated device workspace + the CUDA stream it launches on.
+ * caps: host or NULL (defaults).  cuda_stream: a cudaStream_t / CUstream handle as void*
+ * (NULL = the legacy default stream). */
+int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_stream, lst_ctx** out);
+
+/* Enqueues the chain for n_events events on the context's stream and returns without waiting.
+ * Host input pointers are copied with cudaMemcpyAsync inside this call sequence (page-locked memory
+ * makes that asynchronous); device input pointers are read in place.  seeds may be NULL. */
+int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits, const lst_pls* seeds);
+
+/* Waits for the last lst_ctx_run, reads back the counters (a few hundred bytes) and reports
+ * LST_ERR_CAPACITY / LST_ERR_ARG detected on the device.  summary may be NULL. */
+int lst_ctx_sync(lst_ctx* ctx, lst_batch_summary* summary);
+
+/* After lst_ctx_sync: copies every object array of event `event` of the last batch to the host. */
+int lst_ctx_fetch_event(lst_ctx* ctx, int32_t event, lst_event_out** out);
+
+/* After lst_ctx_sync: copies the track candidates of the whole batch to caller-owned HOST buffers.
+ * tc: [cap_tc][16] int32; tc_event_offsets: n_events+1 int32.  Returns LST_ERR_CAPACITY if the
+ * batch holds more than cap_tc candidates. */
+int lst_ctx_fetch_tc(lst_ctx* ctx, int32_t* tc, int32_t cap_tc, int32_t* tc_event_offsets);
+
+/* Per-kernel device times of the last batch, measured with CUDA events on the context's stream.
+ * enable != 0 switches the recording on for the following lst_ctx_run calls. */
+int lst_ctx_set_timing(lst_ctx* ctx, int32_t enable);
+/* After lst_ctx_sync with timing on: ms[i] = duration of kernel i; returns the number of kernels
+ * (<= cap) or a negative status.  names (may be NULL) receives static strings. */
+int lst_ctx_kernel_times(lst_ctx* ctx, float* ms, const char** names, int32_t cap);
+
+/* Number of kernel launches issued by the last lst_ctx_run. */
+int lst_ctx_launch_count(lst_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LST_H */
