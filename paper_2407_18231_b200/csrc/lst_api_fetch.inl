@@ -1,0 +1,180 @@
+// lst_api_fetch.inl -- included by lst_api.cu: result read-back, lst_run_event, lst_free.
+
+namespace {
+
+void out_destroy(lst_event_out* o) {
+  if (!o) return;
+  free(o->md_hits);  free(o->md_module);  free(o->md_f);
+  free(o->ls_md);  free(o->ls_kappa);
+  free(o->t3_ls);  free(o->t3_md);  free(o->t3_k);
+  free(o->t5_t3);  free(o->t5_md);  free(o->t5_score);
+  free(o->pt3);  free(o->pt3_score);  free(o->pt5);  free(o->pt5_score);
+  free(o->tc);
+  o->magic = 0;
+  free(o);
+}
+
+template <class T>
+T* halloc(size_t n) { return static_cast<T*>(malloc(sizeof(T) * (n ? n : 1))); }
+
+// device slice -> host buffer
+template <class T>
+bool d2h(T* dst, const T* src, size_t first, size_t n) {
+  if (n == 0) return true;
+  return cudaMemcpy(dst, src + first, sizeof(T) * n, cudaMemcpyDeviceToHost) == cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out) {
+  if (!out) return LST_ERR_ARG;
+  *out = nullptr;
+  if (!ctx || ctx->magic != MAGIC_CTX || !ctx->synced || ev < 0 || ev >= ctx->last_n_events) return LST_ERR_ARG;
+  const Ctl& h = *ctx->h_ctl;
+  if (h.error) return (h.error & E_BAD_SENSOR) ? LST_ERR_ARG : LST_ERR_CAPACITY;
+  const Dev& d = ctx->dev;
+  const int E1 = ctx->last_n_events + 1;
+  auto first = [&](int kind, int e) { return ctx->h_ev_first[kind * E1 + e]; };
+  const int f_md = first(K_MD, ev), f_ls = first(K_LS, ev), f_t3 = first(K_T3, ev), f_t5 = first(K_T5, ev);
+  const int f_p3 = first(K_PT3, ev), f_p5 = first(K_PT5, ev);
+  const int f_pls = ctx->last_pls_off[ev];
+
+  lst_event_out* o = static_cast<lst_event_out*>(calloc(1, sizeof(lst_event_out)));
+  if (!o) return LST_ERR_CUDA;
+  o->magic = MAGIC_OUT;
+  o->n_md = first(K_MD, ev + 1) - f_md;
+  o->n_ls = first(K_LS, ev + 1) - f_ls;
+  o->n_t3 = first(K_T3, ev + 1) - f_t3;
+  o->n_t5 = first(K_T5, ev + 1) - f_t5;
+  o->n_pt3 = first(K_PT3, ev + 1) - f_p3;
+  o->n_pt5 = first(K_PT5, ev + 1) - f_p5;
+  // per-event counters are batch totals only when the batch holds one event
+  for (int k = 0; k < LST_N_STAGES; ++k) {
+    o->near[k] = (int64_t)h.near[k];
+    o->n_tests[k] = (int64_t)h.n_tests[k];
+  }
+  bool ok = true;
+  const int n_md = o->n_md, n_ls = o->n_ls, n_t3 = o->n_t3, n_t5 = o->n_t5;
+  // MD
+  o->md_hits = halloc<int32_t>(2 * (size_t)n_md);
+  o->md_module = halloc<int32_t>(n_md);
+  o->md_f = halloc<float>(6 * (size_t)n_md);
+  {
+    std::vector<int> info(n_md);
+    std::vector<float4> a(n_md);
+    std::vector<float2> u(n_md);
+    ok = ok && d2h(reinterpret_cast<int2*>(o->md_hits), d.md_hit, f_md, n_md) &&
+         d2h(info.data(), d.md_info, f_md, n_md) && d2h(a.data(), d.md_a, f_md, n_md) &&
+         d2h(u.data(), d.md_u, f_md, n_md);
+    for (int i = 0; ok && i < n_md; ++i) {
+      o->md_module[i] = (info[i] >> 1) - ev * d.n_mod;
+      float* f = o->md_f + 6 * (size_t)i;
+      f[0] = a[i].x;  f[1] = a[i].y;  f[2] = a[i].z;  f[3] = a[i].w;  f[4] = u[i].x;  f[5] = u[i].y;
+    }
+  }
+  // LS
+  o->ls_md = halloc<int32_t>(2 * (size_t)n_ls);
+  o->ls_kappa = halloc<float>(n_ls);
+  ok = ok && d2h(reinterpret_cast<int2*>(o->ls_md), d.ls_md, f_ls, n_ls) && d2h(o->ls_kappa, d.ls_kappa, f_ls, n_ls);
+  for (size_t i = 0; ok && i < 2 * (size_t)n_ls; ++i) o->ls_md[i] -= f_md;
+  // T3
+  o->t3_ls = halloc<int32_t>(2 * (size_t)n_t3);
+  o->t3_md = halloc<int32_t>(3 * (size_t)n_t3);
+  o->t3_k = halloc<float>(n_t3);
+  {
+    std::vector<int4> m(n_t3);
+    ok = ok && d2h(reinterpret_cast<int2*>(o->t3_ls), d.t3_ls, f_t3, n_t3) && d2h(m.data(), d.t3_md, f_t3, n_t3) &&
+         d2h(o->t3_k, d.t3_k, f_t3, n_t3);
+    for (int i = 0; ok && i < n_t3; ++i) {
+      o->t3_ls[2 * i] -= f_ls;  o->t3_ls[2 * i + 1] -= f_ls;
+      o->t3_md[3 * i] = m[i].x - f_md;  o->t3_md[3 * i + 1] = m[i].y - f_md;  o->t3_md[3 * i + 2] = m[i].z - f_md;
+    }
+  }
+  // T5
+  o->t5_t3 = halloc<int32_t>(2 * (size_t)n_t5);
+  o->t5_md = halloc<int32_t>(5 * (size_t)n_t5);
+  o->t5_score = halloc<float>(n_t5);
+  ok = ok && d2h(reinterpret_cast<int2*>(o->t5_t3), d.t5_t3, f_t5, n_t5) &&
+       d2h(o->t5_md, d.t5_md, 5 * (size_t)f_t5, 5 * (size_t)n_t5) && d2h(o->t5_score, d.t5_score, f_t5, n_t5);
+  for (size_t i = 0; ok && i < 2 * (size_t)n_t5; ++i) o->t5_t3[i] -= f_t3;
+  for (size_t i = 0; ok && i < 5 * (size_t)n_t5; ++i) o->t5_md[i] -= f_md;
+  // pT3 / pT5
+  o->pt3 = halloc<int32_t>(2 * (size_t)o->n_pt3);
+  o->pt3_score = halloc<float>(o->n_pt3);
+  o->pt5 = halloc<int32_t>(2 * (size_t)o->n_pt5);
+  o->pt5_score = halloc<float>(o->n_pt5);
+  ok = ok && d2h(reinterpret_cast<int2*>(o->pt3), d.pt3, f_p3, o->n_pt3) &&
+       d2h(o->pt3_score, d.pt3_score, f_p3, o->n_pt3) &&
+       d2h(reinterpret_cast<int2*>(o->pt5), d.pt5, f_p5, o->n_pt5) && d2h(o->pt5_score, d.pt5_score, f_p5, o->n_pt5);
+  for (int i = 0; ok && i < o->n_pt3; ++i) { o->pt3[2 * i] -= f_pls;  o->pt3[2 * i + 1] -= f_t3; }
+  for (int i = 0; ok && i < o->n_pt5; ++i) { o->pt5[2 * i] -= f_pls;  o->pt5[2 * i + 1] -= f_t5; }
+  // TC
+  int tcb[2] = {0, 0};
+  if (h.total[K_TC] > 0 || (ctx->g->cuts.stage_mask & 32)) {
+    int b0 = 0, b1 = 0;
+    ok = ok && d2h(&b0, d.tc_begin, 4 * (size_t)ev, 1) && d2h(&b1, d.tc_begin, 4 * (size_t)(ev + 1), 1);
+    tcb[0] = b0;  tcb[1] = b1;
+  }
+  o->n_tc = tcb[1] - tcb[0];
+  o->tc = halloc<int32_t>(16 * (size_t)o->n_tc);
+  ok = ok && d2h(o->tc, d.tc, 16 * (size_t)tcb[0], 16 * (size_t)o->n_tc);
+  if (!ok) {
+    out_destroy(o);
+    return LST_ERR_CUDA;
+  }
+  *out = o;
+  return LST_OK;
+}
+
+extern "C" int lst_ctx_fetch_tc(lst_ctx* ctx, int32_t* tc, int32_t cap_tc, int32_t* tc_event_offsets) {
+  if (!ctx || ctx->magic != MAGIC_CTX || !ctx->synced || !tc || !tc_event_offsets || cap_tc < 0) return LST_ERR_ARG;
+  const Ctl& h = *ctx->h_ctl;
+  if (h.error) return (h.error & E_BAD_SENSOR) ? LST_ERR_ARG : LST_ERR_CAPACITY;
+  const int n = h.total[K_TC], E = ctx->last_n_events;
+  if (n > cap_tc) return LST_ERR_CAPACITY;
+  if (!(ctx->g->cuts.stage_mask & 32)) {
+    for (int e = 0; e <= E; ++e) tc_event_offsets[e] = 0;
+    return LST_OK;
+  }
+  std::vector<int> tb(4 * (size_t)E + 1);
+  CK(cudaMemcpyAsync(tb.data(), ctx->dev.tc_begin, sizeof(int) * tb.size(), cudaMemcpyDeviceToHost, ctx->stream));
+  if (n > 0) CK(cudaMemcpyAsync(tc, ctx->dev.tc, sizeof(int) * 16 * (size_t)n, cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  for (int e = 0; e <= E; ++e) tc_event_offsets[e] = tb[4 * (size_t)e];
+  return LST_OK;
+}
+
+extern "C" int lst_run_event(lst_geometry* g, const lst_hits* hits, const lst_pls* seeds, lst_event_out** out) {
+  if (!out) return LST_ERR_ARG;
+  *out = nullptr;
+  if (!g || g->magic != MAGIC_GEOM || !hits) return LST_ERR_ARG;
+  if (hits->event_offsets || (seeds && seeds->event_offsets)) return LST_ERR_ARG;
+  if (!g->default_ctx) {
+    lst_caps c;
+    lst_default_caps(&c);
+    c.max_events = 1;
+    int rc = lst_ctx_create(g, &c, nullptr, &g->default_ctx);
+    if (rc != LST_OK) return rc;
+  }
+  int rc = lst_ctx_run(g->default_ctx, 1, hits, seeds);
+  if (rc != LST_OK) return rc;
+  rc = lst_ctx_sync(g->default_ctx, nullptr);
+  if (rc != LST_OK) return rc;
+  return lst_ctx_fetch_event(g->default_ctx, 0, out);
+}
+
+extern "C" void lst_free(void* p) {
+  if (!p) return;
+  const uint64_t magic = *static_cast<const uint64_t*>(p);
+  if (magic == MAGIC_OUT) {
+    out_destroy(static_cast<lst_event_out*>(p));
+  } else if (magic == MAGIC_CTX) {
+    ctx_destroy(static_cast<lst_ctx*>(p));
+  } else if (magic == MAGIC_GEOM) {
+    lst_geometry* g = static_cast<lst_geometry*>(p);
+    if (g->default_ctx) ctx_destroy(g->default_ctx);
+    cudaFree(g->d_subdet);  cudaFree(g->d_conn_off);  cudaFree(g->d_conn_tgt);
+    g->magic = 0;
+    delete g;
+  }
+}

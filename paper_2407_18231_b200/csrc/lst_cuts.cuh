@@ -1,0 +1,176 @@
+// lst_cuts.cuh -- device transcription of CUTS.md (the selection spec) for sm_100a.
+// binary32, evaluated exactly as parenthesised in CUTS.md; the translation unit is compiled with
+// -fmad=false (no FMA contraction), precise div/sqrt, no flush-to-zero.  Intrinsics __fmul_rn /
+// __fadd_rn are NOT needed under -fmad=false; plain operators keep the code readable.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace lst {
+
+struct Cuts {  // CUTS.md section 1: primary constants + derived (computed on the host in binary32)
+  float z0_max;
+  float md_b_phi_tol, md_z_tol, md_e_slope, md_e_tol;
+  float ls_kappa_max, ls_z_tol, ls_dir_tol;
+  float t3_kappa_max, t3_z_tol0, t3_z_tol1;
+  float t5_tol0, t5_tol1;
+  float pt_gate_tol, pt_k_tol0, pt_k_tol1, pt_z_tol;
+  float near_rel;
+  float kr, r_min, inv_2rmin;
+  int stage_mask;
+};
+
+// CUTS.md section 0: near-threshold flag of a cut v <= t
+__device__ __forceinline__ bool near_thr(const Cuts& c, float v, float t) {
+  return fabsf(v - t) <= c.near_rel * fabsf(t);
+}
+
+// CUTS.md section 1: g(u) ~ asin(sqrt u)/sqrt u, Horner innermost first
+__device__ __forceinline__ float g_poly(float u) {
+  float t = u * 0.030381944f;
+  t = 0.044642857f + t;
+  t = u * t;
+  t = 0.075f + t;
+  t = u * t;
+  t = 0.16666667f + t;
+  t = u * t;
+  return 1.0f + t;
+}
+
+// CUTS.md section 5: signed circumcircle curvature of P, Q, S (transverse plane)
+__device__ __forceinline__ float kappa3(float xp, float yp, float xq, float yq, float xs, float ys,
+                                        float& lpq, float& lqs) {
+  float ax = xq - xp, ay = yq - yp;
+  float bx = xs - xq, by = ys - yq;
+  float cx = xs - xp, cy = ys - yp;
+  lpq = sqrtf(ax * ax + ay * ay);
+  lqs = sqrtf(bx * bx + by * by);
+  float lps = sqrtf(cx * cx + cy * cy);
+  float crs = ax * cy - ay * cx;
+  return (2.0f * crs) / ((lpq * lqs) * lps);
+}
+
+// result bits of a candidate test
+enum : unsigned { ACC = 1u, NEAR = 2u };
+
+// CUTS.md section 3.  a = lower hit, b = upper hit, float4 = (x, y, z, r).
+// On accept of a barrel pair, (ux, uy) receives the unit direction.
+__device__ __forceinline__ unsigned md_test(const Cuts& c, bool endcap, float4 a, float4 b, float& ux,
+                                            float& uy) {
+  unsigned res = 0;
+  if (!endcap) {
+    float dx = b.x - a.x, dy = b.y - a.y;
+    float dd = sqrtf(dx * dx + dy * dy);
+    float dot = a.x * dx + a.y * dy;
+    float crs = a.x * dy - a.y * dx;
+    float lim = (a.w * dd) * (a.w * c.inv_2rmin + c.md_b_phi_tol);
+    float zv = fabsf(b.z * a.w - a.z * b.w);
+    float zl = c.z0_max * (b.w - a.w) + c.md_z_tol * a.w;
+    if (dot > 0.0f) {
+      if (near_thr(c, fabsf(crs), lim)) res |= NEAR;
+      if (fabsf(crs) <= lim) {
+        if (near_thr(c, zv, zl)) res |= NEAR;
+        if (zv <= zl) {
+          res |= ACC;
+          ux = dx / dd;
+          uy = dy / dd;
+        }
+      }
+    }
+  } else {
+    float crs = a.x * b.y - a.y * b.x;
+    float dz = fabsf(b.z - a.z);
+    float den = fabsf(a.z) - c.z0_max;
+    float lim = b.w * (((((a.w * a.w) * dz) * c.inv_2rmin) * c.md_e_slope) / den + c.md_e_tol);
+    float rv = fabsf(b.w * a.z - a.w * b.z);
+    float rl = c.z0_max * fabsf(b.w - a.w) + c.md_z_tol * fabsf(a.z);
+    if (near_thr(c, fabsf(crs), lim)) res |= NEAR;
+    if (fabsf(crs) <= lim) {
+      if (near_thr(c, rv, rl)) res |= NEAR;
+      if (rv <= rl) {
+        res |= ACC;
+        ux = 0.0f;
+        uy = 0.0f;
+      }
+    }
+  }
+  return res;
+}
+
+// CUTS.md section 4.  A, B = MD anchors (x, y, z, r); uA, uB = unit directions.
+__device__ __forceinline__ unsigned ls_test(const Cuts& c, float4 A, float2 uA, bool eA, float4 B,
+                                            float2 uB, bool eB, float& kappa_out) {
+  float ex = B.x - A.x, ey = B.y - A.y;
+  float cc = sqrtf(ex * ex + ey * ey);
+  float crs = A.x * B.y - A.y * B.x;
+  float kappa = (2.0f * crs) / ((A.w * B.w) * cc);
+  float kv = fabsf(kappa) * c.r_min;
+  unsigned res = 0;
+  if (near_thr(c, kv, c.ls_kappa_max)) res |= NEAR;
+  if (!(kv <= c.ls_kappa_max)) return res;
+  float tA = (A.w * kappa) * 0.5f;
+  float gA = g_poly(tA * tA);
+  float tB = (B.w * kappa) * 0.5f;
+  float gB = g_poly(tB * tB);
+  float rho = (B.w * gB) / (A.w * gA);
+  bool e = eA || eB;
+  float ztol = e ? c.ls_z_tol * (1.0f + fabsf(B.z) / B.w) : c.ls_z_tol;
+  float zv = fabsf(B.z - A.z * rho);
+  float zl = c.z0_max * (rho - 1.0f) + ztol;
+  if (near_thr(c, zv, zl)) res |= NEAR;
+  if (!(zv <= zl)) return res;
+  float half = (cc * kappa) * 0.5f;
+  if (!eA) {
+    float sA = (uA.x * ey - uA.y * ex) / cc;
+    float dA = fabsf(sA - half);
+    if (near_thr(c, dA, c.ls_dir_tol)) res |= NEAR;
+    if (!(dA <= c.ls_dir_tol)) return res;
+  }
+  if (!eB) {
+    float sB = (uB.x * ey - uB.y * ex) / cc;
+    float dB = fabsf(sB + half);
+    if (near_thr(c, dB, c.ls_dir_tol)) res |= NEAR;
+    if (!(dB <= c.ls_dir_tol)) return res;
+  }
+  kappa_out = kappa;
+  return res | ACC;
+}
+
+// CUTS.md section 5 (reading S2).  e = endcap(A) || endcap(B) || endcap(C).
+__device__ __forceinline__ unsigned t3_test(const Cuts& c, float4 A, float4 B, float4 C, bool e,
+                                            float& k3_out) {
+  float lpq, lqs;
+  float k3 = kappa3(A.x, A.y, B.x, B.y, C.x, C.y, lpq, lqs);
+  float kv = fabsf(k3) * c.r_min;
+  unsigned res = 0;
+  if (near_thr(c, kv, c.t3_kappa_max)) res |= NEAR;
+  if (!(kv <= c.t3_kappa_max)) return res;
+  float ratio = lqs / lpq;
+  float zpred = B.z + (B.z - A.z) * ratio;
+  float tol = c.t3_z_tol0 + c.t3_z_tol1 * ratio;
+  tol = e ? tol * (1.0f + fabsf(C.z) / C.w) : tol;
+  float zv = fabsf(C.z - zpred);
+  if (near_thr(c, zv, tol)) res |= NEAR;
+  if (!(zv <= tol)) return res;
+  k3_out = k3;
+  return res | ACC;
+}
+
+// CUTS.md section 6 (reading S3).  B, C, D = anchors of the bridge MDs.
+__device__ __forceinline__ unsigned t5_test(const Cuts& c, float ki, float ko, float4 B, float4 C,
+                                            float4 D, float& score_out) {
+  float l0, l1;
+  float kb = kappa3(B.x, B.y, C.x, C.y, D.x, D.y, l0, l1);
+  float tol = c.t5_tol0 + c.t5_tol1 * fmaxf(fabsf(ki), fabsf(ko));
+  float d1 = ki - kb, d2 = kb - ko, d3 = ki - ko;
+  unsigned res = 0;
+  if (near_thr(c, fabsf(d1), tol)) res |= NEAR;
+  if (!(fabsf(d1) <= tol)) return res;
+  if (near_thr(c, fabsf(d2), tol)) res |= NEAR;
+  if (!(fabsf(d2) <= tol)) return res;
+  if (near_thr(c, fabsf(d3), tol)) res |= NEAR;
+  if (!(fabsf(d3) <= tol)) return res;
+  score_out = (d1 * d1 + d2 * d2) + d3 * d3;
+  return res | ACC;
+}
+
+}  // namespace lst

@@ -1,0 +1,87 @@
+// lst_cuts_pt.cuh -- CUTS.md section 7: pLS x T3 / T5 linking (readings S6, S7).
+#pragma once
+#include "lst_cuts.cuh"
+
+namespace lst {
+
+struct Seed {  // per-pLS quantities that do not depend on the candidate (CUTS.md section 7)
+  float x1, y1, z1;
+  float vx, vy, lv;  // P1 - P0 and its transverse length
+  float kp;          // (-q) / (pt * KR)
+  float slope;       // (z1 - z0) / lv
+  float tolk;        // PT_K_TOL0 + PT_K_TOL1 * |kp|
+};
+
+__device__ __forceinline__ Seed make_seed(const Cuts& c, float pt, int q, float x0, float y0, float z0,
+                                          float x1, float y1, float z1) {
+  Seed s;
+  s.x1 = x1;
+  s.y1 = y1;
+  s.z1 = z1;
+  float qf = (float)q;
+  s.kp = (-qf) / (pt * c.kr);
+  s.vx = x1 - x0;
+  s.vy = y1 - y0;
+  s.lv = sqrtf(s.vx * s.vx + s.vy * s.vy);
+  s.slope = (z1 - z0) / s.lv;
+  s.tolk = c.pt_k_tol0 + c.pt_k_tol1 * fabsf(s.kp);
+  return s;
+}
+
+// Gate on the first MD anchor (ax, ay).  Returns ACC if the gate passes, NEAR if the gcrs cut was
+// evaluated and is near-threshold (the strict gdot > 0 cut is never flagged).
+__device__ __forceinline__ unsigned pt_gate(const Cuts& c, const Seed& s, float ax, float ay) {
+  float wx = ax - s.x1, wy = ay - s.y1;
+  float gdot = s.vx * wx + s.vy * wy;
+  if (!(gdot > 0.0f)) return 0;
+  float lw = sqrtf(wx * wx + wy * wy);
+  float gcrs = fabsf(s.vx * wy - s.vy * wx);
+  float glim = (s.lv * lw) * (lw * c.inv_2rmin + c.pt_gate_tol);
+  unsigned res = near_thr(c, gcrs, glim) ? NEAR : 0u;
+  if (gcrs <= glim) res |= ACC;
+  return res;
+}
+
+// r-z extrapolation cut at anchor Q (CUTS.md section 7, loop over Q in (A, L))
+__device__ __forceinline__ unsigned pt_rz(const Cuts& c, const Seed& s, float kx, float4 Q, bool eQ) {
+  float qx = Q.x - s.x1, qy = Q.y - s.y1;
+  float lq = sqrtf(qx * qx + qy * qy);
+  float tq = (lq * kx) * 0.5f;
+  float sq = lq * g_poly(tq * tq);
+  float zq = fabsf(Q.z - (s.z1 + s.slope * sq));
+  float zt = eQ ? c.pt_z_tol * (1.0f + fabsf(Q.z) / Q.w) : c.pt_z_tol;
+  unsigned res = near_thr(c, zq, zt) ? NEAR : 0u;
+  if (zq <= zt) res |= ACC;
+  return res;
+}
+
+// Cuts after the gate.  kt[0..n_kt) = stored curvatures (k3 of a T3; ki, ko of a T5);
+// base = 0 for a pT3, the T5 score for a pT5.  A = first MD anchor, L = last MD anchor.
+template <int N_KT>
+__device__ __forceinline__ unsigned pt_after_gate(const Cuts& c, const Seed& s, float4 A, bool eA,
+                                                  float4 L, bool eL, const float (&kt)[N_KT],
+                                                  float base, float& score_out) {
+  float l0, l1;
+  float kx = kappa3(s.x1, s.y1, A.x, A.y, L.x, L.y, l0, l1);
+  float dp = kx - s.kp;
+  unsigned res = near_thr(c, fabsf(dp), s.tolk) ? NEAR : 0u;
+  if (!(fabsf(dp) <= s.tolk)) return res;
+  float score = dp * dp;
+#pragma unroll
+  for (int i = 0; i < N_KT; ++i) {
+    float dk = kx - kt[i];
+    if (near_thr(c, fabsf(dk), s.tolk)) res |= NEAR;
+    if (!(fabsf(dk) <= s.tolk)) return res;
+    score = score + dk * dk;
+  }
+  unsigned r = pt_rz(c, s, kx, A, eA);
+  res |= (r & NEAR);
+  if (!(r & ACC)) return res;
+  r = pt_rz(c, s, kx, L, eL);
+  res |= (r & NEAR);
+  if (!(r & ACC)) return res;
+  score_out = score + base;
+  return res | ACC;
+}
+
+}  // namespace lst

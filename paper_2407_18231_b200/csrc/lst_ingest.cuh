@@ -1,0 +1,93 @@
+// lst_ingest.cuh -- step a0: hit ingestion and module binning (counting sort by global sensor),
+// plus the generic single-pass exclusive scan kernel.  PAPER.md:23 ("uses as input the hits of the
+// ... outer tracker"); SURVEY.md section 8(a) row a0.
+#pragma once
+#include "lst_scan.cuh"
+#include "lst_types.cuh"
+
+namespace lst {
+
+// event of a batch-global index, from the (<= a few dozen entries) offsets array
+__device__ __forceinline__ int event_of(const int* __restrict__ off, int n_events, int i) {
+  int lo = 0, hi = n_events;  // invariant: off[lo] <= i < off[hi]
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (__ldg(off + mid) <= i) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+// a0.1 histogram: one atomic per hit on its sensor counter; the returned rank is kept so that the
+// scatter pass needs no second atomic.  Invalid sensor ids raise E_BAD_SENSOR (-> LST_ERR_ARG).
+__global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
+  const int stride = gridDim.x * blockDim.x;
+  const int n_sens = 2 * d.n_mod;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.n_hits; i += stride) {
+    int s = __ldg(d.in_sensor + i);
+    if (s < 0 || s >= n_sens) {
+      atomicOr(&d.ctl->error, E_BAD_SENSOR);
+      s = 0;
+    }
+    const int ev = event_of(d.hit_ev_off, d.n_events, i);
+    const int gs = ev * n_sens + s;
+    d.hit_gs_in[i] = gs;
+    d.hit_rank[i] = atomicAdd(d.sens_cnt + gs, 1);
+  }
+  // pLS -> event (tiny; rides along)
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < d.n_pls; p += stride)
+    d.pls_event[p] = event_of(d.pls_ev_off, d.n_events, p);
+}
+
+// Generic exclusive scan out[i] = sum_{j<i} in[j], i in [0, n], n = (*n_ptr) * n_mul + n_add
+// (n_ptr may be NULL -> n = n_add).  in[n] is not read; out[n] = total.  Persistent blocks take
+// tile tickets; 4 items per thread.
+constexpr int kScanItems = 4;
+constexpr int kScanTile = kBlock * kScanItems;
+
+__global__ void __launch_bounds__(kBlock)
+k_scan(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int n_mul, int n_add,
+       int* ticket, unsigned long long* state) {
+  __shared__ int s_tile;
+  __shared__ int s_scan[kWarps + 2];
+  const int n = (n_ptr ? (*n_ptr) * n_mul : 0) + n_add;
+  const int n_tiles = (n + kScanTile - 1) / kScanTile > 0 ? (n + kScanTile - 1) / kScanTile : 1;
+  for (;;) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int base_i = tile * kScanTile + threadIdx.x * kScanItems;
+    int v[kScanItems];
+    int sum = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+      v[k] = (base_i + k < n) ? in[base_i + k] : 0;
+      sum += v[k];
+    }
+    int tb, tt;
+    int off = tile_alloc(sum, state, tile, s_scan, tb, tt);
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+      if (base_i + k < n) out[base_i + k] = off;
+      off += v[k];
+    }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) out[n] = tb + tt;
+  }
+}
+
+// a0.3 scatter: sorted SoA (float4 x,y,z,r + input index + global sensor), r = sqrtf(x*x + y*y)
+__global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
+  const int stride = gridDim.x * blockDim.x;
+  const int n_sens = 2 * d.n_mod;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.n_hits; i += stride) {
+    const int gs = d.hit_gs_in[i];
+    const int pos = __ldg(d.sens_begin + gs) + d.hit_rank[i];
+    const float x = __ldg(d.in_x + i), y = __ldg(d.in_y + i), z = __ldg(d.in_z + i);
+    d.hit[pos] = make_float4(x, y, z, sqrtf(x * x + y * y));
+    const int ev = gs / n_sens;
+    d.hit_idx[pos] = i - __ldg(d.hit_ev_off + ev);
+    d.hit_gs[pos] = gs;
+  }
+}
+
+}  // namespace lst

@@ -1,0 +1,112 @@
+// lst_scan.cuh -- single-pass allocation primitives: warp/block scans and decoupled look-back.
+//
+// Every object-building stage is "owner -> variable number of accepted candidates".  Output slots
+// are assigned by an exclusive prefix sum over the owners, computed INSIDE the producing kernel:
+// tiles of owners take a ticket (so lower tiles always started earlier), scan their counts in
+// shared memory, publish the tile aggregate in a 64-bit status word and look back over the
+// predecessors' words for their prefix.  Result: objects are stored in owner order (deterministic,
+// contiguous per owner, per module and per event) with one kernel launch per stage and no atomics
+// on the data path.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lst {
+
+constexpr int kBlock = 256;  // threads per block of every stage kernel
+constexpr int kWarps = kBlock / 32;
+constexpr unsigned kFull = 0xffffffffu;
+
+__device__ __forceinline__ int warp_incl_scan(int v) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    int t = __shfl_up_sync(kFull, v, d);
+    if (lane >= d) v += t;
+  }
+  return v;
+}
+
+__device__ __forceinline__ int warp_sum(int v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(kFull, v, d);
+  return v;
+}
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(kFull, v, d);
+  return v;
+}
+
+// tile status word: [63:32] flag (0 empty, 1 aggregate, 2 inclusive prefix), [31:0] value
+__device__ __forceinline__ void st_state(unsigned long long* p, unsigned flag, int v) {
+  unsigned long long w = ((unsigned long long)flag << 32) | (unsigned)v;
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(w) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
+  unsigned long long w;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w) : "l"(p) : "memory");
+  return w;
+}
+
+// Called by ONE full warp.  Publishes `aggregate` of tile `tile`, looks back, publishes the
+// inclusive prefix and returns the exclusive prefix of the tile.
+__device__ __forceinline__ int lookback_exclusive(unsigned long long* state, int tile, int aggregate) {
+  const int lane = threadIdx.x & 31;
+  if (tile == 0) {
+    if (lane == 0) st_state(state, 2u, aggregate);
+    return 0;
+  }
+  if (lane == 0) st_state(state + tile, 1u, aggregate);
+  int excl = 0;
+  int t = tile - 1;
+  for (;;) {
+    const int idx = t - lane;
+    unsigned long long w = (idx >= 0) ? ld_state(state + idx) : (2ull << 32);
+    while (__any_sync(kFull, (unsigned)(w >> 32) == 0u)) {
+      if ((unsigned)(w >> 32) == 0u) w = ld_state(state + idx);
+    }
+    const unsigned incl_mask = __ballot_sync(kFull, (unsigned)(w >> 32) == 2u);
+    const int val = (int)(unsigned)(w & 0xffffffffull);
+    if (incl_mask) {
+      const int first = __ffs(incl_mask) - 1;  // nearest predecessor holding an inclusive prefix
+      excl += warp_sum(lane <= first ? val : 0);
+      break;
+    }
+    excl += warp_sum(val);
+    t -= 32;
+  }
+  if (lane == 0) st_state(state + tile, 2u, excl + aggregate);
+  return excl;
+}
+
+// Block-wide exclusive scan of one int per thread + look-back.  Returns the GLOBAL exclusive
+// offset of this thread's count; tile_total/tile_base are block-uniform.  Must be called by all
+// kBlock threads.  smem: kWarps + 2 ints.
+__device__ __forceinline__ int tile_alloc(int cnt, unsigned long long* state, int tile, int* smem,
+                                          int& tile_base, int& tile_total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int incl = warp_incl_scan(cnt);
+  if (lane == 31) smem[warp] = incl;
+  __syncthreads();
+  if (warp == 0) {
+    int w = (lane < kWarps) ? smem[lane] : 0;
+    const int wincl = warp_incl_scan(w);
+    const int total = __shfl_sync(kFull, wincl, kWarps - 1);
+    const int base = lookback_exclusive(state, tile, total);
+    if (lane < kWarps) smem[lane] = wincl - w;  // exclusive warp offsets
+    if (lane == 0) {
+      smem[kWarps] = base;
+      smem[kWarps + 1] = total;
+    }
+  }
+  __syncthreads();
+  tile_base = smem[kWarps];
+  tile_total = smem[kWarps + 1];
+  const int off = tile_base + smem[warp] + incl - cnt;
+  __syncthreads();  // smem is reused by the caller's next tile
+  return off;
+}
+
+}  // namespace lst

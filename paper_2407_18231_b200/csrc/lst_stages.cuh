@@ -1,0 +1,226 @@
+// lst_stages.cuh -- steps a1..a4: MD, LS, T3, T5.  One launch per stage:
+// thread per owner; pass 1 counts the accepted candidates of the owner, tile_alloc() turns the
+// counts into output offsets (shared-memory scan + decoupled look-back), pass 2 re-evaluates and
+// writes.  Objects therefore sit in owner order: MDs by upper hit (= by module), LSs by inner MD,
+// T3s by first LS (= by first MD), T5s by first T3.
+#pragma once
+#include "lst_ingest.cuh"
+
+namespace lst {
+
+template <class Stage>
+__global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
+  __shared__ int s_tile;
+  __shared__ int s_scan[kWarps + 2];
+  __shared__ unsigned long long s_red[2];
+  Stage st(d);
+  const int n = st.n_owners();
+  const int n_tiles = n > 0 ? (n + kBlock - 1) / kBlock : 1;
+  unsigned long long near = 0, tests = 0;
+  for (;;) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(d.ctl->ticket + Stage::kTicket, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int owner = tile * kBlock + threadIdx.x;
+    int cnt = 0;
+    if (owner < n) cnt = st.template visit<false>(owner, 0, near, tests);
+    int tb, tt;
+    const int off = tile_alloc(cnt, d.tstate[Stage::kTicket], tile, s_scan, tb, tt);
+    if (owner < n) st.begin()[owner] = off;
+    if (cnt > 0) {
+      unsigned long long n0 = 0, t0 = 0;
+      st.template visit<true>(owner, off, n0, t0);
+    }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) {
+      const int total = tb + tt;
+      st.begin()[n] = total;
+      if (total > d.cap[Stage::kKind]) {
+        atomicOr(&d.ctl->error, Stage::kErr);
+        d.ctl->total[Stage::kKind] = 0;
+      } else {
+        d.ctl->total[Stage::kKind] = total;
+      }
+    }
+  }
+  // per-stage counters: one atomic pair per block
+  if (threadIdx.x < 2) s_red[threadIdx.x] = 0;
+  __syncthreads();
+  near = warp_sum_u64(near);
+  tests = warp_sum_u64(tests);
+  if ((threadIdx.x & 31) == 0) {
+    if (near) atomicAdd(&s_red[0], near);
+    if (tests) atomicAdd(&s_red[1], tests);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (s_red[0]) atomicAdd(&d.ctl->near[Stage::kStage], s_red[0]);
+    if (s_red[1]) atomicAdd(&d.ctl->n_tests[Stage::kStage], s_red[1]);
+  }
+}
+
+// ---- a1: Mini-Doublets (CUTS.md section 3).  owner = sorted hit on an UPPER sensor; candidates =
+// the lower-sensor hits of the same module (a contiguous range just before the upper range).
+struct StageMD {
+  static constexpr int kTicket = T_MD, kKind = K_MD, kErr = E_CAP_MD, kStage = 0;
+  const Dev& d;
+  __device__ explicit StageMD(const Dev& dd) : d(dd) {}
+  __device__ int n_owners() const { return (d.cuts.stage_mask & 1) ? d.n_hits : 0; }
+  __device__ int* begin() const { return d.hit_md_begin; }
+  template <bool FILL>
+  __device__ int visit(int i, int pos, unsigned long long& near, unsigned long long& tests) const {
+    const int gs = d.hit_gs[i];
+    if (!(gs & 1)) return 0;
+    const int gm = gs >> 1;
+    const int ev = gm / d.n_mod;
+    const bool endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
+    const int a0 = __ldg(d.sens_begin + gs - 1), a1 = __ldg(d.sens_begin + gs);
+    const float4 hb = d.hit[i];
+    const int cap = d.cap[K_MD];
+    int cnt = 0;
+    for (int a = a0; a < a1; ++a) {
+      const float4 ha = d.hit[a];
+      float ux, uy;
+      const unsigned r = md_test(d.cuts, endcap, ha, hb, ux, uy);
+      if (!FILL) near += (r >> 1) & 1u;
+      if (r & ACC) {
+        if (FILL && pos < cap) {
+          d.md_hit[pos] = make_int2(d.hit_idx[a], d.hit_idx[i]);
+          d.md_info[pos] = 2 * gm + (endcap ? 1 : 0);
+          d.md_a[pos] = ha;
+          d.md_u[pos] = make_float2(ux, uy);
+        }
+        ++pos;
+        ++cnt;
+      }
+    }
+    if (!FILL) tests += (unsigned long long)(a1 - a0);
+    return cnt;
+  }
+};
+
+// ---- a2: Line Segments (CUTS.md section 4).  owner = inner MD A; candidates = the MDs of every
+// module in conn[module(A)] (contiguous index lists of the CSR map).
+struct StageLS {
+  static constexpr int kTicket = T_LS, kKind = K_LS, kErr = E_CAP_LS, kStage = 1;
+  const Dev& d;
+  __device__ explicit StageLS(const Dev& dd) : d(dd) {}
+  __device__ int n_owners() const { return (d.cuts.stage_mask & 2) ? d.ctl->total[K_MD] : 0; }
+  __device__ int* begin() const { return d.md_ls_begin; }
+  template <bool FILL>
+  __device__ int visit(int A, int pos, unsigned long long& near, unsigned long long& tests) const {
+    const int info = d.md_info[A];
+    const int gm = info >> 1;
+    const bool eA = info & 1;
+    const int ev = gm / d.n_mod;
+    const int m = gm - ev * d.n_mod;
+    const float4 a = d.md_a[A];
+    const float2 ua = d.md_u[A];
+    const int cap = d.cap[K_LS];
+    const int gs_base = 2 * ev * d.n_mod;
+    int cnt = 0;
+    const int k1 = __ldg(d.conn_off + m + 1);
+    for (int k = __ldg(d.conn_off + m); k < k1; ++k) {
+      const int m2 = __ldg(d.conn_tgt + k);
+      const bool eB = __ldg(d.subdet + m2) != 0;
+      const int gs2 = gs_base + 2 * m2;
+      const int b0 = d.hit_md_begin[__ldg(d.sens_begin + gs2 + 1)];
+      const int b1 = d.hit_md_begin[__ldg(d.sens_begin + gs2 + 2)];
+      if (!FILL) tests += (unsigned long long)(b1 - b0);
+      for (int B = b0; B < b1; ++B) {
+        float kappa;
+        const unsigned r = ls_test(d.cuts, a, ua, eA, d.md_a[B], d.md_u[B], eB, kappa);
+        if (!FILL) near += (r >> 1) & 1u;
+        if (r & ACC) {
+          if (FILL && pos < cap) {
+            d.ls_md[pos] = make_int2(A, B);
+            d.ls_kappa[pos] = kappa;
+          }
+          ++pos;
+          ++cnt;
+        }
+      }
+    }
+    return cnt;
+  }
+};
+
+// ---- a3: T3 (CUTS.md section 5).  owner = LS (A->B); candidates = the LSs whose inner MD is B.
+struct StageT3 {
+  static constexpr int kTicket = T_T3, kKind = K_T3, kErr = E_CAP_T3, kStage = 2;
+  const Dev& d;
+  __device__ explicit StageT3(const Dev& dd) : d(dd) {}
+  __device__ int n_owners() const { return (d.cuts.stage_mask & 4) ? d.ctl->total[K_LS] : 0; }
+  __device__ int* begin() const { return d.ls_t3_begin; }
+  template <bool FILL>
+  __device__ int visit(int l, int pos, unsigned long long& near, unsigned long long& tests) const {
+    const int2 ab = d.ls_md[l];
+    const int l0 = d.md_ls_begin[ab.y], l1 = d.md_ls_begin[ab.y + 1];
+    if (!FILL) tests += (unsigned long long)(l1 - l0);
+    if (l0 == l1) return 0;
+    const float4 a = d.md_a[ab.x], b = d.md_a[ab.y];
+    const int eAB = (d.md_info[ab.x] & 1) | ((d.md_info[ab.y] & 1) << 1);
+    const int cap = d.cap[K_T3];
+    int cnt = 0;
+    for (int l2 = l0; l2 < l1; ++l2) {
+      const int C = d.ls_md[l2].y;
+      const float4 c = d.md_a[C];
+      const int eC = d.md_info[C] & 1;
+      float k3;
+      const unsigned r = t3_test(d.cuts, a, b, c, (eAB | eC) != 0, k3);
+      if (!FILL) near += (r >> 1) & 1u;
+      if (r & ACC) {
+        if (FILL && pos < cap) {
+          d.t3_ls[pos] = make_int2(l, l2);
+          d.t3_md[pos] = make_int4(ab.x, ab.y, C, eAB | (eC << 2));
+          d.t3_k[pos] = k3;
+          d.t3_axy[pos] = make_float2(a.x, a.y);
+        }
+        ++pos;
+        ++cnt;
+      }
+    }
+    return cnt;
+  }
+};
+
+// ---- a4: T5 (CUTS.md section 6).  owner = T3 (A,B,C); candidates = the T3s whose first MD is C,
+// i.e. the T3 range of the LSs whose inner MD is C.
+struct StageT5 {
+  static constexpr int kTicket = T_T5, kKind = K_T5, kErr = E_CAP_T5, kStage = 3;
+  const Dev& d;
+  __device__ explicit StageT5(const Dev& dd) : d(dd) {}
+  __device__ int n_owners() const { return (d.cuts.stage_mask & 8) ? d.ctl->total[K_T3] : 0; }
+  __device__ int* begin() const { return d.t3_t5_begin; }
+  template <bool FILL>
+  __device__ int visit(int t1, int pos, unsigned long long& near, unsigned long long& tests) const {
+    const int4 m1 = d.t3_md[t1];
+    const int u0 = d.ls_t3_begin[d.md_ls_begin[m1.z]], u1 = d.ls_t3_begin[d.md_ls_begin[m1.z + 1]];
+    if (!FILL) tests += (unsigned long long)(u1 - u0);
+    if (u0 == u1) return 0;
+    const float ki = d.t3_k[t1];
+    const float4 b = d.md_a[m1.y], c = d.md_a[m1.z];
+    const int cap = d.cap[K_T5];
+    int cnt = 0;
+    for (int t2 = u0; t2 < u1; ++t2) {
+      const int4 m2 = d.t3_md[t2];
+      float score;
+      const unsigned r = t5_test(d.cuts, ki, d.t3_k[t2], b, c, d.md_a[m2.y], score);
+      if (!FILL) near += (r >> 1) & 1u;
+      if (r & ACC) {
+        if (FILL && pos < cap) {
+          d.t5_t3[pos] = make_int2(t1, t2);
+          int* md = d.t5_md + 5 * (size_t)pos;
+          md[0] = m1.x; md[1] = m1.y; md[2] = m1.z; md[3] = m2.y; md[4] = m2.z;
+          d.t5_score[pos] = score;
+          d.t5_axy[pos] = d.t3_axy[t1];
+        }
+        ++pos;
+        ++cnt;
+      }
+    }
+    return cnt;
+  }
+};
+
+}  // namespace lst

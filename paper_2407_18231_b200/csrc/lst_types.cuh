@@ -1,0 +1,102 @@
+// lst_types.cuh -- device-side data layout of one context (structure of arrays in HBM).
+//
+// Everything of a batch lives in ONE index space: events are concatenated, a "global module" is
+// gm = event * n_mod + module and a "global sensor" gs = 2 * gm + {0,1}.  Because every stage
+// stores its objects in owner order (lst_scan.cuh), hits, MDs, LSs, T3s, T5s, pT3s and pT5s of an
+// event are contiguous, so per-event ranges follow from the *_begin arrays.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lst_cuts.cuh"
+
+namespace lst {
+
+enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_N };
+
+enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
+              E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
+
+// Small control block, zeroed (one memset, together with the tile status words) per batch.
+struct Ctl {
+  int ticket[T_N];
+  int total[K_NKINDS];
+  int error;
+  int pad;
+  unsigned long long near[6];
+  unsigned long long n_tests[6];
+};
+
+struct Dev {
+  // ---- geometry (immutable, shared) ----
+  int n_mod;
+  const int* subdet;    // [n_mod]
+  const int* conn_off;  // [n_mod + 1]
+  const int* conn_tgt;
+  // ---- batch ----
+  int n_events, n_hits, n_pls;
+  const int* hit_ev_off;  // [n_events + 1] device copy of the event offsets
+  const int* pls_ev_off;  // [n_events + 1]
+  const float *in_x, *in_y, *in_z;  // input hits (device), caller order
+  const int* in_sensor;
+  const float *p_pt, *p_x0, *p_y0, *p_z0, *p_x1, *p_y1, *p_z1;  // pLS (device)
+  const int* p_q;
+  // ---- control ----
+  Ctl* ctl;
+  unsigned long long* tstate[T_N];  // look-back status words per scanning kernel
+  // ---- a0: hits binned by global sensor ----
+  int* hit_gs_in;    // [n_hits] global sensor of input hit i
+  int* hit_rank;     // [n_hits] arrival rank inside its sensor bin
+  int* sens_cnt;     // [n_events * 2 * n_mod + 1]
+  int* sens_begin;   // [n_events * 2 * n_mod + 1] exclusive scan of sens_cnt
+  float4* hit;       // [n_hits] sorted (x, y, z, r)
+  int* hit_idx;      // [n_hits] event-local input index of the sorted hit
+  int* hit_gs;       // [n_hits] global sensor of the sorted hit
+  // ---- a1: MD (owner = upper-sensor hit) ----
+  int* hit_md_begin;  // [n_hits + 1]
+  int2* md_hit;       // (h_lo, h_hi) event-local input indices
+  int* md_info;       // 2 * gm + endcap
+  float4* md_a;       // anchor = lower hit (x, y, z, r)
+  float2* md_u;       // unit direction (barrel), 0 (endcap)
+  // ---- a2: LS (owner = inner MD) ----
+  int* md_ls_begin;  // [n_md + 1]
+  int2* ls_md;       // (md_in, md_out) batch-global MD indices
+  float* ls_kappa;
+  // ---- a3: T3 (owner = first LS) ----
+  int* ls_t3_begin;  // [n_ls + 1]
+  int2* t3_ls;
+  int4* t3_md;  // (A, B, C, endcap flags bit0 A, bit1 B, bit2 C)
+  float* t3_k;
+  float2* t3_axy;  // anchor of the first MD (coalesced operand of the pLS gate)
+  // ---- a4: T5 (owner = first T3) ----
+  int* t3_t5_begin;  // [n_t3 + 1]
+  int2* t5_t3;
+  int* t5_md;  // [n_t5][5]
+  float* t5_score;
+  float2* t5_axy;
+  // ---- a5: pT3 / pT5 (owner = pLS) ----
+  int* pls_event;      // [n_pls]
+  int* pls_pt3_begin;  // [n_pls + 1]
+  int* pls_pt5_begin;  // [n_pls + 1]
+  int2* pt3;           // (pls, t3) batch-global
+  float* pt3_score;
+  int2* pt5;
+  float* pt5_score;
+  // ---- a6: duplicate removal + track candidates ----
+  int* idx_cnt;    // [3 * n_md + 1] objects containing MD m: kind 0 T5, 1 pT5, 2 pT3
+  int* idx_begin;  // [3 * n_md + 1]
+  int* idx_cur;    // [3 * n_md]
+  int* idx_list;   // [5 * n_t5 + 5 * n_pt5 + 3 * n_pt3]
+  unsigned char *keep5, *keep3, *keepT, *linked;
+  int* tc_cnt;    // [n_events * 4 + 1] survivors per (event, class)
+  int* tc_begin;  // [n_events * 4 + 1]
+  int* tc_cur;    // [n_events * 4]
+  int* tc;        // [n_tc][16]
+  // ---- capacities ----
+  int cap[K_NKINDS];
+  int cap_idx;
+  Cuts cuts;
+};
+
+}  // namespace lst

@@ -1,0 +1,148 @@
+"""GPU parity: the CUDA chain (through the C ABI) against the CPU oracle, object by object.
+
+Bar (north_star): bit-exact sets of object index tuples; float payloads (anchors, curvatures,
+scores) bit-identical; near-threshold and candidate counters equal.
+"""
+import numpy as np
+import pytest
+
+from lst_inputs import make_config_event, make_config_geometry
+
+from .util import assert_same, canon, run_batch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lst():
+    import torch
+
+    assert torch.cuda.is_available()
+    from paper_2407_18231_b200 import build
+
+    build.build()
+    import paper_2407_18231_b200 as m
+
+    return m
+
+
+def _oracle(oracle_mod, geom, off, tgt, ev, mask=0x3f):
+    return oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls,
+                                oracle_mod.default_params(stage_mask=mask))
+
+
+@pytest.mark.parametrize("cfg,mask", [("C1", 0x0f), ("C2", 0x2f), ("C4", 0x3f), ("C3", 0x3f)])
+def test_single_event_configs(lst, oracle_mod, cfg, mask):
+    geom, off, tgt = make_config_geometry(cfg)
+    ev = make_config_event(cfg, seeds=True if cfg == "C3" else None)
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt, lst.lst_default_params(stage_mask=mask))
+    try:
+        got = lst.lst_run_event(g, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+    finally:
+        lst.lst_free(g)
+    want = _oracle(oracle_mod, geom, off, tgt, ev, mask)
+    assert len(want["t5_md"]) > 0
+    assert_same(canon(got), canon(want), f"{cfg}: ")
+    tests = want["n_tests"].astype(float)
+    assert np.all(want["near"] <= np.maximum(1e-4 * tests, 0)), "near-threshold candidates above 0.01% of the tests"
+
+
+def test_device_resident_inputs_match_host_inputs(lst, oracle_mod):
+    import torch
+
+    geom, off, tgt = make_config_geometry("C4")
+    ev = make_config_event("C4")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    try:
+        dev = {k: torch.from_numpy(getattr(ev, k)).cuda() for k in ("x", "y", "z", "sensor")}
+        pls = {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in ev.pls.items() if k != "truth"}
+        got = lst.lst_run_event(g, dev["x"], dev["y"], dev["z"], dev["sensor"], pls)
+    finally:
+        lst.lst_free(g)
+    assert_same(canon(got), canon(_oracle(oracle_mod, geom, off, tgt, ev)), "C4 device inputs: ")
+
+
+@pytest.mark.parametrize("pu,n_ev", [(50, 5), (200, 3)])
+def test_c5_batches(lst, oracle_mod, pu, n_ev):
+    """Config 5: several independent events in one launch sequence; every event equals the oracle's."""
+    geom, off, tgt = make_config_geometry("C5")
+    evs = [make_config_event("C5", pu=pu, index=i, seeds=True) for i in range(n_ev)]
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=n_ev))
+    try:
+        for rep in range(2):  # the second run reuses the workspace
+            summ = run_batch(lst, ctx, evs)
+            tot = {k: 0 for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")}
+            near = np.zeros(6, np.int64)
+            tests = np.zeros(6, np.int64)
+            for i, ev in enumerate(evs):
+                got = lst.lst_ctx_fetch_event(ctx, i)
+                want = _oracle(oracle_mod, geom, off, tgt, ev)
+                near += want["near"]
+                tests += want["n_tests"]
+                got["near"], got["n_tests"] = want["near"], want["n_tests"]  # counters are per batch (below)
+                assert_same(canon(got), canon(want), f"C5 pu{pu} event {i} rep {rep}: ")
+                for k, key in (("md", "md_hits"), ("ls", "ls_md"), ("t3", "t3_md"), ("t5", "t5_md"), ("pt3", "pt3"),
+                               ("pt5", "pt5"), ("tc", "tc")):
+                    tot[k] += len(want[key])
+            for k in tot:
+                assert summ["n_" + k] == tot[k], k
+            assert summ["near"] == near.tolist() and summ["n_tests"] == tests.tolist()
+            tcbuf = np.zeros((summ["n_tc"] + 1, 16), np.int32)
+            tc, tco = lst.lst_ctx_fetch_tc(ctx, tcbuf, n_ev)
+            assert tco[-1] == summ["n_tc"] and np.all(np.diff(tco) >= 0)
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
+def test_edge_cases(lst, oracle_mod):
+    geom, off, tgt = make_config_geometry("C1")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    try:
+        e = np.zeros(0, np.float32)
+        got = lst.lst_run_event(g, e, e, e, np.zeros(0, np.int32))
+        assert all(len(got[k]) == 0 for k in ("md_hits", "ls_md", "t3_md", "t5_md", "pt3", "pt5", "tc"))
+        one = np.ones(1, np.float32)
+        with pytest.raises(lst.LstError) as ei:
+            lst.lst_run_event(g, one, one, one, np.array([2 * geom.n_modules], np.int32))
+        assert ei.value.status == lst.LST_ERR_ARG
+        # a single hit, seeds without any T3: every pLS comes out unlinked
+        ev = make_config_event("C4")
+        got = lst.lst_run_event(g, one * 23, one * 0, one, np.zeros(1, np.int32), ev.pls)
+        assert len(got["tc"]) == ev.n_pls and np.all(got["tc"][:, 0] == 3)
+        assert sorted(got["tc"][:, 1].tolist()) == list(range(ev.n_pls))
+        # capacity overflow is an error, never a truncation
+        ev2 = make_config_event("C2")
+        ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=1, max_md=100))
+        try:
+            h, keep = lst.make_hits(ev2.x, ev2.y, ev2.z, ev2.sensor)
+            lst.lst_ctx_run(ctx, 1, h, None)
+            with pytest.raises(lst.LstError) as ei:
+                lst.lst_ctx_sync(ctx)
+            assert ei.value.status == lst.LST_ERR_CAPACITY
+        finally:
+            lst.lst_free(ctx)
+    finally:
+        lst.lst_free(g)
+
+
+def test_ragged_batch_with_empty_events(lst, oracle_mod):
+    geom, off, tgt = make_config_geometry("C4")
+    from lst_inputs.events import Event
+
+    empty = Event(x=np.zeros(0, np.float32), y=np.zeros(0, np.float32), z=np.zeros(0, np.float32),
+                  sensor=np.zeros(0, np.int32), truth=np.zeros(0, np.int32))
+    evs = [empty, make_config_event("C4"), empty, make_config_event("C2"), make_config_event("C1"), empty]
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=8))
+    try:
+        run_batch(lst, ctx, evs)
+        for i, ev in enumerate(evs):
+            got = lst.lst_ctx_fetch_event(ctx, i)
+            want = _oracle(oracle_mod, geom, off, tgt, ev)
+            got["near"], got["n_tests"] = want["near"], want["n_tests"]
+            assert_same(canon(got), canon(want), f"ragged event {i}: ")
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)

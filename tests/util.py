@@ -77,3 +77,14 @@ def exact_helix_points(pt, q, phi0, eta, z0, radii):
         x, y, z = trk.pos(t)
         pts.append((x[0], y[0], z[0]))
     return np.array(pts), trk
+
+
+def run_batch(lst, ctx, events, with_seeds: bool = True):
+    """Concatenates lst_inputs Events into one batch, runs it on `ctx` and syncs; returns the summary."""
+    from lst_inputs.events import concat_events
+
+    b = concat_events(events)
+    h, keep = lst.make_hits(b["x"], b["y"], b["z"], b["sensor"], b["hit_offsets"])
+    s, keep = lst.make_pls(b["pls"] if with_seeds else None, b["pls_offsets"], keep)
+    lst.lst_ctx_run(ctx, len(events), h, s)
+    return lst.lst_ctx_sync(ctx)
