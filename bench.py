@@ -1,0 +1,483 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of the LST object-building chain on B200 (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W              # the CUDA path (this repo)
+    python bench.py --impl reference --gpus N --steps K ...    # the CPU oracle, as it stands
+
+Workload (config.workload): BASELINE.json config 5 at PU 200 -- batches of 16 independent
+PU200-like events (config 3's generator, seeds 1000*PU + index, pLS seeds on), pipelined over CUDA
+streams.  One STEP = one batch of 16 events through the whole chain (ingest/binning, MD, LS, T3,
+T5, pT3, pT5, duplicate removal, track-candidate selection) = SURVEY.md section 8(a) rows a0..a6.
+
+  value  : events/s with the batch inputs already resident in HBM (device pointers through the ABI)
+  e2e    : events/s through the same C-ABI calls with HOST (pinned) buffers: H2D of the hits and
+           seeds and D2H of the track candidates inside the timed region
+  roofline / kernels : per-kernel CUDA-event times (lst_ctx_kernel_times) of L2-flushed batches
+  cpu_baseline : the oracle (oracle/) on the host cores over a bounded sample of the same events
+
+Multi-GPU (N > 1): replicas only -- every rank runs its own batches (different seeds), no
+collective on the data path; value = all ranks' events / max-over-ranks device time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "events/sec at PU200-like occupancy (1 B200); fraction of HBM roofline"
+UNIT = "events/s"
+L2_BYTES = 126 << 20
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=("b200", "reference"), default="b200")
+    ap.add_argument("--pu", type=int, default=200)
+    ap.add_argument("--events", type=int, default=16, help="events per batch (= per step)")
+    ap.add_argument("--streams", type=int, default=4, help="contexts / CUDA streams in flight")
+    ap.add_argument("--batches", type=int, default=6, help="distinct input batches rotated through")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile-kernels-only", action="store_true",
+                    help="run only the L2-flushed single-stream loop (the command ncu wraps)")
+    return ap.parse_args()
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ---------------------------------------------------------------------------------------------
+# inputs
+# ---------------------------------------------------------------------------------------------
+def make_batches(pu, n_events, n_batches, first_index):
+    """n_batches distinct batches of n_events C5 events (lst_inputs recipe)."""
+    from lst_inputs import c5_batch
+    from lst_inputs.events import concat_events
+
+    out = []
+    for b in range(n_batches):
+        evs = c5_batch(pu=pu, n_events=n_events, seeds=True, first=first_index + b * n_events)
+        out.append((evs, concat_events(evs)))
+    return out
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed regions run."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self.stop_flag = threading.Event()
+        self.active = threading.Event()
+        self.err = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            names = {
+                nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+            }
+            while not self.stop_flag.is_set():
+                if self.active.is_set():
+                    self.samples.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                    for bit, name in names.items():
+                        if r & bit:
+                            self.reasons.add(name)
+                time.sleep(0.002)
+        except Exception as e:  # the clock record is evidence, not the product: report and go on
+            self.err = repr(e)
+
+    def summary(self):
+        d = {"sm_mhz": int(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+             "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        if self.err:
+            d["error"] = self.err
+        return d
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------
+STAGE_OF_KERNEL = {"md": "md", "ls": "ls", "t3": "t3", "t5": "t5", "pt3": "pt3", "pt5": "pt5"}
+# flops of the FIRST cut of a stage (every candidate evaluates at least that) and of the whole cut
+# list (every accepted object evaluates all of it); counted from CUTS.md, no FMA.
+FLOPS_FIRST = {"md": 19, "ls": 16, "t3": 28, "t5": 33, "pt3": 6, "pt5": 6}
+FLOPS_FULL = {"md": 30, "ls": 64, "t3": 37, "t5": 44, "pt3": 100, "pt5": 107}
+
+
+def algorithmic_work(name, s, n_sens):
+    """(bytes, flops) one launch of kernel `name` must move / compute for batch summary `s`
+    (compulsory traffic: every input array read once, every output written once)."""
+    h, p = s["n_hits"], s["n_pls"]
+    md, ls, t3, t5, p3, p5, tc = (s[k] for k in ("n_md", "n_ls", "n_t3", "n_t5", "n_pt3", "n_pt5", "n_tc"))
+    idx = 5 * t5 + 5 * p5 + 3 * p3
+    table = {
+        "hist": 12 * h + 4 * p,
+        "scan_sensors": 8 * n_sens,
+        "scatter": 44 * h,
+        "md": 28 * h + 8 * n_sens + 36 * md,
+        "ls": 32 * md + 12 * ls,
+        "t3": 12 * ls + 16 * md + 36 * t3,
+        "t5": 24 * t3 + 16 * md + 40 * t5,
+        "pt3": 36 * p + 8 * t3 + 12 * p3,
+        "pt5": 36 * p + 8 * t5 + 12 * p5,
+        "event_ranges": 0,
+        "sel_prepare": 24 * md + p,
+        "index_count": 20 * t5 + 28 * p5 + 24 * p3 + 4 * idx,
+        "scan_index": 24 * md,
+        "index_fill": 20 * t5 + 28 * p5 + 24 * p3 + 8 * idx,
+        "rule1_pt5": 33 * p5,
+        "rule2_pt3": 29 * p3,
+        "rule3_t5": 25 * t5 + p,
+        "scan_tc": 0,
+        "tc_emit": 64 * tc + p5 + p3 + t5 + p,
+    }
+    st = STAGE_OF_KERNEL.get(name)
+    flops = 0
+    if st:
+        i = ("md", "ls", "t3", "t5", "pt3", "pt5").index(st)
+        n_obj = (md, ls, t3, t5, p3, p5)[i]
+        flops = FLOPS_FIRST[st] * s["n_tests"][i] + (FLOPS_FULL[st] - FLOPS_FIRST[st]) * n_obj
+    return table.get(name, 0), flops
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), float(p.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = dist_env()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2407_18231_b200 import build as lst_build
+
+    if rank == 0 or world == 1:
+        lst_build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2407_18231_b200 as lst
+    from lst_inputs import make_config_geometry
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    E, S, NB = args.events, max(1, args.streams), max(1, args.batches)
+    geom, off, tgt = make_config_geometry("C5")
+    n_sens = E * 2 * geom.n_modules
+    t0 = time.time()
+    batches = make_batches(args.pu, E, NB, first_index=rank * NB * E)
+    gen_s = time.time() - t0
+
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    caps = lst.lst_default_caps(max_events=E)
+    streams = [torch.cuda.Stream() for _ in range(S)]
+    ctxs = [lst.lst_ctx_create(g, caps, st.cuda_stream) for st in streams]
+    sampler = ClockSampler(local)
+    sampler.start()
+
+    # device-resident and pinned-host copies of every batch
+    dev_in, host_in = [], []
+    f_hit, f_pls = ("x", "y", "z", "sensor"), ("pt", "x0", "y0", "z0", "x1", "y1", "z1", "q")
+    for _, b in batches:
+        pin = {k: torch.from_numpy(np.ascontiguousarray(b[k])).pin_memory() for k in f_hit}
+        pin_p = {k: torch.from_numpy(np.ascontiguousarray(b["pls"][k])).pin_memory() for k in f_pls}
+        d = {k: v.cuda() for k, v in pin.items()}
+        d_p = {k: v.cuda() for k, v in pin_p.items()}
+        hd, keep_d = lst.make_hits(d["x"], d["y"], d["z"], d["sensor"], b["hit_offsets"])
+        sd, keep_d = lst.make_pls(d_p, b["pls_offsets"], keep_d)
+        hh, keep_h = lst.make_hits(*(pin[k].numpy() for k in f_hit), b["hit_offsets"])
+        sh, keep_h = lst.make_pls({k: v.numpy() for k, v in pin_p.items()}, b["pls_offsets"], keep_h)
+        dev_in.append((hd, sd, keep_d, d, d_p))
+        host_in.append((hh, sh, keep_h, pin, pin_p))
+    in_bytes = [int(b["x"].shape[0]) * 16 + int(b["pls_offsets"][-1]) * 32 + 8 * (E + 1) for _, b in batches]
+    torch.cuda.synchronize()
+
+    def pipelined(inputs, K, fetch):
+        """K steps round-robin over the S contexts; returns (device ms, launches, last summaries)."""
+        inflight = [False] * S
+        launches = 0
+        d2h = 0
+        summ = [None] * S
+        start = torch.cuda.Event(enable_timing=True)
+        ends = [torch.cuda.Event(enable_timing=True) for _ in range(S)]
+        start.record(streams[0])
+        for st in streams:
+            st.wait_event(start)
+
+        def retire(c):
+            nonlocal d2h
+            summ[c] = lst.lst_ctx_sync(ctxs[c])  # status + counters of the batch this context ran
+            if fetch:
+                tc, _ = lst.lst_ctx_fetch_tc(ctxs[c], fetch[c], E)
+                d2h += int(tc.shape[0]) * 64 + 4 * (4 * E + 1) + 160
+            inflight[c] = False
+
+        for i in range(K):
+            c = i % S
+            if inflight[c]:
+                retire(c)
+            h, s = inputs[i % NB][0], inputs[i % NB][1]
+            lst.lst_ctx_run(ctxs[c], E, h, s)
+            launches += lst.lst_ctx_launch_count(ctxs[c])
+            inflight[c] = True
+        for c in range(S):
+            if inflight[c]:
+                retire(c)
+            ends[c].record(streams[c])
+        torch.cuda.synchronize()
+        return max(start.elapsed_time(e) for e in ends), launches, summ, d2h
+
+    if not args.profile_kernels_only:
+        # ---- value: inputs resident in HBM --------------------------------------------------
+        pipelined(dev_in, max(args.warmup, S), None)
+        torch.cuda.synchronize()
+        barrier()
+        sampler.active.set()
+        ms, launches, summ, _ = pipelined(dev_in, args.steps, None)
+        sampler.active.clear()
+        barrier()
+        # ---- e2e: host buffers, H2D + D2H inside ---------------------------------------------
+        tc_pin = [torch.empty((caps.max_tc, 16), dtype=torch.int32).pin_memory().numpy() for _ in range(S)]
+        pipelined(host_in, max(args.warmup, S), tc_pin)
+        torch.cuda.synchronize()
+        barrier()
+        sampler.active.set()
+        ms_e2e, _, _, d2h = pipelined(host_in, args.steps, tc_pin)
+        sampler.active.clear()
+        barrier()
+        if world > 1:
+            t = torch.tensor([ms, ms_e2e], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms, ms_e2e = float(t[0]), float(t[1])
+
+    # ---- per-kernel times: one stream, L2 flushed before every batch -----------------------------
+    hbm_gbs, sm_max_mhz, peak_src = peaks()
+    alu_peak_tflops = 148 * 128 * sm_max_mhz * 1e6 / 1e12  # FP32 lanes x clock, no FMA (CUTS.md section 0)
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device="cuda")
+    reps = 3 if args.profile_kernels_only else 12
+    lst.lst_ctx_set_timing(ctxs[0], True)
+    per_kernel = {}
+    order = []
+    ksum = None
+    sampler.active.set()
+    for r in range(reps + 2):
+        b = r % NB
+        with torch.cuda.stream(streams[0]):
+            flush.zero_()
+        lst.lst_ctx_run(ctxs[0], E, dev_in[b][0], dev_in[b][1])
+        s_b = lst.lst_ctx_sync(ctxs[0])
+        if r < 2:
+            continue  # warm-up
+        for name, t in lst.lst_ctx_kernel_times(ctxs[0]):
+            if name not in per_kernel:
+                per_kernel[name] = []
+                order.append(name)
+            w = algorithmic_work(name, s_b, n_sens)
+            per_kernel[name].append((t, w[0], w[1]))
+        ksum = s_b
+    sampler.active.clear()
+    lst.lst_ctx_set_timing(ctxs[0], False)
+    kernels = []
+    tot_ms = sum(float(np.mean([v[0] for v in per_kernel[n]])) for n in order)
+    for n in order:
+        t = float(np.mean([v[0] for v in per_kernel[n]]))
+        by = float(np.mean([v[1] for v in per_kernel[n]]))
+        fl = float(np.mean([v[2] for v in per_kernel[n]]))
+        gbs = by / (t * 1e-3) / 1e9 if t > 0 else 0.0
+        tf = fl / (t * 1e-3) / 1e12 if t > 0 else 0.0
+        kernels.append({"name": n, "ms": round(t, 5), "share": round(t / tot_ms, 4), "alg_bytes": int(by),
+                        "gbs": round(gbs, 1), "hbm_frac": round(gbs / hbm_gbs, 4), "alg_flops": int(fl),
+                        "tflops": round(tf, 3), "alu_frac": round(tf / alu_peak_tflops, 4)})
+    top = max(kernels, key=lambda k: k["ms"])
+    if top["alu_frac"] >= top["hbm_frac"]:
+        roof = {"bound": "alu", "kernel": top["name"], "achieved": top["tflops"], "peak": round(alu_peak_tflops, 2),
+                "unit": "TFLOP/s", "frac": top["alu_frac"], "traffic": None,
+                "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, 1 flop/lane/clk (no FMA)" % sm_max_mhz}
+    else:
+        roof = {"bound": "hbm", "kernel": top["name"], "achieved": top["gbs"], "peak": hbm_gbs, "unit": "GB/s",
+                "frac": top["hbm_frac"], "traffic": None, "peak_source": peak_src + " copy bandwidth"}
+    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")  # from the committed ncu --set full capture
+    if os.path.exists(traffic_path):
+        with open(traffic_path) as f:
+            roof["traffic"] = json.load(f).get(top["name"])
+    sampler.stop_flag.set()
+    sampler.join(timeout=2)
+
+    if args.profile_kernels_only:
+        if rank == 0:
+            print(json.dumps({"kernels": kernels, "summary": ksum}))
+        for c in ctxs:
+            lst.lst_free(c)
+        lst.lst_free(g)
+        return
+
+    # ---- CPU baseline (rank 0, N = 1 only) -------------------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_rate(batches[0][0][:E], geom, off, tgt)
+
+    n_hits = [int(b["x"].shape[0]) for _, b in batches]
+    line = {
+        "metric": METRIC, "value": round(world * args.steps * E / (ms * 1e-3), 1), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, S), "ms_per_step": round(ms / args.steps, 5),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {
+            "workload": "C5 PU%d: batches of %d PU200-like events (BASELINE.json configs[4]; generator of "
+                        "configs[2] with pLS seeds), %d streams" % (args.pu, E, S),
+            "events_per_step": E, "hits_per_event": int(np.mean(n_hits) / E), "pls_per_event": ksum["n_pls"] // E,
+            "modules": int(geom.n_modules), "parallelism": "replicas x%d, no collective" % world,
+            "l2": "inputs rotate over %d distinct batches + %d context workspaces (> 126 MB L2); per-kernel "
+                  "times taken with an L2 flush (252 MB write) before every batch" % (NB, S),
+            "objects_per_step": {k: ksum["n_" + k] for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
+            "tests_per_step": dict(zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["n_tests"])),
+            "near_threshold_per_step": dict(zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["near"])),
+            "generation_s": round(gen_s, 1),
+        },
+        "e2e": {"value": round(world * args.steps * E / (ms_e2e * 1e-3), 1), "unit": UNIT,
+                "h2d_bytes_per_step": int(np.mean(in_bytes)), "d2h_bytes_per_step": int(d2h / args.steps),
+                "ms_per_step": round(ms_e2e / args.steps, 5)},
+        "gpu_launches": launches,
+        "clocks": sampler.summary(),
+        "roofline": roof,
+        "kernels": kernels,
+        "objects_per_s": {k: round(ksum["n_" + k] / (ms / args.steps * 1e-3), 1)
+                          for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
+        "cpu_baseline": cpu,
+    }
+    if rank == 0:
+        print(json.dumps(line))
+    for c in ctxs:
+        lst.lst_free(c)
+    lst.lst_free(g)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------
+# the CPU oracle: cpu_baseline leg and --impl reference
+# ---------------------------------------------------------------------------------------------
+def oracle_rate(events, geom, off, tgt, single=True):
+    """Times oracle.run_event (as it stands, one thread per event) over `events` on the host cores."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    import oracle
+
+    oracle.build()
+    cores = os.cpu_count() or 1
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except AttributeError:
+        pass
+    threads = max(1, min(cores, len(events)))
+
+    def one(ev):
+        r = oracle.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+        return len(r["tc"])
+
+    t_single = float("nan")
+    if single:
+        t0 = time.perf_counter()
+        one(events[0])
+        t_single = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(threads) as ex:  # ctypes releases the GIL inside the C call
+        list(ex.map(one, events))
+    wall = time.perf_counter() - t0
+    return {"value": round(len(events) / wall, 3), "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d events of the first batch, one oracle.run_event per event, %d threads (host has %d "
+                      "cores); single thread: %.3f events/s" % (len(events), threads, cores, 1.0 / t_single),
+            "single_thread_value": round(1.0 / t_single, 3)}
+
+
+def run_reference(args):
+    """The oracle as it stands on the host cores: same config, metric and unit as the CUDA arm.
+    Each step is a bounded sample of the workload: `cores` events of the step's batch."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    from lst_inputs import make_config_geometry
+
+    geom, off, tgt = make_config_geometry("C5")
+    cores = os.cpu_count() or 1
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except AttributeError:
+        pass
+    per_step = max(1, min(cores, args.events))
+    # keep the whole run within a few minutes: ~1.5 s of one core per PU200 event
+    steps = max(1, min(args.steps, 20))
+    warm = max(0, min(args.warmup, 1))
+    batches = make_batches(args.pu, per_step, 2, first_index=0)
+    for _ in range(warm):
+        oracle_rate(batches[0][0], geom, off, tgt, single=False)
+    t0 = time.perf_counter()
+    res = None
+    for i in range(steps):
+        res = oracle_rate(batches[i % 2][0], geom, off, tgt, single=False)
+    wall = time.perf_counter() - t0
+    n_ev = steps * per_step
+    value = round(n_ev / wall, 3)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": round(wall / steps * 1e3, 3), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "C5 PU%d: batches of %d PU200-like events (BASELINE.json configs[4]); each step "
+                               "a bounded sample of %d events" % (args.pu, args.events, per_step),
+                   "events_per_step": per_step},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": res["cores"], "kind": "oracle",
+                         "sample": "%d steps x %d events, oracle.run_event, %d threads" % (steps, per_step,
+                                                                                           res["cores"])},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()
