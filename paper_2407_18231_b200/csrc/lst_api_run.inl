@@ -117,10 +117,14 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
       d.sens_cnt, d.sens_begin, nullptr, 0, n_sens, d.ctl->ticket + T_SENS, d.tstate[T_SENS]);
   L.mark("scatter");
   k_scatter<<<grid_for(g, hits->n, 8), kBlock, 0, st>>>(d);
+  L.mark("md_pairs");
+  k_scan_f<PairsMD><<<gp, kBlock, 0, st>>>(d, d.pp_md, d.cg0_md, &d.ctl->pair_total[0], T_PMD);
   L.mark("md");
-  k_stage<StageMD><<<grid_for(g, hits->n, 4), kBlock, 0, st>>>(d);
+  k_even<StageMD><<<gp, kBlock, 0, st>>>(d);
+  L.mark("ls_pairs");
+  k_scan_f<PairsLS><<<gp, kBlock, 0, st>>>(d, d.ppe_ls, d.cg0_ls, &d.ctl->pair_total[1], T_PLS);
   L.mark("ls");
-  k_stage<StageLS><<<gp, kBlock, 0, st>>>(d);
+  k_even<StageLS><<<gp, kBlock, 0, st>>>(d);
   L.mark("t3");
   k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
   L.mark("t5");

@@ -65,8 +65,8 @@ __global__ void __launch_bounds__(kBlock) k_pt(Dev d) {
     if (p < n) {
       if (n_cand_total > 0) {
         const int ev = d.pls_event[p];
-        const int md0 = d.hit_md_begin[__ldg(d.hit_ev_off + ev)];
-        const int md1 = d.hit_md_begin[__ldg(d.hit_ev_off + ev + 1)];
+        const int md0 = d.mod_md_begin[ev * d.n_mod];
+        const int md1 = d.mod_md_begin[(ev + 1) * d.n_mod];
         c0 = d.ls_t3_begin[d.md_ls_begin[md0]];
         c1 = d.ls_t3_begin[d.md_ls_begin[md1]];
         if (IS5) {

@@ -4,7 +4,7 @@
 // writes.  Objects therefore sit in owner order: MDs by upper hit (= by module), LSs by inner MD,
 // T3s by first LS (= by first MD), T5s by first T3.
 #pragma once
-#include "lst_ingest.cuh"
+#include "lst_pairs.cuh"
 
 namespace lst {
 
@@ -59,90 +59,173 @@ __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
   }
 }
 
-// ---- a1: Mini-Doublets (CUTS.md section 3).  owner = sorted hit on an UPPER sensor; candidates =
-// the lower-sensor hits of the same module (a contiguous range just before the upper range).
+// ---- a1: Mini-Doublets (CUTS.md section 3).  group = module of one event
+// (gm = event * n_mod + module); owners = hits of its UPPER sensor, candidates = hits of its LOWER
+// sensor (both contiguous ranges of the sorted hits).  MDs come out grouped by module, inside a
+// module by (upper hit, lower hit).
+struct PairsMD {  // pre-pass: candidate pairs per module = upper hits x lower hits
+  const Dev& d;
+  __device__ explicit PairsMD(const Dev& dd) : d(dd) {}
+  __device__ int n_items() const { return (d.cuts.stage_mask & 1) ? d.n_events * d.n_mod : 0; }
+  __device__ int count(int gm) const {
+    const long long p = (long long)d.sens_cnt[2 * gm] * d.sens_cnt[2 * gm + 1];
+    if (p > d.cap_pairs) {
+      atomicOr(&d.ctl->error, E_CAP_MD);
+      return 0;
+    }
+    return (int)p;
+  }
+  __device__ int group(int gm) const { return gm; }
+};
+
 struct StageMD {
-  static constexpr int kTicket = T_MD, kKind = K_MD, kErr = E_CAP_MD, kStage = 0;
+  static constexpr int kTicket = T_MD, kKind = K_MD, kErr = E_CAP_MD, kStage = 0, kPairSlot = 0;
+  struct Group {
+    int gbase, gend, n_c;
+    int a0, b0;  // first lower / first upper sorted hit
+    int endcap;
+  };
+  struct Payload {
+    int a, b;  // sorted hit positions
+    float ux, uy;
+  };
   const Dev& d;
   __device__ explicit StageMD(const Dev& dd) : d(dd) {}
-  __device__ int n_owners() const { return (d.cuts.stage_mask & 1) ? d.n_hits : 0; }
-  __device__ int* begin() const { return d.hit_md_begin; }
-  template <bool FILL>
-  __device__ int visit(int i, int pos, unsigned long long& near, unsigned long long& tests) const {
-    const int gs = d.hit_gs[i];
-    if (!(gs & 1)) return 0;
-    const int gm = gs >> 1;
+  __device__ int n_groups() const { return (d.cuts.stage_mask & 1) ? d.n_events * d.n_mod : 0; }
+  __device__ const int* chunk_g0() const { return d.cg0_md; }
+  __device__ int pp(int g) const { return d.pp_md[g]; }
+  __device__ void load_group(int gm, Group& G) const {
+    G.a0 = __ldg(d.sens_begin + 2 * gm);
+    G.b0 = __ldg(d.sens_begin + 2 * gm + 1);
+    G.n_c = G.b0 - G.a0;
     const int ev = gm / d.n_mod;
-    const bool endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
-    const int a0 = __ldg(d.sens_begin + gs - 1), a1 = __ldg(d.sens_begin + gs);
-    const float4 hb = d.hit[i];
-    const int cap = d.cap[K_MD];
-    int cnt = 0;
-    for (int a = a0; a < a1; ++a) {
-      const float4 ha = d.hit[a];
-      float ux, uy;
-      const unsigned r = md_test(d.cuts, endcap, ha, hb, ux, uy);
-      if (!FILL) near += (r >> 1) & 1u;
-      if (r & ACC) {
-        if (FILL && pos < cap) {
-          d.md_hit[pos] = make_int2(d.hit_idx[a], d.hit_idx[i]);
-          d.md_info[pos] = 2 * gm + (endcap ? 1 : 0);
-          d.md_a[pos] = ha;
-          d.md_u[pos] = make_float2(ux, uy);
-        }
-        ++pos;
-        ++cnt;
-      }
+    G.endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
+  }
+  __device__ unsigned test(const Group& G, int o, int j, Payload& pay) const {
+    pay.a = G.a0 + j;
+    pay.b = G.b0 + o;
+    return md_test(d.cuts, G.endcap, d.hit[pay.a], d.hit[pay.b], pay.ux, pay.uy);
+  }
+  __device__ void emit(int pos, const Payload& pay) const {
+    const int gs = d.hit_gs[pay.a];  // lower sensor: gs = 2 * gm
+    const int ev = (gs >> 1) / d.n_mod;
+    d.md_hit[pos] = make_int2(d.hit_idx[pay.a], d.hit_idx[pay.b]);
+    d.md_info[pos] = gs | (__ldg(d.subdet + ((gs >> 1) - ev * d.n_mod)) != 0);
+    d.md_a[pos] = d.hit[pay.a];
+    d.md_u[pos] = make_float2(pay.ux, pay.uy);
+  }
+  // first MD of every module: rank of the module's first pair
+  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int, int, const TileRank& rank) const {
+    const int n = d.n_events * d.n_mod;
+    if (no_pairs) {
+      for (int g = threadIdx.x; g <= n; g += kBlock) d.mod_md_begin[g] = 0;
+      return;
     }
-    if (!FILL) tests += (unsigned long long)(a1 - a0);
-    return cnt;
+    for (int g = (tile == 0 ? 0 : g_lo + 1) + threadIdx.x; g <= g_hi; g += kBlock) d.mod_md_begin[g] = rank(pp(g));
+  }
+  __device__ void finish_total(int) const {}
+};
+
+// ---- a2: Line Segments (CUTS.md section 4).  group = module gm of one event;
+// owners = its MDs A, candidates = the MDs of the modules in conn[module], concatenated in the
+// order of the CSR row (row length NB).  The pre-pass scans n_MD(source) x n_MD(target) over the
+// edges of all events, so the prefix array ppe_ls is at once the pair prefix of the modules (at a
+// row's first edge) and, divided by n_MD(source), the map candidate j -> (edge, B) inside a row.
+// LSs come out grouped by inner MD, inside an MD by (edge, B).
+struct PairsLS {
+  const Dev& d;
+  __device__ explicit PairsLS(const Dev& dd) : d(dd) {}
+  __device__ int n_items() const {
+    return ((d.cuts.stage_mask & 2) && d.ctl->total[K_MD] > 0) ? d.n_events * d.n_edges : 0;
+  }
+  __device__ int count(int i) const {
+    const int ev = i / d.n_edges, k = i - ev * d.n_edges;
+    const int gs = ev * d.n_mod + __ldg(d.conn_src + k);
+    const int n_o = d.mod_md_begin[gs + 1] - d.mod_md_begin[gs];
+    if (n_o == 0) return 0;
+    const int gt = ev * d.n_mod + __ldg(d.conn_tgt + k);
+    const long long p = (long long)n_o * (d.mod_md_begin[gt + 1] - d.mod_md_begin[gt]);
+    if (p > d.cap_pairs) {
+      atomicOr(&d.ctl->error, E_CAP_LS);
+      return 0;
+    }
+    return (int)p;
+  }
+  __device__ int group(int i) const {
+    const int ev = i / d.n_edges;
+    return ev * d.n_mod + __ldg(d.conn_src + (i - ev * d.n_edges));
   }
 };
 
-// ---- a2: Line Segments (CUTS.md section 4).  owner = inner MD A; candidates = the MDs of every
-// module in conn[module(A)] (contiguous index lists of the CSR map).
 struct StageLS {
-  static constexpr int kTicket = T_LS, kKind = K_LS, kErr = E_CAP_LS, kStage = 1;
+  static constexpr int kTicket = T_LS, kKind = K_LS, kErr = E_CAP_LS, kStage = 1, kPairSlot = 1;
+  struct Group {
+    int gbase, gend, n_c;
+    int n_o, A0;
+    int eb, k0, deg;  // eb = event * n_edges + k0: the row's first entry of ppe_ls
+    int gm_base;      // event * n_mod
+  };
+  struct Payload {
+    int A, B;
+    float kappa;
+  };
   const Dev& d;
   __device__ explicit StageLS(const Dev& dd) : d(dd) {}
-  __device__ int n_owners() const { return (d.cuts.stage_mask & 2) ? d.ctl->total[K_MD] : 0; }
-  __device__ int* begin() const { return d.md_ls_begin; }
-  template <bool FILL>
-  __device__ int visit(int A, int pos, unsigned long long& near, unsigned long long& tests) const {
-    const int info = d.md_info[A];
-    const int gm = info >> 1;
-    const bool eA = info & 1;
-    const int ev = gm / d.n_mod;
-    const int m = gm - ev * d.n_mod;
-    const float4 a = d.md_a[A];
-    const float2 ua = d.md_u[A];
-    const int cap = d.cap[K_LS];
-    const int gs_base = 2 * ev * d.n_mod;
-    int cnt = 0;
-    const int k1 = __ldg(d.conn_off + m + 1);
-    for (int k = __ldg(d.conn_off + m); k < k1; ++k) {
-      const int m2 = __ldg(d.conn_tgt + k);
-      const bool eB = __ldg(d.subdet + m2) != 0;
-      const int gs2 = gs_base + 2 * m2;
-      const int b0 = d.hit_md_begin[__ldg(d.sens_begin + gs2 + 1)];
-      const int b1 = d.hit_md_begin[__ldg(d.sens_begin + gs2 + 2)];
-      if (!FILL) tests += (unsigned long long)(b1 - b0);
-      for (int B = b0; B < b1; ++B) {
-        float kappa;
-        const unsigned r = ls_test(d.cuts, a, ua, eA, d.md_a[B], d.md_u[B], eB, kappa);
-        if (!FILL) near += (r >> 1) & 1u;
-        if (r & ACC) {
-          if (FILL && pos < cap) {
-            d.ls_md[pos] = make_int2(A, B);
-            d.ls_kappa[pos] = kappa;
-          }
-          ++pos;
-          ++cnt;
-        }
-      }
-    }
-    return cnt;
+  __device__ bool enabled() const { return (d.cuts.stage_mask & 2) && d.ctl->total[K_MD] > 0; }
+  __device__ int n_groups() const { return enabled() ? d.n_events * d.n_mod : 0; }
+  __device__ const int* chunk_g0() const { return d.cg0_ls; }
+  __device__ int pp(int g) const {
+    const int ev = g / d.n_mod;
+    return d.ppe_ls[ev * d.n_edges + __ldg(d.conn_off + (g - ev * d.n_mod))];
   }
+  __device__ void load_group(int gm, Group& G) const {
+    const int ev = gm / d.n_mod, m = gm - ev * d.n_mod;
+    G.A0 = d.mod_md_begin[gm];
+    G.n_o = d.mod_md_begin[gm + 1] - G.A0;
+    G.n_c = (G.gend - G.gbase) / G.n_o;  // a group reached through a pair has owners
+    G.k0 = __ldg(d.conn_off + m);
+    G.deg = __ldg(d.conn_off + m + 1) - G.k0;
+    G.eb = ev * d.n_edges + G.k0;
+    G.gm_base = ev * d.n_mod;
+  }
+  __device__ unsigned test(const Group& G, int o, int j, Payload& pay) const {
+    const int target = j * G.n_o;  // < pairs of the group
+    int lo = 0, hi = G.deg;        // largest edge e with (ppe[eb + e] - gbase) <= j * n_o
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (d.ppe_ls[G.eb + mid] - G.gbase <= target) lo = mid; else hi = mid;
+    }
+    const int m2 = __ldg(d.conn_tgt + G.k0 + lo);
+    const int before = (d.ppe_ls[G.eb + lo] - G.gbase) / G.n_o;  // candidates of the row before edge lo
+    pay.A = G.A0 + o;
+    pay.B = d.mod_md_begin[G.gm_base + m2] + (j - before);
+    return ls_test(d.cuts, d.md_a[pay.A], d.md_u[pay.A], d.md_info[pay.A] & 1, d.md_a[pay.B], d.md_u[pay.B],
+                   __ldg(d.subdet + m2) != 0, pay.kappa);
+  }
+  __device__ void emit(int pos, const Payload& pay) const {
+    d.ls_md[pos] = make_int2(pay.A, pay.B);
+    d.ls_kappa[pos] = pay.kappa;
+  }
+  // first LS of every MD A: rank of A's first pair x_A = pp(module) + (A - A0) * NB
+  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int ts, int te, const TileRank& rank) const {
+    const int n_md = d.ctl->total[K_MD];
+    if (no_pairs) {
+      if (enabled())
+        for (int A = threadIdx.x; A < n_md; A += kBlock) d.md_ls_begin[A] = 0;
+      return;
+    }
+    const int n = d.n_events * d.n_mod;
+    const int A_lo = tile == 0 ? 0 : d.mod_md_begin[g_lo];
+    const int A_hi = g_hi >= n ? n_md : d.mod_md_begin[g_hi + 1];
+    for (int A = A_lo + threadIdx.x; A < A_hi; A += kBlock) {
+      const int gm = d.md_info[A] >> 1;
+      const int A0 = d.mod_md_begin[gm], n_o = d.mod_md_begin[gm + 1] - A0;
+      const int base = pp(gm);
+      const int x = base + (A - A0) * ((pp(gm + 1) - base) / n_o);
+      if ((x > ts && x <= te) || (tile == 0 && x == 0)) d.md_ls_begin[A] = rank(x);
+    }
+  }
+  __device__ void finish_total(int total) const { d.md_ls_begin[d.ctl->total[K_MD]] = total; }
 };
 
 // ---- a3: T3 (CUTS.md section 5).  owner = LS (A->B); candidates = the LSs whose inner MD is B.

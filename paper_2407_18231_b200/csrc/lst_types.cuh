@@ -13,7 +13,7 @@
 namespace lst {
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
@@ -26,6 +26,7 @@ struct Ctl {
   int pad;
   unsigned long long near[6];
   unsigned long long n_tests[6];
+  unsigned long long pair_total[2];  // candidate pairs of the batch: 0 MD, 1 LS (lst_pairs.cuh)
 };
 
 struct Dev {
@@ -34,6 +35,8 @@ struct Dev {
   const int* subdet;    // [n_mod]
   const int* conn_off;  // [n_mod + 1]
   const int* conn_tgt;
+  const int* conn_src;  // [n_edges] source module of every CSR entry
+  int n_edges;
   // ---- batch ----
   int n_events, n_hits, n_pls;
   const int* hit_ev_off;  // [n_events + 1] device copy of the event offsets
@@ -53,13 +56,17 @@ struct Dev {
   float4* hit;       // [n_hits] sorted (x, y, z, r)
   int* hit_idx;      // [n_hits] event-local input index of the sorted hit
   int* hit_gs;       // [n_hits] global sensor of the sorted hit
-  // ---- a1: MD (owner = upper-sensor hit) ----
-  int* hit_md_begin;  // [n_hits + 1]
+  // ---- a1: MD (grouped by global module) ----
+  int* pp_md;         // [n_events * n_mod + 1] exclusive prefix of the modules' hit pairs
+  int* cg0_md;        // [cap_pairs / kChunk + 2] module holding the first pair of every chunk
+  int* mod_md_begin;  // [n_events * n_mod + 1] first MD of a global module
   int2* md_hit;       // (h_lo, h_hi) event-local input indices
   int* md_info;       // 2 * gm + endcap
   float4* md_a;       // anchor = lower hit (x, y, z, r)
   float2* md_u;       // unit direction (barrel), 0 (endcap)
   // ---- a2: LS (owner = inner MD) ----
+  int* ppe_ls;       // [n_events * n_edges + 1] exclusive prefix of n_MD(source) * n_MD(target) over edges
+  int* cg0_ls;       // [cap_pairs / kChunk + 2]
   int* md_ls_begin;  // [n_md + 1]
   int2* ls_md;       // (md_in, md_out) batch-global MD indices
   float* ls_kappa;
@@ -96,6 +103,7 @@ struct Dev {
   // ---- capacities ----
   int cap[K_NKINDS];
   int cap_idx;
+  int cap_pairs;  // candidate pairs per stage and batch
   Cuts cuts;
 };
 
