@@ -104,7 +104,7 @@ extern "C" void lst_default_caps(lst_caps* c) {
   c->max_pt3 = 1 << 20;
   c->max_pt5 = 1 << 20;
   c->max_tc = 256 << 10;
-  c->max_pairs = 256 << 20;
+  c->max_pairs = 64 << 20;
 }
 
 static Cuts make_cuts(const lst_params& p) {  // CUTS.md section 1, derived constants in binary32
@@ -208,8 +208,8 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.ctl = b.take<Ctl>(1);
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
   const long long n_einst = (long long)c.max_events * n_edges;
-  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs, kTilePairs));
-  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of(c.max_pairs, kTilePairs));
+  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
+  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
   d.tstate[T_PMD] = b.take<unsigned long long>(tiles_of(n_sens / 2 + 1, kScanTile));
   d.tstate[T_PLS] = b.take<unsigned long long>(tiles_of(n_einst + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
@@ -229,11 +229,16 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.hit_idx = b.take<int>(c.max_hits);
   d.hit_gs = b.take<int>(c.max_hits);
   // --- a1..a4 ---
+  d.ev_cg0 = b.take<int>(c.max_pairs / kChunk + 2);
+  d.ev_cnt = b.take<int2>(c.max_pairs / kChunk + 1);
+  d.ev_mask = b.take<unsigned>(c.max_pairs / 32 + 8);
+  {
+    const size_t a = sizeof(StageMD::Payload) * (size_t)c.max_md, l = sizeof(StageLS::Payload) * (size_t)c.max_ls;
+    d.ev_scratch = b.take<char>(a > l ? a : l);
+  }
   d.pp_md = b.take<int>(n_sens / 2 + 1);
-  d.cg0_md = b.take<int>(c.max_pairs / kChunk + 2);
   d.mod_md_begin = b.take<int>(n_sens / 2 + 1);
   d.ppe_ls = b.take<int>(n_einst + 1);
-  d.cg0_ls = b.take<int>(c.max_pairs / kChunk + 2);
   d.md_hit = b.take<int2>(c.max_md);
   d.md_info = b.take<int>(c.max_md);
   d.md_a = b.take<float4>(c.max_md);

@@ -118,13 +118,17 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   L.mark("scatter");
   k_scatter<<<grid_for(g, hits->n, 8), kBlock, 0, st>>>(d);
   L.mark("md_pairs");
-  k_scan_f<PairsMD><<<gp, kBlock, 0, st>>>(d, d.pp_md, d.cg0_md, &d.ctl->pair_total[0], T_PMD);
+  k_scan_f<PairsMD><<<gp, kBlock, 0, st>>>(d, d.pp_md, d.ev_cg0, &d.ctl->pair_total[0], T_PMD);
   L.mark("md");
-  k_even<StageMD><<<gp, kBlock, 0, st>>>(d);
+  k_eval<StageMD><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  L.mark("md_place");
+  k_place<StageMD><<<gp, kBlock, 0, st>>>(d);
   L.mark("ls_pairs");
-  k_scan_f<PairsLS><<<gp, kBlock, 0, st>>>(d, d.ppe_ls, d.cg0_ls, &d.ctl->pair_total[1], T_PLS);
+  k_scan_f<PairsLS><<<gp, kBlock, 0, st>>>(d, d.ppe_ls, d.ev_cg0, &d.ctl->pair_total[1], T_PLS);
   L.mark("ls");
-  k_even<StageLS><<<gp, kBlock, 0, st>>>(d);
+  k_eval<StageLS><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  L.mark("ls_place");
+  k_place<StageLS><<<gp, kBlock, 0, st>>>(d);
   L.mark("t3");
   k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
   L.mark("t5");

@@ -9,16 +9,19 @@
 //
 // Here the candidate pairs of the whole batch form ONE index space: a pre-pass scans the pair
 // counts of the groups (k_scan_f) and records, for every chunk of kChunk = 256 pairs, the group
-// its first pair falls in.  k_even gives every warp exactly one chunk (8 steps of 32 consecutive
-// pairs; lanes walk pair -> group -> (owner, candidate) with a division by the group's row
-// length), so all warps do the same amount of work whatever the occupancy pattern.  Accepted
-// pairs are compacted in pair order with one ballot per step into the warp's shared-memory
-// staging area, which holds a full chunk: every pair is evaluated exactly once and nothing can
-// overflow.  A tile (8 chunks) gets its output slots from the decoupled look-back of
-// lst_scan.cuh, so objects stay in (group, owner, candidate) order -- deterministic and
-// contiguous per owner, module and event -- with no global atomics on the data path.  The
+// its first pair falls in.  k_eval gives every warp whole chunks (8 steps of 32 consecutive pairs;
+// lanes walk pair -> group -> (owner, candidate) with a division by the group's row length), so
+// all warps do the same amount of work whatever the occupancy pattern, and no warp ever waits for
+// another: accepted pairs are compacted in pair order (one ballot per step) into the warp's
+// staging area, then moved to a scratch list with ONE atomic per chunk; the 8 ballot words and the
+// count of the chunk are kept.  k_place then scans the chunk counts (decoupled look-back over
+// tiny uniform tiles) and moves every object to its final slot, so objects end up in (group,
+// owner, candidate) order -- deterministic and contiguous per owner, module and event.  The
 // begin-offsets of groups and owners ("first object of module m / of MD A") are ranks of pair
-// indices, answered from the staged pair numbers by the tile that holds the pair.
+// indices: chunk offset + popcount of the ballot words below the pair.
+// (A first version kept the look-back inside the evaluating kernel; its tiles then retire in
+// ticket order and every block waits for the slowest chunk in flight -- measured 380 us for the MD
+// stage against 127 us with the wait removed, profiles/r01_v2_even_split.md.)
 #pragma once
 #include "lst_ingest.cuh"
 
@@ -85,124 +88,163 @@ __device__ __forceinline__ void split_pair(int p, int n_c, int& o, int& j) {
   if (j >= n_c) { ++o; j -= n_c; }
 }
 
-// Answers "how many accepted pairs of the batch have a pair index < x" for x inside this tile.
-struct TileRank {
-  const int* woff;                         // [kWarps + 1] global slot of each warp's first object
-  const int* run;                          // [kWarps] accepted pairs per warp
-  const unsigned short (*q)[kChunk];       // staged pair numbers relative to the tile start
-  int ts;
-  __device__ int operator()(int x) const {
-    const int rel = x - ts;
-    const int w = rel / kChunk;
-    if (w >= kWarps) return woff[kWarps];
-    int lo = 0, hi = run[w];  // first staged entry with q >= rel
-    while (lo < hi) {
-      const int mid = (lo + hi) >> 1;
-      if ((int)q[w][mid] < rel) lo = mid + 1; else hi = mid;
-    }
-    return woff[w] + lo;
-  }
-};
 
 // Stage concept (StageMD / StageLS in lst_stages.cuh):
 //   static constexpr int kTicket, kKind, kErr, kStage, kPairSlot;
-//   struct Group { int gbase, gend; ... };  struct Payload;
-//   int  n_groups() const;  const int* chunk_g0() const;
+//   struct Group { int gbase, gend, n_c; ... };  struct Payload;
+//   int  n_groups() const;
 //   int  pp(int g) const;                         // exclusive pair prefix of group g, g in [0, n]
 //   void load_group(int g, Group&) const;         // per lane: row length n_c and what test() needs
 //   unsigned test(const Group&, int o, int j, Payload&) const;     // ACC | NEAR bits
 //   void emit(int pos, const Payload&) const;
-//   void boundaries(int tile, bool only_tile, int g_lo, int g_hi, int ts, int te, const TileRank&) const;
+//   template <class R> void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int ts, int te, const R& rank)
 //   void finish_total(int total) const;
+
+// total candidate pairs of the stage (0 if disabled or beyond the bookkeeping capacity)
 template <class S>
-__global__ void __launch_bounds__(kBlock) k_even(Dev d) {
-  __shared__ int s_tile;
-  __shared__ int s_scan[kWarps + 2];
-  __shared__ int s_woff[kWarps + 1];
-  __shared__ int s_run[kWarps];
-  __shared__ unsigned short s_q[kWarps][kChunk];
+__device__ __forceinline__ int stage_pairs(const Dev& d, const S& st, bool& too_many) {
+  const unsigned long long tp64 = st.n_groups() > 0 ? d.ctl->pair_total[S::kPairSlot] : 0ull;
+  too_many = tp64 > (unsigned long long)d.cap_pairs;
+  return too_many ? 0 : (int)tp64;
+}
+
+// Evaluates every candidate pair of the stage once.  Warp per chunk, grid-stride, no block barrier.
+template <class S>
+__global__ void __launch_bounds__(kBlock) k_eval(Dev d) {
   __shared__ typename S::Payload s_stage[kWarps][kChunk];
   S st(d);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int n = st.n_groups();
-  const unsigned long long tp64 = n > 0 ? d.ctl->pair_total[S::kPairSlot] : 0ull;
-  const bool too_many = tp64 > (unsigned long long)d.cap_pairs;
-  const int TP = too_many ? 0 : (int)tp64;
-  const int n_tiles = TP > 0 ? (TP + kTilePairs - 1) / kTilePairs : 1;
+  bool too_many;
+  const int TP = stage_pairs(d, st, too_many);
+  const int n_chunks = (TP + kChunk - 1) / kChunk;
   const int cap = d.cap[S::kKind];
+  typename S::Payload* scratch = reinterpret_cast<typename S::Payload*>(d.ev_scratch);
   unsigned long long near = 0;
+  for (int c = blockIdx.x * kWarps + warp; c < n_chunks; c += gridDim.x * kWarps) {
+    const int cs = c * kChunk;
+    typename S::Group G;
+    int g = d.ev_cg0[c];  // group holding pair cs
+    G.gbase = st.pp(g);
+    G.gend = st.pp(g + 1);
+    st.load_group(g, G);
+    int run = 0;
+    unsigned my_mask = 0;
+#pragma unroll 1
+    for (int s = 0; s < kChunk / 32; ++s) {
+      const int q = cs + 32 * s + lane;
+      unsigned r = 0;
+      typename S::Payload pay;
+      if (q < TP) {
+        if (q >= G.gend) {  // walk to the group holding q (short linear walk, then bisection)
+          int steps = 0;
+          do {
+            ++g;
+            G.gbase = G.gend;
+            G.gend = st.pp(g + 1);
+          } while (q >= G.gend && ++steps < 4);
+          if (q >= G.gend) {
+            int lo = g, hi = n;  // invariant: pp(lo) <= q < pp(hi)
+            while (hi - lo > 1) {
+              const int mid = (lo + hi) >> 1;
+              if (st.pp(mid) <= q) lo = mid; else hi = mid;
+            }
+            g = lo;
+            G.gbase = st.pp(g);
+            G.gend = st.pp(g + 1);
+          }
+          st.load_group(g, G);
+        }
+        int o, j;
+        split_pair(q - G.gbase, G.n_c, o, j);
+        r = st.test(G, o, j, pay);
+      }
+      near += (r >> 1) & 1u;
+      const unsigned m = __ballot_sync(kFull, r & ACC);
+      if (r & ACC) s_stage[warp][run + __popc(m & ((1u << lane) - 1u))] = pay;
+      if (lane == s) my_mask = m;
+      run += __popc(m);
+    }
+    int base = 0;
+    if (lane == 0 && run > 0) base = atomicAdd(&d.ctl->scratch_cur[S::kPairSlot], run);
+    base = __shfl_sync(kFull, base, 0);
+    __syncwarp();
+    if (base + run <= cap)  // beyond the capacity the stage reports E_CAP (k_place), nothing is placed
+      for (int k = lane; k < run; k += 32) scratch[base + k] = s_stage[warp][k];
+    if (lane < kChunk / 32) d.ev_mask[c * (kChunk / 32) + lane] = my_mask;
+    if (lane == 0) d.ev_cnt[c] = make_int2(run, base);
+    __syncwarp();  // the staging area is reused by the warp's next chunk
+  }
+  near = warp_sum_u64(near);
+  if (lane == 0 && near) atomicAdd(&d.ctl->near[S::kStage], near);
+}
+
+// Rank of pair index x among the accepted pairs of the batch, for x inside the placing tile.
+struct PlaceRank {
+  const int* s_off;      // [kBlock + 1] slot offsets of the tile's chunks relative to tile_base
+  const unsigned* mask;  // ballot words of all chunks
+  int c0, tile_base;
+  __device__ int operator()(int x) const {
+    const int ci = (x >> 8) - c0;
+    if (ci >= kBlock) return tile_base + s_off[kBlock];
+    const int r = x & (kChunk - 1);
+    const unsigned* m = mask + (size_t)(x >> 8) * (kChunk / 32);
+    int cnt = 0;
+    for (int w = 0; w < (r >> 5); ++w) cnt += __popc(m[w]);
+    if (r & 31) cnt += __popc(m[r >> 5] & ((1u << (r & 31)) - 1u));
+    return tile_base + s_off[ci] + cnt;
+  }
+};
+
+// Scans the chunk counts and moves every accepted object from the scratch list to its final slot;
+// fills the begin-offset arrays.  Tile = kBlock chunks (thread per chunk).
+template <class S>
+__global__ void __launch_bounds__(kBlock) k_place(Dev d) {
+  static_assert(kChunk == 256, "PlaceRank shifts by 8");
+  __shared__ int s_tile;
+  __shared__ int s_scan[kWarps + 2];
+  __shared__ int s_off[kBlock + 1];
+  __shared__ int s_base[kBlock];
+  S st(d);
+  const int n = st.n_groups();
+  bool too_many;
+  const int TP = stage_pairs(d, st, too_many);
+  const int n_chunks = (TP + kChunk - 1) / kChunk;
+  const int n_tiles = n_chunks > 0 ? (n_chunks + kBlock - 1) / kBlock : 1;
+  const int cap = d.cap[S::kKind];
+  const bool fits = d.ctl->scratch_cur[S::kPairSlot] <= cap;  // final: k_eval has completed
+  const typename S::Payload* scratch = reinterpret_cast<const typename S::Payload*>(d.ev_scratch);
   for (;;) {
     if (threadIdx.x == 0) s_tile = atomicAdd(d.ctl->ticket + S::kTicket, 1);
     __syncthreads();
     const int tile = s_tile;
     if (tile >= n_tiles) break;
-    const int ts = tile * kTilePairs, te = min(TP, ts + kTilePairs);
-    const int cs = ts + warp * kChunk;
-    // ---- this warp's chunk: every pair once, accepted pairs staged in pair order ----
-    int run = 0;
-    if (cs < te) {
-      typename S::Group G;
-      int g = st.chunk_g0()[tile * kWarps + warp];  // group holding pair cs
-      G.gbase = st.pp(g);
-      G.gend = st.pp(g + 1);
-      st.load_group(g, G);
-#pragma unroll 1
-      for (int s = 0; s < kChunk / 32; ++s) {
-        const int q = cs + 32 * s + lane;
-        unsigned r = 0;
-        typename S::Payload pay;
-        if (q < te) {
-          if (q >= G.gend) {  // walk to the group holding q (short linear walk, then bisection)
-            int steps = 0;
-            do {
-              ++g;
-              G.gbase = G.gend;
-              G.gend = st.pp(g + 1);
-            } while (q >= G.gend && ++steps < 4);
-            if (q >= G.gend) {
-              int lo = g, hi = n;  // invariant: pp(lo) <= q < pp(hi)
-              while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (st.pp(mid) <= q) lo = mid; else hi = mid;
-              }
-              g = lo;
-              G.gbase = st.pp(g);
-              G.gend = st.pp(g + 1);
-            }
-            st.load_group(g, G);
-          }
-          int o, j;
-          split_pair(q - G.gbase, G.n_c, o, j);
-          r = st.test(G, o, j, pay);
+    const int c0 = tile * kBlock, c = c0 + threadIdx.x;
+    int2 cb = make_int2(0, 0);
+    if (c < n_chunks) cb = d.ev_cnt[c];
+    int tb, tt;
+    const int off = tile_alloc(cb.x, d.tstate[S::kTicket], tile, s_scan, tb, tt);
+    s_off[threadIdx.x] = off - tb;
+    s_base[threadIdx.x] = cb.y;
+    if (threadIdx.x == 0) s_off[kBlock] = tt;
+    __syncthreads();
+    if (fits) {
+      for (int e = threadIdx.x; e < tt; e += kBlock) {
+        int lo = 0, hi = kBlock;  // chunk of entry e: largest ci with s_off[ci] <= e
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (s_off[mid] <= e) lo = mid; else hi = mid;
         }
-        near += (r >> 1) & 1u;
-        const unsigned m = __ballot_sync(kFull, r & ACC);
-        if (r & ACC) {
-          const int k = run + __popc(m & ((1u << lane) - 1u));
-          s_stage[warp][k] = pay;
-          s_q[warp][k] = (unsigned short)(q - ts);
-        }
-        run += __popc(m);
+        st.emit(tb + e, scratch[s_base[lo] + (e - s_off[lo])]);
       }
     }
-    // ---- output slots of the tile; objects out of the staging area ----
-    int tb, tt;
-    int off = tile_alloc(lane == 0 ? run : 0, d.tstate[S::kTicket], tile, s_scan, tb, tt);
-    off = __shfl_sync(kFull, off, 0);
-    if (lane == 0) {
-      s_woff[warp] = off;
-      s_run[warp] = run;
-    }
-    if (threadIdx.x == 0) s_woff[kWarps] = tb + tt;
-    __syncthreads();
-    for (int k = lane; k < run; k += 32)
-      if (off + k < cap) st.emit(off + k, s_stage[warp][k]);
-    // ---- begin offsets owned by this tile: groups in (g_lo, g_hi], tile 0 also [0, g_lo] ----
     {
       const bool last = tile == n_tiles - 1;
-      const int g_lo = TP > 0 ? st.chunk_g0()[tile * kWarps] : n;
-      const int g_hi = last ? n : st.chunk_g0()[(tile + 1) * kWarps];
-      const TileRank rank{s_woff, s_run, s_q, ts};
+      const int ts = c0 * kChunk;
+      const int te = last ? TP : ts + kBlock * kChunk;
+      const int g_lo = TP > 0 ? d.ev_cg0[c0] : n;
+      const int g_hi = last ? n : d.ev_cg0[c0 + kBlock];
+      const PlaceRank rank{s_off, d.ev_mask, c0, tb};
       st.boundaries(tile, TP == 0, g_lo, g_hi, ts, te, rank);
       if (last && threadIdx.x == 0) {
         const int total = tb + tt;
@@ -216,10 +258,8 @@ __global__ void __launch_bounds__(kBlock) k_even(Dev d) {
         d.ctl->n_tests[S::kStage] = (unsigned long long)TP;
       }
     }
-    __syncthreads();  // staging and s_woff are reused by the next tile
+    __syncthreads();  // s_off / s_base are reused by the next tile
   }
-  near = warp_sum_u64(near);
-  if (lane == 0 && near) atomicAdd(&d.ctl->near[S::kStage], near);
 }
 
 }  // namespace lst

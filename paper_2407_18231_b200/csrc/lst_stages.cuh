@@ -92,7 +92,6 @@ struct StageMD {
   const Dev& d;
   __device__ explicit StageMD(const Dev& dd) : d(dd) {}
   __device__ int n_groups() const { return (d.cuts.stage_mask & 1) ? d.n_events * d.n_mod : 0; }
-  __device__ const int* chunk_g0() const { return d.cg0_md; }
   __device__ int pp(int g) const { return d.pp_md[g]; }
   __device__ void load_group(int gm, Group& G) const {
     G.a0 = __ldg(d.sens_begin + 2 * gm);
@@ -115,7 +114,8 @@ struct StageMD {
     d.md_u[pos] = make_float2(pay.ux, pay.uy);
   }
   // first MD of every module: rank of the module's first pair
-  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int, int, const TileRank& rank) const {
+  template <class R>
+  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int, int, const R& rank) const {
     const int n = d.n_events * d.n_mod;
     if (no_pairs) {
       for (int g = threadIdx.x; g <= n; g += kBlock) d.mod_md_begin[g] = 0;
@@ -173,7 +173,6 @@ struct StageLS {
   __device__ explicit StageLS(const Dev& dd) : d(dd) {}
   __device__ bool enabled() const { return (d.cuts.stage_mask & 2) && d.ctl->total[K_MD] > 0; }
   __device__ int n_groups() const { return enabled() ? d.n_events * d.n_mod : 0; }
-  __device__ const int* chunk_g0() const { return d.cg0_ls; }
   __device__ int pp(int g) const {
     const int ev = g / d.n_mod;
     return d.ppe_ls[ev * d.n_edges + __ldg(d.conn_off + (g - ev * d.n_mod))];
@@ -207,7 +206,8 @@ struct StageLS {
     d.ls_kappa[pos] = pay.kappa;
   }
   // first LS of every MD A: rank of A's first pair x_A = pp(module) + (A - A0) * NB
-  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int ts, int te, const TileRank& rank) const {
+  template <class R>
+  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int ts, int te, const R& rank) const {
     const int n_md = d.ctl->total[K_MD];
     if (no_pairs) {
       if (enabled())

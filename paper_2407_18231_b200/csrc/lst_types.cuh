@@ -27,6 +27,7 @@ struct Ctl {
   unsigned long long near[6];
   unsigned long long n_tests[6];
   unsigned long long pair_total[2];  // candidate pairs of the batch: 0 MD, 1 LS (lst_pairs.cuh)
+  int scratch_cur[2];                // accepted pairs moved to the scratch list so far
 };
 
 struct Dev {
@@ -56,9 +57,13 @@ struct Dev {
   float4* hit;       // [n_hits] sorted (x, y, z, r)
   int* hit_idx;      // [n_hits] event-local input index of the sorted hit
   int* hit_gs;       // [n_hits] global sensor of the sorted hit
+  // ---- even-split bookkeeping, shared by the MD and LS stages (lst_pairs.cuh) ----
+  int* ev_cg0;          // [cap_pairs / kChunk + 2] group holding the first pair of every chunk
+  int2* ev_cnt;         // [cap_pairs / kChunk + 1] (accepted pairs, scratch position) of every chunk
+  unsigned* ev_mask;    // [cap_pairs / 32 + 8] ballot words of every chunk
+  void* ev_scratch;     // accepted payloads in chunk-arrival order
   // ---- a1: MD (grouped by global module) ----
   int* pp_md;         // [n_events * n_mod + 1] exclusive prefix of the modules' hit pairs
-  int* cg0_md;        // [cap_pairs / kChunk + 2] module holding the first pair of every chunk
   int* mod_md_begin;  // [n_events * n_mod + 1] first MD of a global module
   int2* md_hit;       // (h_lo, h_hi) event-local input indices
   int* md_info;       // 2 * gm + endcap
@@ -66,7 +71,6 @@ struct Dev {
   float2* md_u;       // unit direction (barrel), 0 (endcap)
   // ---- a2: LS (owner = inner MD) ----
   int* ppe_ls;       // [n_events * n_edges + 1] exclusive prefix of n_MD(source) * n_MD(target) over edges
-  int* cg0_ls;       // [cap_pairs / kChunk + 2]
   int* md_ls_begin;  // [n_md + 1]
   int2* ls_md;       // (md_in, md_out) batch-global MD indices
   float* ls_kappa;
