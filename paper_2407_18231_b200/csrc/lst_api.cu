@@ -104,7 +104,7 @@ extern "C" void lst_default_caps(lst_caps* c) {
   c->max_pt3 = 1 << 20;
   c->max_pt5 = 1 << 20;
   c->max_tc = 256 << 10;
-  c->max_pairs = 64 << 20;
+  c->max_pairs = 256 << 20;
 }
 
 static Cuts make_cuts(const lst_params& p) {  // CUTS.md section 1, derived constants in binary32
@@ -214,8 +214,10 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.tstate[T_PLS] = b.take<unsigned long long>(tiles_of(n_einst + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
   d.tstate[T_T5] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
-  d.tstate[T_PT3] = b.take<unsigned long long>(tiles_of(c.max_pls, kWarps));
-  d.tstate[T_PT5] = b.take<unsigned long long>(tiles_of(c.max_pls, kWarps));
+  d.tstate[T_PT3] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
+  d.tstate[T_PT5] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
+  d.tstate[T_PP3] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
+  d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_IDX] = b.take<unsigned long long>(tiles_of(3LL * c.max_md + 1, kScanTile));
   d.tstate[T_TC] = b.take<unsigned long long>(tiles_of(4LL * c.max_events + 1, kScanTile));
   d.sens_cnt = b.take<int>(n_sens + 1);
@@ -233,8 +235,11 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.ev_cnt = b.take<int2>(c.max_pairs / kChunk + 1);
   d.ev_mask = b.take<unsigned>(c.max_pairs / 32 + 8);
   {
-    const size_t a = sizeof(StageMD::Payload) * (size_t)c.max_md, l = sizeof(StageLS::Payload) * (size_t)c.max_ls;
-    d.ev_scratch = b.take<char>(a > l ? a : l);
+    size_t sz = sizeof(StageMD::Payload) * (size_t)c.max_md;
+    const size_t others[3] = {sizeof(StageLS::Payload) * (size_t)c.max_ls, sizeof(StagePT<false>::Payload) * (size_t)c.max_pt3,
+                              sizeof(StagePT<true>::Payload) * (size_t)c.max_pt5};
+    for (size_t o : others) sz = o > sz ? o : sz;
+    d.ev_scratch = b.take<char>(sz);
   }
   d.pp_md = b.take<int>(n_sens / 2 + 1);
   d.mod_md_begin = b.take<int>(n_sens / 2 + 1);
@@ -251,13 +256,16 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.t3_md = b.take<int4>(c.max_t3);
   d.t3_k = b.take<float>(c.max_t3);
   d.t3_axy = b.take<float2>(c.max_t3);
+  d.t3_lxy = b.take<float2>(c.max_t3);
   d.t3_t5_begin = b.take<int>((size_t)c.max_t3 + 1);
   d.t5_t3 = b.take<int2>(c.max_t5);
   d.t5_md = b.take<int>(5 * (size_t)c.max_t5);
   d.t5_score = b.take<float>(c.max_t5);
   d.t5_axy = b.take<float2>(c.max_t5);
+  d.t5_lxy = b.take<float2>(c.max_t5);
   // --- a5 ---
   d.pls_event = b.take<int>(c.max_pls);
+  d.pp_pt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt3_begin = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_begin = b.take<int>((size_t)c.max_pls + 1);
   d.pt3 = b.take<int2>(c.max_pt3);
@@ -304,7 +312,8 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
 
 bool caps_ok(const lst_caps& c) {
   return c.max_events > 0 && c.max_hits > 0 && c.max_pls > 0 && c.max_md > 0 && c.max_ls > 0 && c.max_t3 > 0 &&
-         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_pairs > 0;
+         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_pairs > 0 &&
+         c.max_t3 <= (1 << 22) && c.max_t5 <= (1 << 22);  // candidate index bits of StagePT::Pre
 }
 
 }  // namespace

@@ -258,6 +258,7 @@ struct StageT3 {
           d.t3_md[pos] = make_int4(ab.x, ab.y, C, eAB | (eC << 2));
           d.t3_k[pos] = k3;
           d.t3_axy[pos] = make_float2(a.x, a.y);
+          d.t3_lxy[pos] = make_float2(c.x, c.y);
         }
         ++pos;
         ++cnt;
@@ -297,6 +298,7 @@ struct StageT5 {
           md[0] = m1.x; md[1] = m1.y; md[2] = m1.z; md[3] = m2.y; md[4] = m2.z;
           d.t5_score[pos] = score;
           d.t5_axy[pos] = d.t3_axy[t1];
+          d.t5_lxy[pos] = d.t3_lxy[t2];
         }
         ++pos;
         ++cnt;

@@ -13,7 +13,7 @@
 namespace lst {
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_PP3, T_PP5, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
@@ -26,8 +26,8 @@ struct Ctl {
   int pad;
   unsigned long long near[6];
   unsigned long long n_tests[6];
-  unsigned long long pair_total[2];  // candidate pairs of the batch: 0 MD, 1 LS (lst_pairs.cuh)
-  int scratch_cur[2];                // accepted pairs moved to the scratch list so far
+  unsigned long long pair_total[4];  // candidate pairs of the batch: 0 MD, 1 LS, 2 pT3, 3 pT5 (lst_pairs.cuh)
+  int scratch_cur[4];                // accepted pairs moved to the scratch list so far
 };
 
 struct Dev {
@@ -80,13 +80,16 @@ struct Dev {
   int4* t3_md;  // (A, B, C, endcap flags bit0 A, bit1 B, bit2 C)
   float* t3_k;
   float2* t3_axy;  // anchor of the first MD (coalesced operand of the pLS gate)
+  float2* t3_lxy;  // anchor of the last MD (curvature pre-filter of the pLS linking)
   // ---- a4: T5 (owner = first T3) ----
   int* t3_t5_begin;  // [n_t3 + 1]
   int2* t5_t3;
   int* t5_md;  // [n_t5][5]
   float* t5_score;
   float2* t5_axy;
+  float2* t5_lxy;
   // ---- a5: pT3 / pT5 (owner = pLS) ----
+  int* pp_pt;          // [n_pls + 1] exclusive prefix of the seeds' candidate counts (pT3, then reused for pT5)
   int* pls_event;      // [n_pls]
   int* pls_pt3_begin;  // [n_pls + 1]
   int* pls_pt5_begin;  // [n_pls + 1]
