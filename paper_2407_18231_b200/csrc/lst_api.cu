@@ -214,13 +214,17 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.tstate[T_PLS] = b.take<unsigned long long>(tiles_of(n_einst + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
   d.tstate[T_T5] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
-  d.tstate[T_PT3] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
-  d.tstate[T_PT5] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
+  d.tstate[T_PT3] = nullptr;  // ticket only
+  d.tstate[T_PT5] = nullptr;
   d.tstate[T_PP3] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_IDX] = b.take<unsigned long long>(tiles_of(3LL * c.max_md + 1, kScanTile));
   d.tstate[T_TC] = b.take<unsigned long long>(tiles_of(4LL * c.max_events + 1, kScanTile));
   d.sens_cnt = b.take<int>(n_sens + 1);
+  d.pls_pt3_cnt = b.take<int>((size_t)c.max_pls + 1);
+  d.pls_pt5_cnt = b.take<int>((size_t)c.max_pls + 1);
+  d.pls_pt3_cur = b.take<int>(c.max_pls);
+  d.pls_pt5_cur = b.take<int>(c.max_pls);
   b.off = (b.off + 255) & ~size_t(255);
   if (zero_bytes) *zero_bytes = b.off;
   // --- a0 ---
@@ -236,8 +240,8 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.ev_mask = b.take<unsigned>(c.max_pairs / 32 + 8);
   {
     size_t sz = sizeof(StageMD::Payload) * (size_t)c.max_md;
-    const size_t others[3] = {sizeof(StageLS::Payload) * (size_t)c.max_ls, sizeof(StagePT<false>::Payload) * (size_t)c.max_pt3,
-                              sizeof(StagePT<true>::Payload) * (size_t)c.max_pt5};
+    const size_t others[3] = {sizeof(StageLS::Payload) * (size_t)c.max_ls, sizeof(PtAccepted) * (size_t)c.max_pt3,
+                              sizeof(PtAccepted) * (size_t)c.max_pt5};
     for (size_t o : others) sz = o > sz ? o : sz;
     d.ev_scratch = b.take<char>(sz);
   }
@@ -265,7 +269,7 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.t5_lxy = b.take<float2>(c.max_t5);
   // --- a5 ---
   d.pls_event = b.take<int>(c.max_pls);
-  d.pp_pt = b.take<int>((size_t)c.max_pls + 1);
+  d.pt_ev = b.take<PtEvent>((size_t)c.max_events + 1);
   d.pls_pt3_begin = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_begin = b.take<int>((size_t)c.max_pls + 1);
   d.pt3 = b.take<int2>(c.max_pt3);
@@ -312,8 +316,7 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
 
 bool caps_ok(const lst_caps& c) {
   return c.max_events > 0 && c.max_hits > 0 && c.max_pls > 0 && c.max_md > 0 && c.max_ls > 0 && c.max_t3 > 0 &&
-         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_pairs > 0 &&
-         c.max_t3 <= (1 << 22) && c.max_t5 <= (1 << 22);  // candidate index bits of StagePT::Pre
+         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_pairs > 0;
 }
 
 }  // namespace

@@ -133,19 +133,22 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
   L.mark("t5");
   k_stage<StageT5><<<gp, kBlock, 0, st>>>(d);
-  const int ge = g->n_sm * 6;
-  L.mark("pt3_pairs");
-  k_scan_f<PairsPT<false>><<<gp, kBlock, 0, st>>>(d, d.pp_pt, d.ev_cg0, &d.ctl->pair_total[2], T_PP3);
+  L.mark("pt_tiles");
+  k_pt_tiles<<<1, kBlock, 0, st>>>(d);
   L.mark("pt3");
-  k_eval2<StagePT<false>><<<ge, kBlock, 0, st>>>(d);
+  k_pt_eval<false><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  L.mark("pt3_scan");
+  k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
+      d.pls_pt3_cnt, d.pls_pt3_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP3, d.tstate[T_PP3]);
   L.mark("pt3_place");
-  k_place<StagePT<false>><<<gp, kBlock, 0, st>>>(d);
-  L.mark("pt5_pairs");
-  k_scan_f<PairsPT<true>><<<gp, kBlock, 0, st>>>(d, d.pp_pt, d.ev_cg0, &d.ctl->pair_total[3], T_PP5);
+  k_pt_place<false><<<gp, kBlock, 0, st>>>(d);
   L.mark("pt5");
-  k_eval2<StagePT<true>><<<ge, kBlock, 0, st>>>(d);
+  k_pt_eval<true><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  L.mark("pt5_scan");
+  k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
+      d.pls_pt5_cnt, d.pls_pt5_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP5, d.tstate[T_PP5]);
   L.mark("pt5_place");
-  k_place<StagePT<true>><<<gp, kBlock, 0, st>>>(d);
+  k_pt_place<true><<<gp, kBlock, 0, st>>>(d);
   L.mark("event_ranges");
   k_event_ranges<<<1, 64, 0, st>>>(d, ctx->d_ev_first);
   if (mask & 32) {

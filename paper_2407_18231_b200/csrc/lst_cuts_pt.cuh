@@ -84,4 +84,29 @@ __device__ __forceinline__ unsigned pt_after_gate(const Cuts& c, const Seed& s, 
   return res | ACC;
 }
 
+// Necessary condition of the curvature match |kx - kp| <= tolk, kx = kappa3(P1, A, L) (CUTS.md
+// section 7), without sqrt or division: compares kx^2 = 4 crs^2 / (|P1A|^2 |AL|^2 |P1L|^2) with
+// (|kp| -+ tolk)^2.  crs is formed exactly as in kappa3 (same operands, same order), so its
+// cancellation error is common to both; everything else differs by ~1e-6 relative, near-threshold
+// candidates lie within 1e-5, and the bounds carry a 1e-3 margin.  false = the exact cut rejects.
+__device__ __forceinline__ bool pt_curv_possible(const Cuts& c, float pt, int q, float x1, float y1, float2 A,
+                                                 float2 L) {
+  const float kp = (-(float)q) / (pt * c.kr);
+  const float tolk = c.pt_k_tol0 + c.pt_k_tol1 * fabsf(kp);
+  const float ax = A.x - x1, ay = A.y - y1;
+  const float bx = L.x - A.x, by = L.y - A.y;
+  const float cx = L.x - x1, cy = L.y - y1;
+  const float crs = ax * cy - ay * cx;
+  const float prod = ((ax * ax + ay * ay) * (bx * bx + by * by)) * (cx * cx + cy * cy);
+  const float k2 = 4.0f * (crs * crs);
+  const float hi = (fabsf(kp) + tolk) * 1.001f;
+  if (k2 > (hi * hi) * prod) return false;
+  const float lo = (fabsf(kp) - tolk) * 0.999f;
+  if (lo > 0.0f) {
+    if (k2 < (lo * lo) * prod) return false;
+    if ((crs > 0.0f) != (kp > 0.0f)) return false;  // |kx| >= lo > 0 with the wrong sign: |kx - kp| > tolk
+  }
+  return true;
+}
+
 }  // namespace lst

@@ -179,160 +179,6 @@ __global__ void __launch_bounds__(kBlock) k_eval(Dev d) {
   if (lane == 0 && near) atomicAdd(&d.ctl->near[S::kStage], near);
 }
 
-// Two-phase variant for stages whose candidates fail a cheap necessary condition 90% of the time
-// (pLS x T3 / T5: the direction gate).  Groups have ONE owner (pair = candidate j of group g).
-// A warp takes kSuper consecutive chunks at a time.  Phase 1 runs S::prefilter over their pairs and
-// compacts the survivors into shared memory; phase 1b applies a second necessary condition to the
-// survivors (compacted in place); phase 2 runs the exact cut list S::test_pre over what is left, 32
-// at a time, so the expensive cuts see full warps instead of the 2-3 lanes that pass the gate in a
-// 32-candidate step, and their fixed cost is shared by 1024 pairs.  Both filters must keep a
-// SUPERSET of what the exact cuts accept or flag near-threshold.  If the survivors or the accepted
-// pairs of a super-chunk do not fit the staging areas (kChunk entries), its chunks are redone one
-// by one, which always fits.
-constexpr int kSuper = 4;
-
-template <class S>
-struct Eval2 {
-  typename S::Payload* stage;  // [kChunk] per warp
-  typename S::Pre* pre;        // [kChunk] per warp
-  unsigned* mask;              // [kSuper][kChunk / 32] per warp
-
-  // Evaluates chunks [c_first, c_first + n_ch); false = staging overflow, nothing was recorded.
-  __device__ bool run(const Dev& d, const S& st, int c_first, int n_ch, int TP, int n, int cap,
-                      typename S::Payload* scratch, unsigned long long& near_out) {
-    const int lane = threadIdx.x & 31;
-    const int cs = c_first * kChunk;
-    typename S::Group G;
-    int g = d.ev_cg0[c_first];  // group holding pair cs
-    G.gbase = st.pp(g);
-    G.gend = st.pp(g + 1);
-    st.load_group(g, G);
-    if (lane < kSuper * (kChunk / 32)) mask[lane] = 0;
-    unsigned long long near = 0;
-    // ---- phase 1: cheap necessary condition, survivors compacted in pair order ----
-    int n_pre = 0;
-#pragma unroll 1
-    for (int s = 0; s < n_ch * (kChunk / 32); ++s) {
-      const int q = cs + 32 * s + lane;
-      bool keep = false;
-      typename S::Pre pr;
-      if (q < TP) {
-        if (q >= G.gend) {  // next group with candidates
-          int steps = 0;
-          do {
-            ++g;
-            G.gbase = G.gend;
-            G.gend = st.pp(g + 1);
-          } while (q >= G.gend && ++steps < 4);
-          if (q >= G.gend) {
-            int lo = g, hi = n;  // invariant: pp(lo) <= q < pp(hi)
-            while (hi - lo > 1) {
-              const int mid = (lo + hi) >> 1;
-              if (st.pp(mid) <= q) lo = mid; else hi = mid;
-            }
-            g = lo;
-            G.gbase = st.pp(g);
-            G.gend = st.pp(g + 1);
-          }
-          st.load_group(g, G);
-        }
-        keep = st.prefilter(G, g, q - G.gbase, 32 * s + lane, pr);
-      }
-      const unsigned m = __ballot_sync(kFull, keep);
-      if (n_pre + __popc(m) > kChunk) return false;
-      if (keep) pre[n_pre + __popc(m & ((1u << lane) - 1u))] = pr;
-      n_pre += __popc(m);
-    }
-    __syncwarp();
-    // ---- phase 1b: second necessary condition over the survivors, compacted in place ----
-    {
-      int n2 = 0;
-      for (int k0 = 0; k0 < n_pre; k0 += 32) {
-        bool keep = false;
-        typename S::Pre pr;
-        if (k0 + lane < n_pre) {
-          pr = pre[k0 + lane];
-          keep = st.midfilter(pr, near);
-        }
-        const unsigned m = __ballot_sync(kFull, keep);  // every lane has read its entry: slots <= k0 + lane are free
-        if (keep) pre[n2 + __popc(m & ((1u << lane) - 1u))] = pr;
-        n2 += __popc(m);
-      }
-      n_pre = n2;
-      __syncwarp();
-    }
-    // ---- phase 2: the exact cut list over the survivors ----
-    int run = 0;
-    int cnt[kSuper];
-#pragma unroll
-    for (int k = 0; k < kSuper; ++k) cnt[k] = 0;
-    for (int k0 = 0; k0 < n_pre; k0 += 32) {
-      unsigned r = 0;
-      typename S::Payload pay;
-      int qrel = 0;
-      if (k0 + lane < n_pre) {
-        const typename S::Pre pr = pre[k0 + lane];
-        qrel = st.qrel(pr);  // pair number inside the super-chunk
-        r = st.test_pre(pr, pay);
-      }
-      near += (r >> 1) & 1u;
-      const unsigned m = __ballot_sync(kFull, r & ACC);
-      if (run + __popc(m) > kChunk) return false;
-      if (r & ACC) {
-        stage[run + __popc(m & ((1u << lane) - 1u))] = pay;
-        atomicOr(&mask[qrel >> 5], 1u << (qrel & 31));
-      }
-#pragma unroll
-      for (int k = 0; k < kSuper; ++k) cnt[k] += __popc(__ballot_sync(kFull, (r & ACC) && (qrel >> 8) == k));
-      run += __popc(m);
-    }
-    // ---- record: one atomic for the super-chunk, per-chunk count / scratch position / ballot words ----
-    int base = 0;
-    if (lane == 0 && run > 0) base = atomicAdd(&d.ctl->scratch_cur[S::kPairSlot], run);
-    base = __shfl_sync(kFull, base, 0);
-    __syncwarp();
-    if (base + run <= cap)  // beyond the capacity the stage reports E_CAP (k_place), nothing is placed
-      for (int k = lane; k < run; k += 32) scratch[base + k] = stage[k];
-    if (lane < n_ch * (kChunk / 32)) d.ev_mask[(size_t)c_first * (kChunk / 32) + lane] = mask[lane];
-    int b = base;
-#pragma unroll
-    for (int k = 0; k < kSuper; ++k) {
-      if (lane == 0 && k < n_ch) d.ev_cnt[c_first + k] = make_int2(cnt[k], b);
-      b += cnt[k];
-    }
-    near_out += near;
-    __syncwarp();  // staging areas are reused by the warp's next super-chunk
-    return true;
-  }
-};
-
-template <class S>
-__global__ void __launch_bounds__(kBlock) k_eval2(Dev d) {
-  static_assert(kSuper * (kChunk / 32) <= 32 && kSuper * kChunk <= 1024, "mask words per lane / qrel bits");
-  __shared__ typename S::Payload s_stage[kWarps][kChunk];
-  __shared__ typename S::Pre s_pre[kWarps][kChunk];
-  __shared__ unsigned s_mask[kWarps][kSuper * (kChunk / 32)];
-  S st(d);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int n = st.n_groups();
-  bool too_many;
-  const int TP = stage_pairs(d, st, too_many);
-  const int n_chunks = (TP + kChunk - 1) / kChunk;
-  const int cap = d.cap[S::kKind];
-  typename S::Payload* scratch = reinterpret_cast<typename S::Payload*>(d.ev_scratch);
-  Eval2<S> ev{s_stage[warp], s_pre[warp], s_mask[warp]};
-  unsigned long long near = 0;
-  for (int c = (blockIdx.x * kWarps + warp) * kSuper; c < n_chunks; c += gridDim.x * kWarps * kSuper) {
-    const int n_ch = min(kSuper, n_chunks - c);
-    if (!ev.run(d, st, c, n_ch, TP, n, cap, scratch, near)) {
-      __syncwarp();
-      for (int k = 0; k < n_ch; ++k) ev.run(d, st, c + k, 1, TP, n, cap, scratch, near);
-    }
-  }
-  near = warp_sum_u64(near);
-  if (lane == 0 && near) atomicAdd(&d.ctl->near[S::kStage], near);
-}
-
 // Rank of pair index x among the accepted pairs of the batch, for x inside the placing tile.
 struct PlaceRank {
   const int* s_off;      // [kBlock + 1] slot offsets of the tile's chunks relative to tile_base

@@ -12,6 +12,8 @@
 
 namespace lst {
 
+struct PtEvent;  // lst_pt.cuh
+
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
 enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_PP3, T_PP5, T_N };
 
@@ -26,8 +28,8 @@ struct Ctl {
   int pad;
   unsigned long long near[6];
   unsigned long long n_tests[6];
-  unsigned long long pair_total[4];  // candidate pairs of the batch: 0 MD, 1 LS, 2 pT3, 3 pT5 (lst_pairs.cuh)
-  int scratch_cur[4];                // accepted pairs moved to the scratch list so far
+  unsigned long long pair_total[2];  // candidate pairs of the batch: 0 MD, 1 LS (lst_pairs.cuh)
+  int scratch_cur[4];                // accepted objects in the scratch list: 0 MD, 1 LS, 2 pT3, 3 pT5
 };
 
 struct Dev {
@@ -89,7 +91,9 @@ struct Dev {
   float2* t5_axy;
   float2* t5_lxy;
   // ---- a5: pT3 / pT5 (owner = pLS) ----
-  int* pp_pt;          // [n_pls + 1] exclusive prefix of the seeds' candidate counts (pT3, then reused for pT5)
+  PtEvent* pt_ev;      // [n_events + 1] candidate / seed ranges and first tile of every event
+  int *pls_pt3_cnt, *pls_pt5_cnt;  // [n_pls + 1] accepted per seed (zeroed per batch)
+  int *pls_pt3_cur, *pls_pt5_cur;  // [n_pls] next free slot of a seed's range (zeroed per batch)
   int* pls_event;      // [n_pls]
   int* pls_pt3_begin;  // [n_pls + 1]
   int* pls_pt5_begin;  // [n_pls + 1]
