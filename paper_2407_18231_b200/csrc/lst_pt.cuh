@@ -121,7 +121,8 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
   __shared__ float4 s_seed[kSeedTile];  // x1, y1, vx, vy
   __shared__ float s_lv[kSeedTile];
   __shared__ unsigned short s_q[kQueue][kBlock];  // [entry][thread]: conflict-free per-thread queues
-  const int lane = threadIdx.x & 31;
+  __shared__ unsigned s_w2[kWarps][64];           // phase-2 list of the warp: source lane << 16 | seed slot
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int E = d.n_events;
   const int n_tiles = d.pt_ev[E].tile0[K];
   const int cap = d.cap[kKind];
@@ -167,6 +168,24 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
       A = axy[t];
       L = lxy[t];
     }
+    // ---- phase 2: the exact cut list for one entry of the warp's list; returns its near flag ----
+    const int t_warp = ev.c0[K] + cb * kBlock + warp * 32;
+    auto phase2 = [&](unsigned ent) -> unsigned {
+      const int ks = ent & 0xffff, tt = t_warp + (int)(ent >> 16);
+      const int p = p0 + ks;
+      const float4 sd = s_seed[ks];
+      const Seed full = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p), __ldg(d.p_y0 + p),
+                                  __ldg(d.p_z0 + p), sd.x, sd.y, __ldg(d.p_z1 + p));
+      float score;
+      const unsigned r2 = PtCand<IS5>::test(d, full, tt, score);
+      if (r2 & ACC) {
+        const int slot = atomicAdd(&d.ctl->scratch_cur[IS5 ? 3 : 2], 1);
+        if (slot < cap) scratch[slot] = PtAccepted{p, tt, score};
+        atomicAdd(cnt_p + p, 1);
+      }
+      return (r2 >> 1) & 1u;
+    };
+    int n2 = 0;
     for (int k0 = 0; k0 < n_seed; k0 += kSeedSub) {
       // ---- phase 1: necessary condition of the gate, survivors into the thread's own queue ----
       int nq = 0;
@@ -194,37 +213,41 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
         }
         // a full queue anywhere in the warp: drain now, then go on with the rest of the sub-block
         const bool more = __any_sync(kFull, k < k1);
-        // ---- phase 1b + 2 over the queue, lanes in lockstep ----
+        // ---- phase 1b over the queues, lanes in lockstep; survivors into the warp's phase-2 list ----
         const int nq_max = __reduce_max_sync(kFull, nq);
         for (int i = 0; i < nq_max; ++i) {
+          bool go = false;
+          int ks = 0;
           if (i < nq) {
-            const int ks = s_q[i][threadIdx.x];
-            const int p = p0 + ks;
+            ks = s_q[i][threadIdx.x];
             const float4 sd = s_seed[ks];
             Seed s;
             s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[ks];
             const unsigned r = pt_gate(d.cuts, s, A.x, A.y);  // exact gate (CUTS.md section 7)
-            bool go = (r & ACC) != 0;
+            go = (r & ACC) != 0;
             if (!go) near += (r >> 1) & 1u;
-            if (go && !(r & NEAR)) go = pt_curv_possible(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), sd.x, sd.y, A, L);
-            if (go) {  // ---- phase 2: the exact cut list ----
-              const Seed full = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p),
-                                          __ldg(d.p_y0 + p), __ldg(d.p_z0 + p), sd.x, sd.y, __ldg(d.p_z1 + p));
-              float score;
-              const unsigned r2 = PtCand<IS5>::test(d, full, t, score);
-              near += (r2 >> 1) & 1u;
-              if (r2 & ACC) {
-                const int slot = atomicAdd(&d.ctl->scratch_cur[IS5 ? 3 : 2], 1);
-                if (slot < cap) scratch[slot] = PtAccepted{p, t, score};
-                atomicAdd(cnt_p + p, 1);
-              }
-            }
+            if (go && !(r & NEAR))
+              go = pt_curv_possible(d.cuts, __ldg(d.p_pt + p0 + ks), __ldg(d.p_q + p0 + ks), sd.x, sd.y, A, L);
+          }
+          const unsigned m = __ballot_sync(kFull, go);
+          if (go) s_w2[warp][n2 + __popc(m & ((1u << lane) - 1u))] = ((unsigned)lane << 16) | (unsigned)ks;
+          n2 += __popc(m);
+          if (n2 >= 32) {  // a full warp of phase-2 work
+            __syncwarp();
+            near += phase2(s_w2[warp][lane]);
+            const unsigned rest = (32 + lane < n2) ? s_w2[warp][32 + lane] : 0u;
+            __syncwarp();
+            s_w2[warp][lane] = rest;
+            n2 -= 32;
+            __syncwarp();
           }
         }
         nq = 0;
         if (!more) break;
       }
     }
+    __syncwarp();
+    if (lane < n2) near += phase2(s_w2[warp][lane]);
     __syncthreads();  // the seed tile is reused
   }
   near = warp_sum_u64(near);
