@@ -208,8 +208,8 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.ctl = b.take<Ctl>(1);
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
   const long long n_einst = (long long)c.max_events * n_edges;
-  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
-  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kBlock));
+  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kPlaceChunks));
+  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kPlaceChunks));
   d.tstate[T_PMD] = b.take<unsigned long long>(tiles_of(n_sens / 2 + 1, kScanTile));
   d.tstate[T_PLS] = b.take<unsigned long long>(tiles_of(n_einst + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));

@@ -16,7 +16,8 @@
 // staging area, then moved to a scratch list with ONE atomic per chunk; the 8 ballot words and the
 // count of the chunk are kept.  k_place then scans the chunk counts (decoupled look-back over
 // tiny uniform tiles) and moves every object to its final slot, so objects end up in (group,
-// owner, candidate) order -- deterministic and contiguous per owner, module and event.  The
+// owner, candidate) order -- contiguous per owner, module and event (the order is a function of
+// the sorted-hit order; hits of one sensor are sorted in arrival order, lst_ingest.cuh).  The
 // begin-offsets of groups and owners ("first object of module m / of MD A") are ranks of pair
 // indices: chunk offset + popcount of the ballot words below the pair.
 // (A first version kept the look-back inside the evaluating kernel; its tiles then retire in
@@ -180,13 +181,15 @@ __global__ void __launch_bounds__(kBlock) k_eval(Dev d) {
 }
 
 // Rank of pair index x among the accepted pairs of the batch, for x inside the placing tile.
+constexpr int kPlaceChunks = 64;  // chunks per placing tile: small tiles, many blocks (the work is latency-bound)
+
 struct PlaceRank {
-  const int* s_off;      // [kBlock + 1] slot offsets of the tile's chunks relative to tile_base
+  const int* s_off;      // [kPlaceChunks + 1] slot offsets of the tile's chunks relative to tile_base
   const unsigned* mask;  // ballot words of all chunks
   int c0, tile_base;
   __device__ int operator()(int x) const {
     const int ci = (x >> 8) - c0;
-    if (ci >= kBlock) return tile_base + s_off[kBlock];
+    if (ci >= kPlaceChunks) return tile_base + s_off[kPlaceChunks];
     const int r = x & (kChunk - 1);
     const unsigned* m = mask + (size_t)(x >> 8) * (kChunk / 32);
     int cnt = 0;
@@ -197,20 +200,20 @@ struct PlaceRank {
 };
 
 // Scans the chunk counts and moves every accepted object from the scratch list to its final slot;
-// fills the begin-offset arrays.  Tile = kBlock chunks (thread per chunk).
+// fills the begin-offset arrays.  Tile = kPlaceChunks chunks.
 template <class S>
 __global__ void __launch_bounds__(kBlock) k_place(Dev d) {
   static_assert(kChunk == 256, "PlaceRank shifts by 8");
   __shared__ int s_tile;
   __shared__ int s_scan[kWarps + 2];
-  __shared__ int s_off[kBlock + 1];
-  __shared__ int s_base[kBlock];
+  __shared__ int s_off[kPlaceChunks + 1];
+  __shared__ int s_base[kPlaceChunks];
   S st(d);
   const int n = st.n_groups();
   bool too_many;
   const int TP = stage_pairs(d, st, too_many);
   const int n_chunks = (TP + kChunk - 1) / kChunk;
-  const int n_tiles = n_chunks > 0 ? (n_chunks + kBlock - 1) / kBlock : 1;
+  const int n_tiles = n_chunks > 0 ? (n_chunks + kPlaceChunks - 1) / kPlaceChunks : 1;
   const int cap = d.cap[S::kKind];
   const bool fits = d.ctl->scratch_cur[S::kPairSlot] <= cap;  // final: k_eval has completed
   const typename S::Payload* scratch = reinterpret_cast<const typename S::Payload*>(d.ev_scratch);
@@ -219,18 +222,20 @@ __global__ void __launch_bounds__(kBlock) k_place(Dev d) {
     __syncthreads();
     const int tile = s_tile;
     if (tile >= n_tiles) break;
-    const int c0 = tile * kBlock, c = c0 + threadIdx.x;
+    const int c0 = tile * kPlaceChunks, c = c0 + threadIdx.x;
     int2 cb = make_int2(0, 0);
-    if (c < n_chunks) cb = d.ev_cnt[c];
+    if (threadIdx.x < kPlaceChunks && c < n_chunks) cb = d.ev_cnt[c];
     int tb, tt;
     const int off = tile_alloc(cb.x, d.tstate[S::kTicket], tile, s_scan, tb, tt);
-    s_off[threadIdx.x] = off - tb;
-    s_base[threadIdx.x] = cb.y;
-    if (threadIdx.x == 0) s_off[kBlock] = tt;
+    if (threadIdx.x < kPlaceChunks) {
+      s_off[threadIdx.x] = off - tb;
+      s_base[threadIdx.x] = cb.y;
+    }
+    if (threadIdx.x == 0) s_off[kPlaceChunks] = tt;
     __syncthreads();
     if (fits) {
       for (int e = threadIdx.x; e < tt; e += kBlock) {
-        int lo = 0, hi = kBlock;  // chunk of entry e: largest ci with s_off[ci] <= e
+        int lo = 0, hi = kPlaceChunks;  // chunk of entry e: largest ci with s_off[ci] <= e
         while (hi - lo > 1) {
           const int mid = (lo + hi) >> 1;
           if (s_off[mid] <= e) lo = mid; else hi = mid;
@@ -241,9 +246,9 @@ __global__ void __launch_bounds__(kBlock) k_place(Dev d) {
     {
       const bool last = tile == n_tiles - 1;
       const int ts = c0 * kChunk;
-      const int te = last ? TP : ts + kBlock * kChunk;
+      const int te = last ? TP : ts + kPlaceChunks * kChunk;
       const int g_lo = TP > 0 ? d.ev_cg0[c0] : n;
-      const int g_hi = last ? n : d.ev_cg0[c0 + kBlock];
+      const int g_hi = last ? n : d.ev_cg0[c0 + kPlaceChunks];
       const PlaceRank rank{s_off, d.ev_mask, c0, tb};
       st.boundaries(tile, TP == 0, g_lo, g_hi, ts, te, rank);
       if (last && threadIdx.x == 0) {

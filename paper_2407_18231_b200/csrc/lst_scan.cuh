@@ -4,8 +4,8 @@
 // are assigned by an exclusive prefix sum over the owners, computed INSIDE the producing kernel:
 // tiles of owners take a ticket (so lower tiles always started earlier), scan their counts in
 // shared memory, publish the tile aggregate in a 64-bit status word and look back over the
-// predecessors' words for their prefix.  Result: objects are stored in owner order (deterministic,
-// contiguous per owner, per module and per event) with one kernel launch per stage and no atomics
+// predecessors' words for their prefix.  Result: objects are stored in owner order (contiguous per owner,
+// per module and per event) with one kernel launch per stage and no atomics
 // on the data path.
 #pragma once
 #include <cuda_runtime.h>

@@ -1,0 +1,159 @@
+"""GPU parity, part 2: the even-split pair engine and the tiled seed linking at their edges, and the
+full benchmark configuration (16 PU200 events in one launch sequence, default capacities)."""
+import numpy as np
+import pytest
+
+from lst_inputs import c5_batch, make_config_event, make_config_geometry
+
+from .util import assert_same, canon, run_batch
+
+pytestmark = pytest.mark.gpu
+
+R_LAYER = (23.0, 36.0, 51.0, 68.0, 88.0)
+
+
+@pytest.fixture(scope="module")
+def lst():
+    import torch
+
+    assert torch.cuda.is_available()
+    from paper_2407_18231_b200 import build
+
+    build.build()
+    import paper_2407_18231_b200 as m
+
+    return m
+
+
+def dense_chain_event(n_trk=150, dphi=0.0005, seed=5):
+    """Five barrel modules in a chain, n_trk near-parallel straight tracks through all of them: every
+    module holds n_trk^2 hit pairs (88 chunks of 256 at the default), thousands of MDs share a module,
+    and every MD has hundreds of LS candidates -- the opposite corner from the sparse PU200 modules."""
+    rng = np.random.default_rng(seed)
+    phi = np.arange(n_trk) * dphi + 0.3
+    z0, cot = rng.normal(0, 2, n_trk), rng.normal(0, 0.2, n_trk)
+    xs, ys, zs, ss = [], [], [], []
+    for m, r in enumerate(R_LAYER):
+        for s, rr in enumerate((r, r + 0.26)):
+            ph = phi + rng.normal(0, 0.003, n_trk) / rr
+            xs.append(rr * np.cos(ph))
+            ys.append(rr * np.sin(ph))
+            zs.append(z0 + cot * rr + rng.normal(0, 0.15, n_trk))
+            ss.append(np.full(n_trk, 2 * m + s))
+    perm = rng.permutation(n_trk * 10)
+    f = lambda a, t: np.concatenate(a).astype(t)[perm]
+    table = np.array([[0, m + 1, 0, 0] for m in range(5)], np.int32)
+    return table, np.array([0, 1, 2, 3, 4, 4], np.int32), np.array([1, 2, 3, 4], np.int32), \
+        f(xs, np.float32), f(ys, np.float32), f(zs, np.float32), f(ss, np.int32)
+
+
+def test_dense_modules_span_many_chunks(lst, oracle_mod):
+    table, off, tgt, x, y, z, s = dense_chain_event()
+    g = lst.lst_load_geometry(table, off, tgt)
+    try:
+        got = lst.lst_run_event(g, x, y, z, s)
+    finally:
+        lst.lst_free(g)
+    want = oracle_mod.run_event(table[:, 0].copy(), off, tgt, x, y, z, s, {})
+    assert want["n_tests"][0] == 5 * 150 * 150 and len(want["ls_md"]) > 10_000 and len(want["t5_md"]) > 5_000
+    assert_same(canon(got), canon(want), "dense chain: ")
+    # storage order (what the begin-offset arrays rely on): MDs grouped by module, LSs by inner MD,
+    # T3s by first LS, T5s by first T3
+    for key, col in (("md_module", None), ("ls_md", 0), ("t3_ls", 0), ("t5_t3", 0)):
+        v = got[key] if col is None else got[key][:, col]
+        assert np.all(np.diff(v) >= 0), key
+
+
+def test_pair_capacity_overflow_is_an_error(lst):
+    geom, off, tgt = make_config_geometry("C2")
+    ev = make_config_event("C2")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=1, max_pairs=1000))
+    try:
+        h, keep = lst.make_hits(ev.x, ev.y, ev.z, ev.sensor)
+        lst.lst_ctx_run(ctx, 1, h, None)
+        with pytest.raises(lst.LstError) as ei:
+            lst.lst_ctx_sync(ctx)
+        assert ei.value.status == lst.LST_ERR_CAPACITY
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
+@pytest.mark.parametrize("cap", ["max_ls", "max_t3", "max_t5", "max_pt3", "max_pt5", "max_tc"])
+def test_every_object_capacity_overflow_is_an_error(lst, cap):
+    geom, off, tgt = make_config_geometry("C4")
+    ev = make_config_event("C4")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=1, **{cap: 20}))
+    try:
+        h, keep = lst.make_hits(ev.x, ev.y, ev.z, ev.sensor)
+        s, keep = lst.make_pls(ev.pls, keep=keep)
+        lst.lst_ctx_run(ctx, 1, h, s)
+        with pytest.raises(lst.LstError) as ei:
+            lst.lst_ctx_sync(ctx)
+        assert ei.value.status == lst.LST_ERR_CAPACITY
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
+def test_hits_on_one_sensor_only(lst, oracle_mod):
+    """No module has a hit pair: zero candidate pairs in every stage, every seed comes out unlinked."""
+    geom, off, tgt = make_config_geometry("C4")
+    ev = make_config_event("C4")
+    low = (ev.sensor % 2) == 0
+    x, y, z, s = ev.x[low], ev.y[low], ev.z[low], ev.sensor[low]
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    try:
+        got = lst.lst_run_event(g, x, y, z, s, ev.pls)
+    finally:
+        lst.lst_free(g)
+    want = oracle_mod.run_event(geom.subdet, off, tgt, x, y, z, s, ev.pls)
+    assert len(want["md_hits"]) == 0 and len(want["tc"]) == ev.n_pls
+    assert_same(canon(got), canon(want), "lower sensors only: ")
+
+
+def test_benchmark_configuration(lst, oracle_mod):
+    """BASELINE.json config 5 as bench.py times it: 16 PU200 events (seeds on) in one launch sequence
+    on a non-default stream, default capacities, device-resident inputs, two batches back to back on
+    the same context.  Every event of the last batch is compared with the oracle, object by object."""
+    import torch
+
+    geom, off, tgt = make_config_geometry("C5")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    stream = torch.cuda.Stream()
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=16), stream.cuda_stream)
+    try:
+        from lst_inputs.events import concat_events
+
+        batches = [c5_batch(pu=200, n_events=16, first=0), c5_batch(pu=200, n_events=16, first=16)]
+        keepalive = []
+        for evs in batches:
+            b = concat_events(evs)
+            dev = {k: torch.from_numpy(b[k]).cuda() for k in ("x", "y", "z", "sensor")}
+            pls = {k: torch.from_numpy(v).cuda() for k, v in b["pls"].items()}
+            h, keep = lst.make_hits(dev["x"], dev["y"], dev["z"], dev["sensor"], b["hit_offsets"])
+            s, keep = lst.make_pls(pls, b["pls_offsets"], keep)
+            keepalive.append((dev, pls, keep))
+            torch.cuda.synchronize()
+            lst.lst_ctx_run(ctx, 16, h, s)
+        summ = lst.lst_ctx_sync(ctx)
+        assert summ["n_events"] == 16 and summ["n_hits"] > 16 * 100_000
+        tot = np.zeros(7, np.int64)
+        tests = np.zeros(6, np.int64)
+        near = np.zeros(6, np.int64)
+        for i, ev in enumerate(batches[1]):
+            want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+            got = lst.lst_ctx_fetch_event(ctx, i)
+            got["near"], got["n_tests"] = want["near"], want["n_tests"]  # counters are per batch (checked below)
+            assert_same(canon(got), canon(want), f"bench config, event {i}: ")
+            tot += [len(want[k]) for k in ("md_hits", "ls_md", "t3_md", "t5_md", "pt3", "pt5", "tc")]
+            tests += want["n_tests"]
+            near += want["near"]
+        assert [summ["n_" + k] for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")] == tot.tolist()
+        assert summ["n_tests"] == tests.tolist() and summ["near"] == near.tolist()
+        assert np.all(near <= 1e-4 * tests), "near-threshold candidates above 0.01% (north_star)"
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
