@@ -64,14 +64,16 @@ def dist_env():
 # ---------------------------------------------------------------------------------------------
 # inputs
 # ---------------------------------------------------------------------------------------------
-def make_batches(pu, n_events, n_batches, first_index):
-    """n_batches distinct batches of n_events C5 events (lst_inputs recipe)."""
-    from lst_inputs import c5_batch
+def make_batches(pu, n_events, n_batches, rank=0, world=1):
+    """n_batches distinct batches of n_events C5 events (lst_inputs recipe); every rank
+    takes its own event numbers (paper_2407_18231_b200.replicas: replicas only, no collective)."""
+    from lst_inputs import make_config_event
     from lst_inputs.events import concat_events
+    from paper_2407_18231_b200.replicas import event_indices
 
     out = []
-    for b in range(n_batches):
-        evs = c5_batch(pu=pu, n_events=n_events, seeds=True, first=first_index + b * n_events)
+    for idx in event_indices(rank, world, n_batches, n_events):
+        evs = [make_config_event("C5", pu=pu, index=i, seeds=True) for i in idx]
         out.append((evs, concat_events(evs)))
     return out
 
@@ -142,12 +144,21 @@ def algorithmic_work(name, s, n_sens):
         "hist": 12 * h + 4 * p,
         "scan_sensors": 8 * n_sens,
         "scatter": 44 * h,
-        "md": 28 * h + 8 * n_sens + 36 * md,
-        "ls": 32 * md + 12 * ls,
+        "md_pairs": 8 * n_sens,
+        "md": 16 * h + 4 * n_sens + 16 * md,
+        "md_place": 16 * md + 28 * md + 36 * md + 2 * n_sens,
+        "ls_pairs": 4 * n_sens,
+        "ls": 28 * md + 12 * ls,
+        "ls_place": 24 * ls + 4 * md,
         "t3": 12 * ls + 16 * md + 36 * t3,
         "t5": 24 * t3 + 16 * md + 40 * t5,
-        "pt3": 36 * p + 8 * t3 + 12 * p3,
-        "pt5": 36 * p + 8 * t5 + 12 * p5,
+        "pt_tiles": 0,
+        "pt3": 36 * p + 16 * t3 + 12 * p3,
+        "pt3_scan": 8 * p,
+        "pt3_place": 24 * p3,
+        "pt5": 36 * p + 16 * t5 + 12 * p5,
+        "pt5_scan": 8 * p,
+        "pt5_place": 24 * p5,
         "event_ranges": 0,
         "sel_prepare": 24 * md + p,
         "index_count": 20 * t5 + 28 * p5 + 24 * p3 + 4 * idx,
@@ -203,7 +214,7 @@ def run_b200(args):
     geom, off, tgt = make_config_geometry("C5")
     n_sens = E * 2 * geom.n_modules
     t0 = time.time()
-    batches = make_batches(args.pu, E, NB, first_index=rank * NB * E)
+    batches = make_batches(args.pu, E, NB, rank, world)
     gen_s = time.time() - t0
 
     g = lst.lst_load_geometry(geom.module_table(), off, tgt)
@@ -283,10 +294,10 @@ def run_b200(args):
         ms_e2e, _, _, d2h = pipelined(host_in, args.steps, tc_pin)
         sampler.active.clear()
         barrier()
-        if world > 1:
-            t = torch.tensor([ms, ms_e2e], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms, ms_e2e = float(t[0]), float(t[1])
+        from paper_2407_18231_b200.replicas import max_over_ranks, sum_over_ranks
+
+        ms, ms_e2e = max_over_ranks([ms, ms_e2e], device="cuda")  # the slowest rank sets the job's time
+        launches = int(sum_over_ranks([launches], device="cuda")[0])
 
     # ---- per-kernel times: one stream, L2 flushed before every batch -----------------------------
     hbm_gbs, sm_max_mhz, peak_src = peaks()
@@ -445,7 +456,7 @@ def run_reference(args):
     # keep the whole run within a few minutes: ~1.5 s of one core per PU200 event
     steps = max(1, min(args.steps, 20))
     warm = max(0, min(args.warmup, 1))
-    batches = make_batches(args.pu, per_step, 2, first_index=0)
+    batches = make_batches(args.pu, per_step, 2)
     for _ in range(warm):
         oracle_rate(batches[0][0], geom, off, tgt, single=False)
     t0 = time.perf_counter()
