@@ -15,7 +15,7 @@ __device__ __forceinline__ int ev_of_md(const Dev& d, int md) { return (d.md_inf
 __global__ void k_event_ranges(Dev d, int* ev_first) {
   const int E1 = d.n_events + 1;
   for (int ev = threadIdx.x; ev < E1; ev += blockDim.x) {
-    const int h = d.hit_ev_off[ev], p = d.pls_ev_off[ev];
+    const int p = d.pls_ev_off[ev];
     const int md = d.ctl->total[K_MD] > 0 ? d.mod_md_begin[min(ev, d.n_events) * d.n_mod] : 0;
     const int ls = d.ctl->total[K_LS] > 0 ? d.md_ls_begin[md] : 0;
     const int t3 = d.ctl->total[K_T3] > 0 ? d.ls_t3_begin[ls] : 0;
