@@ -209,7 +209,7 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
   const long long n_einst = (long long)c.max_events * n_edges;
   d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kPlaceChunks));
-  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kPlaceChunks));
+  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kScanTile));
   d.tstate[T_PMD] = b.take<unsigned long long>(tiles_of(n_sens / 2 + 1, kScanTile));
   d.tstate[T_PLS] = b.take<unsigned long long>(tiles_of(n_einst + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
@@ -240,7 +240,7 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.ev_mask = b.take<unsigned>(c.max_pairs / 32 + 8);
   {
     size_t sz = sizeof(StageMD::Payload) * (size_t)c.max_md;
-    const size_t others[3] = {sizeof(StageLS::Payload) * (size_t)c.max_ls, sizeof(PtAccepted) * (size_t)c.max_pt3,
+    const size_t others[3] = {sizeof(LsAccepted) * (size_t)c.max_ls, sizeof(PtAccepted) * (size_t)c.max_pt3,
                               sizeof(PtAccepted) * (size_t)c.max_pt5};
     for (size_t o : others) sz = o > sz ? o : sz;
     d.ev_scratch = b.take<char>(sz);
@@ -253,6 +253,8 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.md_a = b.take<float4>(c.max_md);
   d.md_u = b.take<float2>(c.max_md);
   d.md_ls_begin = b.take<int>((size_t)c.max_md + 1);
+  d.ls_cnt = b.take<int>(c.max_md);
+  d.ls_sbase = b.take<int>(c.max_md);
   d.ls_md = b.take<int2>(c.max_ls);
   d.ls_kappa = b.take<float>(c.max_ls);
   d.ls_t3_begin = b.take<int>((size_t)c.max_ls + 1);

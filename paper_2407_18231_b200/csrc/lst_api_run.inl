@@ -123,12 +123,12 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   k_eval<StageMD><<<g->n_sm * 6, kBlock, 0, st>>>(d);
   L.mark("md_place");
   k_place<StageMD><<<gp, kBlock, 0, st>>>(d);
-  L.mark("ls_pairs");
-  k_scan_f<PairsLS><<<gp, kBlock, 0, st>>>(d, d.ppe_ls, d.ev_cg0, &d.ctl->pair_total[1], T_PLS);
   L.mark("ls");
-  k_eval<StageLS><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  k_ls_eval<<<g->n_sm * 8, kBlock, 0, st>>>(d);
+  L.mark("ls_scan");
+  k_scan<<<gp, kBlock, 0, st>>>(d.ls_cnt, d.md_ls_begin, d.ctl->total + K_MD, 1, 0, d.ctl->ticket + T_LS, d.tstate[T_LS]);
   L.mark("ls_place");
-  k_place<StageLS><<<gp, kBlock, 0, st>>>(d);
+  k_ls_place<<<gp, kBlock, 0, st>>>(d);
   L.mark("t3");
   k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
   L.mark("t5");

@@ -5,6 +5,7 @@
 // object sharing >= 3 of X's 5 MDs contains X.md[0], [2] or [4]; one sharing >= 2 of 5 contains one
 // of X.md[0..3]; one sharing >= 2 of X's 3 MDs contains X.md[0] or [1].
 #pragma once
+#include "lst_ls.cuh"
 #include "lst_pt.cuh"
 
 namespace lst {

@@ -74,6 +74,7 @@ struct Dev {
   // ---- a2: LS (owner = inner MD) ----
   int* ppe_ls;       // [n_events * n_edges + 1] exclusive prefix of n_MD(source) * n_MD(target) over edges
   int* md_ls_begin;  // [n_md + 1]
+  int *ls_cnt, *ls_sbase;  // [n_md] LSs of an inner MD and their position in the scratch list
   int2* ls_md;       // (md_in, md_out) batch-global MD indices
   float* ls_kappa;
   // ---- a3: T3 (owner = first LS) ----
