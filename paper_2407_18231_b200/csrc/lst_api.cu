@@ -141,6 +141,7 @@ extern "C" int lst_load_geometry(const lst_module* modules, int32_t n_modules, c
   for (int m = 0; m < n_modules; ++m)
     if (conn_offsets[m + 1] - conn_offsets[m] > max_deg) max_deg = conn_offsets[m + 1] - conn_offsets[m];
   if (n_edges > 0 && !conn_targets) return LST_ERR_ARG;
+  if (max_deg > kLsRanges) return LST_ERR_GEOMETRY;  // longest connection-map row the LS stage's tables hold
   for (int k = 0; k < n_edges; ++k)
     if (conn_targets[k] < 0 || conn_targets[k] >= n_modules) return LST_ERR_GEOMETRY;
 

@@ -6,11 +6,13 @@
 // (lst_pairs.cuh) costs more in decoding (pair -> module -> MD -> row edge -> B: ~290 thread
 // instructions per pair, ncu) than the cuts themselves (~40), because a 32-pair step crosses a
 // module boundary almost every time.  Here the unit is the list:
-//   * 8 lanes (a "sub-warp") per inner MD, 4 MDs per warp; lane e walks target e, e + 8, ... of the
-//     row, so the CSR walk is done once per (MD, target) and a candidate costs two loads + the cuts;
-//   * the lanes of a warp step through their lists together; accepted (B, kappa) pairs are compacted
-//     per sub-warp with one ballot per step into shared memory, then copied to a scratch list with
-//     one atomic per MD (an MD with more than kLsStage LSs evaluates its row again and writes directly);
+//   * a warp takes 8 consecutive inner MDs and builds, once, the table of their (MD, target) lists
+//     in shared memory (first candidate, length prefix): the CSR walk is done once per list;
+//   * the ~180 candidate pairs of the 8 MDs are then taken 32 at a time (pair -> list by bisection
+//     of the small shared-memory prefix, inner-MD operands from shared memory), so lanes stay busy
+//     whatever the list lengths; accepted (B, kappa) pairs are compacted in pair order with one
+//     ballot per step and copied to a scratch list with one atomic per warp pass (a pass with more
+//     than kLsStage LSs evaluates its pairs again and writes directly);
 //   * k_scan turns the per-MD counts into md_ls_begin; k_ls_place copies each MD's LSs to their slot.
 // LSs therefore sit grouped by inner MD (what T3 building looks up); the order inside an MD's range
 // is free (reading S9).
@@ -19,92 +21,145 @@
 
 namespace lst {
 
-constexpr int kLsSub = 8;     // lanes per inner MD
-constexpr int kLsStage = 48;  // staged LSs per inner MD
+constexpr int kLsOwners = 8;    // inner MDs per warp
+constexpr int kLsRanges = 256;  // (MD, target) lists per warp pass; also the longest row supported
+constexpr int kLsStage = 96;    // staged LSs per warp pass
 
 struct LsAccepted {
   int B;
   float kappa;
 };
 
+struct LsWarp {  // per-warp scratch in shared memory
+  float4 a[kLsOwners];
+  float2 u[kLsOwners];
+  int e[kLsOwners];
+  int cnt[kLsOwners];
+  int dex[kLsOwners + 1];  // exclusive prefix of the row lengths
+  int k0[kLsOwners];
+  int gb[kLsOwners];       // event * n_mod
+  int pref[kLsRanges + 1];  // exclusive prefix of the list lengths
+  int b0[kLsRanges];        // first MD of the list | endcap(target) << 27 | owner slot << 28
+  LsAccepted stage[kLsStage];
+};
+
 __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
-  __shared__ LsAccepted s_stage[kBlock / kLsSub][kLsStage];
-  const int lane = threadIdx.x & 31;
-  const int sl = lane & (kLsSub - 1);             // lane inside the sub-warp
-  const int sw = lane / kLsSub;                   // sub-warp inside the warp
-  const unsigned sub_mask = ((1u << kLsSub) - 1u) << (sw * kLsSub);
-  const int sub_id = threadIdx.x / kLsSub;        // sub-warp inside the block
-  const int per_block = kBlock / kLsSub;
+  __shared__ LsWarp s_w[kWarps];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  LsWarp& w = s_w[warp];
   const bool on = (d.cuts.stage_mask & 2) != 0;
   const int n_md = d.ctl->total[K_MD];
   const int cap = d.cap[K_LS];
   LsAccepted* scratch = reinterpret_cast<LsAccepted*>(d.ev_scratch);
   unsigned long long near = 0, tests = 0;
-  for (int a0 = blockIdx.x * per_block; a0 < n_md; a0 += gridDim.x * per_block) {
-    const int A = a0 + sub_id;
-    const bool have = A < n_md && on;
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-    float2 ua = make_float2(0.f, 0.f);
-    int eA = 0, k0 = 0, deg = 0, gm_base = 0;
-    if (have) {
+  for (int A0 = (blockIdx.x * kWarps + warp) * kLsOwners; A0 < n_md; A0 += gridDim.x * kWarps * kLsOwners) {
+    // ---- lanes 0..7: one inner MD each ----
+    const int A = A0 + lane;
+    int k0 = 0, deg = 0, gm_base = 0;
+    if (lane < kLsOwners && A < n_md && on) {
       const int info = d.md_info[A];
       const int gm = info >> 1;
       const int ev = gm / d.n_mod;
-      eA = info & 1;
-      a = d.md_a[A];
-      ua = d.md_u[A];
+      w.a[lane] = d.md_a[A];
+      w.u[lane] = d.md_u[A];
+      w.e[lane] = info & 1;
       k0 = __ldg(d.conn_off + (gm - ev * d.n_mod));
       deg = __ldg(d.conn_off + (gm - ev * d.n_mod) + 1) - k0;
       gm_base = ev * d.n_mod;
     }
-    int cnt = 0;  // accepted so far for this MD (uniform inside the sub-warp)
-    // pass 0 stages; pass 1 (only if the stage overflowed) writes directly at the reserved base
-    int base = 0;
-    for (int pass = 0; pass < 2; ++pass) {
-      cnt = 0;
-      for (int e0 = 0; __any_sync(kFull, e0 < deg); e0 += kLsSub) {
-        const int e = e0 + sl;
-        int B = 0, b1 = 0, eB = 0;
-        if (e < deg) {
-          const int m2 = __ldg(d.conn_tgt + k0 + e);
-          B = d.mod_md_begin[gm_base + m2];
-          b1 = d.mod_md_begin[gm_base + m2 + 1];
-          eB = __ldg(d.subdet + m2) != 0;
-          if (pass == 0) tests += (unsigned long long)(b1 - B);
+    const int dincl = warp_incl_scan(deg);  // rows of the 8 MDs, concatenated
+    if (lane < kLsOwners) {
+      w.dex[lane] = dincl - deg;
+      w.k0[lane] = k0;
+      w.gb[lane] = gm_base;
+    }
+    if (lane == kLsOwners - 1) w.dex[kLsOwners] = dincl;
+    __syncwarp();
+    int first = 0;                          // MDs [first, first + take) are handled per pass
+    while (first < kLsOwners) {
+      const int d_first = w.dex[first];
+      // as many MDs as fit the range table (a single row always fits: lst_load_geometry checks)
+      const unsigned fit = __ballot_sync(kFull, lane >= first && lane < kLsOwners && dincl - d_first <= kLsRanges);
+      const int take = __popc(fit >> first & ~((fit >> first) + 1u)) ;  // length of the run of ones starting at `first`
+      const int last = first + take;  // exclusive
+      const int R = w.dex[last] - d_first;
+      if (lane < kLsOwners) w.cnt[lane] = 0;
+      // ---- range table: list r = (owner, target e) ----
+      int carry = 0;
+      for (int r0 = 0; r0 < R; r0 += 32) {
+        const int r = r0 + lane;
+        int n_t = 0;
+        if (r < R) {
+          int o = first;  // owner slot of list r: last o with (dex[o] - d_first) <= r
+          for (int k = first + 1; k < last; ++k)
+            if (w.dex[k] - d_first <= r) o = k;
+          const int e = r - (w.dex[o] - d_first);
+          const int m2 = __ldg(d.conn_tgt + w.k0[o] + e);
+          const int gb = w.gb[o];
+          const int B0 = d.mod_md_begin[gb + m2];
+          n_t = d.mod_md_begin[gb + m2 + 1] - B0;
+          w.b0[r] = B0 | ((__ldg(d.subdet + m2) != 0) << 27) | (o << 28);
         }
-        while (__any_sync(kFull, B < b1)) {
-          unsigned r = 0;
-          float kappa = 0.0f;
-          if (B < b1) r = ls_test(d.cuts, a, ua, eA != 0, d.md_a[B], d.md_u[B], eB != 0, kappa);
-          if (pass == 0) near += (r >> 1) & 1u;
-          const unsigned m = __ballot_sync(kFull, r & ACC) & sub_mask;
-          if (r & ACC) {
-            const int pos = cnt + __popc(m & ((1u << lane) - 1u));
+        const int incl = warp_incl_scan(n_t);
+        if (r < R) w.pref[r] = carry + incl - n_t;
+        carry += __shfl_sync(kFull, incl, 31);
+      }
+      const int P = carry;
+      if (lane == 0) w.pref[R] = P;
+      __syncwarp();
+      tests += lane == 0 ? (unsigned long long)P : 0ull;
+      // ---- pairs of the pass, 32 at a time; pass 1 only if the stage overflowed ----
+      int base = 0, run = 0;
+      for (int pass = 0; pass < 2; ++pass) {
+        run = 0;
+        for (int p0 = 0; p0 < P; p0 += 32) {
+          const int p = p0 + lane;
+          unsigned res = 0;
+          LsAccepted acc;
+          int o = 0;
+          if (p < P) {
+            int lo = 0, hi = R;  // list of pair p: largest r with pref[r] <= p
+            while (hi - lo > 1) {
+              const int mid = (lo + hi) >> 1;
+              if (w.pref[mid] <= p) lo = mid; else hi = mid;
+            }
+            const int ent = w.b0[lo];
+            o = (unsigned)ent >> 28;
+            acc.B = (ent & 0x7ffffff) + (p - w.pref[lo]);
+            res = ls_test(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[acc.B], d.md_u[acc.B], (ent >> 27) & 1, acc.kappa);
+          }
+          if (pass == 0) near += (res >> 1) & 1u;
+          const unsigned m = __ballot_sync(kFull, res & ACC);
+          if (res & ACC) {
+            const int pos = run + __popc(m & ((1u << lane) - 1u));
             if (pass == 0) {
-              if (pos < kLsStage) s_stage[sub_id][pos] = LsAccepted{B, kappa};
+              if (pos < kLsStage) w.stage[pos] = acc;
+              atomicAdd(&w.cnt[o], 1);
             } else if (base + pos < cap) {
-              scratch[base + pos] = LsAccepted{B, kappa};
+              scratch[base + pos] = acc;
             }
           }
-          cnt += __popc(m);
-          ++B;
+          run += __popc(m);
         }
-      }
-      if (pass == 0) {
-        if (sl == 0 && cnt > 0) base = atomicAdd(&d.ctl->scratch_cur[1], cnt);
-        base = __shfl_sync(kFull, base, sw * kLsSub);
-        if (A < n_md && sl == 0) {
-          d.ls_cnt[A] = cnt;
-          d.ls_sbase[A] = base;
-        }
+        if (pass == 1) break;
+        // ---- one atomic for the pass; per-MD count and scratch position ----
+        if (lane == 0 && run > 0) base = atomicAdd(&d.ctl->scratch_cur[1], run);
+        base = __shfl_sync(kFull, base, 0);
         __syncwarp();
-        if (cnt <= kLsStage)
-          for (int k = sl; k < cnt; k += kLsSub)
-            if (base + k < cap) scratch[base + k] = s_stage[sub_id][k];
-        __syncwarp();  // the staging rows are reused by the next MD
-        if (!__any_sync(kFull, cnt > kLsStage)) break;
-        if (cnt <= kLsStage) deg = 0;  // only the overflowing sub-warps walk their row again
+        const int c = (lane >= first && lane < last) ? w.cnt[lane] : 0;
+        const int cincl = warp_incl_scan(c);
+        if (lane >= first && lane < last && A < n_md) {
+          d.ls_cnt[A] = c;
+          d.ls_sbase[A] = base + cincl - c;
+        }
+        if (run <= kLsStage) {
+          for (int k = lane; k < run; k += 32)
+            if (base + k < cap) scratch[base + k] = w.stage[k];
+          break;
+        }
       }
+      __syncwarp();  // the tables are reused by the next pass
+      first = last;
     }
   }
   near = warp_sum_u64(near);
