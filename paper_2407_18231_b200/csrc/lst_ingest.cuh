@@ -19,19 +19,37 @@ __device__ __forceinline__ int event_of(const int* __restrict__ off, int n_event
 
 // a0.1 histogram: one atomic per hit on its sensor counter; the returned rank is kept so that the
 // scatter pass needs no second atomic.  Invalid sensor ids raise E_BAD_SENSOR (-> LST_ERR_ARG).
+// kIngestUnroll hits per thread are in flight at once (the kernel is latency-bound: every hit is a
+// chain load -> atomic -> store).
+constexpr int kIngestUnroll = 4;
+
 __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.n_hits; i += stride) {
-    int s = __ldg(d.in_sensor + i);
-    if (s < 0 || s >= n_sens) {
-      atomicOr(&d.ctl->error, E_BAD_SENSOR);
-      s = 0;
+  for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {
+    int s[kIngestUnroll], gs[kIngestUnroll];
+#pragma unroll
+    for (int u = 0; u < kIngestUnroll; ++u) {
+      const int i = i0 + u * stride;
+      s[u] = i < d.n_hits ? __ldg(d.in_sensor + i) : 0;
     }
-    const int ev = event_of(d.hit_ev_off, d.n_events, i);
-    const int gs = ev * n_sens + s;
-    d.hit_gs_in[i] = gs;
-    d.hit_rank[i] = atomicAdd(d.sens_cnt + gs, 1);
+#pragma unroll
+    for (int u = 0; u < kIngestUnroll; ++u) {
+      const int i = i0 + u * stride;
+      if (i < d.n_hits && (s[u] < 0 || s[u] >= n_sens)) {
+        atomicOr(&d.ctl->error, E_BAD_SENSOR);
+        s[u] = 0;
+      }
+      gs[u] = (i < d.n_hits ? event_of(d.hit_ev_off, d.n_events, i) : 0) * n_sens + s[u];
+    }
+#pragma unroll
+    for (int u = 0; u < kIngestUnroll; ++u) {
+      const int i = i0 + u * stride;
+      if (i < d.n_hits) {
+        d.hit_gs_in[i] = gs[u];
+        d.hit_rank[i] = atomicAdd(d.sens_cnt + gs[u], 1);
+      }
+    }
   }
   // pLS -> event (tiny; rides along)
   for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < d.n_pls; p += stride)
@@ -79,14 +97,31 @@ k_scan(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int 
 __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < d.n_hits; i += stride) {
-    const int gs = d.hit_gs_in[i];
-    const int pos = __ldg(d.sens_begin + gs) + d.hit_rank[i];
-    const float x = __ldg(d.in_x + i), y = __ldg(d.in_y + i), z = __ldg(d.in_z + i);
-    d.hit[pos] = make_float4(x, y, z, sqrtf(x * x + y * y));
-    const int ev = gs / n_sens;
-    d.hit_idx[pos] = i - __ldg(d.hit_ev_off + ev);
-    d.hit_gs[pos] = gs;
+  for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {
+    int gs[kIngestUnroll], pos[kIngestUnroll];
+    float x[kIngestUnroll], y[kIngestUnroll], z[kIngestUnroll];
+#pragma unroll
+    for (int u = 0; u < kIngestUnroll; ++u) {
+      const int i = i0 + u * stride;
+      const bool ok = i < d.n_hits;
+      gs[u] = ok ? d.hit_gs_in[i] : 0;
+      pos[u] = ok ? d.hit_rank[i] : 0;
+      x[u] = ok ? __ldg(d.in_x + i) : 0.0f;
+      y[u] = ok ? __ldg(d.in_y + i) : 0.0f;
+      z[u] = ok ? __ldg(d.in_z + i) : 0.0f;
+    }
+#pragma unroll
+    for (int u = 0; u < kIngestUnroll; ++u) pos[u] += __ldg(d.sens_begin + gs[u]);
+#pragma unroll
+    for (int u = 0; u < kIngestUnroll; ++u) {
+      const int i = i0 + u * stride;
+      if (i < d.n_hits) {
+        d.hit[pos[u]] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
+        const int ev = gs[u] / n_sens;
+        d.hit_idx[pos[u]] = i - __ldg(d.hit_ev_off + ev);
+        d.hit_gs[pos[u]] = gs[u];
+      }
+    }
   }
 }
 
