@@ -127,7 +127,7 @@ class ClockSampler(threading.Thread):
 # ---------------------------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------
-STAGE_OF_KERNEL = {"md": "md", "ls": "ls", "t3": "t3", "t5": "t5", "pt3": "pt3", "pt5": "pt5"}
+STAGE_OF_KERNEL = {"md": "md", "ls": "ls", "t3": "t3", "t5": "t5", "pt": "pt"}
 # flops of the FIRST cut of a stage (every candidate evaluates at least that) and of the whole cut
 # list (every accepted object evaluates all of it); counted from CUTS.md, no FMA.
 FLOPS_FIRST = {"md": 19, "ls": 16, "t3": 28, "t5": 33, "pt3": 6, "pt5": 6}
@@ -147,16 +147,16 @@ def algorithmic_work(name, s, n_sens):
         "md_pairs": 8 * n_sens,
         "md": 16 * h + 4 * n_sens + 16 * md,
         "md_place": 16 * md + 28 * md + 36 * md + 2 * n_sens,
-        "ls_pairs": 4 * n_sens,
-        "ls": 28 * md + 12 * ls,
-        "ls_place": 24 * ls + 4 * md,
+        "ls": 28 * md + 8 * ls,
+        "ls_scan": 8 * md,
+        "ls_place": 20 * ls + 12 * md,
         "t3": 12 * ls + 16 * md + 36 * t3,
         "t5": 24 * t3 + 16 * md + 40 * t5,
+        "anchors": 24 * md,
         "pt_tiles": 0,
-        "pt3": 36 * p + 16 * t3 + 12 * p3,
+        "pt": 36 * p + 16 * (t3 + t5) + 12 * (p3 + p5),
         "pt3_scan": 8 * p,
         "pt3_place": 24 * p3,
-        "pt5": 36 * p + 16 * t5 + 12 * p5,
         "pt5_scan": 8 * p,
         "pt5_place": 24 * p5,
         "event_ranges": 0,
@@ -172,9 +172,12 @@ def algorithmic_work(name, s, n_sens):
     }
     st = STAGE_OF_KERNEL.get(name)
     flops = 0
-    if st:
-        i = ("md", "ls", "t3", "t5", "pt3", "pt5").index(st)
-        n_obj = (md, ls, t3, t5, p3, p5)[i]
+    if st == "pt":  # one kernel builds pT3 and pT5
+        for i, key, n_obj in ((4, "pt3", p3), (5, "pt5", p5)):
+            flops += FLOPS_FIRST[key] * s["n_tests"][i] + (FLOPS_FULL[key] - FLOPS_FIRST[key]) * n_obj
+    elif st:
+        i = ("md", "ls", "t3", "t5").index(st)
+        n_obj = (md, ls, t3, t5)[i]
         flops = FLOPS_FIRST[st] * s["n_tests"][i] + (FLOPS_FULL[st] - FLOPS_FIRST[st]) * n_obj
     return table.get(name, 0), flops
 

@@ -133,17 +133,17 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
   L.mark("t5");
   k_stage<StageT5><<<gp, kBlock, 0, st>>>(d);
+  L.mark("anchors");
+  k_anchor<<<gp, kBlock, 0, st>>>(d);
   L.mark("pt_tiles");
   k_pt_tiles<<<1, kBlock, 0, st>>>(d);
-  L.mark("pt3");
-  k_pt_eval<false><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  L.mark("pt");
+  k_pt_eval<<<g->n_sm * 5, kBlock, 0, st>>>(d);
   L.mark("pt3_scan");
   k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
       d.pls_pt3_cnt, d.pls_pt3_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP3, d.tstate[T_PP3]);
   L.mark("pt3_place");
   k_pt_place<false><<<gp, kBlock, 0, st>>>(d);
-  L.mark("pt5");
-  k_pt_eval<true><<<g->n_sm * 6, kBlock, 0, st>>>(d);
   L.mark("pt5_scan");
   k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
       d.pls_pt5_cnt, d.pls_pt5_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP5, d.tstate[T_PP5]);

@@ -89,10 +89,8 @@ __device__ __forceinline__ unsigned pt_after_gate(const Cuts& c, const Seed& s, 
 // (|kp| -+ tolk)^2.  crs is formed exactly as in kappa3 (same operands, same order), so its
 // cancellation error is common to both; everything else differs by ~1e-6 relative, near-threshold
 // candidates lie within 1e-5, and the bounds carry a 1e-3 margin.  false = the exact cut rejects.
-__device__ __forceinline__ bool pt_curv_possible(const Cuts& c, float pt, int q, float x1, float y1, float2 A,
-                                                 float2 L) {
-  const float kp = (-(float)q) / (pt * c.kr);
-  const float tolk = c.pt_k_tol0 + c.pt_k_tol1 * fabsf(kp);
+// kp = (-q) / (pt * KR), tolk = PT_K_TOL0 + PT_K_TOL1 * |kp| (as in make_seed).
+__device__ __forceinline__ bool pt_curv_possible(float kp, float tolk, float x1, float y1, float2 A, float2 L) {
   const float ax = A.x - x1, ay = A.y - y1;
   const float bx = L.x - A.x, by = L.y - A.y;
   const float cx = L.x - x1, cy = L.y - y1;

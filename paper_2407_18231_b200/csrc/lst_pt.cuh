@@ -57,15 +57,50 @@ __device__ __forceinline__ void event_cands(const Dev& d, int ev, int& c0, int& 
   }
 }
 
-constexpr int kSeedTile = 128;   // seeds staged per tile
-constexpr int kSeedSub = 128;    // seeds between two drains of the survivor queues
-constexpr int kQueue = 64;       // survivor queue entries per thread (drained early when one fills up)
+constexpr int kSeedTile = 128;  // seeds staged per tile; the survivor queues are drained after every tile
+constexpr int kQueue = 48;      // survivor queue entries per thread (drained early when one fills up)
 
-// per-event table written by k_pt_tiles: candidate ranges, seed range, first tile (T3 / T5 kernels)
+// ---- anchors: the MDs that start at least one T3 (and therefore every T5) ----------------------
+// The gate of CUTS.md section 7 depends only on the seed and on the FIRST MD of the candidate, and
+// T3s / T5s are stored grouped by first MD: all candidates of an anchor share one gate evaluation.
+// k_anchor compacts the anchors (order preserved, so an event's anchors are contiguous).
+__global__ void __launch_bounds__(kBlock) k_anchor(Dev d) {
+  __shared__ int s_tile;
+  __shared__ int s_scan[kWarps + 2];
+  const bool on = (d.cuts.stage_mask & 16) && d.ctl->total[K_T3] > 0;
+  const bool on5 = d.ctl->total[K_T5] > 0;
+  const int n = d.ctl->total[K_MD];
+  const int n_tiles = n > 0 ? (n + kBlock - 1) / kBlock : 1;
+  for (;;) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(d.ctl->ticket + T_ANC, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int A = tile * kBlock + threadIdx.x;
+    int t0 = 0, t1 = 0;
+    if (on && A < n) {
+      t0 = d.ls_t3_begin[d.md_ls_begin[A]];
+      t1 = d.ls_t3_begin[d.md_ls_begin[A + 1]];
+    }
+    int tb, tt;
+    const int off = tile_alloc(t1 > t0 ? 1 : 0, d.tstate[T_ANC], tile, s_scan, tb, tt);
+    if (A < n) d.anc_begin[A] = off;
+    if (t1 > t0) {
+      const float4 a = d.md_a[A];
+      d.anc_axy[off] = make_float2(a.x, a.y);
+      d.anc_t3[off] = make_int2(t0, t1 - t0);
+      const int u0 = on5 ? d.t3_t5_begin[t0] : 0, u1 = on5 ? d.t3_t5_begin[t1] : 0;
+      d.anc_t5[off] = make_int2(u0, u1 - u0);
+    }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) d.anc_begin[n] = tb + tt;
+  }
+}
+
+// per-event table written by k_pt_tiles: anchor range, seed range, first tile
 struct PtEvent {
-  int c0[2], c1[2];  // [0] T3, [1] T5
+  int a0, a1;
   int s0, s1;
-  int tile0[2];
+  int tile0;
 };
 
 // One block.  Fills pt_ev[0..n_events) and pt_ev[n_events].tile0 = number of tiles; n_tests.
@@ -77,14 +112,20 @@ __global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
     PtEvent ev;
     ev.s0 = d.pls_ev_off[e];
     ev.s1 = d.pls_ev_off[e + 1];
-    ev.c0[0] = ev.c1[0] = ev.c0[1] = ev.c1[1] = 0;
-    if (on && d.ctl->total[K_T3] > 0) event_cands<false>(d, e, ev.c0[0], ev.c1[0]);
-    if (on && d.ctl->total[K_T5] > 0) event_cands<true>(d, e, ev.c0[1], ev.c1[1]);
+    ev.a0 = ev.a1 = 0;
     const int ns = on ? ev.s1 - ev.s0 : 0;
-    for (int k = 0; k < 2; ++k)
-      ev.tile0[k] = ((ev.c1[k] - ev.c0[k] + kBlock - 1) / kBlock) * ((ns + kSeedTile - 1) / kSeedTile);
-    t3 += (unsigned long long)ns * (ev.c1[0] - ev.c0[0]);
-    t5 += (unsigned long long)ns * (ev.c1[1] - ev.c0[1]);
+    int c0 = 0, c1 = 0;
+    if (on && d.ctl->total[K_T3] > 0) {
+      ev.a0 = d.anc_begin[d.mod_md_begin[e * d.n_mod]];
+      ev.a1 = d.anc_begin[d.mod_md_begin[(e + 1) * d.n_mod]];
+      event_cands<false>(d, e, c0, c1);
+      t3 += (unsigned long long)ns * (c1 - c0);  // candidates of CUTS.md section 7: every (seed, T3) of the event
+    }
+    if (on && d.ctl->total[K_T5] > 0) {
+      event_cands<true>(d, e, c0, c1);
+      t5 += (unsigned long long)ns * (c1 - c0);
+    }
+    ev.tile0 = ((ev.a1 - ev.a0 + kBlock - 1) / kBlock) * ((ns + kSeedTile - 1) / kSeedTile);
     d.pt_ev[e] = ev;
   }
   t3 = warp_sum_u64(t3);
@@ -95,16 +136,13 @@ __global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
   }
   __syncthreads();
   if (threadIdx.x == 0) {  // exclusive prefix of the tile counts (n_events is small)
-    int a = 0, b = 0;
+    int a = 0;
     for (int e = 0; e < E; ++e) {
-      const int ta = d.pt_ev[e].tile0[0], tb = d.pt_ev[e].tile0[1];
-      d.pt_ev[e].tile0[0] = a;
-      d.pt_ev[e].tile0[1] = b;
+      const int ta = d.pt_ev[e].tile0;
+      d.pt_ev[e].tile0 = a;
       a += ta;
-      b += tb;
     }
-    d.pt_ev[E].tile0[0] = a;
-    d.pt_ev[E].tile0[1] = b;
+    d.pt_ev[E].tile0 = a;
   }
 }
 
@@ -113,33 +151,39 @@ struct PtAccepted {
   float score;
 };
 
-template <bool IS5>
+struct PtWarp {  // per-warp scratch of k_pt_eval
+  float2 axy[32];      // the warp's anchors
+  int2 r3[32], r5[32];  // (first, count) of their T3s / T5s
+  unsigned w1[64];     // gate survivors: seed slot | anchor lane << 16 | gate-near << 31
+  int pref[33];        // exclusive prefix of the candidate counts of w1[0..32)
+  float kp[32], tolk[32];
+};
+
+// pT3 and pT5 of the whole batch.  Tile = 256 anchors of one event (one per thread) x up to
+// kSeedTile seeds of the same event (shared memory, read as broadcasts).
 __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
-  constexpr int K = IS5 ? 1 : 0;
-  constexpr int kKind = IS5 ? K_PT5 : K_PT3;
   __shared__ int s_tile, s_ev;
   __shared__ float4 s_seed[kSeedTile];  // x1, y1, vx, vy
   __shared__ float s_lv[kSeedTile];
   __shared__ unsigned short s_q[kQueue][kBlock];  // [entry][thread]: conflict-free per-thread queues
-  __shared__ unsigned s_w2[kWarps][64];           // phase-2 list of the warp: source lane << 16 | seed slot
+  __shared__ int2 s_w2[kWarps][64];               // phase-2 list of the warp: (candidate | T5 flag << 31, seed slot)
+  __shared__ PtWarp s_pw[kWarps];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int E = d.n_events;
-  const int n_tiles = d.pt_ev[E].tile0[K];
-  const int cap = d.cap[kKind];
-  const float2* axy = IS5 ? d.t5_axy : d.t3_axy;
-  const float2* lxy = IS5 ? d.t5_lxy : d.t3_lxy;
-  int* cnt_p = IS5 ? d.pls_pt5_cnt : d.pls_pt3_cnt;
-  PtAccepted* scratch = reinterpret_cast<PtAccepted*>(d.ev_scratch);
+  const int n_tiles = d.pt_ev[E].tile0;
+  const int cap3 = d.cap[K_PT3], cap5 = d.cap[K_PT5];
+  PtAccepted* scratch3 = reinterpret_cast<PtAccepted*>(d.ev_scratch);
+  PtAccepted* scratch5 = reinterpret_cast<PtAccepted*>(d.ev_scratch2);
   const float inv_2rmin = d.cuts.inv_2rmin * 1.0001f, gate_tol = d.cuts.pt_gate_tol * 1.0001f;
-  unsigned long long near = 0;
+  unsigned long long near3 = 0, near5 = 0;
   for (;;) {
     if (threadIdx.x == 0) {
-      const int tile = atomicAdd(d.ctl->ticket + (IS5 ? T_PT5 : T_PT3), 1);
+      const int tile = atomicAdd(d.ctl->ticket + T_PT3, 1);
       int lo = 0, hi = E;  // event of the tile: largest e with tile0[e] <= tile
       if (tile < n_tiles)
         while (hi - lo > 1) {
           const int mid = (lo + hi) >> 1;
-          if (d.pt_ev[mid].tile0[K] <= tile) lo = mid; else hi = mid;
+          if (d.pt_ev[mid].tile0 <= tile) lo = mid; else hi = mid;
         }
       s_tile = tile;
       s_ev = lo;
@@ -148,9 +192,9 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     const int tile = s_tile;
     if (tile >= n_tiles) break;
     const PtEvent ev = d.pt_ev[s_ev];
-    const int n_cb = (ev.c1[K] - ev.c0[K] + kBlock - 1) / kBlock;
-    const int local = tile - ev.tile0[K];
-    const int sb = local / n_cb, cb = local - sb * n_cb;
+    const int n_ab = (ev.a1 - ev.a0 + kBlock - 1) / kBlock;
+    const int local = tile - ev.tile0;
+    const int sb = local / n_ab, ab = local - sb * n_ab;
     const int p0 = ev.s0 + sb * kSeedTile;
     const int n_seed = min(kSeedTile, ev.s1 - p0);
     for (int k = threadIdx.x; k < n_seed; k += kBlock) {
@@ -161,97 +205,170 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
       s_lv[k] = sqrtf(vx * vx + vy * vy);
     }
     __syncthreads();
-    const int t = ev.c0[K] + cb * kBlock + threadIdx.x;
-    const bool valid = t < ev.c1[K];
-    float2 A = make_float2(0.0f, 0.0f), L = A;
+    const int anc = ev.a0 + ab * kBlock + threadIdx.x;
+    const bool valid = anc < ev.a1;
+    float2 A = make_float2(0.0f, 0.0f);
+    int2 r3 = make_int2(0, 0), r5 = make_int2(0, 0);  // (first, count) of the anchor's T3s / T5s
     if (valid) {
-      A = axy[t];
-      L = lxy[t];
+      A = d.anc_axy[anc];
+      r3 = d.anc_t3[anc];
+      r5 = d.anc_t5[anc];
     }
-    // ---- phase 2: the exact cut list for one entry of the warp's list; returns its near flag ----
-    const int t_warp = ev.c0[K] + cb * kBlock + warp * 32;
-    auto phase2 = [&](unsigned ent) -> unsigned {
-      const int ks = ent & 0xffff, tt = t_warp + (int)(ent >> 16);
+    // ---- phase 2: the exact cut list for one entry of the warp's list ----
+    auto phase2 = [&](int2 ent) {
+      const bool is5 = ent.x < 0;
+      const int t = ent.x & 0x7fffffff, ks = ent.y;
       const int p = p0 + ks;
       const float4 sd = s_seed[ks];
       const Seed full = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p), __ldg(d.p_y0 + p),
                                   __ldg(d.p_z0 + p), sd.x, sd.y, __ldg(d.p_z1 + p));
       float score;
-      const unsigned r2 = PtCand<IS5>::test(d, full, tt, score);
+      const unsigned r2 = is5 ? PtCand<true>::test(d, full, t, score) : PtCand<false>::test(d, full, t, score);
+      if (is5) near5 += (r2 >> 1) & 1u; else near3 += (r2 >> 1) & 1u;
       if (r2 & ACC) {
-        const int slot = atomicAdd(&d.ctl->scratch_cur[IS5 ? 3 : 2], 1);
-        if (slot < cap) scratch[slot] = PtAccepted{p, tt, score};
-        atomicAdd(cnt_p + p, 1);
+        const int slot = atomicAdd(&d.ctl->scratch_cur[is5 ? 3 : 2], 1);
+        if (slot < (is5 ? cap5 : cap3)) (is5 ? scratch5 : scratch3)[slot] = PtAccepted{p, t, score};
+        atomicAdd((is5 ? d.pls_pt5_cnt : d.pls_pt3_cnt) + p, 1);
       }
-      return (r2 >> 1) & 1u;
     };
     int n2 = 0;
-    for (int k0 = 0; k0 < n_seed; k0 += kSeedSub) {
-      // ---- phase 1: necessary condition of the gate, survivors into the thread's own queue ----
-      int nq = 0;
-      const int k1 = min(n_seed, k0 + kSeedSub);
-      int k = k0;
-      while (k < k1) {
-        if (valid) {
-#pragma unroll 4
-          for (; k < k1 && nq < kQueue; ++k) {
-            const float4 sd = s_seed[k];
-            const float wx = A.x - sd.x, wy = A.y - sd.y;
-            const float gdot = sd.z * wx + sd.w * wy;
-            const float lw2 = wx * wx + wy * wy;
-            float rl;
-            asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
-            const float lw = lw2 * rl;
-            const float gcrs = fabsf(sd.z * wy - sd.w * wx);
-            const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
-            // keep unless surely rejected; out of the approximation's range the exact gate decides
-            const bool keep = gdot > 0.0f && (!(gcrs > lim) || !(lw2 >= 1e-30f) || !(lw2 <= 1e30f));
-            if (keep) s_q[nq++][threadIdx.x] = (unsigned short)k;
-          }
-        } else {
-          k = k1;
-        }
-        // a full queue anywhere in the warp: drain now, then go on with the rest of the sub-block
-        const bool more = __any_sync(kFull, k < k1);
-        // ---- phase 1b over the queues, lanes in lockstep; survivors into the warp's phase-2 list ----
-        const int nq_max = __reduce_max_sync(kFull, nq);
-        for (int i = 0; i < nq_max; ++i) {
-          bool go = false;
-          int ks = 0;
-          if (i < nq) {
-            ks = s_q[i][threadIdx.x];
-            const float4 sd = s_seed[ks];
-            Seed s;
-            s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[ks];
-            const unsigned r = pt_gate(d.cuts, s, A.x, A.y);  // exact gate (CUTS.md section 7)
-            go = (r & ACC) != 0;
-            if (!go) near += (r >> 1) & 1u;
-            if (go && !(r & NEAR))
-              go = pt_curv_possible(d.cuts, __ldg(d.p_pt + p0 + ks), __ldg(d.p_q + p0 + ks), sd.x, sd.y, A, L);
-          }
-          const unsigned m = __ballot_sync(kFull, go);
-          if (go) s_w2[warp][n2 + __popc(m & ((1u << lane) - 1u))] = ((unsigned)lane << 16) | (unsigned)ks;
-          n2 += __popc(m);
-          if (n2 >= 32) {  // a full warp of phase-2 work
-            __syncwarp();
-            near += phase2(s_w2[warp][lane]);
-            const unsigned rest = (32 + lane < n2) ? s_w2[warp][32 + lane] : 0u;
-            __syncwarp();
-            s_w2[warp][lane] = rest;
-            n2 -= 32;
-            __syncwarp();
-          }
-        }
-        nq = 0;
-        if (!more) break;
+    // pushes up to one entry per lane onto the warp's phase-2 list; runs phase 2 whenever 32 are waiting
+    auto push2 = [&](bool go, int cand, int ks) {
+      const unsigned m = __ballot_sync(kFull, go);
+      if (m == 0u) return;
+      if (go) s_w2[warp][n2 + __popc(m & ((1u << lane) - 1u))] = make_int2(cand, ks);
+      n2 += __popc(m);
+      if (n2 >= 32) {
+        __syncwarp();
+        phase2(s_w2[warp][lane]);
+        const int2 rest = (32 + lane < n2) ? s_w2[warp][32 + lane] : make_int2(0, 0);
+        __syncwarp();
+        s_w2[warp][lane] = rest;
+        n2 -= 32;
+        __syncwarp();
       }
+    };
+    // The warp's 32 anchors, readable by every lane (a gate survivor is expanded by whichever lane is free).
+    PtWarp& w = s_pw[warp];
+    w.axy[lane] = A;
+    w.r3[lane] = r3;
+    w.r5[lane] = r5;
+    __syncwarp();
+    // ---- expansion of up to 32 gate survivors (seed slot | anchor lane << 16 | gate-near << 31) into
+    // their (seed, T3) / (seed, T5) candidates, flattened over the lanes; the curvature pre-filter
+    // decides which go on to the exact cuts ----
+    auto expand = [&](int n_ent) {
+      int n_c = 0;
+      if (lane < n_ent) {
+        const unsigned ent = w.w1[lane];
+        const int src = (ent >> 16) & 31, ks = ent & 0xffff;
+        n_c = w.r3[src].y + w.r5[src].y;
+        const float kp = (-(float)__ldg(d.p_q + p0 + ks)) / (__ldg(d.p_pt + p0 + ks) * d.cuts.kr);
+        w.kp[lane] = kp;
+        w.tolk[lane] = d.cuts.pt_k_tol0 + d.cuts.pt_k_tol1 * fabsf(kp);
+      }
+      const int incl = warp_incl_scan(n_c);
+      w.pref[lane] = incl - n_c;
+      const int T = __shfl_sync(kFull, incl, 31);
+      if (lane == 0) w.pref[32] = T;
+      __syncwarp();
+      for (int i0 = 0; i0 < T; i0 += 32) {
+        const int it = i0 + lane;
+        bool go = false;
+        int cand = 0, ks = 0;
+        if (it < T) {
+          int lo = 0, hi = 32;  // entry of item `it`: largest e with pref[e] <= it
+#pragma unroll
+          for (int sft = 0; sft < 5; ++sft) {
+            const int mid = (lo + hi) >> 1;
+            if (w.pref[mid] <= it) lo = mid; else hi = mid;
+          }
+          const unsigned ent = w.w1[lo];
+          const int src = (ent >> 16) & 31, c = it - w.pref[lo];
+          ks = ent & 0xffff;
+          const int2 a3 = w.r3[src], a5 = w.r5[src];
+          const bool is5 = c >= a3.y;
+          const int t = is5 ? a5.x + (c - a3.y) : a3.x + c;
+          cand = t | (is5 ? 0x80000000 : 0);
+          go = true;
+          if (!(ent >> 31)) {
+            const float4 sd = s_seed[ks];
+            go = pt_curv_possible(w.kp[lo], w.tolk[lo], sd.x, sd.y, w.axy[src], is5 ? d.t5_lxy[t] : d.t3_lxy[t]);
+          }
+        }
+        push2(go, cand, ks);
+      }
+      __syncwarp();
+    };
+    int n1 = 0;  // gate survivors waiting in w.w1
+    // ---- phase 1: necessary condition of the gate, survivors into the thread's own queue ----
+    int k = 0;
+    for (;;) {
+      int nq = 0;
+      if (valid) {
+#pragma unroll 4
+        for (; k < n_seed && nq < kQueue; ++k) {
+          const float4 sd = s_seed[k];
+          const float wx = A.x - sd.x, wy = A.y - sd.y;
+          const float gdot = sd.z * wx + sd.w * wy;
+          const float lw2 = wx * wx + wy * wy;
+          float rl;
+          asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
+          const float lw = lw2 * rl;
+          const float gcrs = fabsf(sd.z * wy - sd.w * wx);
+          const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
+          // keep unless surely rejected; out of the approximation's range the exact gate decides
+          const bool keep = gdot > 0.0f && (!(gcrs > lim) || !(lw2 >= 1e-30f) || !(lw2 <= 1e30f));
+          if (keep) s_q[nq++][threadIdx.x] = (unsigned short)k;
+        }
+      } else {
+        k = n_seed;
+      }
+      const bool more = __any_sync(kFull, k < n_seed);  // a queue filled up: drain, then go on
+      // ---- phase 1b: exact gate per (seed, anchor); survivors onto the warp's list ----
+      const int nq_max = __reduce_max_sync(kFull, nq);
+      for (int i = 0; i < nq_max; ++i) {
+        bool pass = false;
+        unsigned ent = 0;
+        if (i < nq) {
+          const int ks = s_q[i][threadIdx.x];
+          const float4 sd = s_seed[ks];
+          Seed s;
+          s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[ks];
+          const unsigned r = pt_gate(d.cuts, s, A.x, A.y);  // exact gate (CUTS.md section 7)
+          pass = (r & ACC) != 0;
+          if (!pass && (r & NEAR)) {  // every candidate of the anchor fails the gate near its threshold
+            near3 += (unsigned)r3.y;
+            near5 += (unsigned)r5.y;
+          }
+          ent = (unsigned)ks | ((unsigned)lane << 16) | ((r & NEAR) ? 0x80000000u : 0u);
+        }
+        const unsigned m = __ballot_sync(kFull, pass);
+        if (pass) w.w1[n1 + __popc(m & ((1u << lane) - 1u))] = ent;
+        n1 += __popc(m);
+        if (n1 >= 32) {
+          __syncwarp();
+          expand(32);
+          const unsigned rest = (32 + lane < n1) ? w.w1[32 + lane] : 0u;
+          __syncwarp();
+          w.w1[lane] = rest;
+          n1 -= 32;
+          __syncwarp();
+        }
+      }
+      if (!more) break;
     }
     __syncwarp();
-    if (lane < n2) near += phase2(s_w2[warp][lane]);
+    if (n1 > 0) expand(n1);
+    if (lane < n2) phase2(s_w2[warp][lane]);
     __syncthreads();  // the seed tile is reused
   }
-  near = warp_sum_u64(near);
-  if (lane == 0 && near) atomicAdd(&d.ctl->near[IS5 ? 5 : 4], near);
+  near3 = warp_sum_u64(near3);
+  near5 = warp_sum_u64(near5);
+  if (lane == 0) {
+    if (near3) atomicAdd(&d.ctl->near[4], near3);
+    if (near5) atomicAdd(&d.ctl->near[5], near5);
+  }
 }
 
 // Groups the accepted pairs by seed: begin = exclusive scan of the per-seed counts (k_scan, before
@@ -265,7 +382,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
   int* cur = IS5 ? d.pls_pt5_cur : d.pls_pt3_cur;
   int2* out = IS5 ? d.pt5 : d.pt3;
   float* out_s = IS5 ? d.pt5_score : d.pt3_score;
-  const PtAccepted* scratch = reinterpret_cast<const PtAccepted*>(d.ev_scratch);
+  const PtAccepted* scratch = reinterpret_cast<const PtAccepted*>(IS5 ? d.ev_scratch2 : d.ev_scratch);
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     if (n > cap) {
       atomicOr(&d.ctl->error, IS5 ? E_CAP_PT5 : E_CAP_PT3);

@@ -15,7 +15,7 @@ namespace lst {
 struct PtEvent;  // lst_pt.cuh
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_PP3, T_PP5, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_PP3, T_PP5, T_ANC, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
@@ -64,6 +64,7 @@ struct Dev {
   int2* ev_cnt;         // [cap_pairs / kChunk + 1] (accepted pairs, scratch position) of every chunk
   unsigned* ev_mask;    // [cap_pairs / 32 + 8] ballot words of every chunk
   void* ev_scratch;     // accepted payloads in chunk-arrival order
+  void* ev_scratch2;    // second scratch list (pT5, filled by the same kernel as pT3)
   // ---- a1: MD (grouped by global module) ----
   int* pp_md;         // [n_events * n_mod + 1] exclusive prefix of the modules' hit pairs
   int* mod_md_begin;  // [n_events * n_mod + 1] first MD of a global module
@@ -92,7 +93,10 @@ struct Dev {
   float2* t5_axy;
   float2* t5_lxy;
   // ---- a5: pT3 / pT5 (owner = pLS) ----
-  PtEvent* pt_ev;      // [n_events + 1] candidate / seed ranges and first tile of every event
+  PtEvent* pt_ev;      // [n_events + 1] anchor / seed ranges and first tile of every event
+  int* anc_begin;      // [n_md + 1] anchors before MD A (anchor = MD starting at least one T3)
+  float2* anc_axy;     // [n_anchor] anchor position
+  int2 *anc_t3, *anc_t5;  // [n_anchor] (first, count) of the T3s / T5s starting at the anchor
   int *pls_pt3_cnt, *pls_pt5_cnt;  // [n_pls + 1] accepted per seed (zeroed per batch)
   int *pls_pt3_cur, *pls_pt5_cur;  // [n_pls] next free slot of a seed's range (zeroed per batch)
   int* pls_event;      // [n_pls]
