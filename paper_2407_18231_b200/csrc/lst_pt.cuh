@@ -156,6 +156,7 @@ struct PtWarp {  // per-warp scratch of k_pt_eval
   int2 r3[32], r5[32];  // (first, count) of their T3s / T5s
   unsigned w1[64];     // gate survivors: seed slot | anchor lane << 16 | gate-near << 31
   int pref[33];        // exclusive prefix of the candidate counts of w1[0..32)
+  unsigned heads[32];  // head bits of the entries over the first 1024 items
   float kp[32], tolk[32];
 };
 
@@ -270,18 +271,30 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
       const int incl = warp_incl_scan(n_c);
       w.pref[lane] = incl - n_c;
       const int T = __shfl_sync(kFull, incl, 31);
-      if (lane == 0) w.pref[32] = T;
+      // item -> entry in O(1): one head bit per entry at the position of its first item; the entry of
+      // item `it` = number of head bits at or before it, minus one (falls back to bisection beyond 1024 items)
+      w.heads[lane] = 0u;
       __syncwarp();
+      if (n_c > 0 && incl - n_c < 1024) atomicOr(&w.heads[(incl - n_c) >> 5], 1u << ((incl - n_c) & 31));
+      __syncwarp();
+      int heads_before = 0;
       for (int i0 = 0; i0 < T; i0 += 32) {
         const int it = i0 + lane;
         bool go = false;
         int cand = 0, ks = 0;
+        const unsigned hw = i0 < 1024 ? w.heads[i0 >> 5] : 0u;
         if (it < T) {
-          int lo = 0, hi = 32;  // entry of item `it`: largest e with pref[e] <= it
+          int lo;
+          if (i0 < 1024) {
+            lo = heads_before + __popc(hw & (0xffffffffu >> (31 - lane))) - 1;
+          } else {
+            lo = 0;
+            int hi = 32;  // largest e with pref[e] <= it
 #pragma unroll
-          for (int sft = 0; sft < 5; ++sft) {
-            const int mid = (lo + hi) >> 1;
-            if (w.pref[mid] <= it) lo = mid; else hi = mid;
+            for (int sft = 0; sft < 5; ++sft) {
+              const int mid = (lo + hi) >> 1;
+              if (w.pref[mid] <= it) lo = mid; else hi = mid;
+            }
           }
           const unsigned ent = w.w1[lo];
           const int src = (ent >> 16) & 31, c = it - w.pref[lo];
@@ -296,6 +309,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
             go = pt_curv_possible(w.kp[lo], w.tolk[lo], sd.x, sd.y, w.axy[src], is5 ? d.t5_lxy[t] : d.t3_lxy[t]);
           }
         }
+        heads_before += __popc(hw);
         push2(go, cand, ks);
       }
       __syncwarp();
@@ -317,9 +331,13 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
           const float lw = lw2 * rl;
           const float gcrs = fabsf(sd.z * wy - sd.w * wx);
           const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
-          // keep unless surely rejected; out of the approximation's range the exact gate decides
-          const bool keep = gdot > 0.0f && (!(gcrs > lim) || !(lw2 >= 1e-30f) || !(lw2 <= 1e30f));
-          if (keep) s_q[nq++][threadIdx.x] = (unsigned short)k;
+          // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact
+          // gate is skipped), uncertain = within 2e-4 of the threshold or out of the approximation's
+          // range (the exact gate decides, flag bit 15)
+          const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f;
+          const bool keep = gdot > 0.0f && (!(gcrs > lim) || !in_range);
+          const bool sure = in_range && gcrs <= lim * 0.9998f;
+          if (keep) s_q[nq++][threadIdx.x] = (unsigned short)(k | (sure ? 0 : 0x8000));
         }
       } else {
         k = n_seed;
@@ -331,11 +349,15 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
         bool pass = false;
         unsigned ent = 0;
         if (i < nq) {
-          const int ks = s_q[i][threadIdx.x];
-          const float4 sd = s_seed[ks];
-          Seed s;
-          s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[ks];
-          const unsigned r = pt_gate(d.cuts, s, A.x, A.y);  // exact gate (CUTS.md section 7)
+          const int qe = s_q[i][threadIdx.x];
+          const int ks = qe & 0x7fff;
+          unsigned r = ACC;
+          if (qe & 0x8000) {  // uncertain: the exact gate (CUTS.md section 7) decides and flags near-threshold
+            const float4 sd = s_seed[ks];
+            Seed s;
+            s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[ks];
+            r = pt_gate(d.cuts, s, A.x, A.y);
+          }
           pass = (r & ACC) != 0;
           if (!pass && (r & NEAR)) {  // every candidate of the anchor fails the gate near its threshold
             near3 += (unsigned)r3.y;
