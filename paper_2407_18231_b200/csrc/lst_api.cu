@@ -217,12 +217,13 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   d.tstate[T_T5] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
   d.tstate[T_PT3] = nullptr;  // ticket only
   d.tstate[T_PT5] = nullptr;
-  d.tstate[T_ANC] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kBlock));
+  d.tstate[T_ANC] = b.take<unsigned long long>(tiles_of((long long)c.max_events * kAncBins + 1, kScanTile));
   d.tstate[T_PP3] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_IDX] = b.take<unsigned long long>(tiles_of(3LL * c.max_md + 1, kScanTile));
   d.tstate[T_TC] = b.take<unsigned long long>(tiles_of(4LL * c.max_events + 1, kScanTile));
   d.sens_cnt = b.take<int>(n_sens + 1);
+  d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins + 1);
   d.pls_pt3_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt3_cur = b.take<int>(c.max_pls);
@@ -275,7 +276,9 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   // --- a5 ---
   d.pls_event = b.take<int>(c.max_pls);
   d.pt_ev = b.take<PtEvent>((size_t)c.max_events + 1);
-  d.anc_begin = b.take<int>((size_t)c.max_md + 1);
+  d.anc_bin = b.take<int>(c.max_md);
+  d.anc_rank = b.take<int>(c.max_md);
+  d.anc_bin_begin = b.take<int>((size_t)c.max_events * kAncBins + 1);
   d.anc_axy = b.take<float2>(c.max_md);
   d.anc_t3 = b.take<int2>(c.max_md);
   d.anc_t5 = b.take<int2>(c.max_md);

@@ -135,6 +135,11 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   k_stage<StageT5><<<gp, kBlock, 0, st>>>(d);
   L.mark("anchors");
   k_anchor<<<gp, kBlock, 0, st>>>(d);
+  L.mark("anchor_scan");
+  k_scan<<<grid_for(g, (n_events * kAncBins + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
+      d.anc_bin_cnt, d.anc_bin_begin, nullptr, 0, n_events * kAncBins, d.ctl->ticket + T_ANC, d.tstate[T_ANC]);
+  L.mark("anchor_sort");
+  k_anchor_sort<<<gp, kBlock, 0, st>>>(d);
   L.mark("pt_tiles");
   k_pt_tiles<<<1, kBlock, 0, st>>>(d);
   L.mark("pt");

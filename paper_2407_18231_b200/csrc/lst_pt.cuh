@@ -63,36 +63,52 @@ constexpr int kQueue = 48;      // survivor queue entries per thread (drained ea
 // ---- anchors: the MDs that start at least one T3 (and therefore every T5) ----------------------
 // The gate of CUTS.md section 7 depends only on the seed and on the FIRST MD of the candidate, and
 // T3s / T5s are stored grouped by first MD: all candidates of an anchor share one gate evaluation.
-// k_anchor compacts the anchors (order preserved, so an event's anchors are contiguous).
+// The anchors of an event are sorted into kAncBins = 8 radial classes x 32 azimuthal sectors
+// (counting sort: k_anchor counts and keeps the arrival rank, k_scan, k_anchor_sort places), so the
+// 32 anchors of a warp of k_pt_eval sit within a few cm of each other and a seed whose gate cone
+// misses their bounding circle is skipped for the whole warp.
+constexpr int kAncBins = 256;
+
+__device__ __forceinline__ int anchor_bin(float x, float y, float r) {
+  const int rc = (r >= 29.5f) + (r >= 43.5f) + (r >= 59.5f) + (r >= 78.0f) + (r >= 98.0f) + (r >= 125.0f);
+  const float a = fabsf(x) + fabsf(y);
+  const float t = a > 0.0f ? y / a : 0.0f;                                  // diamond angle, monotone in azimuth
+  const float ps = x >= 0.0f ? (y >= 0.0f ? t : 4.0f + t) : 2.0f - t;      // [0, 4)
+  int sec = (int)(ps * 8.0f);
+  sec = sec < 0 ? 0 : (sec > 31 ? 31 : sec);
+  return rc * 32 + sec;  // any finite or non-finite input lands in [0, 256): binning never affects results
+}
+
 __global__ void __launch_bounds__(kBlock) k_anchor(Dev d) {
-  __shared__ int s_tile;
-  __shared__ int s_scan[kWarps + 2];
   const bool on = (d.cuts.stage_mask & 16) && d.ctl->total[K_T3] > 0;
+  const int n = d.ctl->total[K_MD];
+  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < n; A += gridDim.x * blockDim.x) {
+    int bin = -1, rank = 0;
+    if (on && d.ls_t3_begin[d.md_ls_begin[A + 1]] > d.ls_t3_begin[d.md_ls_begin[A]]) {
+      const float4 a = d.md_a[A];
+      const int ev = (d.md_info[A] >> 1) / d.n_mod;
+      bin = ev * kAncBins + anchor_bin(a.x, a.y, a.w);
+      rank = atomicAdd(d.anc_bin_cnt + bin, 1);
+    }
+    d.anc_bin[A] = bin;
+    d.anc_rank[A] = rank;
+  }
+}
+
+// after k_scan(anc_bin_cnt -> anc_bin_begin)
+__global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
   const bool on5 = d.ctl->total[K_T5] > 0;
   const int n = d.ctl->total[K_MD];
-  const int n_tiles = n > 0 ? (n + kBlock - 1) / kBlock : 1;
-  for (;;) {
-    if (threadIdx.x == 0) s_tile = atomicAdd(d.ctl->ticket + T_ANC, 1);
-    __syncthreads();
-    const int tile = s_tile;
-    if (tile >= n_tiles) break;
-    const int A = tile * kBlock + threadIdx.x;
-    int t0 = 0, t1 = 0;
-    if (on && A < n) {
-      t0 = d.ls_t3_begin[d.md_ls_begin[A]];
-      t1 = d.ls_t3_begin[d.md_ls_begin[A + 1]];
-    }
-    int tb, tt;
-    const int off = tile_alloc(t1 > t0 ? 1 : 0, d.tstate[T_ANC], tile, s_scan, tb, tt);
-    if (A < n) d.anc_begin[A] = off;
-    if (t1 > t0) {
-      const float4 a = d.md_a[A];
-      d.anc_axy[off] = make_float2(a.x, a.y);
-      d.anc_t3[off] = make_int2(t0, t1 - t0);
-      const int u0 = on5 ? d.t3_t5_begin[t0] : 0, u1 = on5 ? d.t3_t5_begin[t1] : 0;
-      d.anc_t5[off] = make_int2(u0, u1 - u0);
-    }
-    if (tile == n_tiles - 1 && threadIdx.x == 0) d.anc_begin[n] = tb + tt;
+  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < n; A += gridDim.x * blockDim.x) {
+    const int bin = d.anc_bin[A];
+    if (bin < 0) continue;
+    const int pos = d.anc_bin_begin[bin] + d.anc_rank[A];
+    const int t0 = d.ls_t3_begin[d.md_ls_begin[A]], t1 = d.ls_t3_begin[d.md_ls_begin[A + 1]];
+    const float4 a = d.md_a[A];
+    d.anc_axy[pos] = make_float2(a.x, a.y);
+    d.anc_t3[pos] = make_int2(t0, t1 - t0);
+    const int u0 = on5 ? d.t3_t5_begin[t0] : 0, u1 = on5 ? d.t3_t5_begin[t1] : 0;
+    d.anc_t5[pos] = make_int2(u0, u1 - u0);
   }
 }
 
@@ -116,8 +132,8 @@ __global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
     const int ns = on ? ev.s1 - ev.s0 : 0;
     int c0 = 0, c1 = 0;
     if (on && d.ctl->total[K_T3] > 0) {
-      ev.a0 = d.anc_begin[d.mod_md_begin[e * d.n_mod]];
-      ev.a1 = d.anc_begin[d.mod_md_begin[(e + 1) * d.n_mod]];
+      ev.a0 = d.anc_bin_begin[e * kAncBins];
+      ev.a1 = d.anc_bin_begin[(e + 1) * kAncBins];
       event_cands<false>(d, e, c0, c1);
       t3 += (unsigned long long)ns * (c1 - c0);  // candidates of CUTS.md section 7: every (seed, T3) of the event
     }
@@ -315,35 +331,9 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
       __syncwarp();
     };
     int n1 = 0;  // gate survivors waiting in w.w1
-    // ---- phase 1: necessary condition of the gate, survivors into the thread's own queue ----
-    int k = 0;
-    for (;;) {
-      int nq = 0;
-      if (valid) {
-#pragma unroll 4
-        for (; k < n_seed && nq < kQueue; ++k) {
-          const float4 sd = s_seed[k];
-          const float wx = A.x - sd.x, wy = A.y - sd.y;
-          const float gdot = sd.z * wx + sd.w * wy;
-          const float lw2 = wx * wx + wy * wy;
-          float rl;
-          asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
-          const float lw = lw2 * rl;
-          const float gcrs = fabsf(sd.z * wy - sd.w * wx);
-          const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
-          // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact
-          // gate is skipped), uncertain = within 2e-4 of the threshold or out of the approximation's
-          // range (the exact gate decides, flag bit 15)
-          const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f;
-          const bool keep = gdot > 0.0f && (!(gcrs > lim) || !in_range);
-          const bool sure = in_range && gcrs <= lim * 0.9998f;
-          if (keep) s_q[nq++][threadIdx.x] = (unsigned short)(k | (sure ? 0 : 0x8000));
-        }
-      } else {
-        k = n_seed;
-      }
-      const bool more = __any_sync(kFull, k < n_seed);  // a queue filled up: drain, then go on
-      // ---- phase 1b: exact gate per (seed, anchor); survivors onto the warp's list ----
+    int nq = 0;  // entries in this thread's queue
+    // ---- phase 1b: exact gate per queued (seed, anchor) where needed; survivors onto the warp's list ----
+    auto drain = [&]() {
       const int nq_max = __reduce_max_sync(kFull, nq);
       for (int i = 0; i < nq_max; ++i) {
         bool pass = false;
@@ -378,8 +368,67 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
           __syncwarp();
         }
       }
-      if (!more) break;
+      nq = 0;
+    };
+    // ---- bounding circle of the warp's anchors (sorted by radius class and azimuth: a few cm) ----
+    float bx0 = valid ? A.x : 3e38f, bx1 = valid ? A.x : -3e38f, by0 = valid ? A.y : 3e38f, by1 = valid ? A.y : -3e38f;
+#pragma unroll
+    for (int sh = 16; sh > 0; sh >>= 1) {
+      bx0 = fminf(bx0, __shfl_xor_sync(kFull, bx0, sh));
+      bx1 = fmaxf(bx1, __shfl_xor_sync(kFull, bx1, sh));
+      by0 = fminf(by0, __shfl_xor_sync(kFull, by0, sh));
+      by1 = fmaxf(by1, __shfl_xor_sync(kFull, by1, sh));
     }
+    const bool warp_has = bx0 <= bx1;
+    const float bcx = 0.5f * (bx0 + bx1), bcy = 0.5f * (by0 + by1);
+    const float bh = 0.5f * sqrtf((bx1 - bx0) * (bx1 - bx0) + (by1 - by0) * (by1 - by0)) * 1.001f + 1e-3f;
+    // ---- phase 1, 32 seeds at a time ----
+    for (int kb = 0; kb < n_seed && warp_has; kb += 32) {
+      // (a) one seed per lane against the circle: can its gate accept ANY point within bh of the centre?
+      //     gdot(A) <= v.wc + lv*bh and gcrs(A) >= |v x wc| - lv*bh, glim(A) <= glim at |wc| + bh; margins
+      //     1e-3 cover the rounding of both sides (~1e-6 relative).  Out of range: tested by every lane.
+      bool maybe = false;
+      if (kb + lane < n_seed) {
+        const float4 sd = s_seed[kb + lane];
+        const float lv = s_lv[kb + lane];
+        const float wx = bcx - sd.x, wy = bcy - sd.y;
+        const float lw2 = wx * wx + wy * wy;
+        float rl;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
+        const float Lw = (lw2 * rl + bh) * 1.001f;
+        const float slack = lv * (bh * 1.001f + 1e-4f);
+        const float dotc = sd.z * wx + sd.w * wy;
+        const float crsc = fabsf(sd.z * wy - sd.w * wx);
+        const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f && lv <= 1e30f;
+        maybe = !in_range || (dotc + slack > 0.0f && crsc - slack <= (lv * Lw) * (Lw * inv_2rmin + gate_tol));
+      }
+      unsigned word = __ballot_sync(kFull, maybe);
+      // (b) the seeds that may match: every lane tests its own anchor
+      while (word) {
+        const int k = kb + __ffs(word) - 1;
+        word &= word - 1;
+        if (valid) {
+          const float4 sd = s_seed[k];
+          const float wx = A.x - sd.x, wy = A.y - sd.y;
+          const float gdot = sd.z * wx + sd.w * wy;
+          const float lw2 = wx * wx + wy * wy;
+          float rl;
+          asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
+          const float lw = lw2 * rl;
+          const float gcrs = fabsf(sd.z * wy - sd.w * wx);
+          const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
+          // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact
+          // gate is skipped), uncertain = within 2e-4 of the threshold or out of the approximation's
+          // range (the exact gate decides, flag bit 15)
+          const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f;
+          const bool keep = gdot > 0.0f && (!(gcrs > lim) || !in_range);
+          const bool sure = in_range && gcrs <= lim * 0.9998f;
+          if (keep) s_q[nq++][threadIdx.x] = (unsigned short)(k | (sure ? 0 : 0x8000));
+        }
+        if (__any_sync(kFull, nq >= kQueue)) drain();
+      }
+    }
+    drain();
     __syncwarp();
     if (n1 > 0) expand(n1);
     if (lane < n2) phase2(s_w2[warp][lane]);

@@ -94,7 +94,8 @@ struct Dev {
   float2* t5_lxy;
   // ---- a5: pT3 / pT5 (owner = pLS) ----
   PtEvent* pt_ev;      // [n_events + 1] anchor / seed ranges and first tile of every event
-  int* anc_begin;      // [n_md + 1] anchors before MD A (anchor = MD starting at least one T3)
+  int *anc_bin, *anc_rank;  // [n_md] bin (event * 256 + radial class * 32 + sector, -1 = no anchor) and arrival rank
+  int *anc_bin_cnt, *anc_bin_begin;  // [n_events * 256 + 1] (counts zeroed per batch)
   float2* anc_axy;     // [n_anchor] anchor position
   int2 *anc_t3, *anc_t5;  // [n_anchor] (first, count) of the T3s / T5s starting at the anchor
   int *pls_pt3_cnt, *pls_pt5_cnt;  // [n_pls + 1] accepted per seed (zeroed per batch)
