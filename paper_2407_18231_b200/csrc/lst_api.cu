@@ -400,6 +400,11 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
     ctx_destroy(ctx);
     return LST_ERR_CUDA;
   }
+  if (cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(PtWarp) * kWarps)) !=
+      cudaSuccess) {
+    ctx_destroy(ctx);
+    return LST_ERR_CUDA;
+  }
   *out = ctx;
   return LST_OK;
 }

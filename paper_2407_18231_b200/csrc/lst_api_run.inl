@@ -143,7 +143,7 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   L.mark("pt_tiles");
   k_pt_tiles<<<1, kBlock, 0, st>>>(d);
   L.mark("pt");
-  k_pt_eval<<<g->n_sm * 5, kBlock, 0, st>>>(d);
+  k_pt_eval<<<g->n_sm * 4, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
   L.mark("pt3_scan");
   k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
       d.pls_pt3_cnt, d.pls_pt3_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP3, d.tstate[T_PP3]);

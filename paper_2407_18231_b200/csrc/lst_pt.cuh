@@ -58,7 +58,7 @@ __device__ __forceinline__ void event_cands(const Dev& d, int ev, int& c0, int& 
 }
 
 constexpr int kSeedTile = 128;  // seeds staged per tile; the survivor queues are drained after every tile
-constexpr int kQueue = 48;      // survivor queue entries per thread (drained early when one fills up)
+constexpr int kQueue = 32;      // survivor queue entries per thread (drained early when one fills up)
 
 // ---- anchors: the MDs that start at least one T3 (and therefore every T5) ----------------------
 // The gate of CUTS.md section 7 depends only on the seed and on the FIRST MD of the candidate, and
@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
       event_cands<true>(d, e, c0, c1);
       t5 += (unsigned long long)ns * (c1 - c0);
     }
-    ev.tile0 = ((ev.a1 - ev.a0 + kBlock - 1) / kBlock) * ((ns + kSeedTile - 1) / kSeedTile);
+    ev.tile0 = ((ev.a1 - ev.a0 + 31) / 32) * ((ns + kSeedTile - 1) / kSeedTile);  // warp tiles
     d.pt_ev[e] = ev;
   }
   t3 = warp_sum_u64(t3);
@@ -167,7 +167,11 @@ struct PtAccepted {
   float score;
 };
 
-struct PtWarp {  // per-warp scratch of k_pt_eval
+struct PtWarp {  // per-warp scratch of k_pt_eval (dynamic shared memory: kWarps of these)
+  float4 seed[kSeedTile];  // x1, y1, vx, vy of the tile's seeds
+  float lv[kSeedTile];
+  unsigned short q[kQueue][32];  // [entry][lane]: per-thread survivor queues
+  int2 w2[64];         // phase-2 list: (candidate | T5 flag << 31, seed slot)
   float2 axy[32];      // the warp's anchors
   int2 r3[32], r5[32];  // (first, count) of their T3s / T5s
   unsigned w1[64];     // gate survivors: seed slot | anchor lane << 16 | gate-near << 31
@@ -176,16 +180,16 @@ struct PtWarp {  // per-warp scratch of k_pt_eval
   float kp[32], tolk[32];
 };
 
-// pT3 and pT5 of the whole batch.  Tile = 256 anchors of one event (one per thread) x up to
-// kSeedTile seeds of the same event (shared memory, read as broadcasts).
+// pT3 and pT5 of the whole batch.  A tile = 32 anchors of one event (one per lane) x up to kSeedTile
+// seeds of the same event (shared memory, read as broadcasts).  Warps take tiles by ticket and never
+// wait for one another (with a block-wide tile, a quarter of the warp time was spent at the barrier
+// behind the warp whose anchors matched the most seeds; profiles/).
 __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
-  __shared__ int s_tile, s_ev;
-  __shared__ float4 s_seed[kSeedTile];  // x1, y1, vx, vy
-  __shared__ float s_lv[kSeedTile];
-  __shared__ unsigned short s_q[kQueue][kBlock];  // [entry][thread]: conflict-free per-thread queues
-  __shared__ int2 s_w2[kWarps][64];               // phase-2 list of the warp: (candidate | T5 flag << 31, seed slot)
-  __shared__ PtWarp s_pw[kWarps];
+  extern __shared__ __align__(16) unsigned char s_dyn[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  PtWarp& w = reinterpret_cast<PtWarp*>(s_dyn)[warp];
+  float4* const s_seed = w.seed;
+  float* const s_lv = w.lv;
   const int E = d.n_events;
   const int n_tiles = d.pt_ev[E].tile0;
   const int cap3 = d.cap[K_PT3], cap5 = d.cap[K_PT5];
@@ -194,35 +198,34 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
   const float inv_2rmin = d.cuts.inv_2rmin * 1.0001f, gate_tol = d.cuts.pt_gate_tol * 1.0001f;
   unsigned long long near3 = 0, near5 = 0;
   for (;;) {
-    if (threadIdx.x == 0) {
-      const int tile = atomicAdd(d.ctl->ticket + T_PT3, 1);
-      int lo = 0, hi = E;  // event of the tile: largest e with tile0[e] <= tile
+    int tile = 0, evi = 0;
+    if (lane == 0) {
+      tile = atomicAdd(d.ctl->ticket + T_PT3, 1);
+      int hi = E;  // event of the tile: largest e with tile0[e] <= tile
       if (tile < n_tiles)
-        while (hi - lo > 1) {
-          const int mid = (lo + hi) >> 1;
-          if (d.pt_ev[mid].tile0 <= tile) lo = mid; else hi = mid;
+        while (hi - evi > 1) {
+          const int mid = (evi + hi) >> 1;
+          if (d.pt_ev[mid].tile0 <= tile) evi = mid; else hi = mid;
         }
-      s_tile = tile;
-      s_ev = lo;
     }
-    __syncthreads();
-    const int tile = s_tile;
+    tile = __shfl_sync(kFull, tile, 0);
+    evi = __shfl_sync(kFull, evi, 0);
     if (tile >= n_tiles) break;
-    const PtEvent ev = d.pt_ev[s_ev];
-    const int n_ab = (ev.a1 - ev.a0 + kBlock - 1) / kBlock;
+    const PtEvent ev = d.pt_ev[evi];
+    const int n_ab = (ev.a1 - ev.a0 + 31) / 32;
     const int local = tile - ev.tile0;
     const int sb = local / n_ab, ab = local - sb * n_ab;
     const int p0 = ev.s0 + sb * kSeedTile;
     const int n_seed = min(kSeedTile, ev.s1 - p0);
-    for (int k = threadIdx.x; k < n_seed; k += kBlock) {
+    for (int k = lane; k < n_seed; k += 32) {
       const int p = p0 + k;
       const float x1 = __ldg(d.p_x1 + p), y1 = __ldg(d.p_y1 + p);
       const float vx = x1 - __ldg(d.p_x0 + p), vy = y1 - __ldg(d.p_y0 + p);
       s_seed[k] = make_float4(x1, y1, vx, vy);
       s_lv[k] = sqrtf(vx * vx + vy * vy);
     }
-    __syncthreads();
-    const int anc = ev.a0 + ab * kBlock + threadIdx.x;
+    __syncwarp();
+    const int anc = ev.a0 + ab * 32 + lane;
     const bool valid = anc < ev.a1;
     float2 A = make_float2(0.0f, 0.0f);
     int2 r3 = make_int2(0, 0), r5 = make_int2(0, 0);  // (first, count) of the anchor's T3s / T5s
@@ -253,20 +256,19 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     auto push2 = [&](bool go, int cand, int ks) {
       const unsigned m = __ballot_sync(kFull, go);
       if (m == 0u) return;
-      if (go) s_w2[warp][n2 + __popc(m & ((1u << lane) - 1u))] = make_int2(cand, ks);
+      if (go) w.w2[n2 + __popc(m & ((1u << lane) - 1u))] = make_int2(cand, ks);
       n2 += __popc(m);
       if (n2 >= 32) {
         __syncwarp();
-        phase2(s_w2[warp][lane]);
-        const int2 rest = (32 + lane < n2) ? s_w2[warp][32 + lane] : make_int2(0, 0);
+        phase2(w.w2[lane]);
+        const int2 rest = (32 + lane < n2) ? w.w2[32 + lane] : make_int2(0, 0);
         __syncwarp();
-        s_w2[warp][lane] = rest;
+        w.w2[lane] = rest;
         n2 -= 32;
         __syncwarp();
       }
     };
     // The warp's 32 anchors, readable by every lane (a gate survivor is expanded by whichever lane is free).
-    PtWarp& w = s_pw[warp];
     w.axy[lane] = A;
     w.r3[lane] = r3;
     w.r5[lane] = r5;
@@ -339,7 +341,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
         bool pass = false;
         unsigned ent = 0;
         if (i < nq) {
-          const int qe = s_q[i][threadIdx.x];
+          const int qe = w.q[i][lane];
           const int ks = qe & 0x7fff;
           unsigned r = ACC;
           if (qe & 0x8000) {  // uncertain: the exact gate (CUTS.md section 7) decides and flags near-threshold
@@ -423,7 +425,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
           const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f;
           const bool keep = gdot > 0.0f && (!(gcrs > lim) || !in_range);
           const bool sure = in_range && gcrs <= lim * 0.9998f;
-          if (keep) s_q[nq++][threadIdx.x] = (unsigned short)(k | (sure ? 0 : 0x8000));
+          if (keep) w.q[nq++][lane] = (unsigned short)(k | (sure ? 0 : 0x8000));
         }
         if (__any_sync(kFull, nq >= kQueue)) drain();
       }
@@ -431,8 +433,8 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     drain();
     __syncwarp();
     if (n1 > 0) expand(n1);
-    if (lane < n2) phase2(s_w2[warp][lane]);
-    __syncthreads();  // the seed tile is reused
+    if (lane < n2) phase2(w.w2[lane]);
+    __syncwarp();  // the seed tile is reused
   }
   near3 = warp_sum_u64(near3);
   near5 = warp_sum_u64(near5);
