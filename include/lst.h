@@ -70,15 +70,13 @@ typedef struct lst_caps {
   int32_t max_events;
   int32_t max_hits, max_pls;
   int32_t max_md, max_ls, max_t3, max_t5, max_pt3, max_pt5, max_tc;
-  int32_t max_pairs; /* candidate pairs one stage may test per batch (hit pairs of the MD stage, MD pairs of
-                        the LS stage); sizes the even-split bookkeeping only */
+  int32_t max_pairs; /* hit pairs the MD stage may test per batch; sizes the even-split bookkeeping only */
 } lst_caps;
 
 /* Defaults sized for 16 PU250-like events (a few hundred MB; the B200 has 180 GB). */
 void lst_default_caps(lst_caps* c);
-/* Device bytes a context with these capacities allocates for a geometry of n_modules modules and
- * n_edges connection-map entries. */
-size_t lst_workspace_bytes(const lst_caps* c, int32_t n_modules, int32_t n_edges);
+/* Device bytes a context with these capacities allocates for a geometry of n_modules. */
+size_t lst_workspace_bytes(const lst_caps* c, int32_t n_modules);
 
 /* Outer-tracker hits of a batch, structure of arrays.  x, y, z in cm. */
 typedef struct lst_hits {

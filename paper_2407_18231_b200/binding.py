@@ -113,7 +113,7 @@ def _lib():
     L.lst_default_params.restype = None
     L.lst_default_caps.argtypes = [C.POINTER(lst_caps)]
     L.lst_default_caps.restype = None
-    L.lst_workspace_bytes.argtypes = [C.POINTER(lst_caps), C.c_int32, C.c_int32]
+    L.lst_workspace_bytes.argtypes = [C.POINTER(lst_caps), C.c_int32]
     L.lst_workspace_bytes.restype = C.c_size_t
     L.lst_load_geometry.argtypes = [C.POINTER(lst_module), C.c_int32, _ip, _ip, C.POINTER(lst_params), C.POINTER(vp)]
     L.lst_run_event.argtypes = [vp, C.POINTER(lst_hits), C.POINTER(lst_pls), C.POINTER(C.POINTER(lst_event_out))]
@@ -156,8 +156,8 @@ def lst_default_caps(**overrides) -> lst_caps:
     return c
 
 
-def lst_workspace_bytes(caps: lst_caps | None, n_modules: int, n_edges: int) -> int:
-    return int(_lib().lst_workspace_bytes(C.byref(caps) if caps is not None else None, int(n_modules), int(n_edges)))
+def lst_workspace_bytes(caps: lst_caps | None, n_modules: int) -> int:
+    return int(_lib().lst_workspace_bytes(C.byref(caps) if caps is not None else None, int(n_modules)))
 
 
 def lst_free(handle) -> None:

@@ -32,7 +32,7 @@ constexpr int kMaxKernels = 32;
 struct lst_geometry {
   uint64_t magic;
   int n_mod, n_edges, max_deg;
-  int *d_subdet, *d_conn_off, *d_conn_tgt, *d_conn_src;
+  int *d_subdet, *d_conn_off, *d_conn_tgt;
   lst_params params;
   Cuts cuts;
   lst_ctx* default_ctx;
@@ -160,22 +160,17 @@ extern "C" int lst_load_geometry(const lst_module* modules, int32_t n_modules, c
     delete g;
     return LST_ERR_CUDA;
   }
-  std::vector<int> sub(n_modules), src(n_edges > 0 ? n_edges : 1);
-  for (int m = 0; m < n_modules; ++m) {
-    sub[m] = modules[m].subdet;
-    for (int k = conn_offsets[m]; k < conn_offsets[m + 1]; ++k) src[k] = m;
-  }
+  std::vector<int> sub(n_modules);
+  for (int m = 0; m < n_modules; ++m) sub[m] = modules[m].subdet;
   bool ok = cudaMalloc(&g->d_subdet, sizeof(int) * n_modules) == cudaSuccess &&
             cudaMalloc(&g->d_conn_off, sizeof(int) * (n_modules + 1)) == cudaSuccess &&
-            cudaMalloc(&g->d_conn_tgt, sizeof(int) * (n_edges > 0 ? n_edges : 1)) == cudaSuccess &&
-            cudaMalloc(&g->d_conn_src, sizeof(int) * (n_edges > 0 ? n_edges : 1)) == cudaSuccess;
+            cudaMalloc(&g->d_conn_tgt, sizeof(int) * (n_edges > 0 ? n_edges : 1)) == cudaSuccess;
   ok = ok && cudaMemcpy(g->d_subdet, sub.data(), sizeof(int) * n_modules, cudaMemcpyHostToDevice) == cudaSuccess;
   ok = ok && cudaMemcpy(g->d_conn_off, conn_offsets, sizeof(int) * (n_modules + 1), cudaMemcpyHostToDevice) == cudaSuccess;
   if (ok && n_edges > 0)
-    ok = cudaMemcpy(g->d_conn_tgt, conn_targets, sizeof(int) * n_edges, cudaMemcpyHostToDevice) == cudaSuccess &&
-         cudaMemcpy(g->d_conn_src, src.data(), sizeof(int) * n_edges, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = cudaMemcpy(g->d_conn_tgt, conn_targets, sizeof(int) * n_edges, cudaMemcpyHostToDevice) == cudaSuccess;
   if (!ok) {
-    cudaFree(g->d_subdet);  cudaFree(g->d_conn_off);  cudaFree(g->d_conn_tgt);  cudaFree(g->d_conn_src);
+    cudaFree(g->d_subdet);  cudaFree(g->d_conn_off);  cudaFree(g->d_conn_tgt);
     delete g;
     return LST_ERR_CUDA;
   }
@@ -202,17 +197,15 @@ inline int tiles_of(long long n, int tile) { return (int)((n + tile - 1) / tile)
 
 // Fills the pointer table of `dev` (pointers are offsets from `base`; base == nullptr only sizes).
 // Returns total bytes; *zero_bytes = size of the leading region that is memset per batch.
-size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst_ctx* ctx, size_t* zero_bytes) {
+size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, size_t* zero_bytes) {
   Bump b{base, 0};
   const long long n_sens = (long long)c.max_events * 2 * n_mod;
   // --- zeroed per batch ---
   d.ctl = b.take<Ctl>(1);
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
-  const long long n_einst = (long long)c.max_events * n_edges;
   d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kPlaceChunks));
   d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kScanTile));
   d.tstate[T_PMD] = b.take<unsigned long long>(tiles_of(n_sens / 2 + 1, kScanTile));
-  d.tstate[T_PLS] = b.take<unsigned long long>(tiles_of(n_einst + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
   d.tstate[T_T5] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
   d.tstate[T_PT3] = nullptr;  // ticket only
@@ -251,7 +244,6 @@ size_t layout(const lst_caps& c, int n_mod, int n_edges, char* base, Dev& d, lst
   }
   d.pp_md = b.take<int>(n_sens / 2 + 1);
   d.mod_md_begin = b.take<int>(n_sens / 2 + 1);
-  d.ppe_ls = b.take<int>(n_einst + 1);
   d.md_hit = b.take<int2>(c.max_md);
   d.md_info = b.take<int>(c.max_md);
   d.md_a = b.take<float4>(c.max_md);
@@ -333,12 +325,12 @@ bool caps_ok(const lst_caps& c) {
 
 }  // namespace
 
-extern "C" size_t lst_workspace_bytes(const lst_caps* caps, int32_t n_modules, int32_t n_edges) {
+extern "C" size_t lst_workspace_bytes(const lst_caps* caps, int32_t n_modules) {
   lst_caps c;
   if (caps) c = *caps; else lst_default_caps(&c);
-  if (!caps_ok(c) || n_modules <= 0 || n_edges < 0) return 0;
+  if (!caps_ok(c) || n_modules <= 0) return 0;
   Dev d;
-  return layout(c, n_modules, n_edges, nullptr, d, nullptr, nullptr);
+  return layout(c, n_modules, nullptr, d, nullptr, nullptr);
 }
 
 static void ctx_destroy(lst_ctx* ctx) {
@@ -360,7 +352,6 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   if (caps) c = *caps; else lst_default_caps(&c);
   if (!caps_ok(c)) return LST_ERR_ARG;
   if ((long long)c.max_events * 2 * g->n_mod + 1 > 0x7fffffffLL) return LST_ERR_ARG;
-  if ((long long)c.max_events * g->n_edges + 1 > 0x7fffffffLL) return LST_ERR_ARG;
   lst_ctx* ctx = new (std::nothrow) lst_ctx();
   if (!ctx) return LST_ERR_CUDA;
   ctx->magic = MAGIC_CTX;
@@ -375,7 +366,7 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   ctx->last_n_events = 0;
   ctx->synced = true;
   Dev probe;
-  ctx->bytes = layout(c, g->n_mod, g->n_edges, nullptr, probe, nullptr, nullptr);
+  ctx->bytes = layout(c, g->n_mod, nullptr, probe, nullptr, nullptr);
   char* base = nullptr;
   if (cudaMalloc(&base, ctx->bytes) != cudaSuccess) {
     cudaGetLastError();
@@ -384,14 +375,12 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   }
   ctx->allocs.push_back(base);
   memset(&ctx->dev, 0, sizeof(Dev));
-  layout(c, g->n_mod, g->n_edges, base, ctx->dev, ctx, &ctx->zero_bytes);
+  layout(c, g->n_mod, base, ctx->dev, ctx, &ctx->zero_bytes);
   ctx->zero_region = base;
   ctx->dev.n_mod = g->n_mod;
   ctx->dev.subdet = g->d_subdet;
   ctx->dev.conn_off = g->d_conn_off;
   ctx->dev.conn_tgt = g->d_conn_tgt;
-  ctx->dev.conn_src = g->d_conn_src;
-  ctx->dev.n_edges = g->n_edges;
   ctx->dev.cuts = g->cuts;
   bool ok = cudaMallocHost(&ctx->h_ctl, sizeof(Ctl)) == cudaSuccess &&
             cudaMallocHost(&ctx->h_ev_first, sizeof(int) * (K_PT5 + 1) * (c.max_events + 1)) == cudaSuccess;

@@ -173,7 +173,7 @@ extern "C" void lst_free(void* p) {
   } else if (magic == MAGIC_GEOM) {
     lst_geometry* g = static_cast<lst_geometry*>(p);
     if (g->default_ctx) ctx_destroy(g->default_ctx);
-    cudaFree(g->d_subdet);  cudaFree(g->d_conn_off);  cudaFree(g->d_conn_tgt);  cudaFree(g->d_conn_src);
+    cudaFree(g->d_subdet);  cudaFree(g->d_conn_off);  cudaFree(g->d_conn_tgt);
     g->magic = 0;
     delete g;
   }

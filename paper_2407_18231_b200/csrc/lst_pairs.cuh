@@ -1,8 +1,9 @@
-// lst_pairs.cuh -- the evenly split candidate-pair engine of the MD and LS stages.
+// lst_pairs.cuh -- the evenly split candidate-pair engine (used by the MD stage).
 //
 // A stage is "group -> (owners x candidates) -> accepted subset": for Mini-Doublets the group is a
-// module of one event (upper hits x lower hits), for Line Segments a module (its MDs x the MDs of
-// the modules its connection-map row lists).  Pair counts per group differ by 100x (a layer-1
+// module of one event (upper hits x lower hits).  (Line Segments used this engine too until their
+// tiny lists made the pair decoding dearer than the cuts; see lst_ls.cuh.)  Pair counts per group
+// differ by 100x (a layer-1
 // barrel module holds ~1000 hit pairs, an outer endcap module a handful), so neither
 // thread-per-owner nor warp-per-group keeps the machine busy (profiles/r01_v1_first_path.md: 10 of
 // 32 lanes active; r01 notes: warp-per-module stalls the look-back chain behind hot modules).
@@ -90,7 +91,7 @@ __device__ __forceinline__ void split_pair(int p, int n_c, int& o, int& j) {
 }
 
 
-// Stage concept (StageMD / StageLS in lst_stages.cuh):
+// Stage concept (StageMD in lst_stages.cuh):
 //   static constexpr int kTicket, kKind, kErr, kStage, kPairSlot;
 //   struct Group { int gbase, gend, n_c; ... };  struct Payload;
 //   int  n_groups() const;

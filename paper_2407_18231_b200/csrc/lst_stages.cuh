@@ -126,107 +126,7 @@ struct StageMD {
   __device__ void finish_total(int) const {}
 };
 
-// ---- a2: Line Segments (CUTS.md section 4).  group = module gm of one event;
-// owners = its MDs A, candidates = the MDs of the modules in conn[module], concatenated in the
-// order of the CSR row (row length NB).  The pre-pass scans n_MD(source) x n_MD(target) over the
-// edges of all events, so the prefix array ppe_ls is at once the pair prefix of the modules (at a
-// row's first edge) and, divided by n_MD(source), the map candidate j -> (edge, B) inside a row.
-// LSs come out grouped by inner MD, inside an MD by (edge, B).
-struct PairsLS {
-  const Dev& d;
-  __device__ explicit PairsLS(const Dev& dd) : d(dd) {}
-  __device__ int n_items() const {
-    return ((d.cuts.stage_mask & 2) && d.ctl->total[K_MD] > 0) ? d.n_events * d.n_edges : 0;
-  }
-  __device__ int count(int i) const {
-    const int ev = i / d.n_edges, k = i - ev * d.n_edges;
-    const int gs = ev * d.n_mod + __ldg(d.conn_src + k);
-    const int n_o = d.mod_md_begin[gs + 1] - d.mod_md_begin[gs];
-    if (n_o == 0) return 0;
-    const int gt = ev * d.n_mod + __ldg(d.conn_tgt + k);
-    const long long p = (long long)n_o * (d.mod_md_begin[gt + 1] - d.mod_md_begin[gt]);
-    if (p > d.cap_pairs) {
-      atomicOr(&d.ctl->error, E_CAP_LS);
-      return 0;
-    }
-    return (int)p;
-  }
-  __device__ int group(int i) const {
-    const int ev = i / d.n_edges;
-    return ev * d.n_mod + __ldg(d.conn_src + (i - ev * d.n_edges));
-  }
-};
-
-struct StageLS {
-  static constexpr int kTicket = T_LS, kKind = K_LS, kErr = E_CAP_LS, kStage = 1, kPairSlot = 1;
-  struct Group {
-    int gbase, gend, n_c;
-    int n_o, A0;
-    int eb, k0, deg;  // eb = event * n_edges + k0: the row's first entry of ppe_ls
-    int gm_base;      // event * n_mod
-  };
-  struct Payload {
-    int A, B;
-    float kappa;
-  };
-  const Dev& d;
-  __device__ explicit StageLS(const Dev& dd) : d(dd) {}
-  __device__ bool enabled() const { return (d.cuts.stage_mask & 2) && d.ctl->total[K_MD] > 0; }
-  __device__ int n_groups() const { return enabled() ? d.n_events * d.n_mod : 0; }
-  __device__ int pp(int g) const {
-    const int ev = g / d.n_mod;
-    return d.ppe_ls[ev * d.n_edges + __ldg(d.conn_off + (g - ev * d.n_mod))];
-  }
-  __device__ void load_group(int gm, Group& G) const {
-    const int ev = gm / d.n_mod, m = gm - ev * d.n_mod;
-    G.A0 = d.mod_md_begin[gm];
-    G.n_o = d.mod_md_begin[gm + 1] - G.A0;
-    G.n_c = (G.gend - G.gbase) / G.n_o;  // a group reached through a pair has owners
-    G.k0 = __ldg(d.conn_off + m);
-    G.deg = __ldg(d.conn_off + m + 1) - G.k0;
-    G.eb = ev * d.n_edges + G.k0;
-    G.gm_base = ev * d.n_mod;
-  }
-  __device__ unsigned test(const Group& G, int o, int j, Payload& pay) const {
-    const int target = j * G.n_o;  // < pairs of the group
-    int lo = 0, hi = G.deg;        // largest edge e with (ppe[eb + e] - gbase) <= j * n_o
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (d.ppe_ls[G.eb + mid] - G.gbase <= target) lo = mid; else hi = mid;
-    }
-    const int m2 = __ldg(d.conn_tgt + G.k0 + lo);
-    const int before = (d.ppe_ls[G.eb + lo] - G.gbase) / G.n_o;  // candidates of the row before edge lo
-    pay.A = G.A0 + o;
-    pay.B = d.mod_md_begin[G.gm_base + m2] + (j - before);
-    return ls_test(d.cuts, d.md_a[pay.A], d.md_u[pay.A], d.md_info[pay.A] & 1, d.md_a[pay.B], d.md_u[pay.B],
-                   __ldg(d.subdet + m2) != 0, pay.kappa);
-  }
-  __device__ void emit(int pos, const Payload& pay) const {
-    d.ls_md[pos] = make_int2(pay.A, pay.B);
-    d.ls_kappa[pos] = pay.kappa;
-  }
-  // first LS of every MD A: rank of A's first pair x_A = pp(module) + (A - A0) * NB
-  template <class R>
-  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int ts, int te, const R& rank) const {
-    const int n_md = d.ctl->total[K_MD];
-    if (no_pairs) {
-      if (enabled())
-        for (int A = threadIdx.x; A < n_md; A += kBlock) d.md_ls_begin[A] = 0;
-      return;
-    }
-    const int n = d.n_events * d.n_mod;
-    const int A_lo = tile == 0 ? 0 : d.mod_md_begin[g_lo];
-    const int A_hi = g_hi >= n ? n_md : d.mod_md_begin[g_hi + 1];
-    for (int A = A_lo + threadIdx.x; A < A_hi; A += kBlock) {
-      const int gm = d.md_info[A] >> 1;
-      const int A0 = d.mod_md_begin[gm], n_o = d.mod_md_begin[gm + 1] - A0;
-      const int base = pp(gm);
-      const int x = base + (A - A0) * ((pp(gm + 1) - base) / n_o);
-      if ((x > ts && x <= te) || (tile == 0 && x == 0)) d.md_ls_begin[A] = rank(x);
-    }
-  }
-  __device__ void finish_total(int total) const { d.md_ls_begin[d.ctl->total[K_MD]] = total; }
-};
+// ---- a2: Line Segments: lst_ls.cuh ----
 
 // ---- a3: T3 (CUTS.md section 5).  owner = LS (A->B); candidates = the LSs whose inner MD is B.
 struct StageT3 {

@@ -15,7 +15,7 @@ namespace lst {
 struct PtEvent;  // lst_pt.cuh
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PLS, T_PP3, T_PP5, T_ANC, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PP3, T_PP5, T_ANC, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
@@ -28,7 +28,7 @@ struct Ctl {
   int pad;
   unsigned long long near[6];
   unsigned long long n_tests[6];
-  unsigned long long pair_total[2];  // candidate pairs of the batch: 0 MD, 1 LS (lst_pairs.cuh)
+  unsigned long long pair_total[2];  // candidate pairs of the batch: [0] MD (lst_pairs.cuh)
   int scratch_cur[4];                // accepted objects in the scratch list: 0 MD, 1 LS, 2 pT3, 3 pT5
 };
 
@@ -38,8 +38,6 @@ struct Dev {
   const int* subdet;    // [n_mod]
   const int* conn_off;  // [n_mod + 1]
   const int* conn_tgt;
-  const int* conn_src;  // [n_edges] source module of every CSR entry
-  int n_edges;
   // ---- batch ----
   int n_events, n_hits, n_pls;
   const int* hit_ev_off;  // [n_events + 1] device copy of the event offsets
@@ -73,7 +71,6 @@ struct Dev {
   float4* md_a;       // anchor = lower hit (x, y, z, r)
   float2* md_u;       // unit direction (barrel), 0 (endcap)
   // ---- a2: LS (owner = inner MD) ----
-  int* ppe_ls;       // [n_events * n_edges + 1] exclusive prefix of n_MD(source) * n_MD(target) over edges
   int* md_ls_begin;  // [n_md + 1]
   int *ls_cnt, *ls_sbase;  // [n_md] LSs of an inner MD and their position in the scratch list
   int2* ls_md;       // (md_in, md_out) batch-global MD indices

@@ -66,11 +66,11 @@ def test_strerror_and_caps(lst):
     assert len(set(msgs.values())) == 6
     caps = lst.lst_default_caps()
     assert caps.max_events == 16 and caps.max_hits >= 16 * 150_000 and caps.max_pairs >= 1 << 27
-    b1 = lst.lst_workspace_bytes(caps, 9512, 72887)
-    b2 = lst.lst_workspace_bytes(lst.lst_default_caps(max_events=32), 9512, 72887)
+    b1 = lst.lst_workspace_bytes(caps, 9512)
+    b2 = lst.lst_workspace_bytes(lst.lst_default_caps(max_events=32), 9512)
     assert 0 < b1 < b2 < 8 << 30  # a few hundred MB of the B200's 180 GB
-    assert lst.lst_workspace_bytes(lst.lst_default_caps(max_md=0), 9512, 72887) == 0
-    assert lst.lst_workspace_bytes(caps, 0, 0) == 0
+    assert lst.lst_workspace_bytes(lst.lst_default_caps(max_md=0), 9512) == 0
+    assert lst.lst_workspace_bytes(caps, 0) == 0
 
 
 def test_argument_errors_are_reported_before_any_cuda_call(lst):
