@@ -8,8 +8,8 @@
 // module boundary almost every time.  Here the unit is the list:
 //   * a warp takes 8 consecutive inner MDs and builds, once, the table of their (MD, target) lists
 //     in shared memory (first candidate, length prefix): the CSR walk is done once per list;
-//   * the ~180 candidate pairs of the 8 MDs are then taken 32 at a time (pair -> list by bisection
-//     of the small shared-memory prefix, inner-MD operands from shared memory), so lanes stay busy
+//   * the ~180 candidate pairs of the 8 MDs are then taken 32 at a time (pair -> list through a
+//     bit mask of list starts, inner-MD operands from shared memory), so lanes stay busy
 //     whatever the list lengths; accepted (B, kappa) pairs are compacted in pair order with one
 //     ballot per step and copied to a scratch list with one atomic per warp pass (a pass with more
 //     than kLsStage LSs evaluates its pairs again and writes directly);
@@ -24,6 +24,7 @@ namespace lst {
 constexpr int kLsOwners = 8;    // inner MDs per warp
 constexpr int kLsRanges = 256;  // (MD, target) lists per warp pass; also the longest row supported
 constexpr int kLsStage = 96;    // staged LSs per warp pass
+constexpr int kLsHeadWords = 64;
 
 struct LsAccepted {
   int B;
@@ -40,6 +41,7 @@ struct LsWarp {  // per-warp scratch in shared memory
   int gb[kLsOwners];       // event * n_mod
   int pref[kLsRanges + 1];  // exclusive prefix of the list lengths
   int b0[kLsRanges];        // first MD of the list | endcap(target) << 27 | owner slot << 28
+  unsigned heads[kLsHeadWords];  // bit p set = a list starts at pair p (pairs below 32 * kLsHeadWords)
   LsAccepted stage[kLsStage];
 };
 
@@ -84,11 +86,13 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
       const int last = first + take;  // exclusive
       const int R = w.dex[last] - d_first;
       if (lane < kLsOwners) w.cnt[lane] = 0;
-      // ---- range table: list r = (owner, target e) ----
-      int carry = 0;
+      // ---- table of the non-empty lists (owner, target e) in row order, and their head bits ----
+      for (int k = lane; k < kLsHeadWords; k += 32) w.heads[k] = 0u;
+      __syncwarp();
+      int carry = 0, Rn = 0;
       for (int r0 = 0; r0 < R; r0 += 32) {
         const int r = r0 + lane;
-        int n_t = 0;
+        int n_t = 0, ent = 0;
         if (r < R) {
           int o = first;  // owner slot of list r: last o with (dex[o] - d_first) <= r
           for (int k = first + 1; k < last; ++k)
@@ -98,30 +102,46 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
           const int gb = w.gb[o];
           const int B0 = d.mod_md_begin[gb + m2];
           n_t = d.mod_md_begin[gb + m2 + 1] - B0;
-          w.b0[r] = B0 | ((__ldg(d.subdet + m2) != 0) << 27) | (o << 28);
+          ent = B0 | ((__ldg(d.subdet + m2) != 0) << 27) | (o << 28);
         }
         const int incl = warp_incl_scan(n_t);
-        if (r < R) w.pref[r] = carry + incl - n_t;
+        const unsigned nz = __ballot_sync(kFull, n_t > 0);
+        if (n_t > 0) {
+          const int idx = Rn + __popc(nz & ((1u << lane) - 1u));
+          const int start = carry + incl - n_t;
+          w.pref[idx] = start;
+          w.b0[idx] = ent;
+          if (start < 32 * kLsHeadWords) atomicOr(&w.heads[start >> 5], 1u << (start & 31));
+        }
+        Rn += __popc(nz);
         carry += __shfl_sync(kFull, incl, 31);
       }
       const int P = carry;
-      if (lane == 0) w.pref[R] = P;
+      if (lane == 0) w.pref[Rn] = P;
       __syncwarp();
       tests += lane == 0 ? (unsigned long long)P : 0ull;
       // ---- pairs of the pass, 32 at a time; pass 1 only if the stage overflowed ----
       int base = 0, run = 0;
       for (int pass = 0; pass < 2; ++pass) {
         run = 0;
+        int heads_before = 0;
         for (int p0 = 0; p0 < P; p0 += 32) {
           const int p = p0 + lane;
           unsigned res = 0;
           LsAccepted acc;
           int o = 0;
+          const unsigned hw = p0 < 32 * kLsHeadWords ? w.heads[p0 >> 5] : 0u;
           if (p < P) {
-            int lo = 0, hi = R;  // list of pair p: largest r with pref[r] <= p
-            while (hi - lo > 1) {
-              const int mid = (lo + hi) >> 1;
-              if (w.pref[mid] <= p) lo = mid; else hi = mid;
+            int lo;  // list of pair p: the last list starting at or before p
+            if (p0 < 32 * kLsHeadWords) {
+              lo = heads_before + __popc(hw & (0xffffffffu >> (31 - lane))) - 1;
+            } else {
+              lo = 0;
+              int hi = Rn;
+              while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (w.pref[mid] <= p) lo = mid; else hi = mid;
+              }
             }
             const int ent = w.b0[lo];
             o = (unsigned)ent >> 28;
@@ -140,6 +160,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
             }
           }
           run += __popc(m);
+          heads_before += __popc(hw);
         }
         if (pass == 1) break;
         // ---- one atomic for the pass; per-MD count and scratch position ----
