@@ -62,6 +62,7 @@ struct lst_ctx {
   std::vector<int> last_hit_off, last_pls_off;
   int last_n_events;
   bool synced;
+  int grid_md, grid_ls, grid_pt;  // resident blocks of the three heavy kernels (occupancy x SMs)
   // timing
   bool timing;
   cudaEvent_t ev[kMaxKernels + 1];
@@ -389,11 +390,20 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
     ctx_destroy(ctx);
     return LST_ERR_CUDA;
   }
-  if (cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(PtWarp) * kWarps)) !=
-      cudaSuccess) {
+  // grid-stride kernels are launched with exactly the blocks that fit the GPU at once
+  int occ_md = 0, occ_ls = 0, occ_pt = 0;
+  const size_t pt_smem = sizeof(PtWarp) * kWarps;
+  if (cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_md, k_eval<StageMD>, kBlock, 0) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_ls, k_ls_eval, kBlock, 0) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pt, k_pt_eval, kBlock, pt_smem) != cudaSuccess ||
+      occ_md < 1 || occ_ls < 1 || occ_pt < 1) {
     ctx_destroy(ctx);
     return LST_ERR_CUDA;
   }
+  ctx->grid_md = g->n_sm * occ_md;
+  ctx->grid_ls = g->n_sm * occ_ls;
+  ctx->grid_pt = g->n_sm * occ_pt;
   *out = ctx;
   return LST_OK;
 }

@@ -120,11 +120,11 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   L.mark("md_pairs");
   k_scan_f<PairsMD><<<gp, kBlock, 0, st>>>(d, d.pp_md, d.ev_cg0, &d.ctl->pair_total[0], T_PMD);
   L.mark("md");
-  k_eval<StageMD><<<g->n_sm * 6, kBlock, 0, st>>>(d);
+  k_eval<StageMD><<<ctx->grid_md, kBlock, 0, st>>>(d);
   L.mark("md_place");
   k_place<StageMD><<<gp, kBlock, 0, st>>>(d);
   L.mark("ls");
-  k_ls_eval<<<g->n_sm * 8, kBlock, 0, st>>>(d);
+  k_ls_eval<<<ctx->grid_ls, kBlock, 0, st>>>(d);
   L.mark("ls_scan");
   k_scan<<<gp, kBlock, 0, st>>>(d.ls_cnt, d.md_ls_begin, d.ctl->total + K_MD, 1, 0, d.ctl->ticket + T_LS, d.tstate[T_LS]);
   L.mark("ls_place");
@@ -143,7 +143,7 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   L.mark("pt_tiles");
   k_pt_tiles<<<1, kBlock, 0, st>>>(d);
   L.mark("pt");
-  k_pt_eval<<<g->n_sm * 4, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
+  k_pt_eval<<<ctx->grid_pt, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
   L.mark("pt3_scan");
   k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
       d.pls_pt3_cnt, d.pls_pt3_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP3, d.tstate[T_PP3]);

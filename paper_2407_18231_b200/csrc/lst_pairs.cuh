@@ -77,14 +77,15 @@ __global__ void __launch_bounds__(kBlock) k_scan_f(Dev d, int* __restrict__ out,
   }
 }
 
-// p = o * n_c + j with 0 <= j < n_c (float reciprocal + integer fix-up below 2^24)
-__device__ __forceinline__ void split_pair(int p, int n_c, int& o, int& j) {
+// p = o * n_c + j with 0 <= j < n_c.  inv_nc ~ 1 / n_c (computed once per group); the float quotient
+// is off by at most one below 2^24, which the integer fix-up repairs.
+__device__ __forceinline__ void split_pair(int p, int n_c, float inv_nc, int& o, int& j) {
   if (p >= (1 << 24)) {
     o = p / n_c;
     j = p - o * n_c;
     return;
   }
-  o = __float2int_rz(__fdividef(__int2float_rn(p), __int2float_rn(n_c)));
+  o = __float2int_rz(__int2float_rn(p) * inv_nc);
   j = p - o * n_c;
   if (j < 0) { --o; j += n_c; }
   if (j >= n_c) { ++o; j -= n_c; }
@@ -93,7 +94,7 @@ __device__ __forceinline__ void split_pair(int p, int n_c, int& o, int& j) {
 
 // Stage concept (StageMD in lst_stages.cuh):
 //   static constexpr int kTicket, kKind, kErr, kStage, kPairSlot;
-//   struct Group { int gbase, gend, n_c; ... };  struct Payload;
+//   struct Group { int gbase, gend, n_c; float inv_nc; ... };  struct Payload;
 //   int  n_groups() const;
 //   int  pp(int g) const;                         // exclusive pair prefix of group g, g in [0, n]
 //   void load_group(int g, Group&) const;         // per lane: row length n_c and what test() needs
@@ -158,7 +159,7 @@ __global__ void __launch_bounds__(kBlock) k_eval(Dev d) {
           st.load_group(g, G);
         }
         int o, j;
-        split_pair(q - G.gbase, G.n_c, o, j);
+        split_pair(q - G.gbase, G.n_c, G.inv_nc, o, j);
         r = st.test(G, o, j, pay);
       }
       near += (r >> 1) & 1u;

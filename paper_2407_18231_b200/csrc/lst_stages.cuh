@@ -82,6 +82,7 @@ struct StageMD {
   static constexpr int kTicket = T_MD, kKind = K_MD, kErr = E_CAP_MD, kStage = 0, kPairSlot = 0;
   struct Group {
     int gbase, gend, n_c;
+    float inv_nc;
     int a0, b0;  // first lower / first upper sorted hit
     int endcap;
   };
@@ -97,6 +98,7 @@ struct StageMD {
     G.a0 = __ldg(d.sens_begin + 2 * gm);
     G.b0 = __ldg(d.sens_begin + 2 * gm + 1);
     G.n_c = G.b0 - G.a0;
+    G.inv_nc = __frcp_rn(__int2float_rn(G.n_c));
     const int ev = gm / d.n_mod;
     G.endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
   }
