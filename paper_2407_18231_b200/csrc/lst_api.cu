@@ -229,8 +229,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.hit_rank = b.take<int>(c.max_hits);
   d.sens_begin = b.take<int>(n_sens + 1);
   d.hit = b.take<float4>(c.max_hits);
-  d.hit_idx = b.take<int>(c.max_hits);
-  d.hit_gs = b.take<int>(c.max_hits);
+  d.hit_ig = b.take<int2>(c.max_hits);
   // --- a1..a4 ---
   d.ev_cg0 = b.take<int>(c.max_pairs / kChunk + 2);
   d.ev_cnt = b.take<int2>(c.max_pairs / kChunk + 1);

@@ -93,7 +93,7 @@ k_scan(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int 
   }
 }
 
-// a0.3 scatter: sorted SoA (float4 x,y,z,r + input index + global sensor), r = sqrtf(x*x + y*y)
+// a0.3 scatter: sorted SoA (float4 x,y,z,r + int2 input index, global sensor), r = sqrtf(x*x + y*y)
 __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
@@ -118,8 +118,7 @@ __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
       if (i < d.n_hits) {
         d.hit[pos[u]] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
         const int ev = gs[u] / n_sens;
-        d.hit_idx[pos[u]] = i - __ldg(d.hit_ev_off + ev);
-        d.hit_gs[pos[u]] = gs[u];
+        d.hit_ig[pos[u]] = make_int2(i - __ldg(d.hit_ev_off + ev), gs[u]);
       }
     }
   }

@@ -108,9 +108,10 @@ struct StageMD {
     return md_test(d.cuts, G.endcap, d.hit[pay.a], d.hit[pay.b], pay.ux, pay.uy);
   }
   __device__ void emit(int pos, const Payload& pay) const {
-    const int gs = d.hit_gs[pay.a];  // lower sensor: gs = 2 * gm
+    const int2 ia = d.hit_ig[pay.a];
+    const int gs = ia.y;  // lower sensor: gs = 2 * gm
     const int ev = (gs >> 1) / d.n_mod;
-    d.md_hit[pos] = make_int2(d.hit_idx[pay.a], d.hit_idx[pay.b]);
+    d.md_hit[pos] = make_int2(ia.x, d.hit_ig[pay.b].x);
     d.md_info[pos] = gs | (__ldg(d.subdet + ((gs >> 1) - ev * d.n_mod)) != 0);
     d.md_a[pos] = d.hit[pay.a];
     d.md_u[pos] = make_float2(pay.ux, pay.uy);

@@ -55,8 +55,7 @@ struct Dev {
   int* sens_cnt;     // [n_events * 2 * n_mod + 1]
   int* sens_begin;   // [n_events * 2 * n_mod + 1] exclusive scan of sens_cnt
   float4* hit;       // [n_hits] sorted (x, y, z, r)
-  int* hit_idx;      // [n_hits] event-local input index of the sorted hit
-  int* hit_gs;       // [n_hits] global sensor of the sorted hit
+  int2* hit_ig;      // [n_hits] (event-local input index, global sensor) of the sorted hit
   // ---- even-split bookkeeping, shared by the MD and LS stages (lst_pairs.cuh) ----
   int* ev_cg0;          // [cap_pairs / kChunk + 2] group holding the first pair of every chunk
   int2* ev_cnt;         // [cap_pairs / kChunk + 1] (accepted pairs, scratch position) of every chunk
