@@ -70,7 +70,6 @@ typedef struct lst_caps {
   int32_t max_events;
   int32_t max_hits, max_pls;
   int32_t max_md, max_ls, max_t3, max_t5, max_pt3, max_pt5, max_tc;
-  int32_t max_pairs; /* hit pairs the MD stage may test per batch; sizes the even-split bookkeeping only */
 } lst_caps;
 
 /* Defaults sized for 16 PU250-like events (a few hundred MB; the B200 has 180 GB). */

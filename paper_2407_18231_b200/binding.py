@@ -48,7 +48,7 @@ class lst_params(C.Structure):
 
 class lst_caps(C.Structure):
     _fields_ = [(f, C.c_int32) for f in ("max_events", "max_hits", "max_pls", "max_md", "max_ls", "max_t3",
-                                          "max_t5", "max_pt3", "max_pt5", "max_tc", "max_pairs")]
+                                          "max_t5", "max_pt3", "max_pt5", "max_tc")]
 
 
 class lst_hits(C.Structure):

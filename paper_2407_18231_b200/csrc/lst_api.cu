@@ -105,7 +105,6 @@ extern "C" void lst_default_caps(lst_caps* c) {
   c->max_pt3 = 1 << 20;
   c->max_pt5 = 1 << 20;
   c->max_tc = 256 << 10;
-  c->max_pairs = 256 << 20;
 }
 
 static Cuts make_cuts(const lst_params& p) {  // CUTS.md section 1, derived constants in binary32
@@ -204,9 +203,8 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   // --- zeroed per batch ---
   d.ctl = b.take<Ctl>(1);
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
-  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of(c.max_pairs / kChunk + 1, kPlaceChunks));
+  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of((long long)c.max_hits + 1, kScanTile));
   d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kScanTile));
-  d.tstate[T_PMD] = b.take<unsigned long long>(tiles_of(n_sens / 2 + 1, kScanTile));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
   d.tstate[T_T5] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
   d.tstate[T_PT3] = nullptr;  // ticket only
@@ -231,18 +229,16 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.hit = b.take<float4>(c.max_hits);
   d.hit_ig = b.take<int2>(c.max_hits);
   // --- a1..a4 ---
-  d.ev_cg0 = b.take<int>(c.max_pairs / kChunk + 2);
-  d.ev_cnt = b.take<int2>(c.max_pairs / kChunk + 1);
-  d.ev_mask = b.take<unsigned>(c.max_pairs / 32 + 8);
   {
-    size_t sz = sizeof(StageMD::Payload) * (size_t)c.max_md;
-    const size_t others[3] = {sizeof(LsAccepted) * (size_t)c.max_ls, sizeof(PtAccepted) * (size_t)c.max_pt3,
-                              sizeof(PtAccepted) * (size_t)c.max_pt5};
-    for (size_t o : others) sz = o > sz ? o : sz;
+    size_t sz = sizeof(LsAccepted) * (size_t)c.max_ls;
+    const size_t other = sizeof(PtAccepted) * (size_t)c.max_pt3;
+    sz = other > sz ? other : sz;
     d.ev_scratch = b.take<char>(sz);
     d.ev_scratch2 = b.take<char>(sizeof(PtAccepted) * (size_t)c.max_pt5);
   }
-  d.pp_md = b.take<int>(n_sens / 2 + 1);
+  d.md_cnt = b.take<int>(c.max_hits);
+  d.md_stash = b.take<int>(4 * (size_t)c.max_hits);
+  d.hit_md_begin = b.take<int>((size_t)c.max_hits + 1);
   d.mod_md_begin = b.take<int>(n_sens / 2 + 1);
   d.md_hit = b.take<int2>(c.max_md);
   d.md_info = b.take<int>(c.max_md);
@@ -313,14 +309,13 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
     ctx->d_hit_ev_off = ho;  ctx->d_pls_ev_off = po;  ctx->d_ev_first = ef;
   }
   d.cap[K_MD] = c.max_md;  d.cap[K_LS] = c.max_ls;  d.cap[K_T3] = c.max_t3;  d.cap[K_T5] = c.max_t5;
-  d.cap_pairs = c.max_pairs;
   d.cap[K_PT3] = c.max_pt3;  d.cap[K_PT5] = c.max_pt5;  d.cap[K_TC] = c.max_tc;
   return (b.off + 255) & ~size_t(255);
 }
 
 bool caps_ok(const lst_caps& c) {
   return c.max_events > 0 && c.max_hits > 0 && c.max_pls > 0 && c.max_md > 0 && c.max_ls > 0 && c.max_t3 > 0 &&
-         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_pairs > 0;
+         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0;
 }
 
 }  // namespace
@@ -393,7 +388,7 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   int occ_md = 0, occ_ls = 0, occ_pt = 0;
   const size_t pt_smem = sizeof(PtWarp) * kWarps;
   if (cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem) != cudaSuccess ||
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_md, k_eval<StageMD>, kBlock, 0) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_md, k_md_eval, kBlock, 0) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_ls, k_ls_eval, kBlock, 0) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pt, k_pt_eval, kBlock, pt_smem) != cudaSuccess ||
       occ_md < 1 || occ_ls < 1 || occ_pt < 1) {

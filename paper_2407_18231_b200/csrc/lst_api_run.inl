@@ -117,12 +117,13 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
       d.sens_cnt, d.sens_begin, nullptr, 0, n_sens, d.ctl->ticket + T_SENS, d.tstate[T_SENS]);
   L.mark("scatter");
   k_scatter<<<grid_for(g, hits->n, 8), kBlock, 0, st>>>(d);
-  L.mark("md_pairs");
-  k_scan_f<PairsMD><<<gp, kBlock, 0, st>>>(d, d.pp_md, d.ev_cg0, &d.ctl->pair_total[0], T_PMD);
   L.mark("md");
-  k_eval<StageMD><<<ctx->grid_md, kBlock, 0, st>>>(d);
+  k_md_eval<<<ctx->grid_md, kBlock, 0, st>>>(d);
+  L.mark("md_scan");
+  k_scan_t<16><<<grid_for(g, (hits->n + 16) / 16, 4), kBlock, 0, st>>>(
+      d.md_cnt, d.hit_md_begin, nullptr, 0, hits->n, d.ctl->ticket + T_MD, d.tstate[T_MD]);
   L.mark("md_place");
-  k_place<StageMD><<<gp, kBlock, 0, st>>>(d);
+  k_md_place<<<grid_for(g, hits->n, 8), kBlock, 0, st>>>(d);
   L.mark("ls");
   k_ls_eval<<<ctx->grid_ls, kBlock, 0, st>>>(d);
   L.mark("ls_scan");

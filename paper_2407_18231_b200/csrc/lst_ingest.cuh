@@ -58,40 +58,52 @@ __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
 
 // Generic exclusive scan out[i] = sum_{j<i} in[j], i in [0, n], n = (*n_ptr) * n_mul + n_add
 // (n_ptr may be NULL -> n = n_add).  in[n] is not read; out[n] = total.  Persistent blocks take
-// tile tickets; 4 items per thread.
+// tile tickets; ITEMS consecutive items per thread (16 for the million-item scans: the cost of a scan
+// is its number of tiles, i.e. look-back round trips).
 constexpr int kScanItems = 4;
 constexpr int kScanTile = kBlock * kScanItems;
 
+template <int ITEMS>
 __global__ void __launch_bounds__(kBlock)
-k_scan(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int n_mul, int n_add,
-       int* ticket, unsigned long long* state) {
+k_scan_t(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int n_mul, int n_add,
+         int* ticket, unsigned long long* state) {
+  constexpr int kTile = kBlock * ITEMS;
   __shared__ int s_tile;
   __shared__ int s_scan[kWarps + 2];
   const int n = (n_ptr ? (*n_ptr) * n_mul : 0) + n_add;
-  const int n_tiles = (n + kScanTile - 1) / kScanTile > 0 ? (n + kScanTile - 1) / kScanTile : 1;
+  const int n_tiles = (n + kTile - 1) / kTile > 0 ? (n + kTile - 1) / kTile : 1;
   for (;;) {
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1);
     __syncthreads();
     const int tile = s_tile;
     if (tile >= n_tiles) break;
-    const int base_i = tile * kScanTile + threadIdx.x * kScanItems;
-    int v[kScanItems];
+    const int base_i = tile * kTile + threadIdx.x * ITEMS;
+    int v[ITEMS];
     int sum = 0;
+    if (ITEMS % 4 == 0 && base_i + ITEMS <= n) {  // full thread: 16-byte loads (arrays are 256-byte aligned)
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-      v[k] = (base_i + k < n) ? in[base_i + k] : 0;
-      sum += v[k];
+      for (int k = 0; k < ITEMS; k += 4) {
+        const int4 q = *reinterpret_cast<const int4*>(in + base_i + k);
+        v[k] = q.x;  v[k + 1] = q.y;  v[k + 2] = q.z;  v[k + 3] = q.w;
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < ITEMS; ++k) v[k] = (base_i + k < n) ? in[base_i + k] : 0;
     }
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) sum += v[k];
     int tb, tt;
     int off = tile_alloc(sum, state, tile, s_scan, tb, tt);
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
+    for (int k = 0; k < ITEMS; ++k) {
       if (base_i + k < n) out[base_i + k] = off;
       off += v[k];
     }
     if (tile == n_tiles - 1 && threadIdx.x == 0) out[n] = tb + tt;
   }
 }
+
+#define k_scan k_scan_t<kScanItems>
 
 // a0.3 scatter: sorted SoA (float4 x,y,z,r + int2 input index, global sensor), r = sqrtf(x*x + y*y)
 __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {

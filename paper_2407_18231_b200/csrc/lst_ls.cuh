@@ -2,8 +2,8 @@
 //
 // Candidates of an inner MD A: the MDs of every module in conn[module(A)] (the CSR row of the
 // precomputed connection map).  A PU200 batch holds 2.1e5 MDs, rows of 7.7 targets on average and
-// 1.4 MDs per target: 5e6 candidate pairs in 1.6e6 tiny (MD, target) lists.  Flattening the pairs
-// (lst_pairs.cuh) costs more in decoding (pair -> module -> MD -> row edge -> B: ~290 thread
+// 1.4 MDs per target: 5e6 candidate pairs in 1.6e6 tiny (MD, target) lists.  Flattening the pairs of
+// the whole batch (an earlier engine, profiles/r01_v2_even_split.md) costs more in decoding (pair -> module -> MD -> row edge -> B: ~290 thread
 // instructions per pair, ncu) than the cuts themselves (~40), because a 32-pair step crosses a
 // module boundary almost every time.  Here the unit is the list:
 //   * a warp takes 8 consecutive inner MDs and builds, once, the table of their (MD, target) lists
@@ -17,7 +17,7 @@
 // LSs therefore sit grouped by inner MD (what T3 building looks up); the order inside an MD's range
 // is free (reading S9).
 #pragma once
-#include "lst_stages.cuh"
+#include "lst_md.cuh"
 
 namespace lst {
 

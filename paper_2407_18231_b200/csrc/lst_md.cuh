@@ -1,0 +1,143 @@
+// lst_md.cuh -- step a1: Mini-Doublets (CUDA transcription of CUTS.md section 3).
+//
+// Candidates of an upper-sensor hit b: the hits of the lower sensor of the same module (a contiguous
+// range of the sorted hits, just before the module's upper range).  1.4e7 hit pairs per PU200 batch,
+// 1.5 % accepted.  One LANE per upper hit, the lower hits are walked in a plain loop: no pair
+// decoding, no ballot per step (the even-split pair engine spent 100 of its 151 instructions per 32
+// pairs on those; profiles/).  Lanes of a warp hold consecutive upper hits, i.e. hits of the same or
+// neighbouring modules, so their loops have similar lengths (the hot layer-1 modules fill whole warps)
+// and their loads hit the same cache lines.
+//   * k_md_eval: a warp takes windows of 64 sorted hits, compacts the upper-sensor ones (ballot),
+//     and every lane tests its hit against its module's lower hits; the positions of the first
+//     kMdStash accepted lower hits are stashed per upper hit, the count is exact;
+//   * k_scan turns the counts into hit_md_begin (MDs grouped by upper hit = by module);
+//   * k_md_place writes each upper hit's MDs (re-evaluating only the rare hit with more than kMdStash
+//     MDs) and the first MD of every module.
+#pragma once
+#include "lst_stages.cuh"
+
+namespace lst {
+
+constexpr int kMdStash = 4;  // stashed MDs per upper hit
+
+__global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
+  __shared__ int s_own[kWarps][64];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int n = (d.cuts.stage_mask & 1) ? d.n_hits : 0;
+  unsigned long long near = 0, tests = 0;
+  for (int w0 = (blockIdx.x * kWarps + warp) * 64; w0 < d.n_hits; w0 += gridDim.x * kWarps * 64) {
+    // ---- the upper-sensor hits of the window, compacted in order ----
+    const int i0 = w0 + lane, i1 = w0 + 32 + lane;
+    const int gs0 = i0 < n ? d.hit_ig[i0].y : 0, gs1 = i1 < n ? d.hit_ig[i1].y : 0;
+    const unsigned m0 = __ballot_sync(kFull, gs0 & 1), m1 = __ballot_sync(kFull, gs1 & 1);
+    const int n0 = __popc(m0), n_own = n0 + __popc(m1);
+    if (gs0 & 1) s_own[warp][__popc(m0 & ((1u << lane) - 1u))] = i0;
+    if (gs1 & 1) s_own[warp][n0 + __popc(m1 & ((1u << lane) - 1u))] = i1;
+    if (i0 < d.n_hits && !(gs0 & 1)) d.md_cnt[i0] = 0;  // lower-sensor hits own no MD
+    if (i1 < d.n_hits && !(gs1 & 1)) d.md_cnt[i1] = 0;
+    __syncwarp();
+    for (int r0 = 0; r0 < n_own; r0 += 32) {
+      int i = -1, a = 0, a1 = 0, endcap = 0;
+      float4 hb = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (r0 + lane < n_own) {
+        i = s_own[warp][r0 + lane];
+        const int gs = d.hit_ig[i].y;
+        const int gm = gs >> 1;
+        a = __ldg(d.sens_begin + gs - 1);
+        a1 = __ldg(d.sens_begin + gs);
+        endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
+        hb = d.hit[i];
+        tests += (unsigned long long)(a1 - a);
+      }
+      int cnt = 0;
+      int stash[kMdStash];
+#pragma unroll
+      for (int k = 0; k < kMdStash; ++k) stash[k] = 0;
+      for (; a < a1; ++a) {
+        float ux, uy;
+        const unsigned r = md_test(d.cuts, endcap, d.hit[a], hb, ux, uy);
+        near += (r >> 1) & 1u;
+        if (r & ACC) {
+#pragma unroll
+          for (int k = 0; k < kMdStash; ++k)
+            if (cnt == k) stash[k] = a;
+          ++cnt;
+        }
+      }
+      if (i >= 0) {
+        d.md_cnt[i] = cnt;
+        int4 st4 = make_int4(stash[0], stash[1], stash[2], stash[3]);
+        reinterpret_cast<int4*>(d.md_stash)[i] = st4;
+      }
+    }
+    __syncwarp();  // s_own is reused by the next window
+  }
+  near = warp_sum_u64(near);
+  tests = warp_sum_u64(tests);
+  if (lane == 0) {
+    if (near) atomicAdd(&d.ctl->near[0], near);
+    if (tests) atomicAdd(&d.ctl->n_tests[0], tests);
+  }
+}
+
+// After k_scan(md_cnt -> hit_md_begin).  MDs of upper hit i go to hit_md_begin[i] ..., in lower-hit order.
+__global__ void __launch_bounds__(kBlock) k_md_place(Dev d) {
+  static_assert(kMdStash == 4, "the stash is stored as one int4 per hit");
+  const bool on = (d.cuts.stage_mask & 1) != 0;
+  const int n = on ? d.n_hits : 0;
+  const int total = on ? d.hit_md_begin[d.n_hits] : 0;
+  const int cap = d.cap[K_MD];
+  const int stride = gridDim.x * blockDim.x, t0 = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t0 == 0) {
+    if (total > cap) {
+      atomicOr(&d.ctl->error, E_CAP_MD);
+      d.ctl->total[K_MD] = 0;
+    } else {
+      d.ctl->total[K_MD] = total;
+    }
+  }
+  // first MD of every module (MDs are owned by upper hits, so any hit of the lower range marks the start)
+  const int n_gm = d.n_events * d.n_mod;
+  for (int gm = t0; gm <= n_gm; gm += stride)
+    d.mod_md_begin[gm] = (on && total <= cap) ? d.hit_md_begin[gm < n_gm ? __ldg(d.sens_begin + 2 * gm) : d.n_hits] : 0;
+  if (total > cap) return;
+  for (int i = t0; i < n; i += stride) {
+    const int cnt = d.md_cnt[i];
+    if (cnt == 0) continue;
+    const int2 ib = d.hit_ig[i];
+    const int gs = ib.y, gm = gs >> 1;
+    const int endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
+    const float4 hb = d.hit[i];
+    int pos = d.hit_md_begin[i];
+    auto emit = [&](int a) {  // unit direction exactly as in md_test (CUTS.md section 3)
+      const float4 ha = d.hit[a];
+      float ux = 0.0f, uy = 0.0f;
+      if (!endcap) {
+        const float dx = hb.x - ha.x, dy = hb.y - ha.y;
+        const float dd = sqrtf(dx * dx + dy * dy);
+        ux = dx / dd;
+        uy = dy / dd;
+      }
+      d.md_hit[pos] = make_int2(d.hit_ig[a].x, ib.x);
+      d.md_info[pos] = (gs - 1) | endcap;
+      d.md_a[pos] = ha;
+      d.md_u[pos] = make_float2(ux, uy);
+      ++pos;
+    };
+    if (cnt <= kMdStash) {
+      const int4 st = reinterpret_cast<const int4*>(d.md_stash)[i];
+      emit(st.x);
+      if (cnt > 1) emit(st.y);
+      if (cnt > 2) emit(st.z);
+      if (cnt > 3) emit(st.w);
+    } else {  // rare: more MDs than the stash holds -> evaluate this hit's candidates again
+      const int a1 = __ldg(d.sens_begin + gs);
+      for (int a = __ldg(d.sens_begin + gs - 1); a < a1; ++a) {
+        float ux, uy;
+        if (md_test(d.cuts, endcap, d.hit[a], hb, ux, uy) & ACC) emit(a);
+      }
+    }
+  }
+}
+
+}  // namespace lst

@@ -1,10 +1,9 @@
-// lst_stages.cuh -- steps a1..a4: MD, LS, T3, T5.  One launch per stage:
-// thread per owner; pass 1 counts the accepted candidates of the owner, tile_alloc() turns the
-// counts into output offsets (shared-memory scan + decoupled look-back), pass 2 re-evaluates and
-// writes.  Objects therefore sit in owner order: MDs by upper hit (= by module), LSs by inner MD,
-// T3s by first LS (= by first MD), T5s by first T3.
+// lst_stages.cuh -- steps a3, a4: T3 and T5.  One launch per stage: thread per owner;
+// pass 1 counts the accepted candidates of the owner, tile_alloc() turns the counts into output
+// offsets (shared-memory scan + decoupled look-back), pass 2 re-evaluates and writes.  T3s therefore
+// sit grouped by first LS (= by first MD), T5s by first T3.  (MD: lst_md.cuh, LS: lst_ls.cuh.)
 #pragma once
-#include "lst_pairs.cuh"
+#include "lst_ingest.cuh"
 
 namespace lst {
 
@@ -59,76 +58,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
   }
 }
 
-// ---- a1: Mini-Doublets (CUTS.md section 3).  group = module of one event
-// (gm = event * n_mod + module); owners = hits of its UPPER sensor, candidates = hits of its LOWER
-// sensor (both contiguous ranges of the sorted hits).  MDs come out grouped by module, inside a
-// module by (upper hit, lower hit).
-struct PairsMD {  // pre-pass: candidate pairs per module = upper hits x lower hits
-  const Dev& d;
-  __device__ explicit PairsMD(const Dev& dd) : d(dd) {}
-  __device__ int n_items() const { return (d.cuts.stage_mask & 1) ? d.n_events * d.n_mod : 0; }
-  __device__ int count(int gm) const {
-    const long long p = (long long)d.sens_cnt[2 * gm] * d.sens_cnt[2 * gm + 1];
-    if (p > d.cap_pairs) {
-      atomicOr(&d.ctl->error, E_CAP_MD);
-      return 0;
-    }
-    return (int)p;
-  }
-  __device__ int group(int gm) const { return gm; }
-};
-
-struct StageMD {
-  static constexpr int kTicket = T_MD, kKind = K_MD, kErr = E_CAP_MD, kStage = 0, kPairSlot = 0;
-  struct Group {
-    int gbase, gend, n_c;
-    float inv_nc;
-    int a0, b0;  // first lower / first upper sorted hit
-    int endcap;
-  };
-  struct Payload {
-    int a, b;  // sorted hit positions
-    float ux, uy;
-  };
-  const Dev& d;
-  __device__ explicit StageMD(const Dev& dd) : d(dd) {}
-  __device__ int n_groups() const { return (d.cuts.stage_mask & 1) ? d.n_events * d.n_mod : 0; }
-  __device__ int pp(int g) const { return d.pp_md[g]; }
-  __device__ void load_group(int gm, Group& G) const {
-    G.a0 = __ldg(d.sens_begin + 2 * gm);
-    G.b0 = __ldg(d.sens_begin + 2 * gm + 1);
-    G.n_c = G.b0 - G.a0;
-    G.inv_nc = __frcp_rn(__int2float_rn(G.n_c));
-    const int ev = gm / d.n_mod;
-    G.endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
-  }
-  __device__ unsigned test(const Group& G, int o, int j, Payload& pay) const {
-    pay.a = G.a0 + j;
-    pay.b = G.b0 + o;
-    return md_test(d.cuts, G.endcap, d.hit[pay.a], d.hit[pay.b], pay.ux, pay.uy);
-  }
-  __device__ void emit(int pos, const Payload& pay) const {
-    const int2 ia = d.hit_ig[pay.a];
-    const int gs = ia.y;  // lower sensor: gs = 2 * gm
-    const int ev = (gs >> 1) / d.n_mod;
-    d.md_hit[pos] = make_int2(ia.x, d.hit_ig[pay.b].x);
-    d.md_info[pos] = gs | (__ldg(d.subdet + ((gs >> 1) - ev * d.n_mod)) != 0);
-    d.md_a[pos] = d.hit[pay.a];
-    d.md_u[pos] = make_float2(pay.ux, pay.uy);
-  }
-  // first MD of every module: rank of the module's first pair
-  template <class R>
-  __device__ void boundaries(int tile, bool no_pairs, int g_lo, int g_hi, int, int, const R& rank) const {
-    const int n = d.n_events * d.n_mod;
-    if (no_pairs) {
-      for (int g = threadIdx.x; g <= n; g += kBlock) d.mod_md_begin[g] = 0;
-      return;
-    }
-    for (int g = (tile == 0 ? 0 : g_lo + 1) + threadIdx.x; g <= g_hi; g += kBlock) d.mod_md_begin[g] = rank(pp(g));
-  }
-  __device__ void finish_total(int) const {}
-};
-
+// ---- a1: Mini-Doublets: lst_md.cuh ----
 // ---- a2: Line Segments: lst_ls.cuh ----
 
 // ---- a3: T3 (CUTS.md section 5).  owner = LS (A->B); candidates = the LSs whose inner MD is B.

@@ -15,7 +15,7 @@ namespace lst {
 struct PtEvent;  // lst_pt.cuh
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PMD, T_PP3, T_PP5, T_ANC, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PP3, T_PP5, T_ANC, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
@@ -28,8 +28,7 @@ struct Ctl {
   int pad;
   unsigned long long near[6];
   unsigned long long n_tests[6];
-  unsigned long long pair_total[2];  // candidate pairs of the batch: [0] MD (lst_pairs.cuh)
-  int scratch_cur[4];                // accepted objects in the scratch list: 0 MD, 1 LS, 2 pT3, 3 pT5
+  int scratch_cur[4];                // accepted objects in the scratch lists: [1] LS, [2] pT3, [3] pT5
 };
 
 struct Dev {
@@ -56,14 +55,13 @@ struct Dev {
   int* sens_begin;   // [n_events * 2 * n_mod + 1] exclusive scan of sens_cnt
   float4* hit;       // [n_hits] sorted (x, y, z, r)
   int2* hit_ig;      // [n_hits] (event-local input index, global sensor) of the sorted hit
-  // ---- even-split bookkeeping, shared by the MD and LS stages (lst_pairs.cuh) ----
-  int* ev_cg0;          // [cap_pairs / kChunk + 2] group holding the first pair of every chunk
-  int2* ev_cnt;         // [cap_pairs / kChunk + 1] (accepted pairs, scratch position) of every chunk
-  unsigned* ev_mask;    // [cap_pairs / 32 + 8] ballot words of every chunk
-  void* ev_scratch;     // accepted payloads in chunk-arrival order
-  void* ev_scratch2;    // second scratch list (pT5, filled by the same kernel as pT3)
+  // ---- scratch lists of accepted objects in arrival order (LS, then pT3; pT5) ----
+  void* ev_scratch;
+  void* ev_scratch2;
   // ---- a1: MD (grouped by global module) ----
-  int* pp_md;         // [n_events * n_mod + 1] exclusive prefix of the modules' hit pairs
+  int* md_cnt;        // [n_hits] MDs owned by a sorted hit (upper-sensor hits only)
+  int* md_stash;      // [n_hits][4] sorted positions of the first accepted lower hits
+  int* hit_md_begin;  // [n_hits + 1] exclusive scan of md_cnt
   int* mod_md_begin;  // [n_events * n_mod + 1] first MD of a global module
   int2* md_hit;       // (h_lo, h_hi) event-local input indices
   int* md_info;       // 2 * gm + endcap
@@ -116,7 +114,6 @@ struct Dev {
   // ---- capacities ----
   int cap[K_NKINDS];
   int cap_idx;
-  int cap_pairs;  // candidate pairs per stage and batch
   Cuts cuts;
 };
 

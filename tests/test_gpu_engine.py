@@ -1,5 +1,5 @@
-"""GPU parity, part 2: the even-split pair engine and the tiled seed linking at their edges, and the
-full benchmark configuration (16 PU200 events in one launch sequence, default capacities)."""
+"""GPU parity, part 2: the MD / LS / seed-linking kernels at their edges (dense modules, stash and
+stage overflows, capacities), and the full benchmark configuration (16 PU200 events in one launch sequence, default capacities)."""
 import numpy as np
 import pytest
 
@@ -27,8 +27,8 @@ def lst():
 
 def dense_chain_event(n_trk=150, dphi=0.0005, seed=5):
     """Five barrel modules in a chain, n_trk near-parallel straight tracks through all of them: every
-    module holds n_trk^2 hit pairs (88 chunks of 256 at the default), thousands of MDs share a module,
-    and every MD has hundreds of LS candidates -- the opposite corner from the sparse PU200 modules."""
+    module holds n_trk^2 hit pairs, thousands of MDs share a module (upper hits with more MDs than the
+    stash holds), and every MD has hundreds of LS candidates (more LSs per warp pass than the stage holds) -- the opposite corner from the sparse PU200 modules."""
     rng = np.random.default_rng(seed)
     phi = np.arange(n_trk) * dphi + 0.3
     z0, cot = rng.normal(0, 2, n_trk), rng.normal(0, 0.2, n_trk)
@@ -64,23 +64,7 @@ def test_dense_modules_span_many_chunks(lst, oracle_mod):
         assert np.all(np.diff(v) >= 0), key
 
 
-def test_pair_capacity_overflow_is_an_error(lst):
-    geom, off, tgt = make_config_geometry("C2")
-    ev = make_config_event("C2")
-    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
-    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=1, max_pairs=1000))
-    try:
-        h, keep = lst.make_hits(ev.x, ev.y, ev.z, ev.sensor)
-        lst.lst_ctx_run(ctx, 1, h, None)
-        with pytest.raises(lst.LstError) as ei:
-            lst.lst_ctx_sync(ctx)
-        assert ei.value.status == lst.LST_ERR_CAPACITY
-    finally:
-        lst.lst_free(ctx)
-        lst.lst_free(g)
-
-
-@pytest.mark.parametrize("cap", ["max_ls", "max_t3", "max_t5", "max_pt3", "max_pt5", "max_tc"])
+@pytest.mark.parametrize("cap", ["max_md", "max_ls", "max_t3", "max_t5", "max_pt3", "max_pt5", "max_tc"])
 def test_every_object_capacity_overflow_is_an_error(lst, cap):
     geom, off, tgt = make_config_geometry("C4")
     ev = make_config_event("C4")
