@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--impl", choices=("b200", "reference"), default="b200")
     ap.add_argument("--pu", type=int, default=200)
     ap.add_argument("--events", type=int, default=16, help="events per batch (= per step)")
-    ap.add_argument("--streams", type=int, default=4, help="contexts / CUDA streams in flight")
+    ap.add_argument("--streams", type=int, default=8, help="contexts / CUDA streams in flight")
     ap.add_argument("--batches", type=int, default=6, help="distinct input batches rotated through")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels-only", action="store_true",
@@ -144,9 +144,9 @@ def algorithmic_work(name, s, n_sens):
         "hist": 12 * h + 4 * p,
         "scan_sensors": 8 * n_sens,
         "scatter": 44 * h,
-        "md_pairs": 8 * n_sens,
-        "md": 16 * h + 4 * n_sens + 16 * md,
-        "md_place": 16 * md + 28 * md + 36 * md + 2 * n_sens,
+        "md": 24 * h + 4 * n_sens + 20 * h,
+        "md_scan": 8 * h,
+        "md_place": 24 * h + 52 * md + 2 * n_sens,
         "ls": 28 * md + 8 * ls,
         "ls_scan": 8 * md,
         "ls_place": 20 * ls + 12 * md,

@@ -57,8 +57,7 @@ __device__ __forceinline__ void event_cands(const Dev& d, int ev, int& c0, int& 
   }
 }
 
-constexpr int kSeedTile = 128;  // seeds staged per tile; the survivor queues are drained after every tile
-constexpr int kQueue = 32;      // survivor queue entries per thread (drained early when one fills up)
+constexpr int kSeedTile = 128;  // seeds staged per tile
 
 // ---- anchors: the MDs that start at least one T3 (and therefore every T5) ----------------------
 // The gate of CUTS.md section 7 depends only on the seed and on the FIRST MD of the candidate, and
@@ -170,7 +169,6 @@ struct PtAccepted {
 struct PtWarp {  // per-warp scratch of k_pt_eval (dynamic shared memory: kWarps of these)
   float4 seed[kSeedTile];  // x1, y1, vx, vy of the tile's seeds
   float lv[kSeedTile];
-  unsigned short q[kQueue][32];  // [entry][lane]: per-thread survivor queues
   int2 w2[64];         // phase-2 list: (candidate | T5 flag << 31, seed slot)
   float2 axy[32];      // the warp's anchors
   int2 r3[32], r5[32];  // (first, count) of their T3s / T5s
@@ -333,45 +331,6 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
       __syncwarp();
     };
     int n1 = 0;  // gate survivors waiting in w.w1
-    int nq = 0;  // entries in this thread's queue
-    // ---- phase 1b: exact gate per queued (seed, anchor) where needed; survivors onto the warp's list ----
-    auto drain = [&]() {
-      const int nq_max = __reduce_max_sync(kFull, nq);
-      for (int i = 0; i < nq_max; ++i) {
-        bool pass = false;
-        unsigned ent = 0;
-        if (i < nq) {
-          const int qe = w.q[i][lane];
-          const int ks = qe & 0x7fff;
-          unsigned r = ACC;
-          if (qe & 0x8000) {  // uncertain: the exact gate (CUTS.md section 7) decides and flags near-threshold
-            const float4 sd = s_seed[ks];
-            Seed s;
-            s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[ks];
-            r = pt_gate(d.cuts, s, A.x, A.y);
-          }
-          pass = (r & ACC) != 0;
-          if (!pass && (r & NEAR)) {  // every candidate of the anchor fails the gate near its threshold
-            near3 += (unsigned)r3.y;
-            near5 += (unsigned)r5.y;
-          }
-          ent = (unsigned)ks | ((unsigned)lane << 16) | ((r & NEAR) ? 0x80000000u : 0u);
-        }
-        const unsigned m = __ballot_sync(kFull, pass);
-        if (pass) w.w1[n1 + __popc(m & ((1u << lane) - 1u))] = ent;
-        n1 += __popc(m);
-        if (n1 >= 32) {
-          __syncwarp();
-          expand(32);
-          const unsigned rest = (32 + lane < n1) ? w.w1[32 + lane] : 0u;
-          __syncwarp();
-          w.w1[lane] = rest;
-          n1 -= 32;
-          __syncwarp();
-        }
-      }
-      nq = 0;
-    };
     // ---- bounding circle of the warp's anchors (sorted by radius class and azimuth: a few cm) ----
     float bx0 = valid ? A.x : 3e38f, bx1 = valid ? A.x : -3e38f, by0 = valid ? A.y : 3e38f, by1 = valid ? A.y : -3e38f;
 #pragma unroll
@@ -409,6 +368,8 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
       while (word) {
         const int k = kb + __ffs(word) - 1;
         word &= word - 1;
+        bool pass = false;
+        unsigned ent = 0u;
         if (valid) {
           const float4 sd = s_seed[k];
           const float wx = A.x - sd.x, wy = A.y - sd.y;
@@ -421,16 +382,39 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
           const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
           // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact
           // gate is skipped), uncertain = within 2e-4 of the threshold or out of the approximation's
-          // range (the exact gate decides, flag bit 15)
+          // range (the exact gate decides)
           const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f;
-          const bool keep = gdot > 0.0f && (!(gcrs > lim) || !in_range);
-          const bool sure = in_range && gcrs <= lim * 0.9998f;
-          if (keep) w.q[nq++][lane] = (unsigned short)(k | (sure ? 0 : 0x8000));
+          pass = gdot > 0.0f && (!(gcrs > lim) || !in_range);
+          if (pass && !(in_range && gcrs <= lim * 0.9998f)) {
+            // phase 1b: the exact gate (CUTS.md section 7) decides and flags near-threshold
+            Seed s;
+            s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[k];
+            const unsigned r = pt_gate(d.cuts, s, A.x, A.y);
+            pass = (r & ACC) != 0;
+            if (!pass && (r & NEAR)) {  // every candidate of the anchor fails the gate near its threshold
+              near3 += (unsigned)r3.y;
+              near5 += (unsigned)r5.y;
+            }
+            if (r & NEAR) ent = 0x80000000u;
+          }
+          ent |= (unsigned)k | ((unsigned)lane << 16);
         }
-        if (__any_sync(kFull, nq >= kQueue)) drain();
+        // gate survivors onto the warp's list, in (seed, lane) order; a full warp of them is expanded at once
+        const unsigned m = __ballot_sync(kFull, pass);
+        if (m == 0u) continue;
+        if (pass) w.w1[n1 + __popc(m & ((1u << lane) - 1u))] = ent;
+        n1 += __popc(m);
+        if (n1 >= 32) {
+          __syncwarp();
+          expand(32);
+          const unsigned rest = (32 + lane < n1) ? w.w1[32 + lane] : 0u;
+          __syncwarp();
+          w.w1[lane] = rest;
+          n1 -= 32;
+          __syncwarp();
+        }
       }
     }
-    drain();
     __syncwarp();
     if (n1 > 0) expand(n1);
     if (lane < n2) phase2(w.w2[lane]);
