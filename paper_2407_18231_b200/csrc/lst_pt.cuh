@@ -62,20 +62,20 @@ constexpr int kSeedTile = 128;  // seeds staged per tile
 // ---- anchors: the MDs that start at least one T3 (and therefore every T5) ----------------------
 // The gate of CUTS.md section 7 depends only on the seed and on the FIRST MD of the candidate, and
 // T3s / T5s are stored grouped by first MD: all candidates of an anchor share one gate evaluation.
-// The anchors of an event are sorted into kAncBins = 8 radial classes x 32 azimuthal sectors
+// The anchors of an event are sorted into kAncBins = 8 radial classes x 64 azimuthal sectors
 // (counting sort: k_anchor counts and keeps the arrival rank, k_scan, k_anchor_sort places), so the
 // 32 anchors of a warp of k_pt_eval sit within a few cm of each other and a seed whose gate cone
 // misses their bounding circle is skipped for the whole warp.
-constexpr int kAncBins = 256;
+constexpr int kAncBins = 512;
 
 __device__ __forceinline__ int anchor_bin(float x, float y, float r) {
   const int rc = (r >= 29.5f) + (r >= 43.5f) + (r >= 59.5f) + (r >= 78.0f) + (r >= 98.0f) + (r >= 125.0f);
   const float a = fabsf(x) + fabsf(y);
   const float t = a > 0.0f ? y / a : 0.0f;                                  // diamond angle, monotone in azimuth
   const float ps = x >= 0.0f ? (y >= 0.0f ? t : 4.0f + t) : 2.0f - t;      // [0, 4)
-  int sec = (int)(ps * 8.0f);
-  sec = sec < 0 ? 0 : (sec > 31 ? 31 : sec);
-  return rc * 32 + sec;  // any finite or non-finite input lands in [0, 256): binning never affects results
+  int sec = (int)(ps * 16.0f);
+  sec = sec < 0 ? 0 : (sec > 63 ? 63 : sec);
+  return rc * 64 + sec;  // any finite or non-finite input lands in [0, 512): binning never affects results
 }
 
 __global__ void __launch_bounds__(kBlock) k_anchor(Dev d) {
