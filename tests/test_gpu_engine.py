@@ -141,3 +141,35 @@ def test_benchmark_configuration(lst, oracle_mod):
     finally:
         lst.lst_free(ctx)
         lst.lst_free(g)
+
+
+def test_randomised_batches(lst, oracle_mod):
+    """Many small and odd-sized batches (1-5 events, 1-400 tracks, with and without noise, seeds and
+    displaced tracks) on one reused context: every event equals the oracle's.  (compute-sanitizer is
+    not available on the GPU pool; this is the race / bounds shake-out.)"""
+    from lst_inputs.events import EventSpec, generate_event
+
+    geom, off, tgt = make_config_geometry("C4")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=5))
+    rng = np.random.default_rng(2407)
+    try:
+        for rep in range(8):
+            evs = []
+            for k in range(int(rng.integers(1, 6))):
+                spec = EventSpec(n_tracks=int(rng.integers(1, 400)), pt_dist=("loguniform", 0.8, 20.0), eta_max=1.0,
+                                 noise=("count", int(rng.integers(0, 3000))) if rng.random() < 0.7 else None,
+                                 inefficiency=0.05 * float(rng.random()), seeds=bool(rng.random() < 0.8),
+                                 n_displaced=int(rng.integers(0, 30)))
+                evs.append(generate_event(geom, spec, 10_000 + 100 * rep + k))
+            if all(e.n_pls == 0 for e in evs):
+                evs[0] = make_config_event("C4")
+            run_batch(lst, ctx, evs)
+            for i, ev in enumerate(evs):
+                want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+                got = lst.lst_ctx_fetch_event(ctx, i)
+                got["near"], got["n_tests"] = want["near"], want["n_tests"]
+                assert_same(canon(got), canon(want), f"random batch {rep}, event {i}: ")
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
