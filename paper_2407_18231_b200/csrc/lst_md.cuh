@@ -7,8 +7,8 @@
 // pairs on those; profiles/).  Lanes of a warp hold consecutive upper hits, i.e. hits of the same or
 // neighbouring modules, so their loops have similar lengths (the hot layer-1 modules fill whole warps)
 // and their loads hit the same cache lines.
-//   * k_md_eval: a warp takes windows of 64 sorted hits, compacts the upper-sensor ones (ballot),
-//     and every lane tests its hit against its module's lower hits; the positions of the first
+//   * k_md_eval: a warp takes windows of 64 sorted hits, queues the upper-sensor ones (ballot), and
+//     whenever 32 are waiting every lane tests one against its module's lower hits; the positions of the first
 //     kMdStash accepted lower hits are stashed per upper hit, the count is exact;
 //   * k_scan turns the counts into hit_md_begin (MDs grouped by upper hit = by module);
 //   * k_md_place writes each upper hit's MDs (re-evaluating only the rare hit with more than kMdStash
@@ -21,57 +21,69 @@ namespace lst {
 constexpr int kMdStash = 4;  // stashed MDs per upper hit
 
 __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
-  __shared__ int s_own[kWarps][64];
+  __shared__ int s_own[kWarps][96];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int n = (d.cuts.stage_mask & 1) ? d.n_hits : 0;
   unsigned long long near = 0, tests = 0;
+  // one round: up to 32 queued upper hits, one per lane, each against its module's lower hits
+  auto round = [&](int n_now) {
+    int i = -1, a = 0, a1 = 0, endcap = 0;
+    float4 hb = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (lane < n_now) {
+      i = s_own[warp][lane];
+      const int gs = d.hit_ig[i].y;
+      const int gm = gs >> 1;
+      a = __ldg(d.sens_begin + gs - 1);
+      a1 = __ldg(d.sens_begin + gs);
+      endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
+      hb = d.hit[i];
+      tests += (unsigned long long)(a1 - a);
+    }
+    int cnt = 0;
+    int stash[kMdStash];
+#pragma unroll
+    for (int k = 0; k < kMdStash; ++k) stash[k] = 0;
+    for (; a < a1; ++a) {
+      float ux, uy;
+      const unsigned r = md_test(d.cuts, endcap, d.hit[a], hb, ux, uy);
+      near += (r >> 1) & 1u;
+      if (r & ACC) {
+#pragma unroll
+        for (int k = 0; k < kMdStash; ++k)
+          if (cnt == k) stash[k] = a;
+        ++cnt;
+      }
+    }
+    if (i >= 0) {
+      d.md_cnt[i] = cnt;
+      reinterpret_cast<int4*>(d.md_stash)[i] = make_int4(stash[0], stash[1], stash[2], stash[3]);
+    }
+  };
+  int n_q = 0;  // upper hits waiting in s_own (always < 32 between windows, so 96 slots suffice)
   for (int w0 = (blockIdx.x * kWarps + warp) * 64; w0 < d.n_hits; w0 += gridDim.x * kWarps * 64) {
-    // ---- the upper-sensor hits of the window, compacted in order ----
+    // ---- the upper-sensor hits of the window join the queue, in order ----
     const int i0 = w0 + lane, i1 = w0 + 32 + lane;
     const int gs0 = i0 < n ? d.hit_ig[i0].y : 0, gs1 = i1 < n ? d.hit_ig[i1].y : 0;
     const unsigned m0 = __ballot_sync(kFull, gs0 & 1), m1 = __ballot_sync(kFull, gs1 & 1);
-    const int n0 = __popc(m0), n_own = n0 + __popc(m1);
-    if (gs0 & 1) s_own[warp][__popc(m0 & ((1u << lane) - 1u))] = i0;
-    if (gs1 & 1) s_own[warp][n0 + __popc(m1 & ((1u << lane) - 1u))] = i1;
+    const int n0 = __popc(m0);
+    if (gs0 & 1) s_own[warp][n_q + __popc(m0 & ((1u << lane) - 1u))] = i0;
+    if (gs1 & 1) s_own[warp][n_q + n0 + __popc(m1 & ((1u << lane) - 1u))] = i1;
     if (i0 < d.n_hits && !(gs0 & 1)) d.md_cnt[i0] = 0;  // lower-sensor hits own no MD
     if (i1 < d.n_hits && !(gs1 & 1)) d.md_cnt[i1] = 0;
+    n_q += n0 + __popc(m1);
     __syncwarp();
-    for (int r0 = 0; r0 < n_own; r0 += 32) {
-      int i = -1, a = 0, a1 = 0, endcap = 0;
-      float4 hb = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (r0 + lane < n_own) {
-        i = s_own[warp][r0 + lane];
-        const int gs = d.hit_ig[i].y;
-        const int gm = gs >> 1;
-        a = __ldg(d.sens_begin + gs - 1);
-        a1 = __ldg(d.sens_begin + gs);
-        endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
-        hb = d.hit[i];
-        tests += (unsigned long long)(a1 - a);
-      }
-      int cnt = 0;
-      int stash[kMdStash];
-#pragma unroll
-      for (int k = 0; k < kMdStash; ++k) stash[k] = 0;
-      for (; a < a1; ++a) {
-        float ux, uy;
-        const unsigned r = md_test(d.cuts, endcap, d.hit[a], hb, ux, uy);
-        near += (r >> 1) & 1u;
-        if (r & ACC) {
-#pragma unroll
-          for (int k = 0; k < kMdStash; ++k)
-            if (cnt == k) stash[k] = a;
-          ++cnt;
-        }
-      }
-      if (i >= 0) {
-        d.md_cnt[i] = cnt;
-        int4 st4 = make_int4(stash[0], stash[1], stash[2], stash[3]);
-        reinterpret_cast<int4*>(d.md_stash)[i] = st4;
-      }
+    while (n_q >= 32) {  // full rounds only; the remainder waits for the next window
+      round(32);
+      const int r0 = (32 + lane < n_q) ? s_own[warp][32 + lane] : 0;
+      const int r1 = (64 + lane < n_q) ? s_own[warp][64 + lane] : 0;
+      __syncwarp();
+      s_own[warp][lane] = r0;
+      s_own[warp][32 + lane] = r1;
+      n_q -= 32;
+      __syncwarp();
     }
-    __syncwarp();  // s_own is reused by the next window
   }
+  if (n_q > 0) round(n_q);
   near = warp_sum_u64(near);
   tests = warp_sum_u64(tests);
   if (lane == 0) {
