@@ -173,3 +173,46 @@ def test_randomised_batches(lst, oracle_mod):
     finally:
         lst.lst_free(ctx)
         lst.lst_free(g)
+
+
+def test_many_small_events_in_one_batch(lst, oracle_mod):
+    """40 events per launch sequence (more events than any table is sized for by default)."""
+    geom, off, tgt = make_config_geometry("C4")
+    from lst_inputs.events import EventSpec, generate_event
+
+    evs = [generate_event(geom, EventSpec(n_tracks=30 + 5 * (k % 7), pt_dist=("loguniform", 0.8, 10.0), eta_max=1.0,
+                                          noise=("count", 100), seeds=True), 5000 + k) for k in range(40)]
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=40))
+    try:
+        summ = run_batch(lst, ctx, evs)
+        assert summ["n_events"] == 40
+        n_tc = 0
+        for i, ev in enumerate(evs):
+            want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+            got = lst.lst_ctx_fetch_event(ctx, i)
+            got["near"], got["n_tests"] = want["near"], want["n_tests"]
+            assert_same(canon(got), canon(want), f"40-event batch, event {i}: ")
+            n_tc += len(want["tc"])
+        assert summ["n_tc"] == n_tc
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
+def test_pu250_events(lst, oracle_mod):
+    """The densest point of the BASELINE.json sweep (8,750 tracks per event)."""
+    geom, off, tgt = make_config_geometry("C5")
+    evs = c5_batch(pu=250, n_events=2)
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=2))
+    try:
+        run_batch(lst, ctx, evs)
+        for i, ev in enumerate(evs):
+            want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+            got = lst.lst_ctx_fetch_event(ctx, i)
+            got["near"], got["n_tests"] = want["near"], want["n_tests"]
+            assert_same(canon(got), canon(want), f"PU250 event {i}: ")
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
