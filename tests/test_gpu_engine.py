@@ -43,19 +43,27 @@ def dense_chain_event(n_trk=150, dphi=0.0005, seed=5):
     perm = rng.permutation(n_trk * 10)
     f = lambda a, t: np.concatenate(a).astype(t)[perm]
     table = np.array([[0, m + 1, 0, 0] for m in range(5)], np.int32)
+    # seeds on every 5th track (straight: very high pT): each sees hundreds of T3s / T5s behind one anchor
+    k = np.arange(0, n_trk, 5)
+    pls = {"pt": np.full(k.size, 200.0), "q": np.where(k % 2 == 0, 1, -1)}
+    for name, r in (("0", 3.0), ("1", 7.0)):
+        pls["x" + name], pls["y" + name] = r * np.cos(phi[k]), r * np.sin(phi[k])
+        pls["z" + name] = z0[k] + cot[k] * r
+    pls = {key: np.ascontiguousarray(v, dtype=np.int32 if key == "q" else np.float32) for key, v in pls.items()}
     return table, np.array([0, 1, 2, 3, 4, 4], np.int32), np.array([1, 2, 3, 4], np.int32), \
-        f(xs, np.float32), f(ys, np.float32), f(zs, np.float32), f(ss, np.int32)
+        f(xs, np.float32), f(ys, np.float32), f(zs, np.float32), f(ss, np.int32), pls
 
 
 def test_dense_modules_span_many_chunks(lst, oracle_mod):
-    table, off, tgt, x, y, z, s = dense_chain_event()
+    table, off, tgt, x, y, z, s, pls = dense_chain_event()
     g = lst.lst_load_geometry(table, off, tgt)
     try:
-        got = lst.lst_run_event(g, x, y, z, s)
+        got = lst.lst_run_event(g, x, y, z, s, pls)
     finally:
         lst.lst_free(g)
-    want = oracle_mod.run_event(table[:, 0].copy(), off, tgt, x, y, z, s, {})
+    want = oracle_mod.run_event(table[:, 0].copy(), off, tgt, x, y, z, s, pls)
     assert want["n_tests"][0] == 5 * 150 * 150 and len(want["ls_md"]) > 10_000 and len(want["t5_md"]) > 5_000
+    assert len(want["pt3"]) > 100 and len(want["pt5"]) > 100  # anchors with more candidates than a warp list holds
     assert_same(canon(got), canon(want), "dense chain: ")
     # storage order (what the begin-offset arrays rely on): MDs grouped by module, LSs by inner MD,
     # T3s by first LS, T5s by first T3
