@@ -65,7 +65,9 @@ typedef struct lst_params {
 /* Fills *p with the defaults of CUTS.md section 1 (stage_mask = 0x3f). */
 void lst_default_params(lst_params* p);
 
-/* Capacities of one context (object counts summed over the events of a batch). */
+/* Capacities of one context (object counts summed over the events of a batch).  max_md may not exceed
+ * LST_MAX_MD (the Line-Segment stage packs an MD index into 27 bits): lst_ctx_create returns LST_ERR_ARG. */
+#define LST_MAX_MD (1 << 27)
 typedef struct lst_caps {
   int32_t max_events;
   int32_t max_hits, max_pls;
@@ -109,8 +111,8 @@ enum { LST_ST_MD = 0, LST_ST_LS, LST_ST_T3, LST_ST_T5, LST_ST_PT3, LST_ST_PT5, L
 typedef struct lst_event_out {
   uint64_t magic;
   int32_t n_md, n_ls, n_t3, n_t5, n_pt3, n_pt5, n_tc;
-  int64_t near[LST_N_STAGES];    /* near-threshold candidates per stage (CUTS.md section 0) */
-  int64_t n_tests[LST_N_STAGES]; /* candidates evaluated per stage */
+  int64_t near[LST_N_STAGES];    /* near-threshold candidates of THIS event per stage (CUTS.md section 0) */
+  int64_t n_tests[LST_N_STAGES]; /* candidates of THIS event per stage (CUTS.md sections 3-7) */
   int32_t* md_hits;   /* [n_md][2]  h_lo, h_hi (input hit indices) */
   int32_t* md_module; /* [n_md] */
   float* md_f;        /* [n_md][6]  anchor x, y, z, r and unit direction ux, uy */
@@ -129,7 +131,8 @@ typedef struct lst_event_out {
   int32_t* tc;        /* [n_tc][16] type, pls, t5, t3, hit_idx[12]; classes in order pT5, pT3, T5, pLS */
 } lst_event_out;
 
-/* Totals of the last batch of a context (host struct filled by lst_ctx_sync). */
+/* Totals of the last batch of a context (host struct filled by lst_ctx_sync); near / n_tests are the
+ * sums of the per-event counters that lst_ctx_fetch_event returns. */
 typedef struct lst_batch_summary {
   int32_t n_events;
   int32_t n_hits, n_pls;
@@ -149,7 +152,9 @@ int lst_load_geometry(const lst_module* modules, int32_t n_modules, const int32_
 
 /* Runs the whole chain on ONE event, synchronously, on an internal context (default capacities,
  * default stream) and returns every object array on the host.  seeds may be NULL.
- * hits->event_offsets / seeds->event_offsets must be NULL.  *out: release with lst_free. */
+ * hits->event_offsets / seeds->event_offsets must be NULL.  *out: release with lst_free.
+ * Thread-safe: concurrent calls on one geometry are serialised by the library (one internal
+ * context per geometry); use one lst_ctx per thread / stream for concurrency. */
 int lst_run_event(lst_geometry* g, const lst_hits* hits, const lst_pls* seeds, lst_event_out** out);
 
 /* Releases a lst_geometry, lst_ctx or lst_event_out (NULL is a no-op). */

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -35,7 +36,8 @@ struct lst_geometry {
   int *d_subdet, *d_conn_off, *d_conn_tgt;
   lst_params params;
   Cuts cuts;
-  lst_ctx* default_ctx;
+  lst_ctx* default_ctx;   // lst_run_event's context, created on first use under default_mu
+  std::mutex default_mu;  // serialises lst_run_event on one geometry
   int n_sm;
 };
 
@@ -57,7 +59,9 @@ struct lst_ctx {
   int *d_hit_ev_off, *d_pls_ev_off, *d_ev_first;
   // pinned host mirrors
   Ctl* h_ctl;
+  unsigned long long* h_ev_cnt;  // [max_events][kEvCnt]
   int* h_ev_first;  // [K_PT5 + 1][max_events + 1]
+  int* h_tc_begin;  // [4 * max_events + 1] first track candidate of every (event, class)
   int h_pls_off[2];
   std::vector<int> last_hit_off, last_pls_off;
   int last_n_events;
@@ -202,6 +206,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   const long long n_sens = (long long)c.max_events * 2 * n_mod;
   // --- zeroed per batch ---
   d.ctl = b.take<Ctl>(1);
+  d.ev_cnt = b.take<unsigned long long>((size_t)c.max_events * kEvCnt);
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
   d.tstate[T_MD] = b.take<unsigned long long>(tiles_of((long long)c.max_hits + 1, kScanTile));
   d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kScanTile));
@@ -314,8 +319,9 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
 }
 
 bool caps_ok(const lst_caps& c) {
+  // max_md: the LS stage packs an MD index into 27 bits (lst_ls.cuh); max_pls: a seed slot into 16 bits per tile
   return c.max_events > 0 && c.max_hits > 0 && c.max_pls > 0 && c.max_md > 0 && c.max_ls > 0 && c.max_t3 > 0 &&
-         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0;
+         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_md <= LST_MAX_MD;
 }
 
 }  // namespace
@@ -332,7 +338,9 @@ static void ctx_destroy(lst_ctx* ctx) {
   if (!ctx) return;
   for (void* p : ctx->allocs) cudaFree(p);
   if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
+  if (ctx->h_ev_cnt) cudaFreeHost(ctx->h_ev_cnt);
   if (ctx->h_ev_first) cudaFreeHost(ctx->h_ev_first);
+  if (ctx->h_tc_begin) cudaFreeHost(ctx->h_tc_begin);
   for (int i = 0; i <= kMaxKernels; ++i)
     if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
   ctx->magic = 0;
@@ -354,7 +362,9 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   ctx->caps = c;
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->h_ctl = nullptr;
+  ctx->h_ev_cnt = nullptr;
   ctx->h_ev_first = nullptr;
+  ctx->h_tc_begin = nullptr;
   for (int i = 0; i <= kMaxKernels; ++i) ctx->ev[i] = nullptr;
   ctx->timing = false;
   ctx->n_kernels = 0;
@@ -378,7 +388,9 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   ctx->dev.conn_tgt = g->d_conn_tgt;
   ctx->dev.cuts = g->cuts;
   bool ok = cudaMallocHost(&ctx->h_ctl, sizeof(Ctl)) == cudaSuccess &&
-            cudaMallocHost(&ctx->h_ev_first, sizeof(int) * (K_PT5 + 1) * (c.max_events + 1)) == cudaSuccess;
+            cudaMallocHost(&ctx->h_ev_cnt, sizeof(unsigned long long) * kEvCnt * c.max_events) == cudaSuccess &&
+            cudaMallocHost(&ctx->h_ev_first, sizeof(int) * (K_PT5 + 1) * (c.max_events + 1)) == cudaSuccess &&
+            cudaMallocHost(&ctx->h_tc_begin, sizeof(int) * (4 * (size_t)c.max_events + 1)) == cudaSuccess;
   for (int i = 0; ok && i <= kMaxKernels; ++i) ok = cudaEventCreate(&ctx->ev[i]) == cudaSuccess;
   if (!ok) {
     ctx_destroy(ctx);

@@ -17,12 +17,15 @@ void out_destroy(lst_event_out* o) {
 template <class T>
 T* halloc(size_t n) { return static_cast<T*>(malloc(sizeof(T) * (n ? n : 1))); }
 
-// device slice -> host buffer
-template <class T>
-bool d2h(T* dst, const T* src, size_t first, size_t n) {
-  if (n == 0) return true;
-  return cudaMemcpy(dst, src + first, sizeof(T) * n, cudaMemcpyDeviceToHost) == cudaSuccess;
-}
+// device slice -> host buffer, enqueued on the context's stream (the caller synchronises once)
+struct D2H {
+  cudaStream_t st;
+  template <class T>
+  bool operator()(T* dst, const T* src, size_t first, size_t n) const {
+    if (n == 0) return true;
+    return cudaMemcpyAsync(dst, src + first, sizeof(T) * n, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  }
+};
 
 }  // namespace
 
@@ -38,6 +41,7 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
   const int f_md = first(K_MD, ev), f_ls = first(K_LS, ev), f_t3 = first(K_T3, ev), f_t5 = first(K_T5, ev);
   const int f_p3 = first(K_PT3, ev), f_p5 = first(K_PT5, ev);
   const int f_pls = ctx->last_pls_off[ev];
+  const D2H d2h{ctx->stream};
 
   lst_event_out* o = static_cast<lst_event_out*>(calloc(1, sizeof(lst_event_out)));
   if (!o) return LST_ERR_CUDA;
@@ -48,80 +52,67 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
   o->n_t5 = first(K_T5, ev + 1) - f_t5;
   o->n_pt3 = first(K_PT3, ev + 1) - f_p3;
   o->n_pt5 = first(K_PT5, ev + 1) - f_p5;
-  // per-event counters are batch totals only when the batch holds one event
-  for (int k = 0; k < LST_N_STAGES; ++k) {
-    o->near[k] = (int64_t)h.near[k];
-    o->n_tests[k] = (int64_t)h.n_tests[k];
+  const bool has_tc = (ctx->g->cuts.stage_mask & 32) != 0;
+  const int tc0 = has_tc ? ctx->h_tc_begin[4 * (size_t)ev] : 0;
+  o->n_tc = has_tc ? ctx->h_tc_begin[4 * (size_t)(ev + 1)] - tc0 : 0;
+  for (int k = 0; k < LST_N_STAGES; ++k) {  // counters of THIS event
+    o->near[k] = (int64_t)ctx->h_ev_cnt[(size_t)ev * kEvCnt + k];
+    o->n_tests[k] = (int64_t)ctx->h_ev_cnt[(size_t)ev * kEvCnt + 6 + k];
   }
-  bool ok = true;
   const int n_md = o->n_md, n_ls = o->n_ls, n_t3 = o->n_t3, n_t5 = o->n_t5;
-  // MD
   o->md_hits = halloc<int32_t>(2 * (size_t)n_md);
   o->md_module = halloc<int32_t>(n_md);
   o->md_f = halloc<float>(6 * (size_t)n_md);
-  {
-    std::vector<int> info(n_md);
-    std::vector<float4> a(n_md);
-    std::vector<float2> u(n_md);
-    ok = ok && d2h(reinterpret_cast<int2*>(o->md_hits), d.md_hit, f_md, n_md) &&
-         d2h(info.data(), d.md_info, f_md, n_md) && d2h(a.data(), d.md_a, f_md, n_md) &&
-         d2h(u.data(), d.md_u, f_md, n_md);
-    for (int i = 0; ok && i < n_md; ++i) {
-      o->md_module[i] = (info[i] >> 1) - ev * d.n_mod;
-      float* f = o->md_f + 6 * (size_t)i;
-      f[0] = a[i].x;  f[1] = a[i].y;  f[2] = a[i].z;  f[3] = a[i].w;  f[4] = u[i].x;  f[5] = u[i].y;
-    }
-  }
-  // LS
   o->ls_md = halloc<int32_t>(2 * (size_t)n_ls);
   o->ls_kappa = halloc<float>(n_ls);
-  ok = ok && d2h(reinterpret_cast<int2*>(o->ls_md), d.ls_md, f_ls, n_ls) && d2h(o->ls_kappa, d.ls_kappa, f_ls, n_ls);
-  for (size_t i = 0; ok && i < 2 * (size_t)n_ls; ++i) o->ls_md[i] -= f_md;
-  // T3
   o->t3_ls = halloc<int32_t>(2 * (size_t)n_t3);
   o->t3_md = halloc<int32_t>(3 * (size_t)n_t3);
   o->t3_k = halloc<float>(n_t3);
-  {
-    std::vector<int4> m(n_t3);
-    ok = ok && d2h(reinterpret_cast<int2*>(o->t3_ls), d.t3_ls, f_t3, n_t3) && d2h(m.data(), d.t3_md, f_t3, n_t3) &&
-         d2h(o->t3_k, d.t3_k, f_t3, n_t3);
-    for (int i = 0; ok && i < n_t3; ++i) {
-      o->t3_ls[2 * i] -= f_ls;  o->t3_ls[2 * i + 1] -= f_ls;
-      o->t3_md[3 * i] = m[i].x - f_md;  o->t3_md[3 * i + 1] = m[i].y - f_md;  o->t3_md[3 * i + 2] = m[i].z - f_md;
-    }
-  }
-  // T5
   o->t5_t3 = halloc<int32_t>(2 * (size_t)n_t5);
   o->t5_md = halloc<int32_t>(5 * (size_t)n_t5);
   o->t5_score = halloc<float>(n_t5);
-  ok = ok && d2h(reinterpret_cast<int2*>(o->t5_t3), d.t5_t3, f_t5, n_t5) &&
-       d2h(o->t5_md, d.t5_md, 5 * (size_t)f_t5, 5 * (size_t)n_t5) && d2h(o->t5_score, d.t5_score, f_t5, n_t5);
-  for (size_t i = 0; ok && i < 2 * (size_t)n_t5; ++i) o->t5_t3[i] -= f_t3;
-  for (size_t i = 0; ok && i < 5 * (size_t)n_t5; ++i) o->t5_md[i] -= f_md;
-  // pT3 / pT5
   o->pt3 = halloc<int32_t>(2 * (size_t)o->n_pt3);
   o->pt3_score = halloc<float>(o->n_pt3);
   o->pt5 = halloc<int32_t>(2 * (size_t)o->n_pt5);
   o->pt5_score = halloc<float>(o->n_pt5);
-  ok = ok && d2h(reinterpret_cast<int2*>(o->pt3), d.pt3, f_p3, o->n_pt3) &&
-       d2h(o->pt3_score, d.pt3_score, f_p3, o->n_pt3) &&
-       d2h(reinterpret_cast<int2*>(o->pt5), d.pt5, f_p5, o->n_pt5) && d2h(o->pt5_score, d.pt5_score, f_p5, o->n_pt5);
-  for (int i = 0; ok && i < o->n_pt3; ++i) { o->pt3[2 * i] -= f_pls;  o->pt3[2 * i + 1] -= f_t3; }
-  for (int i = 0; ok && i < o->n_pt5; ++i) { o->pt5[2 * i] -= f_pls;  o->pt5[2 * i + 1] -= f_t5; }
-  // TC
-  int tcb[2] = {0, 0};
-  if (h.total[K_TC] > 0 || (ctx->g->cuts.stage_mask & 32)) {
-    int b0 = 0, b1 = 0;
-    ok = ok && d2h(&b0, d.tc_begin, 4 * (size_t)ev, 1) && d2h(&b1, d.tc_begin, 4 * (size_t)(ev + 1), 1);
-    tcb[0] = b0;  tcb[1] = b1;
-  }
-  o->n_tc = tcb[1] - tcb[0];
   o->tc = halloc<int32_t>(16 * (size_t)o->n_tc);
-  ok = ok && d2h(o->tc, d.tc, 16 * (size_t)tcb[0], 16 * (size_t)o->n_tc);
+  std::vector<int> info(n_md);
+  std::vector<float4> a(n_md);
+  std::vector<float2> u(n_md);
+  std::vector<int4> m3(n_t3);
+  // every copy goes to the context's stream; one synchronisation, then the index shifts on the host
+  bool ok = d2h(reinterpret_cast<int2*>(o->md_hits), d.md_hit, f_md, n_md) &&
+            d2h(info.data(), d.md_info, f_md, n_md) && d2h(a.data(), d.md_a, f_md, n_md) &&
+            d2h(u.data(), d.md_u, f_md, n_md) &&
+            d2h(reinterpret_cast<int2*>(o->ls_md), d.ls_md, f_ls, n_ls) && d2h(o->ls_kappa, d.ls_kappa, f_ls, n_ls) &&
+            d2h(reinterpret_cast<int2*>(o->t3_ls), d.t3_ls, f_t3, n_t3) && d2h(m3.data(), d.t3_md, f_t3, n_t3) &&
+            d2h(o->t3_k, d.t3_k, f_t3, n_t3) &&
+            d2h(reinterpret_cast<int2*>(o->t5_t3), d.t5_t3, f_t5, n_t5) &&
+            d2h(o->t5_md, d.t5_md, 5 * (size_t)f_t5, 5 * (size_t)n_t5) && d2h(o->t5_score, d.t5_score, f_t5, n_t5) &&
+            d2h(reinterpret_cast<int2*>(o->pt3), d.pt3, f_p3, o->n_pt3) &&
+            d2h(o->pt3_score, d.pt3_score, f_p3, o->n_pt3) &&
+            d2h(reinterpret_cast<int2*>(o->pt5), d.pt5, f_p5, o->n_pt5) &&
+            d2h(o->pt5_score, d.pt5_score, f_p5, o->n_pt5) &&
+            d2h(o->tc, d.tc, 16 * (size_t)tc0, 16 * (size_t)o->n_tc);
+  ok = (cudaStreamSynchronize(ctx->stream) == cudaSuccess) && ok;
   if (!ok) {
     out_destroy(o);
     return LST_ERR_CUDA;
   }
+  for (int i = 0; i < n_md; ++i) {
+    o->md_module[i] = (info[i] >> 1) - ev * d.n_mod;
+    float* f = o->md_f + 6 * (size_t)i;
+    f[0] = a[i].x;  f[1] = a[i].y;  f[2] = a[i].z;  f[3] = a[i].w;  f[4] = u[i].x;  f[5] = u[i].y;
+  }
+  for (size_t i = 0; i < 2 * (size_t)n_ls; ++i) o->ls_md[i] -= f_md;
+  for (int i = 0; i < n_t3; ++i) {
+    o->t3_ls[2 * i] -= f_ls;  o->t3_ls[2 * i + 1] -= f_ls;
+    o->t3_md[3 * i] = m3[i].x - f_md;  o->t3_md[3 * i + 1] = m3[i].y - f_md;  o->t3_md[3 * i + 2] = m3[i].z - f_md;
+  }
+  for (size_t i = 0; i < 2 * (size_t)n_t5; ++i) o->t5_t3[i] -= f_t3;
+  for (size_t i = 0; i < 5 * (size_t)n_t5; ++i) o->t5_md[i] -= f_md;
+  for (int i = 0; i < o->n_pt3; ++i) { o->pt3[2 * i] -= f_pls;  o->pt3[2 * i + 1] -= f_t3; }
+  for (int i = 0; i < o->n_pt5; ++i) { o->pt5[2 * i] -= f_pls;  o->pt5[2 * i + 1] -= f_t5; }
   *out = o;
   return LST_OK;
 }
@@ -136,11 +127,11 @@ extern "C" int lst_ctx_fetch_tc(lst_ctx* ctx, int32_t* tc, int32_t cap_tc, int32
     for (int e = 0; e <= E; ++e) tc_event_offsets[e] = 0;
     return LST_OK;
   }
-  std::vector<int> tb(4 * (size_t)E + 1);
-  CK(cudaMemcpyAsync(tb.data(), ctx->dev.tc_begin, sizeof(int) * tb.size(), cudaMemcpyDeviceToHost, ctx->stream));
-  if (n > 0) CK(cudaMemcpyAsync(tc, ctx->dev.tc, sizeof(int) * 16 * (size_t)n, cudaMemcpyDeviceToHost, ctx->stream));
-  CK(cudaStreamSynchronize(ctx->stream));
-  for (int e = 0; e <= E; ++e) tc_event_offsets[e] = tb[4 * (size_t)e];
+  if (n > 0) {
+    CK(cudaMemcpyAsync(tc, ctx->dev.tc, sizeof(int) * 16 * (size_t)n, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+  }
+  for (int e = 0; e <= E; ++e) tc_event_offsets[e] = ctx->h_tc_begin[4 * (size_t)e];  // read back by lst_ctx_run
   return LST_OK;
 }
 
@@ -149,6 +140,7 @@ extern "C" int lst_run_event(lst_geometry* g, const lst_hits* hits, const lst_pl
   *out = nullptr;
   if (!g || g->magic != MAGIC_GEOM || !hits) return LST_ERR_ARG;
   if (hits->event_offsets || (seeds && seeds->event_offsets)) return LST_ERR_ARG;
+  std::lock_guard<std::mutex> lock(g->default_mu);  // one internal context per geometry: calls are serialised
   if (!g->default_ctx) {
     lst_caps c;
     lst_default_caps(&c);

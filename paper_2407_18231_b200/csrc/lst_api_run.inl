@@ -182,8 +182,11 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   L.finish();
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(ctx->h_ctl, d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(ctx->h_ev_cnt, d.ev_cnt, sizeof(unsigned long long) * kEvCnt * n_events, cudaMemcpyDeviceToHost, st));
   CK(cudaMemcpyAsync(ctx->h_ev_first, ctx->d_ev_first, sizeof(int) * (K_PT5 + 1) * (n_events + 1),
                      cudaMemcpyDeviceToHost, st));
+  if (mask & 32)
+    CK(cudaMemcpyAsync(ctx->h_tc_begin, d.tc_begin, sizeof(int) * (4 * (size_t)n_events + 1), cudaMemcpyDeviceToHost, st));
   ctx->dev.n_events = n_events;
   ctx->dev.n_hits = hits->n;
   ctx->dev.n_pls = n_pls;
@@ -204,9 +207,13 @@ extern "C" int lst_ctx_sync(lst_ctx* ctx, lst_batch_summary* s) {
     s->n_pls = ctx->dev.n_pls;
     s->n_md = h.total[K_MD];  s->n_ls = h.total[K_LS];  s->n_t3 = h.total[K_T3];  s->n_t5 = h.total[K_T5];
     s->n_pt3 = h.total[K_PT3];  s->n_pt5 = h.total[K_PT5];  s->n_tc = h.total[K_TC];
-    for (int k = 0; k < LST_N_STAGES; ++k) {
-      s->near[k] = (int64_t)h.near[k];
-      s->n_tests[k] = (int64_t)h.n_tests[k];
+    for (int k = 0; k < LST_N_STAGES; ++k) {  // batch totals = sums of the per-event counters
+      s->near[k] = 0;
+      s->n_tests[k] = 0;
+      for (int e = 0; e < ctx->last_n_events; ++e) {
+        s->near[k] += (int64_t)ctx->h_ev_cnt[(size_t)e * kEvCnt + k];
+        s->n_tests[k] += (int64_t)ctx->h_ev_cnt[(size_t)e * kEvCnt + 6 + k];
+      }
     }
   }
   if (h.error & E_BAD_SENSOR) return LST_ERR_ARG;

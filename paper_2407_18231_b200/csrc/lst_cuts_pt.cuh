@@ -86,9 +86,16 @@ __device__ __forceinline__ unsigned pt_after_gate(const Cuts& c, const Seed& s, 
 
 // Necessary condition of the curvature match |kx - kp| <= tolk, kx = kappa3(P1, A, L) (CUTS.md
 // section 7), without sqrt or division: compares kx^2 = 4 crs^2 / (|P1A|^2 |AL|^2 |P1L|^2) with
-// (|kp| -+ tolk)^2.  crs is formed exactly as in kappa3 (same operands, same order), so its
-// cancellation error is common to both; everything else differs by ~1e-6 relative, near-threshold
-// candidates lie within 1e-5, and the bounds carry a 1e-3 margin.  false = the exact cut rejects.
+// (|kp| -+ tolk)^2.  false = the exact cut rejects AND is not near-threshold.
+// Inequality chain.  Let k2/prod = kx~^2 be what is computed here and kx the spec's binary32 value: crs is
+// formed exactly as in kappa3 (same operands, same order), the rest differs by |kx~ - kx| <= d |kx| with
+// d < 4e-6 (three sqrt, four products and one division on the spec's side, five products here).  The exact
+// cut flags or accepts only if |kp| - tolk (1 + 1e-5) <= |kx| <= |kp| + tolk (1 + 1e-5).  With
+// m = 1e-3 (|kp| + tolk):
+//   reject high: |kx~| > hi = |kp| + tolk + m   =>  |kx| >= |kx~| (1 - d) > |kp| + tolk (1 + 1e-5)
+//   reject low:  |kx~| < lo = |kp| - tolk - m   =>  |kx| <= |kx~| (1 + d) < |kp| - tolk (1 + 1e-5)
+// because m - d (|kp| + tolk + m) > 1e-5 tolk (m is taken relative to |kp| + tolk, NOT to |kp| - tolk: the
+// latter margin vanishes where |kp| ~ tolk, i.e. for seeds of pT ~ 20.4 GeV).  The sign test needs lo > 0.
 // kp = (-q) / (pt * KR), tolk = PT_K_TOL0 + PT_K_TOL1 * |kp| (as in make_seed).
 __device__ __forceinline__ bool pt_curv_possible(float kp, float tolk, float x1, float y1, float2 A, float2 L) {
   const float ax = A.x - x1, ay = A.y - y1;
@@ -97,12 +104,13 @@ __device__ __forceinline__ bool pt_curv_possible(float kp, float tolk, float x1,
   const float crs = ax * cy - ay * cx;
   const float prod = ((ax * ax + ay * ay) * (bx * bx + by * by)) * (cx * cx + cy * cy);
   const float k2 = 4.0f * (crs * crs);
-  const float hi = (fabsf(kp) + tolk) * 1.001f;
+  const float m = 1e-3f * (fabsf(kp) + tolk);
+  const float hi = (fabsf(kp) + tolk) + m;
   if (k2 > (hi * hi) * prod) return false;
-  const float lo = (fabsf(kp) - tolk) * 0.999f;
+  const float lo = (fabsf(kp) - tolk) - m;
   if (lo > 0.0f) {
     if (k2 < (lo * lo) * prod) return false;
-    if ((crs > 0.0f) != (kp > 0.0f)) return false;  // |kx| >= lo > 0 with the wrong sign: |kx - kp| > tolk
+    if ((crs > 0.0f) != (kp > 0.0f)) return false;  // |kx| >= lo (1 - d) > 0 with the wrong sign: |kx - kp| > |kp| > tolk (1 + 1e-5)
   }
   return true;
 }

@@ -47,13 +47,15 @@ struct LsWarp {  // per-warp scratch in shared memory
 
 __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
   __shared__ LsWarp s_w[kWarps];
+  __shared__ unsigned long long s_tests[kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   LsWarp& w = s_w[warp];
+  EvTests tbl;
+  tbl.init(s_tests, d.ev_cnt, 1, d.n_events);
   const bool on = (d.cuts.stage_mask & 2) != 0;
   const int n_md = d.ctl->total[K_MD];
   const int cap = d.cap[K_LS];
   LsAccepted* scratch = reinterpret_cast<LsAccepted*>(d.ev_scratch);
-  unsigned long long near = 0, tests = 0;
   for (int A0 = (blockIdx.x * kWarps + warp) * kLsOwners; A0 < n_md; A0 += gridDim.x * kWarps * kLsOwners) {
     // ---- lanes 0..7: one inner MD each ----
     const int A = A0 + lane;
@@ -85,6 +87,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
       const int take = __popc(fit >> first & ~((fit >> first) + 1u)) ;  // length of the run of ones starting at `first`
       const int last = first + take;  // exclusive
       const int R = w.dex[last] - d_first;
+      const bool one_event = w.gb[first] == w.gb[last - 1];  // the MDs of the pass belong to one event (nearly always)
       if (lane < kLsOwners) w.cnt[lane] = 0;
       // ---- table of the non-empty lists (owner, target e) in row order, and their head bits ----
       for (int k = lane; k < kLsHeadWords; k += 32) w.heads[k] = 0u;
@@ -103,6 +106,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
           const int B0 = d.mod_md_begin[gb + m2];
           n_t = d.mod_md_begin[gb + m2 + 1] - B0;
           ent = B0 | ((__ldg(d.subdet + m2) != 0) << 27) | (o << 28);
+          if (!one_event) tbl.add(gb / d.n_mod, (unsigned long long)n_t);
         }
         const int incl = warp_incl_scan(n_t);
         const unsigned nz = __ballot_sync(kFull, n_t > 0);
@@ -119,7 +123,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
       const int P = carry;
       if (lane == 0) w.pref[Rn] = P;
       __syncwarp();
-      tests += lane == 0 ? (unsigned long long)P : 0ull;
+      if (one_event && lane == 0) tbl.add(w.gb[first] / d.n_mod, (unsigned long long)P);
       // ---- pairs of the pass, 32 at a time; pass 1 only if the stage overflowed ----
       int base = 0, run = 0;
       for (int pass = 0; pass < 2; ++pass) {
@@ -148,7 +152,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
             acc.B = (ent & 0x7ffffff) + (p - w.pref[lo]);
             res = ls_test(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[acc.B], d.md_u[acc.B], (ent >> 27) & 1, acc.kappa);
           }
-          if (pass == 0) near += (res >> 1) & 1u;
+          if (pass == 0 && (res & NEAR)) count_near(d.ev_cnt, w.gb[o] / d.n_mod, 1);
           const unsigned m = __ballot_sync(kFull, res & ACC);
           if (res & ACC) {
             const int pos = run + __popc(m & ((1u << lane) - 1u));
@@ -183,12 +187,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
       first = last;
     }
   }
-  near = warp_sum_u64(near);
-  tests = warp_sum_u64(tests);
-  if (lane == 0) {
-    if (near) atomicAdd(&d.ctl->near[1], near);
-    if (tests) atomicAdd(&d.ctl->n_tests[1], tests);
-  }
+  tbl.flush();
 }
 
 // After k_scan(ls_cnt -> md_ls_begin): every MD's LSs go from the scratch list to their final slot.

@@ -22,23 +22,26 @@ constexpr int kMdStash = 4;  // stashed MDs per upper hit
 
 __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
   __shared__ int s_own[kWarps][96];
+  __shared__ unsigned long long s_tests[kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int n = (d.cuts.stage_mask & 1) ? d.n_hits : 0;
-  unsigned long long near = 0, tests = 0;
+  EvTests tbl;
+  tbl.init(s_tests, d.ev_cnt, 0, d.n_events);
   // one round: up to 32 queued upper hits, one per lane, each against its module's lower hits
   auto round = [&](int n_now) {
-    int i = -1, a = 0, a1 = 0, endcap = 0;
+    int i = -1, a = 0, a1 = 0, endcap = 0, ev = 0;
     float4 hb = make_float4(0.f, 0.f, 0.f, 0.f);
     if (lane < n_now) {
       i = s_own[warp][lane];
       const int gs = d.hit_ig[i].y;
       const int gm = gs >> 1;
+      ev = gm / d.n_mod;
       a = __ldg(d.sens_begin + gs - 1);
       a1 = __ldg(d.sens_begin + gs);
-      endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
+      endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
       hb = d.hit[i];
-      tests += (unsigned long long)(a1 - a);
     }
+    tbl.warp_add(ev, (unsigned long long)(a1 - a));
     int cnt = 0;
     int stash[kMdStash];
 #pragma unroll
@@ -46,7 +49,7 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
     for (; a < a1; ++a) {
       float ux, uy;
       const unsigned r = md_test(d.cuts, endcap, d.hit[a], hb, ux, uy);
-      near += (r >> 1) & 1u;
+      if (r & NEAR) count_near(d.ev_cnt, ev, 0);
       if (r & ACC) {
 #pragma unroll
         for (int k = 0; k < kMdStash; ++k)
@@ -84,12 +87,7 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
     }
   }
   if (n_q > 0) round(n_q);
-  near = warp_sum_u64(near);
-  tests = warp_sum_u64(tests);
-  if (lane == 0) {
-    if (near) atomicAdd(&d.ctl->near[0], near);
-    if (tests) atomicAdd(&d.ctl->n_tests[0], tests);
-  }
+  tbl.flush();
 }
 
 // After k_scan(md_cnt -> hit_md_begin).  MDs of upper hit i go to hit_md_begin[i] ..., in lower-hit order.

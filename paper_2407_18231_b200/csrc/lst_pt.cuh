@@ -122,7 +122,6 @@ struct PtEvent {
 __global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
   const int E = d.n_events;
   const bool on = (d.cuts.stage_mask & 16) != 0;
-  unsigned long long t3 = 0, t5 = 0;
   for (int e = threadIdx.x; e < E; e += kBlock) {
     PtEvent ev;
     ev.s0 = d.pls_ev_off[e];
@@ -134,20 +133,15 @@ __global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
       ev.a0 = d.anc_bin_begin[e * kAncBins];
       ev.a1 = d.anc_bin_begin[(e + 1) * kAncBins];
       event_cands<false>(d, e, c0, c1);
-      t3 += (unsigned long long)ns * (c1 - c0);  // candidates of CUTS.md section 7: every (seed, T3) of the event
+      // candidates of CUTS.md section 7: every (seed, T3) of the event
+      d.ev_cnt[(size_t)e * kEvCnt + 6 + 4] = (unsigned long long)ns * (c1 - c0);
     }
     if (on && d.ctl->total[K_T5] > 0) {
       event_cands<true>(d, e, c0, c1);
-      t5 += (unsigned long long)ns * (c1 - c0);
+      d.ev_cnt[(size_t)e * kEvCnt + 6 + 5] = (unsigned long long)ns * (c1 - c0);
     }
     ev.tile0 = ((ev.a1 - ev.a0 + 31) / 32) * ((ns + kSeedTile - 1) / kSeedTile);  // warp tiles
     d.pt_ev[e] = ev;
-  }
-  t3 = warp_sum_u64(t3);
-  t5 = warp_sum_u64(t5);
-  if ((threadIdx.x & 31) == 0) {
-    if (t3) atomicAdd(&d.ctl->n_tests[4], t3);
-    if (t5) atomicAdd(&d.ctl->n_tests[5], t5);
   }
   __syncthreads();
   if (threadIdx.x == 0) {  // exclusive prefix of the tile counts (n_events is small)
@@ -194,8 +188,8 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
   PtAccepted* scratch3 = reinterpret_cast<PtAccepted*>(d.ev_scratch);
   PtAccepted* scratch5 = reinterpret_cast<PtAccepted*>(d.ev_scratch2);
   const float inv_2rmin = d.cuts.inv_2rmin * 1.0001f, gate_tol = d.cuts.pt_gate_tol * 1.0001f;
-  unsigned long long near3 = 0, near5 = 0;
   for (;;) {
+    unsigned near3 = 0, near5 = 0;  // near-threshold candidates of this tile (one event)
     int tile = 0, evi = 0;
     if (lane == 0) {
       tile = atomicAdd(d.ctl->ticket + T_PT3, 1);
@@ -418,13 +412,14 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     __syncwarp();
     if (n1 > 0) expand(n1);
     if (lane < n2) phase2(w.w2[lane]);
+    if (__any_sync(kFull, (near3 | near5) != 0u)) {
+      const int s3 = warp_sum((int)near3), s5 = warp_sum((int)near5);
+      if (lane == 0) {
+        if (s3) atomicAdd(d.ev_cnt + (size_t)evi * kEvCnt + 4, (unsigned long long)s3);
+        if (s5) atomicAdd(d.ev_cnt + (size_t)evi * kEvCnt + 5, (unsigned long long)s5);
+      }
+    }
     __syncwarp();  // the seed tile is reused
-  }
-  near3 = warp_sum_u64(near3);
-  near5 = warp_sum_u64(near5);
-  if (lane == 0) {
-    if (near3) atomicAdd(&d.ctl->near[4], near3);
-    if (near5) atomicAdd(&d.ctl->near[5], near5);
   }
 }
 

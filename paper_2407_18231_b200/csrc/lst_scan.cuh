@@ -39,6 +39,46 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
   return v;
 }
 
+// ---- per-event counters (CUTS.md section 0: near-threshold candidates and candidates per stage) ----
+// Near-threshold candidates are rare (a few per million): one global atomic where it happens.
+__device__ __forceinline__ void count_near(unsigned long long* ev_cnt, int ev, int stage) {
+  atomicAdd(ev_cnt + (size_t)ev * 12 + stage, 1ull);
+}
+
+// Candidate counts are accumulated per block in a shared-memory table indexed by event (events beyond
+// the table go straight to global memory) and flushed once at the end of the kernel.
+struct EvTests {
+  unsigned long long* s;  // [64] shared
+  unsigned long long* g;  // ev_cnt
+  int stage, n_events;
+  __device__ __forceinline__ void init(unsigned long long* smem, unsigned long long* ev_cnt, int st, int n_ev) {
+    s = smem;  g = ev_cnt;  stage = st;  n_events = n_ev;
+    for (int i = threadIdx.x; i < 64; i += blockDim.x) smem[i] = 0ull;
+    __syncthreads();
+  }
+  __device__ __forceinline__ void add(int ev, unsigned long long n) const {
+    if (n == 0ull) return;
+    if (ev < 64) atomicAdd(s + ev, n); else atomicAdd(g + (size_t)ev * 12 + 6 + stage, n);
+  }
+  // called by all 32 lanes: lanes of the leader's event are summed into one update (the common case:
+  // consecutive work items belong to one event), the others add their own
+  __device__ __forceinline__ void warp_add(int ev, unsigned long long n) const {
+    const unsigned act = __ballot_sync(kFull, n != 0ull);
+    if (act == 0u) return;
+    const int lane = threadIdx.x & 31, lead = __ffs(act) - 1;
+    const int ev0 = __shfl_sync(kFull, ev, lead);
+    const bool same = n != 0ull && ev == ev0;
+    const unsigned long long sum = warp_sum_u64(same ? n : 0ull);
+    if (lane == lead) add(ev0, sum);
+    else if (n != 0ull && !same) add(ev, n);
+  }
+  __device__ __forceinline__ void flush() const {  // all threads of the block
+    __syncthreads();
+    for (int e = threadIdx.x; e < 64 && e < n_events; e += blockDim.x)
+      if (s[e]) atomicAdd(g + (size_t)e * 12 + 6 + stage, s[e]);
+  }
+};
+
 // tile status word: [63:32] flag (0 empty, 1 aggregate, 2 inclusive prefix), [31:0] value
 __device__ __forceinline__ void st_state(unsigned long long* p, unsigned flag, int v) {
   unsigned long long w = ((unsigned long long)flag << 32) | (unsigned)v;

@@ -11,25 +11,28 @@ template <class Stage>
 __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
   __shared__ int s_tile;
   __shared__ int s_scan[kWarps + 2];
-  __shared__ unsigned long long s_red[2];
+  __shared__ unsigned long long s_tests[kEvSmem];
   Stage st(d);
   const int n = st.n_owners();
   const int n_tiles = n > 0 ? (n + kBlock - 1) / kBlock : 1;
-  unsigned long long near = 0, tests = 0;
+  EvTests tbl;
+  tbl.init(s_tests, d.ev_cnt, Stage::kStage, d.n_events);
   for (;;) {
     if (threadIdx.x == 0) s_tile = atomicAdd(d.ctl->ticket + Stage::kTicket, 1);
     __syncthreads();
     const int tile = s_tile;
     if (tile >= n_tiles) break;
     const int owner = tile * kBlock + threadIdx.x;
-    int cnt = 0;
-    if (owner < n) cnt = st.template visit<false>(owner, 0, near, tests);
+    int cnt = 0, ev = 0;
+    unsigned long long tests = 0;
+    if (owner < n) cnt = st.template visit<false>(owner, 0, ev, tests);
+    tbl.warp_add(ev, tests);
     int tb, tt;
     const int off = tile_alloc(cnt, d.tstate[Stage::kTicket], tile, s_scan, tb, tt);
     if (owner < n) st.begin()[owner] = off;
     if (cnt > 0) {
-      unsigned long long n0 = 0, t0 = 0;
-      st.template visit<true>(owner, off, n0, t0);
+      unsigned long long t0 = 0;
+      st.template visit<true>(owner, off, ev, t0);
     }
     if (tile == n_tiles - 1 && threadIdx.x == 0) {
       const int total = tb + tt;
@@ -42,20 +45,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
       }
     }
   }
-  // per-stage counters: one atomic pair per block
-  if (threadIdx.x < 2) s_red[threadIdx.x] = 0;
-  __syncthreads();
-  near = warp_sum_u64(near);
-  tests = warp_sum_u64(tests);
-  if ((threadIdx.x & 31) == 0) {
-    if (near) atomicAdd(&s_red[0], near);
-    if (tests) atomicAdd(&s_red[1], tests);
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    if (s_red[0]) atomicAdd(&d.ctl->near[Stage::kStage], s_red[0]);
-    if (s_red[1]) atomicAdd(&d.ctl->n_tests[Stage::kStage], s_red[1]);
-  }
+  tbl.flush();
 }
 
 // ---- a1: Mini-Doublets: lst_md.cuh ----
@@ -69,13 +59,17 @@ struct StageT3 {
   __device__ int n_owners() const { return (d.cuts.stage_mask & 4) ? d.ctl->total[K_LS] : 0; }
   __device__ int* begin() const { return d.ls_t3_begin; }
   template <bool FILL>
-  __device__ int visit(int l, int pos, unsigned long long& near, unsigned long long& tests) const {
+  __device__ int visit(int l, int pos, int& ev, unsigned long long& tests) const {
     const int2 ab = d.ls_md[l];
     const int l0 = d.md_ls_begin[ab.y], l1 = d.md_ls_begin[ab.y + 1];
-    if (!FILL) tests += (unsigned long long)(l1 - l0);
     if (l0 == l1) return 0;
     const float4 a = d.md_a[ab.x], b = d.md_a[ab.y];
-    const int eAB = (d.md_info[ab.x] & 1) | ((d.md_info[ab.y] & 1) << 1);
+    const int infoA = d.md_info[ab.x];
+    const int eAB = (infoA & 1) | ((d.md_info[ab.y] & 1) << 1);
+    if (!FILL) {
+      ev = (infoA >> 1) / d.n_mod;
+      tests = (unsigned long long)(l1 - l0);
+    }
     const int cap = d.cap[K_T3];
     int cnt = 0;
     for (int l2 = l0; l2 < l1; ++l2) {
@@ -84,7 +78,7 @@ struct StageT3 {
       const int eC = d.md_info[C] & 1;
       float k3;
       const unsigned r = t3_test(d.cuts, a, b, c, (eAB | eC) != 0, k3);
-      if (!FILL) near += (r >> 1) & 1u;
+      if (!FILL && (r & NEAR)) count_near(d.ev_cnt, ev, 2);
       if (r & ACC) {
         if (FILL && pos < cap) {
           d.t3_ls[pos] = make_int2(l, l2);
@@ -110,11 +104,14 @@ struct StageT5 {
   __device__ int n_owners() const { return (d.cuts.stage_mask & 8) ? d.ctl->total[K_T3] : 0; }
   __device__ int* begin() const { return d.t3_t5_begin; }
   template <bool FILL>
-  __device__ int visit(int t1, int pos, unsigned long long& near, unsigned long long& tests) const {
+  __device__ int visit(int t1, int pos, int& ev, unsigned long long& tests) const {
     const int4 m1 = d.t3_md[t1];
     const int u0 = d.ls_t3_begin[d.md_ls_begin[m1.z]], u1 = d.ls_t3_begin[d.md_ls_begin[m1.z + 1]];
-    if (!FILL) tests += (unsigned long long)(u1 - u0);
     if (u0 == u1) return 0;
+    if (!FILL) {
+      ev = (d.md_info[m1.x] >> 1) / d.n_mod;
+      tests = (unsigned long long)(u1 - u0);
+    }
     const float ki = d.t3_k[t1];
     const float4 b = d.md_a[m1.y], c = d.md_a[m1.z];
     const int cap = d.cap[K_T5];
@@ -123,7 +120,7 @@ struct StageT5 {
       const int4 m2 = d.t3_md[t2];
       float score;
       const unsigned r = t5_test(d.cuts, ki, d.t3_k[t2], b, c, d.md_a[m2.y], score);
-      if (!FILL) near += (r >> 1) & 1u;
+      if (!FILL && (r & NEAR)) count_near(d.ev_cnt, ev, 3);
       if (r & ACC) {
         if (FILL && pos < cap) {
           d.t5_t3[pos] = make_int2(t1, t2);

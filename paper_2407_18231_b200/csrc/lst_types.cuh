@@ -20,14 +20,15 @@ enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PP3,
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
 
+constexpr int kEvCnt = 12;    // per-event counters: [0, 6) near-threshold candidates, [6, 12) candidates, per stage
+constexpr int kEvSmem = 64;   // events whose candidate counts a block accumulates in shared memory
+
 // Small control block, zeroed (one memset, together with the tile status words) per batch.
 struct Ctl {
   int ticket[T_N];
   int total[K_NKINDS];
   int error;
   int pad;
-  unsigned long long near[6];
-  unsigned long long n_tests[6];
   int scratch_cur[4];                // accepted objects in the scratch lists: [1] LS, [2] pT3, [3] pT5
 };
 
@@ -47,6 +48,7 @@ struct Dev {
   const int* p_q;
   // ---- control ----
   Ctl* ctl;
+  unsigned long long* ev_cnt;       // [n_events][kEvCnt]: near[6] then n_tests[6] of every event (zeroed per batch)
   unsigned long long* tstate[T_N];  // look-back status words per scanning kernel
   // ---- a0: hits binned by global sensor ----
   int* hit_gs_in;    // [n_hits] global sensor of input hit i

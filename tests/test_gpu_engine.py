@@ -138,14 +138,13 @@ def test_benchmark_configuration(lst, oracle_mod):
         for i, ev in enumerate(batches[1]):
             want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
             got = lst.lst_ctx_fetch_event(ctx, i)
-            got["near"], got["n_tests"] = want["near"], want["n_tests"]  # counters are per batch (checked below)
             assert_same(canon(got), canon(want), f"bench config, event {i}: ")
             tot += [len(want[k]) for k in ("md_hits", "ls_md", "t3_md", "t5_md", "pt3", "pt5", "tc")]
             tests += want["n_tests"]
             near += want["near"]
         assert [summ["n_" + k] for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")] == tot.tolist()
         assert summ["n_tests"] == tests.tolist() and summ["near"] == near.tolist()
-        assert np.all(near <= 1e-4 * tests), "near-threshold candidates above 0.01% (north_star)"
+        assert np.all(near <= 1e-4 * tests), "near-threshold candidates above 0.01% of the candidates (DESIGN.md N2)"
     finally:
         lst.lst_free(ctx)
         lst.lst_free(g)
@@ -176,7 +175,6 @@ def test_randomised_batches(lst, oracle_mod):
             for i, ev in enumerate(evs):
                 want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
                 got = lst.lst_ctx_fetch_event(ctx, i)
-                got["near"], got["n_tests"] = want["near"], want["n_tests"]
                 assert_same(canon(got), canon(want), f"random batch {rep}, event {i}: ")
     finally:
         lst.lst_free(ctx)
@@ -199,7 +197,6 @@ def test_many_small_events_in_one_batch(lst, oracle_mod):
         for i, ev in enumerate(evs):
             want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
             got = lst.lst_ctx_fetch_event(ctx, i)
-            got["near"], got["n_tests"] = want["near"], want["n_tests"]
             assert_same(canon(got), canon(want), f"40-event batch, event {i}: ")
             n_tc += len(want["tc"])
         assert summ["n_tc"] == n_tc
@@ -219,7 +216,6 @@ def test_pu250_events(lst, oracle_mod):
         for i, ev in enumerate(evs):
             want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
             got = lst.lst_ctx_fetch_event(ctx, i)
-            got["near"], got["n_tests"] = want["near"], want["n_tests"]
             assert_same(canon(got), canon(want), f"PU250 event {i}: ")
     finally:
         lst.lst_free(ctx)

@@ -44,7 +44,8 @@ def test_single_event_configs(lst, oracle_mod, cfg, mask):
     assert len(want["t5_md"]) > 0
     assert_same(canon(got), canon(want), f"{cfg}: ")
     tests = want["n_tests"].astype(float)
-    assert np.all(want["near"] <= np.maximum(1e-4 * tests, 0)), "near-threshold candidates above 0.01% of the tests"
+    # DESIGN.md reading N2: the 0.01 % bar is checked against the candidates of the stage
+    assert np.all(want["near"] <= np.maximum(1e-4 * tests, 0)), "near-threshold candidates above 0.01% of the candidates"
 
 
 def test_device_resident_inputs_match_host_inputs(lst, oracle_mod):
@@ -80,7 +81,6 @@ def test_c5_batches(lst, oracle_mod, pu, n_ev):
                 want = _oracle(oracle_mod, geom, off, tgt, ev)
                 near += want["near"]
                 tests += want["n_tests"]
-                got["near"], got["n_tests"] = want["near"], want["n_tests"]  # counters are per batch (below)
                 assert_same(canon(got), canon(want), f"C5 pu{pu} event {i} rep {rep}: ")
                 for k, key in (("md", "md_hits"), ("ls", "ls_md"), ("t3", "t3_md"), ("t5", "t5_md"), ("pt3", "pt3"),
                                ("pt5", "pt5"), ("tc", "tc")):
@@ -141,7 +141,6 @@ def test_ragged_batch_with_empty_events(lst, oracle_mod):
         for i, ev in enumerate(evs):
             got = lst.lst_ctx_fetch_event(ctx, i)
             want = _oracle(oracle_mod, geom, off, tgt, ev)
-            got["near"], got["n_tests"] = want["near"], want["n_tests"]
             assert_same(canon(got), canon(want), f"ragged event {i}: ")
     finally:
         lst.lst_free(ctx)
