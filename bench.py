@@ -141,33 +141,23 @@ def algorithmic_work(name, s, n_sens):
     md, ls, t3, t5, p3, p5, tc = (s[k] for k in ("n_md", "n_ls", "n_t3", "n_t5", "n_pt3", "n_pt5", "n_tc"))
     idx = 5 * t5 + 5 * p5 + 3 * p3
     table = {
-        "hist": 12 * h + 4 * p,
+        "hist": 12 * h + 4 * p + 32 * p + 36 * p,            # sensor ids in, bin + rank out; seeds in, seed table out
         "scan_sensors": 8 * n_sens,
         "scatter": 44 * h,
         "md": 24 * h + 4 * n_sens + 20 * h,
-        "md_scan": 8 * h,
-        "md_place": 24 * h + 52 * md + 2 * n_sens,
+        "md_place": 28 * h + 52 * md + 2 * n_sens,            # counts + stash in, MDs + module offsets out
         "ls": 28 * md + 8 * ls,
-        "ls_scan": 8 * md,
-        "ls_place": 20 * ls + 12 * md,
-        "t3": 12 * ls + 16 * md + 36 * t3,
-        "t5": 24 * t3 + 16 * md + 40 * t5,
-        "anchors": 24 * md,
-        "pt_tiles": 0,
-        "pt": 36 * p + 16 * (t3 + t5) + 12 * (p3 + p5),
-        "pt3_scan": 8 * p,
-        "pt3_place": 24 * p3,
-        "pt5_scan": 8 * p,
-        "pt5_place": 24 * p5,
-        "event_ranges": 0,
-        "sel_prepare": 24 * md + p,
-        "index_count": 20 * t5 + 28 * p5 + 24 * p3 + 4 * idx,
-        "scan_index": 24 * md,
-        "index_fill": 20 * t5 + 28 * p5 + 24 * p3 + 8 * idx,
+        "ls_place": 12 * md + 20 * ls + 16 * md,              # counts in, offsets + LSs out, index heads cleared
+        "t3": 12 * ls + 16 * md + 44 * t3,
+        "t5": 24 * t3 + 16 * md + 56 * t5 + 16 * md,          # + anchor bins and ranks
+        "anchor_sort": 12 * md + 32 * md // 3,                # bins and ranks in, ~1/3 of the MDs are anchors
+        "pt": 40 * p + 32 * md // 3 + 16 * (t3 + t5) + 8 * (p3 + p5),
+        "pt_exact": 80 * (p3 + p5) + 12 * (p3 + p5),
+        "pt_scan": 16 * p,
+        "pt_place": 24 * (p3 + p5) + 4 * idx + 8 * idx,       # grouped by seed + the MD index of pT3, pT5, T5
         "rule1_pt5": 33 * p5,
         "rule2_pt3": 29 * p3,
         "rule3_t5": 25 * t5 + p,
-        "scan_tc": 0,
         "tc_emit": 64 * tc + p5 + p3 + t5 + p,
     }
     st = STAGE_OF_KERNEL.get(name)

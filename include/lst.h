@@ -194,6 +194,12 @@ int lst_ctx_kernel_times(lst_ctx* ctx, float* ms, const char** names, int32_t ca
 /* Number of kernel launches issued by the last lst_ctx_run. */
 int lst_ctx_launch_count(lst_ctx* ctx);
 
+/* Diagnostics of the last synchronised batch (after lst_ctx_sync).  LST_STAT_PT_QUEUE: (seed, T3 / T5)
+ * candidates that reached the exact cut list of the seed linking (CUTS.md section 7) -- the accepted ones plus
+ * those the approximate pre-filters could not decide.  Returns the value (>= 0) or a negative lst_status. */
+enum { LST_STAT_PT_QUEUE = 0, LST_STAT_WORKSPACE_MB = 1 };
+int64_t lst_ctx_stat(lst_ctx* ctx, int32_t which);
+
 #ifdef __cplusplus
 }
 #endif

@@ -172,3 +172,13 @@ def lst_ctx_kernel_times(ctx) -> list:
 
 def lst_ctx_launch_count(ctx) -> int:
     return int(_lib().lst_ctx_launch_count(ctx))
+
+
+LST_STAT_PT_QUEUE, LST_STAT_WORKSPACE_MB = 0, 1
+
+
+def lst_ctx_stat(ctx, which: int) -> int:
+    v = int(_lib().lst_ctx_stat(ctx, int(which)))
+    if v < 0:
+        raise LstError(v, "lst_ctx_stat")
+    return v

@@ -56,7 +56,11 @@ struct lst_ctx {
   int* in_sensor;
   float *p_pt, *p_x0, *p_y0, *p_z0, *p_x1, *p_y1, *p_z1;
   int* p_q;
-  int *d_hit_ev_off, *d_pls_ev_off, *d_ev_first;
+  int *d_hit_ev_off, *d_pls_ev_off;
+  Batch* d_batch;
+  cudaStream_t owned_stream;  // non-null: created by the library (lst_run_event's context), destroyed with the context
+  cudaGraphExec_t graph;   // the launch sequence of one batch, captured on first use (kernel arguments never change)
+  bool use_graph;
   // pinned host mirrors
   Ctl* h_ctl;
   unsigned long long* h_ev_cnt;  // [max_events][kEvCnt]
@@ -208,23 +212,22 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.ctl = b.take<Ctl>(1);
   d.ev_cnt = b.take<unsigned long long>((size_t)c.max_events * kEvCnt);
   d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
-  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of((long long)c.max_hits + 1, kScanTile));
-  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kScanTile));
+  d.tstate[T_MD] = b.take<unsigned long long>(tiles_of((long long)c.max_hits + 1, kBlock * kMdPlaceItems));
+  d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kBlock));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
   d.tstate[T_T5] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
-  d.tstate[T_PT3] = nullptr;  // ticket only
-  d.tstate[T_PT5] = nullptr;
-  d.tstate[T_ANC] = b.take<unsigned long long>(tiles_of((long long)c.max_events * kAncBins + 1, kScanTile));
+  d.tstate[T_PT] = nullptr;  // ticket only
   d.tstate[T_PP3] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
-  d.tstate[T_IDX] = b.take<unsigned long long>(tiles_of(3LL * c.max_md + 1, kScanTile));
-  d.tstate[T_TC] = b.take<unsigned long long>(tiles_of(4LL * c.max_events + 1, kScanTile));
   d.sens_cnt = b.take<int>(n_sens + 1);
-  d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins + 1);
+  d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins);
   d.pls_pt3_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt3_cur = b.take<int>(c.max_pls);
   d.pls_pt5_cur = b.take<int>(c.max_pls);
+  d.tc_cnt = b.take<int>(4 * (size_t)c.max_events + 1);
+  d.tc_cur = b.take<int>(4 * (size_t)c.max_events + 1);
+  d.linked = b.take<unsigned char>(c.max_pls);
   b.off = (b.off + 255) & ~size_t(255);
   if (zero_bytes) *zero_bytes = b.off;
   // --- a0 ---
@@ -243,7 +246,6 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   }
   d.md_cnt = b.take<int>(c.max_hits);
   d.md_stash = b.take<int>(4 * (size_t)c.max_hits);
-  d.hit_md_begin = b.take<int>((size_t)c.max_hits + 1);
   d.mod_md_begin = b.take<int>(n_sens / 2 + 1);
   d.md_hit = b.take<int2>(c.max_md);
   d.md_info = b.take<int>(c.max_md);
@@ -258,23 +260,26 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.t3_ls = b.take<int2>(c.max_t3);
   d.t3_md = b.take<int4>(c.max_t3);
   d.t3_k = b.take<float>(c.max_t3);
-  d.t3_axy = b.take<float2>(c.max_t3);
-  d.t3_lxy = b.take<float2>(c.max_t3);
+  d.t3_l = b.take<float4>(c.max_t3);
   d.t3_t5_begin = b.take<int>((size_t)c.max_t3 + 1);
   d.t5_t3 = b.take<int2>(c.max_t5);
   d.t5_md = b.take<int>(5 * (size_t)c.max_t5);
   d.t5_score = b.take<float>(c.max_t5);
-  d.t5_axy = b.take<float2>(c.max_t5);
-  d.t5_lxy = b.take<float2>(c.max_t5);
+  d.t5_l = b.take<float4>(c.max_t5);
+  d.t5_kio = b.take<float2>(c.max_t5);
   // --- a5 ---
+  d.seed_a = b.take<float4>(c.max_pls);
+  d.seed_b = b.take<float4>(c.max_pls);
+  d.seed_z1 = b.take<float>(c.max_pls);
   d.pls_event = b.take<int>(c.max_pls);
   d.pt_ev = b.take<PtEvent>((size_t)c.max_events + 1);
   d.anc_bin = b.take<int>(c.max_md);
   d.anc_rank = b.take<int>(c.max_md);
-  d.anc_bin_begin = b.take<int>((size_t)c.max_events * kAncBins + 1);
-  d.anc_axy = b.take<float2>(c.max_md);
-  d.anc_t3 = b.take<int2>(c.max_md);
-  d.anc_t5 = b.take<int2>(c.max_md);
+  d.anc_a = b.take<float4>(c.max_md);
+  d.anc_t = b.take<int4>(c.max_md);
+  d.cap_queue = (int)(2LL * ((long long)c.max_pt3 + c.max_pt5) < 0x7fffffffLL ? 2LL * ((long long)c.max_pt3 + c.max_pt5)
+                                                                             : 0x7fffffffLL);
+  d.pt_queue = b.take<int2>(d.cap_queue);
   d.pls_pt3_begin = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_begin = b.take<int>((size_t)c.max_pls + 1);
   d.pt3 = b.take<int2>(c.max_pt3);
@@ -282,21 +287,15 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.pt5 = b.take<int2>(c.max_pt5);
   d.pt5_score = b.take<float>(c.max_pt5);
   // --- a6 ---
-  d.cap_idx = (int)(5LL * c.max_t5 + 5LL * c.max_pt5 + 3LL * c.max_pt3 < 0x7fffffffLL
-                        ? 5LL * c.max_t5 + 5LL * c.max_pt5 + 3LL * c.max_pt3 : 0x7fffffffLL);
-  d.idx_cnt = b.take<int>(3 * (size_t)c.max_md + 1);
-  d.idx_begin = b.take<int>(3 * (size_t)c.max_md + 1);
-  d.idx_cur = b.take<int>(3 * (size_t)c.max_md + 1);
-  d.idx_list = b.take<int>(d.cap_idx);
+  d.idx_head = b.take<int>(3 * (size_t)c.max_md);
+  d.idx_next = b.take<int>(5 * (size_t)c.max_t5 + 5 * (size_t)c.max_pt5 + 3 * (size_t)c.max_pt3);
   d.keep5 = b.take<unsigned char>(c.max_pt5);
   d.keep3 = b.take<unsigned char>(c.max_pt3);
   d.keepT = b.take<unsigned char>(c.max_t5);
-  d.linked = b.take<unsigned char>(c.max_pls);
-  d.tc_cnt = b.take<int>(4 * (size_t)c.max_events + 1);
   d.tc_begin = b.take<int>(4 * (size_t)c.max_events + 1);
-  d.tc_cur = b.take<int>(4 * (size_t)c.max_events + 1);
   d.tc = b.take<int>(16 * (size_t)c.max_tc);
-  // --- staging of host inputs + per-event tables ---
+  d.ev_first = b.take<int>((size_t)(K_PT5 + 1) * (c.max_events + 1));
+  // --- staging of host inputs + per-event tables + the batch record ---
   float* fx = b.take<float>(c.max_hits);
   float* fy = b.take<float>(c.max_hits);
   float* fz = b.take<float>(c.max_hits);
@@ -306,12 +305,15 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   int* pq = b.take<int>(c.max_pls);
   int* ho = b.take<int>((size_t)c.max_events + 1);
   int* po = b.take<int>((size_t)c.max_events + 1);
-  int* ef = b.take<int>((size_t)(K_PT5 + 1) * (c.max_events + 1));
+  Batch* bt = b.take<Batch>(1);
+  d.batch = bt;
+  d.hit_ev_off = ho;
+  d.pls_ev_off = po;
   if (ctx) {
     ctx->in_x = fx;  ctx->in_y = fy;  ctx->in_z = fz;  ctx->in_sensor = is;
     ctx->p_pt = pf[0];  ctx->p_x0 = pf[1];  ctx->p_y0 = pf[2];  ctx->p_z0 = pf[3];
     ctx->p_x1 = pf[4];  ctx->p_y1 = pf[5];  ctx->p_z1 = pf[6];  ctx->p_q = pq;
-    ctx->d_hit_ev_off = ho;  ctx->d_pls_ev_off = po;  ctx->d_ev_first = ef;
+    ctx->d_hit_ev_off = ho;  ctx->d_pls_ev_off = po;  ctx->d_batch = bt;
   }
   d.cap[K_MD] = c.max_md;  d.cap[K_LS] = c.max_ls;  d.cap[K_T3] = c.max_t3;  d.cap[K_T5] = c.max_t5;
   d.cap[K_PT3] = c.max_pt3;  d.cap[K_PT5] = c.max_pt5;  d.cap[K_TC] = c.max_tc;
@@ -321,7 +323,8 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
 bool caps_ok(const lst_caps& c) {
   // max_md: the LS stage packs an MD index into 27 bits (lst_ls.cuh); max_pls: a seed slot into 16 bits per tile
   return c.max_events > 0 && c.max_hits > 0 && c.max_pls > 0 && c.max_md > 0 && c.max_ls > 0 && c.max_t3 > 0 &&
-         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_md <= LST_MAX_MD;
+         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_md <= LST_MAX_MD &&
+         5LL * c.max_t5 + 5LL * c.max_pt5 + 3LL * c.max_pt3 < 0x7fffffffLL && 16LL * c.max_tc < 0x7fffffffLL;
 }
 
 }  // namespace
@@ -336,6 +339,11 @@ extern "C" size_t lst_workspace_bytes(const lst_caps* caps, int32_t n_modules) {
 
 static void ctx_destroy(lst_ctx* ctx) {
   if (!ctx) return;
+  if (ctx->graph) cudaGraphExecDestroy(ctx->graph);
+  if (ctx->owned_stream) {
+    cudaStreamSynchronize(ctx->owned_stream);
+    cudaStreamDestroy(ctx->owned_stream);
+  }
   for (void* p : ctx->allocs) cudaFree(p);
   if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
   if (ctx->h_ev_cnt) cudaFreeHost(ctx->h_ev_cnt);
@@ -367,6 +375,9 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   ctx->h_tc_begin = nullptr;
   for (int i = 0; i <= kMaxKernels; ++i) ctx->ev[i] = nullptr;
   ctx->timing = false;
+  ctx->graph = nullptr;
+  ctx->owned_stream = nullptr;
+  ctx->use_graph = getenv("LST_NO_GRAPH") == nullptr && cuda_stream != nullptr;  // the legacy default stream cannot be captured
   ctx->n_kernels = 0;
   ctx->last_n_events = 0;
   ctx->synced = true;

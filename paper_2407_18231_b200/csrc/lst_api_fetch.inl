@@ -145,8 +145,16 @@ extern "C" int lst_run_event(lst_geometry* g, const lst_hits* hits, const lst_pl
     lst_caps c;
     lst_default_caps(&c);
     c.max_events = 1;
-    int rc = lst_ctx_create(g, &c, nullptr, &g->default_ctx);
-    if (rc != LST_OK) return rc;
+    // a stream of its own (a blocking one: ordered after the caller's work on the legacy default stream),
+    // so that the launch sequence can run as a CUDA graph
+    cudaStream_t own = nullptr;
+    if (cudaStreamCreate(&own) != cudaSuccess) return LST_ERR_CUDA;
+    int rc = lst_ctx_create(g, &c, own, &g->default_ctx);
+    if (rc != LST_OK) {
+      cudaStreamDestroy(own);
+      return rc;
+    }
+    g->default_ctx->owned_stream = own;
   }
   int rc = lst_ctx_run(g->default_ctx, 1, hits, seeds);
   if (rc != LST_OK) return rc;

@@ -13,8 +13,9 @@ inline int grid_for(const lst_geometry* g, long long n, int per_sm) {
 struct Launcher {
   lst_ctx* ctx;
   int k = 0;
+  bool capturing = false;
   void mark(const char* name) {
-    if (ctx->timing && k < kMaxKernels) {
+    if (ctx->timing && !capturing && k < kMaxKernels) {
       cudaEventRecord(ctx->ev[k], ctx->stream);
       ctx->kname[k] = name;
     }
@@ -25,6 +26,61 @@ struct Launcher {
     ctx->n_kernels = k;
   }
 };
+
+// The launch sequence of one batch on stream st.  Grids do not depend on the batch (every kernel is a
+// grid-stride or ticket loop over sizes read from device memory), so the sequence can be captured once.
+int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
+  Launcher& L = *Lp;
+  const lst_geometry* g = ctx->g;
+  const Dev& d = ctx->dev;
+  const int mask = g->cuts.stage_mask;
+  const int gp = g->n_sm * 4;  // persistent ticket / grid-stride kernels
+  const int gw = g->n_sm * 8;
+  CK(cudaMemsetAsync(ctx->zero_region, 0, ctx->zero_bytes, st));
+  L.mark("hist");
+  k_hist<<<gw, kBlock, 0, st>>>(d);
+  L.mark("scan_sensors");
+  k_scan<<<gp, kBlock, 0, st>>>(d.sens_cnt, d.sens_begin, &d.batch->n_events, 2 * g->n_mod, 0, d.ctl->ticket + T_SENS,
+                                d.tstate[T_SENS]);
+  L.mark("scatter");
+  k_scatter<<<gw, kBlock, 0, st>>>(d);
+  L.mark("md");
+  k_md_eval<<<ctx->grid_md, kBlock, 0, st>>>(d);
+  L.mark("md_place");
+  k_md_place<<<gw, kBlock, 0, st>>>(d);
+  L.mark("ls");
+  k_ls_eval<<<ctx->grid_ls, kBlock, 0, st>>>(d);
+  L.mark("ls_place");
+  k_ls_place<<<gp, kBlock, 0, st>>>(d);
+  L.mark("t3");
+  k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
+  L.mark("t5");
+  k_stage<StageT5><<<gp, kBlock, 0, st>>>(d);
+  L.mark("anchor_sort");
+  k_anchor_sort<<<ctx->caps.max_events * kAncBlocksPerEvent, kBlock, 0, st>>>(d);
+  L.mark("pt");
+  k_pt_eval<<<ctx->grid_pt, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
+  L.mark("pt_exact");
+  k_pt_exact<<<gp, kBlock, 0, st>>>(d);
+  L.mark("pt_scan");
+  k_scan2<<<dim3(g->n_sm, 2), kBlock, 0, st>>>(
+      ScanJob{d.pls_pt3_cnt, d.pls_pt3_begin, &d.batch->n_pls, 1, 0, d.ctl->ticket + T_PP3, d.tstate[T_PP3]},
+      ScanJob{d.pls_pt5_cnt, d.pls_pt5_begin, &d.batch->n_pls, 1, 0, d.ctl->ticket + T_PP5, d.tstate[T_PP5]});
+  L.mark("pt_place");
+  k_pt_place<<<gp, kBlock, 0, st>>>(d);
+  if (mask & 32) {
+    L.mark("rule1_pt5");
+    k_rule1<<<gp, kBlock, 0, st>>>(d);
+    L.mark("rule2_pt3");
+    k_rule2<<<gp, kBlock, 0, st>>>(d);
+    L.mark("rule3_t5");
+    k_rule3<<<gp, kBlock, 0, st>>>(d);
+    L.mark("tc_emit");
+    k_tc_emit<<<gp, kBlock, 0, st>>>(d);
+  }
+  CK(cudaGetLastError());
+  return LST_OK;
+}
 
 bool offsets_ok(const int32_t* off, int n_events, int n) {
   if (off[0] != 0 || off[n_events] != n) return false;
@@ -70,120 +126,75 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   CK(cudaMemcpyAsync(ctx->d_hit_ev_off, ctx->last_hit_off.data(), eo, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(ctx->d_pls_ev_off, ctx->last_pls_off.data(), eo, cudaMemcpyHostToDevice, st));
 
-  Dev d = ctx->dev;
-  d.n_events = n_events;
-  d.n_hits = hits->n;
-  d.n_pls = n_pls;
-  d.hit_ev_off = ctx->d_hit_ev_off;
-  d.pls_ev_off = ctx->d_pls_ev_off;
+  Batch bt;
+  memset(&bt, 0, sizeof(bt));
+  bt.n_events = n_events;
+  bt.n_hits = hits->n;
+  bt.n_pls = n_pls;
   if (hits->on_device || hits->n == 0) {
-    d.in_x = hits->x;  d.in_y = hits->y;  d.in_z = hits->z;  d.in_sensor = hits->sensor;
+    bt.in_x = hits->x;  bt.in_y = hits->y;  bt.in_z = hits->z;  bt.in_sensor = hits->sensor;
   } else {
     const size_t nb = sizeof(float) * hits->n;
     CK(cudaMemcpyAsync(ctx->in_x, hits->x, nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->in_y, hits->y, nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->in_z, hits->z, nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->in_sensor, hits->sensor, nb, cudaMemcpyHostToDevice, st));
-    d.in_x = ctx->in_x;  d.in_y = ctx->in_y;  d.in_z = ctx->in_z;  d.in_sensor = ctx->in_sensor;
+    bt.in_x = ctx->in_x;  bt.in_y = ctx->in_y;  bt.in_z = ctx->in_z;  bt.in_sensor = ctx->in_sensor;
   }
   if (n_pls > 0) {
     if (seeds->on_device) {
-      d.p_pt = seeds->pt;  d.p_q = seeds->q;
-      d.p_x0 = seeds->x0;  d.p_y0 = seeds->y0;  d.p_z0 = seeds->z0;
-      d.p_x1 = seeds->x1;  d.p_y1 = seeds->y1;  d.p_z1 = seeds->z1;
+      bt.p_pt = seeds->pt;  bt.p_q = seeds->q;
+      bt.p_x0 = seeds->x0;  bt.p_y0 = seeds->y0;  bt.p_z0 = seeds->z0;
+      bt.p_x1 = seeds->x1;  bt.p_y1 = seeds->y1;  bt.p_z1 = seeds->z1;
     } else {
       const size_t nb = sizeof(float) * n_pls;
       const float* src[7] = {seeds->pt, seeds->x0, seeds->y0, seeds->z0, seeds->x1, seeds->y1, seeds->z1};
       float* dst[7] = {ctx->p_pt, ctx->p_x0, ctx->p_y0, ctx->p_z0, ctx->p_x1, ctx->p_y1, ctx->p_z1};
       for (int k = 0; k < 7; ++k) CK(cudaMemcpyAsync(dst[k], src[k], nb, cudaMemcpyHostToDevice, st));
       CK(cudaMemcpyAsync(ctx->p_q, seeds->q, nb, cudaMemcpyHostToDevice, st));
-      d.p_pt = ctx->p_pt;  d.p_q = ctx->p_q;
-      d.p_x0 = ctx->p_x0;  d.p_y0 = ctx->p_y0;  d.p_z0 = ctx->p_z0;
-      d.p_x1 = ctx->p_x1;  d.p_y1 = ctx->p_y1;  d.p_z1 = ctx->p_z1;
+      bt.p_pt = ctx->p_pt;  bt.p_q = ctx->p_q;
+      bt.p_x0 = ctx->p_x0;  bt.p_y0 = ctx->p_y0;  bt.p_z0 = ctx->p_z0;
+      bt.p_x1 = ctx->p_x1;  bt.p_y1 = ctx->p_y1;  bt.p_z1 = ctx->p_z1;
     }
   }
+  // the batch record (pageable source: staged by the runtime before this call returns)
+  CK(cudaMemcpyAsync(ctx->d_batch, &bt, sizeof(Batch), cudaMemcpyHostToDevice, st));
 
-  const lst_geometry* g = ctx->g;
-  const int mask = g->cuts.stage_mask;
-  const int n_sens = n_events * 2 * g->n_mod;
-  const int gp = g->n_sm * 4;  // persistent ticket kernels
-  Launcher L{ctx};
-
-  CK(cudaMemsetAsync(ctx->zero_region, 0, ctx->zero_bytes, st));
-  L.mark("hist");
-  k_hist<<<grid_for(g, hits->n > n_pls ? hits->n : n_pls, 8), kBlock, 0, st>>>(d);
-  L.mark("scan_sensors");
-  k_scan<<<grid_for(g, (n_sens + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
-      d.sens_cnt, d.sens_begin, nullptr, 0, n_sens, d.ctl->ticket + T_SENS, d.tstate[T_SENS]);
-  L.mark("scatter");
-  k_scatter<<<grid_for(g, hits->n, 8), kBlock, 0, st>>>(d);
-  L.mark("md");
-  k_md_eval<<<ctx->grid_md, kBlock, 0, st>>>(d);
-  L.mark("md_scan");
-  k_scan_t<16><<<grid_for(g, (hits->n + 16) / 16, 4), kBlock, 0, st>>>(
-      d.md_cnt, d.hit_md_begin, nullptr, 0, hits->n, d.ctl->ticket + T_MD, d.tstate[T_MD]);
-  L.mark("md_place");
-  k_md_place<<<grid_for(g, hits->n, 8), kBlock, 0, st>>>(d);
-  L.mark("ls");
-  k_ls_eval<<<ctx->grid_ls, kBlock, 0, st>>>(d);
-  L.mark("ls_scan");
-  k_scan<<<gp, kBlock, 0, st>>>(d.ls_cnt, d.md_ls_begin, d.ctl->total + K_MD, 1, 0, d.ctl->ticket + T_LS, d.tstate[T_LS]);
-  L.mark("ls_place");
-  k_ls_place<<<gp, kBlock, 0, st>>>(d);
-  L.mark("t3");
-  k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
-  L.mark("t5");
-  k_stage<StageT5><<<gp, kBlock, 0, st>>>(d);
-  L.mark("anchors");
-  k_anchor<<<gp, kBlock, 0, st>>>(d);
-  L.mark("anchor_scan");
-  k_scan<<<grid_for(g, (n_events * kAncBins + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
-      d.anc_bin_cnt, d.anc_bin_begin, nullptr, 0, n_events * kAncBins, d.ctl->ticket + T_ANC, d.tstate[T_ANC]);
-  L.mark("anchor_sort");
-  k_anchor_sort<<<gp, kBlock, 0, st>>>(d);
-  L.mark("pt_tiles");
-  k_pt_tiles<<<1, kBlock, 0, st>>>(d);
-  L.mark("pt");
-  k_pt_eval<<<ctx->grid_pt, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
-  L.mark("pt3_scan");
-  k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
-      d.pls_pt3_cnt, d.pls_pt3_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP3, d.tstate[T_PP3]);
-  L.mark("pt3_place");
-  k_pt_place<false><<<gp, kBlock, 0, st>>>(d);
-  L.mark("pt5_scan");
-  k_scan<<<grid_for(g, (n_pls + kScanItems) / kScanItems, 4), kBlock, 0, st>>>(
-      d.pls_pt5_cnt, d.pls_pt5_begin, nullptr, 0, n_pls, d.ctl->ticket + T_PP5, d.tstate[T_PP5]);
-  L.mark("pt5_place");
-  k_pt_place<true><<<gp, kBlock, 0, st>>>(d);
-  L.mark("event_ranges");
-  k_event_ranges<<<1, 64, 0, st>>>(d, ctx->d_ev_first);
-  if (mask & 32) {
-    L.mark("sel_prepare");
-    k_sel_prepare<<<gp, kBlock, 0, st>>>(d);
-    L.mark("index_count");
-    k_index<false><<<gp, kBlock, 0, st>>>(d);
-    L.mark("scan_index");
-    k_scan<<<gp, kBlock, 0, st>>>(d.idx_cnt, d.idx_begin, d.ctl->total + K_MD, 3, 0, d.ctl->ticket + T_IDX,
-                                  d.tstate[T_IDX]);
-    L.mark("index_fill");
-    k_index<true><<<gp, kBlock, 0, st>>>(d);
-    L.mark("rule1_pt5");
-    k_rule1<<<gp, kBlock, 0, st>>>(d);
-    L.mark("rule2_pt3");
-    k_rule2<<<gp, kBlock, 0, st>>>(d);
-    L.mark("rule3_t5");
-    k_rule3<<<gp, kBlock, 0, st>>>(d);
-    L.mark("scan_tc");
-    k_scan<<<1, kBlock, 0, st>>>(d.tc_cnt, d.tc_begin, nullptr, 0, 4 * n_events, d.ctl->ticket + T_TC,
-                                 d.tstate[T_TC]);
-    L.mark("tc_emit");
-    k_tc_emit<<<gp, kBlock, 0, st>>>(d, ctx->d_ev_first);
+  // ---- the launch sequence: memset + 18 kernels (12 without the selection), as a CUDA graph ----
+  const int mask = ctx->g->cuts.stage_mask;
+  if (ctx->timing || !ctx->use_graph) {
+    Launcher L{ctx};
+    int rc = enqueue(ctx, st, &L);
+    if (rc != LST_OK) return rc;
+    L.finish();
+  } else {
+    if (!ctx->graph) {
+      cudaGraph_t graph = nullptr;
+      CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+      Launcher L{ctx};
+      L.capturing = true;
+      const int rc = enqueue(ctx, st, &L);
+      const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+      if (rc != LST_OK || ce != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return LST_ERR_CUDA;
+      }
+      const cudaError_t ie = cudaGraphInstantiate(&ctx->graph, graph, 0);
+      cudaGraphDestroy(graph);
+      if (ie != cudaSuccess) {
+        ctx->graph = nullptr;
+        return LST_ERR_CUDA;
+      }
+      ctx->n_kernels = L.k;
+    }
+    CK(cudaGraphLaunch(ctx->graph, st));
   }
-  L.finish();
   CK(cudaGetLastError());
+  const Dev& d = ctx->dev;
   CK(cudaMemcpyAsync(ctx->h_ctl, d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
   CK(cudaMemcpyAsync(ctx->h_ev_cnt, d.ev_cnt, sizeof(unsigned long long) * kEvCnt * n_events, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(ctx->h_ev_first, ctx->d_ev_first, sizeof(int) * (K_PT5 + 1) * (n_events + 1),
+  CK(cudaMemcpyAsync(ctx->h_ev_first, d.ev_first, sizeof(int) * (K_PT5 + 1) * (n_events + 1),
                      cudaMemcpyDeviceToHost, st));
   if (mask & 32)
     CK(cudaMemcpyAsync(ctx->h_tc_begin, d.tc_begin, sizeof(int) * (4 * (size_t)n_events + 1), cudaMemcpyDeviceToHost, st));
@@ -241,4 +252,13 @@ extern "C" int lst_ctx_kernel_times(lst_ctx* ctx, float* ms, const char** names,
 extern "C" int lst_ctx_launch_count(lst_ctx* ctx) {
   if (!ctx || ctx->magic != MAGIC_CTX) return LST_ERR_ARG;
   return ctx->n_kernels;
+}
+
+extern "C" int64_t lst_ctx_stat(lst_ctx* ctx, int32_t which) {
+  if (!ctx || ctx->magic != MAGIC_CTX) return LST_ERR_ARG;
+  switch (which) {
+    case LST_STAT_PT_QUEUE: return ctx->synced ? (int64_t)ctx->h_ctl->queue_cur : (int64_t)LST_ERR_ARG;
+    case LST_STAT_WORKSPACE_MB: return (int64_t)(ctx->bytes >> 20);
+    default: return LST_ERR_ARG;
+  }
 }

@@ -84,35 +84,69 @@ __device__ __forceinline__ unsigned pt_after_gate(const Cuts& c, const Seed& s, 
   return res | ACC;
 }
 
-// Necessary condition of the curvature match |kx - kp| <= tolk, kx = kappa3(P1, A, L) (CUTS.md
-// section 7), without sqrt or division: compares kx^2 = 4 crs^2 / (|P1A|^2 |AL|^2 |P1L|^2) with
-// (|kp| -+ tolk)^2.  false = the exact cut rejects AND is not near-threshold.
-// Inequality chain.  Let k2/prod = kx~^2 be what is computed here and kx the spec's binary32 value: crs is
-// formed exactly as in kappa3 (same operands, same order), the rest differs by |kx~ - kx| <= d |kx| with
-// d < 4e-6 (three sqrt, four products and one division on the spec's side, five products here).  The exact
-// cut flags or accepts only if |kp| - tolk (1 + 1e-5) <= |kx| <= |kp| + tolk (1 + 1e-5).  With
-// m = 1e-3 (|kp| + tolk):
-//   reject high: |kx~| > hi = |kp| + tolk + m   =>  |kx| >= |kx~| (1 - d) > |kp| + tolk (1 + 1e-5)
-//   reject low:  |kx~| < lo = |kp| - tolk - m   =>  |kx| <= |kx~| (1 + d) < |kp| - tolk (1 + 1e-5)
-// because m - d (|kp| + tolk + m) > 1e-5 tolk (m is taken relative to |kp| + tolk, NOT to |kp| - tolk: the
-// latter margin vanishes where |kp| ~ tolk, i.e. for seeds of pT ~ 20.4 GeV).  The sign test needs lo > 0.
-// kp = (-q) / (pt * KR), tolk = PT_K_TOL0 + PT_K_TOL1 * |kp| (as in make_seed).
-__device__ __forceinline__ bool pt_curv_possible(float kp, float tolk, float x1, float y1, float2 A, float2 L) {
-  const float ax = A.x - x1, ay = A.y - y1;
-  const float bx = L.x - A.x, by = L.y - A.y;
-  const float cx = L.x - x1, cy = L.y - y1;
-  const float crs = ax * cy - ay * cx;
-  const float prod = ((ax * ax + ay * ay) * (bx * bx + by * by)) * (cx * cx + cy * cy);
-  const float k2 = 4.0f * (crs * crs);
-  const float m = 1e-3f * (fabsf(kp) + tolk);
-  const float hi = (fabsf(kp) + tolk) + m;
-  if (k2 > (hi * hi) * prod) return false;
-  const float lo = (fabsf(kp) - tolk) - m;
-  if (lo > 0.0f) {
-    if (k2 < (lo * lo) * prod) return false;
-    if ((crs > 0.0f) != (kp > 0.0f)) return false;  // |kx| >= lo (1 - d) > 0 with the wrong sign: |kx - kp| > |kp| > tolk (1 + 1e-5)
-  }
-  return true;
+// ---- approximate cascade: which candidates can the exact cuts accept or flag? -------------------------
+// The seed linking evaluates ~1e7 (seed, T3 / T5) candidates per batch behind the gate and accepts 0.06 %.
+// The exact cut list (precise sqrt and division, ~700 thread instructions) is therefore run only on the
+// candidates that an APPROXIMATE evaluation of the same cuts, in the same order, cannot reject for sure:
+//   * kx~ ~ kappa3(P1, A, L): crs is formed exactly as in kappa3 (same operands, same order, no FMA), the
+//     three lengths by ONE rsqrt.approx of the product of the squared lengths.  Against the spec's binary32
+//     kx: |kx~ - kx| <= d |kx|, d < 1.2e-6 (spec side: three sqrt, two products, one division <= 9 ulp;
+//     here: three fused squares, two products, rsqrt.approx (2^-22), one product <= 8 ulp; 1 ulp = 6e-8);
+//     the bands below take d = 4e-6.
+//   * a cut v <= t is classified with a band b >= |v~ - v| + 1e-5 t (the near-threshold window):
+//     v~ > t + b: the exact cut fails and is not near; v~ < t - b: it passes and is not near; otherwise
+//     (or when an operand is NaN / out of the approximation's range) the candidate goes to the exact cuts.
+//   * a candidate is dropped only at a cut that surely fails AFTER cuts that surely pass: it is then
+//     rejected by the spec at that cut without a near flag, so objects AND counters are unchanged
+//     (CUTS.md section 0: evaluation stops at the first failed cut).
+// Bands: curvature cuts b = 1.2e-5 tolk + 4e-6 |kx~| (|dp~ - dp| <= d |kx|);
+//        r-z cuts      b = 1.2e-5 zt + 8e-6 |slope sq~| + 1e-6 (|z1| + |zQ|)
+//        (sq = lq g((lq kx / 2)^2): rel. error <= 3 ulp (lq) + 0.43 * 2 (d + 5 ulp) (g, u g'/g <= 0.43 on
+//        u <= 1) + polynomial rounding < 5e-6; the last term covers the roundings of the sum).
+enum PtClass : int { PT_FAIL = 0, PT_PASS = 1, PT_UNSURE = 2 };
+
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// kx~; ok = false when the product of the squared lengths leaves the range where the bound holds
+__device__ __forceinline__ float kx_approx(float x1, float y1, float xa, float ya, float xl, float yl, bool& ok) {
+  const float ax = xa - x1, ay = ya - y1;
+  const float bx = xl - xa, by = yl - ya;
+  const float cx = xl - x1, cy = yl - y1;
+  const float crs = ax * cy - ay * cx;  // no FMA contraction in this translation unit: the spec's crs
+  const float prod = (fmaf(ax, ax, ay * ay) * fmaf(bx, bx, by * by)) * fmaf(cx, cx, cy * cy);
+  ok = prod >= 1e-30f && prod <= 1e30f;
+  return (2.0f * crs) * rsqrt_approx(prod);
+}
+
+__device__ __forceinline__ int classify(float v, float t, float band, bool ok) {
+  if (ok && v > t + band) return PT_FAIL;
+  if (ok && v < t - band) return PT_PASS;
+  return PT_UNSURE;  // includes every NaN
+}
+
+__device__ __forceinline__ int pt_class_curv(float kx, float kref, float tolk, bool ok) {
+  return classify(fabsf(kx - kref), tolk, 1.2e-5f * fabsf(tolk) + 4e-6f * fabsf(kx), ok);
+}
+
+// r-z cut at Q = (x, y, z, r | endcap << 31)
+__device__ __forceinline__ int pt_class_rz(const Cuts& c, float x1, float y1, float z1, float slope, float kx,
+                                           float4 Q, bool ok) {
+  const float qx = Q.x - x1, qy = Q.y - y1;
+  const float lq2 = fmaf(qx, qx, qy * qy);
+  ok = ok && lq2 >= 1e-30f && lq2 <= 1e30f;
+  const float lq = lq2 * rsqrt_approx(lq2);
+  const float tq = (lq * kx) * 0.5f;
+  const float sq = lq * g_poly(tq * tq);
+  const float pred = slope * sq;
+  const float zq = fabsf(Q.z - (z1 + pred));
+  const bool eQ = __float_as_int(Q.w) < 0;
+  const float zt = eQ ? c.pt_z_tol * (1.0f + __fdividef(fabsf(Q.z), fabsf(Q.w))) : c.pt_z_tol;
+  const float band = 1.2e-5f * fabsf(zt) + 8e-6f * fabsf(pred) + 1e-6f * (fabsf(z1) + fabsf(Q.z));
+  return classify(zq, zt, band, ok && fabsf(tq) <= 1.0f);
 }
 
 }  // namespace lst

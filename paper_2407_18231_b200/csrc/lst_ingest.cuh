@@ -2,6 +2,7 @@
 // plus the generic single-pass exclusive scan kernel.  PAPER.md:23 ("uses as input the hits of the
 // ... outer tracker"); SURVEY.md section 8(a) row a0.
 #pragma once
+#include "lst_cuts_pt.cuh"
 #include "lst_scan.cuh"
 #include "lst_types.cuh"
 
@@ -24,6 +25,7 @@ __device__ __forceinline__ int event_of(const int* __restrict__ off, int n_event
 constexpr int kIngestUnroll = 4;
 
 __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
+  load_batch(d);
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
   for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {
@@ -51,9 +53,16 @@ __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
       }
     }
   }
-  // pLS -> event (tiny; rides along)
-  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < d.n_pls; p += stride)
+  // pLS -> event, and the per-seed quantities of CUTS.md section 7 (computed once per seed, exactly as
+  // written there: lv, kp, tolk, slope); tiny, rides along
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < d.n_pls; p += stride) {
     d.pls_event[p] = event_of(d.pls_ev_off, d.n_events, p);
+    const Seed s = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p), __ldg(d.p_y0 + p),
+                             __ldg(d.p_z0 + p), __ldg(d.p_x1 + p), __ldg(d.p_y1 + p), __ldg(d.p_z1 + p));
+    d.seed_a[p] = make_float4(s.x1, s.y1, s.vx, s.vy);
+    d.seed_b[p] = make_float4(s.lv, s.kp, s.tolk, s.slope);
+    d.seed_z1[p] = s.z1;
+  }
 }
 
 // Generic exclusive scan out[i] = sum_{j<i} in[j], i in [0, n], n = (*n_ptr) * n_mul + n_add
@@ -63,17 +72,26 @@ __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
 constexpr int kScanItems = 4;
 constexpr int kScanTile = kBlock * kScanItems;
 
+struct ScanJob {
+  const int* in;
+  int* out;
+  const int* n_ptr;
+  int n_mul, n_add;
+  int* ticket;
+  unsigned long long* state;
+};
+
 template <int ITEMS>
-__global__ void __launch_bounds__(kBlock)
-k_scan_t(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int n_mul, int n_add,
-         int* ticket, unsigned long long* state) {
+__device__ __forceinline__ void scan_body(const ScanJob& j) {
   constexpr int kTile = kBlock * ITEMS;
   __shared__ int s_tile;
   __shared__ int s_scan[kWarps + 2];
-  const int n = (n_ptr ? (*n_ptr) * n_mul : 0) + n_add;
+  const int* __restrict__ in = j.in;
+  int* __restrict__ out = j.out;
+  const int n = (j.n_ptr ? (*j.n_ptr) * j.n_mul : 0) + j.n_add;
   const int n_tiles = (n + kTile - 1) / kTile > 0 ? (n + kTile - 1) / kTile : 1;
   for (;;) {
-    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1);
+    if (threadIdx.x == 0) s_tile = atomicAdd(j.ticket, 1);
     __syncthreads();
     const int tile = s_tile;
     if (tile >= n_tiles) break;
@@ -93,7 +111,7 @@ k_scan_t(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, in
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) sum += v[k];
     int tb, tt;
-    int off = tile_alloc(sum, state, tile, s_scan, tb, tt);
+    int off = tile_alloc(sum, j.state, tile, s_scan, tb, tt);
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
       if (base_i + k < n) out[base_i + k] = off;
@@ -103,10 +121,23 @@ k_scan_t(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, in
   }
 }
 
+template <int ITEMS>
+__global__ void __launch_bounds__(kBlock)
+k_scan_t(const int* __restrict__ in, int* __restrict__ out, const int* n_ptr, int n_mul, int n_add,
+         int* ticket, unsigned long long* state) {
+  scan_body<ITEMS>(ScanJob{in, out, n_ptr, n_mul, n_add, ticket, state});
+}
+
+// two independent scans in one launch (blockIdx.y picks the job)
+__global__ void __launch_bounds__(kBlock) k_scan2(ScanJob j0, ScanJob j1) {
+  scan_body<kScanItems>(blockIdx.y ? j1 : j0);
+}
+
 #define k_scan k_scan_t<kScanItems>
 
 // a0.3 scatter: sorted SoA (float4 x,y,z,r + int2 input index, global sensor), r = sqrtf(x*x + y*y)
 __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
+  load_batch(d);
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
   for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {

@@ -13,7 +13,7 @@
 //     whatever the list lengths; accepted (B, kappa) pairs are compacted in pair order with one
 //     ballot per step and copied to a scratch list with one atomic per warp pass (a pass with more
 //     than kLsStage LSs evaluates its pairs again and writes directly);
-//   * k_scan turns the per-MD counts into md_ls_begin; k_ls_place copies each MD's LSs to their slot.
+//   * k_ls_place scans the per-MD counts into md_ls_begin (fused, look-back) and copies each MD's LSs to their slot.
 // LSs therefore sit grouped by inner MD (what T3 building looks up); the order inside an MD's range
 // is free (reading S9).
 #pragma once
@@ -46,6 +46,7 @@ struct LsWarp {  // per-warp scratch in shared memory
 };
 
 __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
+  load_batch(d);
   __shared__ LsWarp s_w[kWarps];
   __shared__ unsigned long long s_tests[kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -190,28 +191,48 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
   tbl.flush();
 }
 
-// After k_scan(ls_cnt -> md_ls_begin): every MD's LSs go from the scratch list to their final slot.
+// Placement with the exclusive scan of ls_cnt fused in (tiles of kBlock inner MDs by ticket, block scan +
+// look-back): every MD's LSs go from the scratch list to their final slot, md_ls_begin is written on the
+// way.  Rides along: the three list heads of every MD of the duplicate-removal index are cleared.
 __global__ void __launch_bounds__(kBlock) k_ls_place(Dev d) {
+  load_batch(d);
+  __shared__ int s_tile;
+  __shared__ int s_scan[kWarps + 2];
   const int n_md = d.ctl->total[K_MD];
   const int total = d.ctl->scratch_cur[1];
   const int cap = d.cap[K_LS];
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    if (total > cap) {
-      atomicOr(&d.ctl->error, E_CAP_LS);
-      d.ctl->total[K_LS] = 0;
-    } else {
-      d.ctl->total[K_LS] = total;
-    }
-  }
-  if (total > cap) return;
+  const bool fits = total <= cap;
+  const int n_tiles = n_md > 0 ? (n_md + kBlock - 1) / kBlock : 1;
   const LsAccepted* scratch = reinterpret_cast<const LsAccepted*>(d.ev_scratch);
-  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < n_md; A += gridDim.x * blockDim.x) {
-    const int n = d.ls_cnt[A], src = d.ls_sbase[A];
-    const int dst = d.md_ls_begin[A];
-    for (int k = 0; k < n; ++k) {
-      const LsAccepted s = scratch[src + k];
-      d.ls_md[dst + k] = make_int2(A, s.B);
-      d.ls_kappa[dst + k] = s.kappa;
+  for (;;) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(d.ctl->ticket + T_LS, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int A = tile * kBlock + threadIdx.x;
+    const int n = (A < n_md && fits) ? d.ls_cnt[A] : 0;
+    int tb, tt;
+    const int dst = tile_alloc(n, d.tstate[T_LS], tile, s_scan, tb, tt);
+    if (A < n_md) {
+      d.md_ls_begin[A] = dst;
+      d.idx_head[A] = 0;
+      d.idx_head[n_md + A] = 0;
+      d.idx_head[2 * n_md + A] = 0;
+      const int src = d.ls_sbase[A];
+      for (int k = 0; k < n; ++k) {
+        const LsAccepted s = scratch[src + k];
+        d.ls_md[dst + k] = make_int2(A, s.B);
+        d.ls_kappa[dst + k] = s.kappa;
+      }
+    }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) {
+      d.md_ls_begin[n_md] = tb + tt;
+      if (!fits) {
+        atomicOr(&d.ctl->error, E_CAP_LS);
+        d.ctl->total[K_LS] = 0;
+      } else {
+        d.ctl->total[K_LS] = total;
+      }
     }
   }
 }

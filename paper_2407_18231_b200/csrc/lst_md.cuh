@@ -10,9 +10,8 @@
 //   * k_md_eval: a warp takes windows of 64 sorted hits, queues the upper-sensor ones (ballot), and
 //     whenever 32 are waiting every lane tests one against its module's lower hits; the positions of the first
 //     kMdStash accepted lower hits are stashed per upper hit, the count is exact;
-//   * k_scan turns the counts into hit_md_begin (MDs grouped by upper hit = by module);
-//   * k_md_place writes each upper hit's MDs (re-evaluating only the rare hit with more than kMdStash
-//     MDs) and the first MD of every module.
+//   * k_md_place scans the counts (fused, look-back) and writes each upper hit's MDs (re-evaluating only
+//     the rare hit with more than kMdStash MDs) and the first MD of every module.
 #pragma once
 #include "lst_stages.cuh"
 
@@ -21,6 +20,7 @@ namespace lst {
 constexpr int kMdStash = 4;  // stashed MDs per upper hit
 
 __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
+  load_batch(d);
   __shared__ int s_own[kWarps][96];
   __shared__ unsigned long long s_tests[kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -90,63 +90,120 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
   tbl.flush();
 }
 
-// After k_scan(md_cnt -> hit_md_begin).  MDs of upper hit i go to hit_md_begin[i] ..., in lower-hit order.
+// Placement with the exclusive scan of md_cnt fused in (tiles of kBlock * kMdPlaceItems sorted hits taken
+// by ticket, block scan + decoupled look-back): the MDs of upper hit i go to the running offset, in
+// lower-hit order, so MDs end up grouped by module.  The thread of the FIRST hit after a module boundary
+// also writes mod_md_begin for the modules that start there (empty modules in between included); gaps
+// longer than kMdGapSerial modules (sparse batches) are filled by the whole block.
+constexpr int kMdPlaceItems = 4;
+constexpr int kMdGapSerial = 16;
+constexpr int kMdBigGaps = 16;
+
 __global__ void __launch_bounds__(kBlock) k_md_place(Dev d) {
+  load_batch(d);
   static_assert(kMdStash == 4, "the stash is stored as one int4 per hit");
+  constexpr int kTile = kBlock * kMdPlaceItems;
+  __shared__ int s_tile;
+  __shared__ int s_scan[kWarps + 2];
+  __shared__ int s_nbig;
+  __shared__ int s_big[kMdBigGaps][3];  // (first module, one past the last, offset)
   const bool on = (d.cuts.stage_mask & 1) != 0;
   const int n = on ? d.n_hits : 0;
-  const int total = on ? d.hit_md_begin[d.n_hits] : 0;
   const int cap = d.cap[K_MD];
-  const int stride = gridDim.x * blockDim.x, t0 = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t0 == 0) {
-    if (total > cap) {
-      atomicOr(&d.ctl->error, E_CAP_MD);
-      d.ctl->total[K_MD] = 0;
-    } else {
-      d.ctl->total[K_MD] = total;
-    }
-  }
-  // first MD of every module (MDs are owned by upper hits, so any hit of the lower range marks the start)
   const int n_gm = d.n_events * d.n_mod;
-  for (int gm = t0; gm <= n_gm; gm += stride)
-    d.mod_md_begin[gm] = (on && total <= cap) ? d.hit_md_begin[gm < n_gm ? __ldg(d.sens_begin + 2 * gm) : d.n_hits] : 0;
-  if (total > cap) return;
-  for (int i = t0; i < n; i += stride) {
-    const int cnt = d.md_cnt[i];
-    if (cnt == 0) continue;
-    const int2 ib = d.hit_ig[i];
-    const int gs = ib.y, gm = gs >> 1;
-    const int endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
-    const float4 hb = d.hit[i];
-    int pos = d.hit_md_begin[i];
-    auto emit = [&](int a) {  // unit direction exactly as in md_test (CUTS.md section 3)
-      const float4 ha = d.hit[a];
-      float ux = 0.0f, uy = 0.0f;
-      if (!endcap) {
-        const float dx = hb.x - ha.x, dy = hb.y - ha.y;
-        const float dd = sqrtf(dx * dx + dy * dy);
-        ux = dx / dd;
-        uy = dy / dd;
-      }
-      d.md_hit[pos] = make_int2(d.hit_ig[a].x, ib.x);
-      d.md_info[pos] = (gs - 1) | endcap;
-      d.md_a[pos] = ha;
-      d.md_u[pos] = make_float2(ux, uy);
-      ++pos;
-    };
-    if (cnt <= kMdStash) {
-      const int4 st = reinterpret_cast<const int4*>(d.md_stash)[i];
-      emit(st.x);
-      if (cnt > 1) emit(st.y);
-      if (cnt > 2) emit(st.z);
-      if (cnt > 3) emit(st.w);
-    } else {  // rare: more MDs than the stash holds -> evaluate this hit's candidates again
-      const int a1 = __ldg(d.sens_begin + gs);
-      for (int a = __ldg(d.sens_begin + gs - 1); a < a1; ++a) {
-        float ux, uy;
-        if (md_test(d.cuts, endcap, d.hit[a], hb, ux, uy) & ACC) emit(a);
+  const int n_tiles = n > 0 ? (n + kTile - 1) / kTile : 1;
+  // mod_md_begin[g0 .. g1) = off
+  auto fill = [&](int g0, int g1, int off) {
+    if (g1 - g0 <= kMdGapSerial) {
+      for (int g = g0; g < g1; ++g) d.mod_md_begin[g] = off;
+      return;
+    }
+    const int slot = atomicAdd(&s_nbig, 1);
+    if (slot < kMdBigGaps) {
+      s_big[slot][0] = g0;  s_big[slot][1] = g1;  s_big[slot][2] = off;
+    } else {
+      for (int g = g0; g < g1; ++g) d.mod_md_begin[g] = off;
+    }
+  };
+  for (;;) {
+    if (threadIdx.x == 0) {
+      s_tile = atomicAdd(d.ctl->ticket + T_MD, 1);
+      s_nbig = 0;
+    }
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int i0 = tile * kTile + threadIdx.x * kMdPlaceItems;
+    int cnt[kMdPlaceItems], sum = 0;
+#pragma unroll
+    for (int k = 0; k < kMdPlaceItems; ++k) {
+      cnt[k] = (i0 + k < n) ? d.md_cnt[i0 + k] : 0;
+      sum += cnt[k];
+    }
+    int tb, tt;
+    int pos = tile_alloc(sum, d.tstate[T_MD], tile, s_scan, tb, tt);
+    int gm_prev = (i0 > 0 && i0 <= n) ? (d.hit_ig[i0 - 1].y >> 1) : -1;
+#pragma unroll
+    for (int k = 0; k < kMdPlaceItems; ++k) {
+      const int i = i0 + k;
+      if (i >= n) break;
+      const int2 ib = d.hit_ig[i];
+      const int gs = ib.y, gm = gs >> 1;
+      if (gm != gm_prev) fill(gm_prev + 1, gm + 1, pos);  // the modules that begin at hit i
+      gm_prev = gm;
+      if (cnt[k] == 0) continue;
+      const int endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
+      const float4 hb = d.hit[i];
+      auto emit = [&](int a) {  // unit direction exactly as in md_test (CUTS.md section 3)
+        if (pos < cap) {
+          const float4 ha = d.hit[a];
+          float ux = 0.0f, uy = 0.0f;
+          if (!endcap) {
+            const float dx = hb.x - ha.x, dy = hb.y - ha.y;
+            const float dd = sqrtf(dx * dx + dy * dy);
+            ux = dx / dd;
+            uy = dy / dd;
+          }
+          d.md_hit[pos] = make_int2(d.hit_ig[a].x, ib.x);
+          d.md_info[pos] = (gs - 1) | endcap;
+          d.md_a[pos] = ha;
+          d.md_u[pos] = make_float2(ux, uy);
+        }
+        ++pos;
+      };
+      if (cnt[k] <= kMdStash) {
+        const int4 st = reinterpret_cast<const int4*>(d.md_stash)[i];
+        emit(st.x);
+        if (cnt[k] > 1) emit(st.y);
+        if (cnt[k] > 2) emit(st.z);
+        if (cnt[k] > 3) emit(st.w);
+      } else {  // rare: more MDs than the stash holds -> evaluate this hit's candidates again
+        const int a1 = __ldg(d.sens_begin + gs);
+        for (int a = __ldg(d.sens_begin + gs - 1); a < a1; ++a) {
+          float ux, uy;
+          if (md_test(d.cuts, endcap, d.hit[a], hb, ux, uy) & ACC) emit(a);
+        }
       }
     }
+    const int total = tb + tt;
+    if (tile == n_tiles - 1) {
+      // the modules after the last hit (all of them when there is no hit), and the totals
+      const int last = n - 1 - tile * kTile;  // position of the last hit in this tile, -1 = no hit at all
+      if (n == 0 ? threadIdx.x == 0 : (last / kMdPlaceItems == threadIdx.x)) fill(n == 0 ? 0 : gm_prev + 1, n_gm + 1, total);
+      if (threadIdx.x == 0) {
+        if (total > cap) {
+          atomicOr(&d.ctl->error, E_CAP_MD);
+          d.ctl->total[K_MD] = 0;
+        } else {
+          d.ctl->total[K_MD] = total;
+        }
+      }
+    }
+    __syncthreads();
+    const int nbig = min(s_nbig, kMdBigGaps);
+    for (int b = 0; b < nbig; ++b)
+      for (int g = s_big[b][0] + threadIdx.x; g < s_big[b][1]; g += kBlock) d.mod_md_begin[g] = s_big[b][2];
+    __syncthreads();  // s_nbig / s_big are reset by the next tile
   }
 }
 

@@ -1,48 +1,75 @@
 // lst_pt.cuh -- step a5: pLS x T3 -> pT3 and pLS x T5 -> pT5 (CUTS.md section 7).
-// Candidates of a seed = every T3 / T5 of its event (CUTS.md section 7; the direction gate of the
-// spec replaces the IT->OT connection map): ~1.2e8 (seed, T3) pairs per 16-event PU200 batch, of
-// which 8% pass the gate and 0.06% are accepted.  This is the heaviest loop of the chain, so its
-// inner step is stripped to the arithmetic of a NECESSARY condition of the gate:
-//   * a tile = 256 candidates of one event (one per thread, first/last anchor in registers) x up
-//     to kSeedTile seeds of the same event (staged in shared memory, read as broadcasts);
-//   * phase 1 (every pair): gdot > 0 exactly as in the spec and gcrs <= glim with |A - P1| from
-//     the approximate reciprocal square root and a 1e-4 margin; a survivor costs one store into
-//     the thread's own queue -- no ballot, no index arithmetic;
-//   * phase 1b (8%): the exact gate (near-threshold accounting of CUTS.md section 0 happens here)
-//     and a sqrt-free necessary condition of the curvature match;
-//   * phase 2 (<1%): the exact cut list.
-// Accepted pairs go to a scratch list (atomics per accepted object, ~4 per 10^4 tests); k_pt_place
-// groups them by seed with a counting sort (count in phase 2, generic scan, scatter).  Order
-// inside a seed's range is arrival order -- free by the spec (reading S9).
+// Candidates of a seed = every T3 / T5 of its event (the direction gate of the spec replaces the IT->OT
+// connection map): ~1.2e8 (seed, T3) + 2.5e7 (seed, T5) pairs per 16-event PU200 batch, of which 8 % pass
+// the gate, 0.9 % the curvature match with the seed and 0.06 % are accepted.  Structure:
+//   * anchors: the gate depends only on the seed and the FIRST MD of the candidate, and T3s / T5s are stored
+//     grouped by first MD, so the gate is evaluated once per (seed, anchor) and shared by pT3 and pT5;
+//     anchors are sorted into radius x azimuth bins (lst_stages.cuh, k_anchor_sort);
+//   * k_pt_eval, tile = 32 anchors (one per lane) x 64 seeds of the same event (shared memory, broadcast):
+//     (1a) one seed per lane against the bounding circle of the warp's anchors;
+//     (1b) every lane tests its anchor against the seeds that may match: a necessary condition of the gate
+//          with |A - P1| from rsqrt.approx; only within 1e-4 of the threshold the exact gate decides (and
+//          flags near-threshold);
+//     (2)  gate survivors are expanded into their (seed, T3 / T5) candidates, flattened over the lanes;
+//          kx~ (lst_cuts_pt.cuh) drops those whose curvature match with the seed surely fails;
+//     (3)  the rest of the approximate cascade (stored curvatures, r-z at both ends) on full warps;
+//     what cannot be rejected for sure goes to a queue;
+//   * k_pt_exact runs the exact cut list of CUTS.md section 7 on the queue (1.1 x the accepted objects):
+//     accepted pairs go to scratch lists with a count per seed; k_scan2 + k_pt_place group them by seed.
+// Objects and both counters are those of the spec: lst_cuts_pt.cuh states why no pre-filter can change them.
 #pragma once
 #include "lst_cuts_pt.cuh"
 #include "lst_stages.cuh"
 
 namespace lst {
 
+__device__ __forceinline__ Seed seed_from_table(const Dev& d, int p) {
+  const float4 a = d.seed_a[p], b = d.seed_b[p];
+  Seed s;
+  s.x1 = a.x;  s.y1 = a.y;  s.z1 = d.seed_z1[p];
+  s.vx = a.z;  s.vy = a.w;  s.lv = b.x;
+  s.kp = b.y;  s.tolk = b.z;  s.slope = b.w;
+  return s;
+}
+
 template <bool IS5>
 struct PtCand {
-  // evaluates candidate t for seed s; returns ACC/NEAR bits, score on accept
+  // the exact cut list for seed s and candidate t; returns ACC/NEAR bits, score on accept
   static __device__ __forceinline__ unsigned test(const Dev& d, const Seed& s, int t, float& score) {
-    const float2 axy = IS5 ? d.t5_axy[t] : d.t3_axy[t];
-    unsigned r = pt_gate(d.cuts, s, axy.x, axy.y);
+    int A, L, eA, eL;
+    if (IS5) {
+      const int* md = d.t5_md + 5 * (size_t)t;
+      A = md[0];  L = md[4];
+      eA = d.md_info[A] & 1;  eL = d.md_info[L] & 1;
+    } else {
+      const int4 m = d.t3_md[t];
+      A = m.x;  L = m.z;
+      eA = m.w & 1;  eL = (m.w >> 2) & 1;
+    }
+    const float4 a = d.md_a[A];
+    unsigned r = pt_gate(d.cuts, s, a.x, a.y);
     if (!(r & ACC)) return r;
     r &= NEAR;
     if (IS5) {
-      const int* md = d.t5_md + 5 * (size_t)t;
-      const int A = md[0], L = md[4];
-      const int2 tt = d.t5_t3[t];
-      const float kt[2] = {d.t3_k[tt.x], d.t3_k[tt.y]};
-      r |= pt_after_gate<2>(d.cuts, s, d.md_a[A], d.md_info[A] & 1, d.md_a[L], d.md_info[L] & 1, kt,
-                            d.t5_score[t], score);
+      const float2 kio = d.t5_kio[t];
+      const float kt[2] = {kio.x, kio.y};
+      r |= pt_after_gate<2>(d.cuts, s, a, eA, d.md_a[L], eL, kt, d.t5_score[t], score);
     } else {
-      const int4 m = d.t3_md[t];
       const float kt[1] = {d.t3_k[t]};
-      r |= pt_after_gate<1>(d.cuts, s, d.md_a[m.x], m.w & 1, d.md_a[m.z], (m.w >> 2) & 1, kt, 0.0f,
-                            score);
+      r |= pt_after_gate<1>(d.cuts, s, a, eA, d.md_a[L], eL, kt, 0.0f, score);
     }
     return r;
   }
+};
+
+constexpr int kSeedTile = 64;           // seeds staged per tile
+constexpr int kAncBlocksPerEvent = 8;   // blocks of k_anchor_sort per event
+
+// per-event table written by k_anchor_sort: anchor range, seed range, first tile
+struct PtEvent {
+  int a0, a1;
+  int s0, s1;
+  int tile0;
 };
 
 // first candidate (T3 or T5) of event ev and one past its last
@@ -57,98 +84,76 @@ __device__ __forceinline__ void event_cands(const Dev& d, int ev, int& c0, int& 
   }
 }
 
-constexpr int kSeedTile = 128;  // seeds staged per tile
-
-// ---- anchors: the MDs that start at least one T3 (and therefore every T5) ----------------------
-// The gate of CUTS.md section 7 depends only on the seed and on the FIRST MD of the candidate, and
-// T3s / T5s are stored grouped by first MD: all candidates of an anchor share one gate evaluation.
-// The anchors of an event are sorted into kAncBins = 8 radial classes x 64 azimuthal sectors
-// (counting sort: k_anchor counts and keeps the arrival rank, k_scan, k_anchor_sort places), so the
-// 32 anchors of a warp of k_pt_eval sit within a few cm of each other and a seed whose gate cone
-// misses their bounding circle is skipped for the whole warp.
-constexpr int kAncBins = 512;
-
-__device__ __forceinline__ int anchor_bin(float x, float y, float r) {
-  const int rc = (r >= 29.5f) + (r >= 43.5f) + (r >= 59.5f) + (r >= 78.0f) + (r >= 98.0f) + (r >= 125.0f);
-  const float a = fabsf(x) + fabsf(y);
-  const float t = a > 0.0f ? y / a : 0.0f;                                  // diamond angle, monotone in azimuth
-  const float ps = x >= 0.0f ? (y >= 0.0f ? t : 4.0f + t) : 2.0f - t;      // [0, 4)
-  int sec = (int)(ps * 16.0f);
-  sec = sec < 0 ? 0 : (sec > 63 ? 63 : sec);
-  return rc * 64 + sec;  // any finite or non-finite input lands in [0, 512): binning never affects results
-}
-
-__global__ void __launch_bounds__(kBlock) k_anchor(Dev d) {
-  const bool on = (d.cuts.stage_mask & 16) && d.ctl->total[K_T3] > 0;
-  const int n = d.ctl->total[K_MD];
-  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < n; A += gridDim.x * blockDim.x) {
-    int bin = -1, rank = 0;
-    if (on && d.ls_t3_begin[d.md_ls_begin[A + 1]] > d.ls_t3_begin[d.md_ls_begin[A]]) {
-      const float4 a = d.md_a[A];
-      const int ev = (d.md_info[A] >> 1) / d.n_mod;
-      bin = ev * kAncBins + anchor_bin(a.x, a.y, a.w);
-      rank = atomicAdd(d.anc_bin_cnt + bin, 1);
-    }
-    d.anc_bin[A] = bin;
-    d.anc_rank[A] = rank;
-  }
-}
-
-// after k_scan(anc_bin_cnt -> anc_bin_begin)
+// Counting sort of an event's anchors by bin (the counts and arrival ranks come from the T5 kernel's
+// prologue).  grid = n_events * kAncBlocksPerEvent; every block scans the 512 bin counts of its event in
+// shared memory and places its share of the event's MDs; the anchors of event e start at the event's
+// first MD (an event has no more anchors than MDs), so no prefix across events is needed.  Block 0 also
+// writes the per-event table of k_pt_eval (ranges, tile prefix) and the candidate counts of stages 4, 5.
 __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
-  const bool on5 = d.ctl->total[K_T5] > 0;
-  const int n = d.ctl->total[K_MD];
-  for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < n; A += gridDim.x * blockDim.x) {
-    const int bin = d.anc_bin[A];
-    if (bin < 0) continue;
-    const int pos = d.anc_bin_begin[bin] + d.anc_rank[A];
-    const int t0 = d.ls_t3_begin[d.md_ls_begin[A]], t1 = d.ls_t3_begin[d.md_ls_begin[A + 1]];
-    const float4 a = d.md_a[A];
-    d.anc_axy[pos] = make_float2(a.x, a.y);
-    d.anc_t3[pos] = make_int2(t0, t1 - t0);
-    const int u0 = on5 ? d.t3_t5_begin[t0] : 0, u1 = on5 ? d.t3_t5_begin[t1] : 0;
-    d.anc_t5[pos] = make_int2(u0, u1 - u0);
-  }
-}
-
-// per-event table written by k_pt_tiles: anchor range, seed range, first tile
-struct PtEvent {
-  int a0, a1;
-  int s0, s1;
-  int tile0;
-};
-
-// One block.  Fills pt_ev[0..n_events) and pt_ev[n_events].tile0 = number of tiles; n_tests.
-__global__ void __launch_bounds__(kBlock) k_pt_tiles(Dev d) {
+  load_batch(d);
+  __shared__ int s_begin[kAncBins];
+  __shared__ int s_warp[kWarps];
   const int E = d.n_events;
-  const bool on = (d.cuts.stage_mask & 16) != 0;
-  for (int e = threadIdx.x; e < E; e += kBlock) {
-    PtEvent ev;
-    ev.s0 = d.pls_ev_off[e];
-    ev.s1 = d.pls_ev_off[e + 1];
-    ev.a0 = ev.a1 = 0;
-    const int ns = on ? ev.s1 - ev.s0 : 0;
-    int c0 = 0, c1 = 0;
-    if (on && d.ctl->total[K_T3] > 0) {
-      ev.a0 = d.anc_bin_begin[e * kAncBins];
-      ev.a1 = d.anc_bin_begin[(e + 1) * kAncBins];
-      event_cands<false>(d, e, c0, c1);
-      // candidates of CUTS.md section 7: every (seed, T3) of the event
-      d.ev_cnt[(size_t)e * kEvCnt + 6 + 4] = (unsigned long long)ns * (c1 - c0);
+  const int e = blockIdx.x / kAncBlocksPerEvent, part = blockIdx.x - e * kAncBlocksPerEvent;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool on = (d.cuts.stage_mask & 16) && d.ctl->total[K_T3] > 0 && d.n_pls > 0;
+  const bool on5 = d.ctl->total[K_T5] > 0;
+  if (on) {
+    // exclusive scan of the event's 512 bin counts: 2 per thread
+    const int c0 = d.anc_bin_cnt[e * kAncBins + 2 * threadIdx.x], c1 = d.anc_bin_cnt[e * kAncBins + 2 * threadIdx.x + 1];
+    const int incl = warp_incl_scan(c0 + c1);
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int base = 0;
+    for (int w = 0; w < warp; ++w) base += s_warp[w];
+    s_begin[2 * threadIdx.x] = base + incl - c0 - c1;
+    s_begin[2 * threadIdx.x + 1] = base + incl - c1;
+    __syncthreads();
+    const int md0 = d.mod_md_begin[e * d.n_mod], md1 = d.mod_md_begin[(e + 1) * d.n_mod];
+    for (int A = md0 + part * kBlock + threadIdx.x; A < md1; A += kAncBlocksPerEvent * kBlock) {
+      const int bin = d.anc_bin[A];
+      if (bin < 0) continue;
+      const int pos = md0 + s_begin[bin] + d.anc_rank[A];
+      const int t0 = d.ls_t3_begin[d.md_ls_begin[A]], t1 = d.ls_t3_begin[d.md_ls_begin[A + 1]];
+      const int u0 = on5 ? d.t3_t5_begin[t0] : 0, u1 = on5 ? d.t3_t5_begin[t1] : 0;
+      d.anc_a[pos] = pack_flag(d.md_a[A], d.md_info[A] & 1);
+      d.anc_t[pos] = make_int4(t0, t1 - t0, u0, u1 - u0);
     }
-    if (on && d.ctl->total[K_T5] > 0) {
-      event_cands<true>(d, e, c0, c1);
-      d.ev_cnt[(size_t)e * kEvCnt + 6 + 5] = (unsigned long long)ns * (c1 - c0);
+  }
+  if (blockIdx.x != 0) return;
+  __syncthreads();
+  // ---- the event table (block 0): anchors = sum of the event's bin counts ----
+  for (int ev = warp; ev < E; ev += kWarps) {
+    int n_a = 0;
+    if (on)
+      for (int b = lane; b < kAncBins; b += 32) n_a += d.anc_bin_cnt[ev * kAncBins + b];
+    n_a = warp_sum(n_a);
+    if (lane == 0) {
+      PtEvent pe;
+      pe.s0 = d.pls_ev_off[ev];
+      pe.s1 = d.pls_ev_off[ev + 1];
+      pe.a0 = on ? d.mod_md_begin[ev * d.n_mod] : 0;
+      pe.a1 = pe.a0 + n_a;
+      const int ns = on ? pe.s1 - pe.s0 : 0;
+      pe.tile0 = ((n_a + 31) / 32) * ((ns + kSeedTile - 1) / kSeedTile);  // warp tiles; prefix below
+      d.pt_ev[ev] = pe;
+      int c0 = 0, c1 = 0;
+      if (on) {  // candidates of CUTS.md section 7: every (seed, T3) and (seed, T5) of the event
+        event_cands<false>(d, ev, c0, c1);
+        d.ev_cnt[(size_t)ev * kEvCnt + 6 + 4] = (unsigned long long)ns * (c1 - c0);
+        if (on5) {
+          event_cands<true>(d, ev, c0, c1);
+          d.ev_cnt[(size_t)ev * kEvCnt + 6 + 5] = (unsigned long long)ns * (c1 - c0);
+        }
+      }
     }
-    ev.tile0 = ((ev.a1 - ev.a0 + 31) / 32) * ((ns + kSeedTile - 1) / kSeedTile);  // warp tiles
-    d.pt_ev[e] = ev;
   }
   __syncthreads();
   if (threadIdx.x == 0) {  // exclusive prefix of the tile counts (n_events is small)
     int a = 0;
-    for (int e = 0; e < E; ++e) {
-      const int ta = d.pt_ev[e].tile0;
-      d.pt_ev[e].tile0 = a;
+    for (int ev = 0; ev < E; ++ev) {
+      const int ta = d.pt_ev[ev].tile0;
+      d.pt_ev[ev].tile0 = a;
       a += ta;
     }
     d.pt_ev[E].tile0 = a;
@@ -161,38 +166,45 @@ struct PtAccepted {
 };
 
 struct PtWarp {  // per-warp scratch of k_pt_eval (dynamic shared memory: kWarps of these)
-  float4 seed[kSeedTile];  // x1, y1, vx, vy of the tile's seeds
-  float lv[kSeedTile];
-  int2 w2[64];         // phase-2 list: (candidate | T5 flag << 31, seed slot)
-  float2 axy[32];      // the warp's anchors
-  int2 r3[32], r5[32];  // (first, count) of their T3s / T5s
-  unsigned w1[64];     // gate survivors: seed slot | anchor lane << 16 | gate-near << 31
-  int pref[33];        // exclusive prefix of the candidate counts of w1[0..32)
-  unsigned heads[32];  // head bits of the entries over the first 1024 items
-  float kp[32], tolk[32];
+  float4 sa[kSeedTile];  // x1, y1, vx, vy of the tile's seeds
+  float4 sg[kSeedTile];  // gate limit lw (lw c1 + c2), c1 = lv INV_2RMIN, c2 = lv PT_GATE_TOL: upper (c1h, c2h) and lower (c1l, c2l) versions
+  float2 sk[kSeedTile];  // kp, tolk
+  int2 w2[64];           // candidates behind the curvature pre-filter: (T3 / T5 index | T5 flag << 31, seed slot | anchor lane << 16)
+  float4 anc[32];        // the warp's anchors (x, y, z, r | endcap << 31)
+  int4 at[32];           // (first T3, number of T3s, first T5, number of T5s) of each
+  unsigned w1[64];       // gate survivors: seed slot | anchor lane << 16 | gate-near << 31
+  int pref[33];          // exclusive prefix of the candidate counts of w1[0..32)
+  unsigned heads[32];    // head bits of the entries over the first 1024 items
 };
 
-// pT3 and pT5 of the whole batch.  A tile = 32 anchors of one event (one per lane) x up to kSeedTile
-// seeds of the same event (shared memory, read as broadcasts).  Warps take tiles by ticket and never
-// wait for one another (with a block-wide tile, a quarter of the warp time was spent at the barrier
-// behind the warp whose anchors matched the most seeds; profiles/).
+// pT3 and pT5 candidates of the whole batch -> queue of the exact cuts.  Warps take tiles by ticket and
+// never wait for one another.
 __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
+  load_batch(d);
   extern __shared__ __align__(16) unsigned char s_dyn[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   PtWarp& w = reinterpret_cast<PtWarp*>(s_dyn)[warp];
-  float4* const s_seed = w.seed;
-  float* const s_lv = w.lv;
   const int E = d.n_events;
   const int n_tiles = d.pt_ev[E].tile0;
-  const int cap3 = d.cap[K_PT3], cap5 = d.cap[K_PT5];
-  PtAccepted* scratch3 = reinterpret_cast<PtAccepted*>(d.ev_scratch);
-  PtAccepted* scratch5 = reinterpret_cast<PtAccepted*>(d.ev_scratch2);
-  const float inv_2rmin = d.cuts.inv_2rmin * 1.0001f, gate_tol = d.cuts.pt_gate_tol * 1.0001f;
+  const int cap_q = d.cap_queue;
+  const float inv = d.cuts.inv_2rmin, gtol = d.cuts.pt_gate_tol;
+  // the circle test of phase 1a bounds the gate limit at |w| + h, which needs a limit growing with |w|
+  const bool can_prune = inv >= 0.0f && gtol >= 0.0f;
+  // warp-aggregated append to the queue of the exact cuts
+  auto push_q = [&](bool go, int p, int cand) {
+    const unsigned m = __ballot_sync(kFull, go);
+    if (m == 0u) return;
+    int base = 0;
+    if (lane == __ffs(m) - 1) base = atomicAdd(&d.ctl->queue_cur, __popc(m));
+    base = __shfl_sync(kFull, base, __ffs(m) - 1);
+    const int pos = base + __popc(m & ((1u << lane) - 1u));
+    if (go && pos < cap_q) d.pt_queue[pos] = make_int2(p, cand);
+  };
   for (;;) {
-    unsigned near3 = 0, near5 = 0;  // near-threshold candidates of this tile (one event)
+    unsigned near3 = 0, near5 = 0;  // candidates failing the gate near its threshold, this tile (one event)
     int tile = 0, evi = 0;
     if (lane == 0) {
-      tile = atomicAdd(d.ctl->ticket + T_PT3, 1);
+      tile = atomicAdd(d.ctl->ticket + T_PT, 1);
       int hi = E;  // event of the tile: largest e with tile0[e] <= tile
       if (tile < n_tiles)
         while (hi - evi > 1) {
@@ -210,49 +222,64 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     const int p0 = ev.s0 + sb * kSeedTile;
     const int n_seed = min(kSeedTile, ev.s1 - p0);
     for (int k = lane; k < n_seed; k += 32) {
-      const int p = p0 + k;
-      const float x1 = __ldg(d.p_x1 + p), y1 = __ldg(d.p_y1 + p);
-      const float vx = x1 - __ldg(d.p_x0 + p), vy = y1 - __ldg(d.p_y0 + p);
-      s_seed[k] = make_float4(x1, y1, vx, vy);
-      s_lv[k] = sqrtf(vx * vx + vy * vy);
+      const float4 a = d.seed_a[p0 + k], b = d.seed_b[p0 + k];
+      const float c1 = b.x * inv, c2 = b.x * gtol;
+      w.sa[k] = a;
+      w.sg[k] = make_float4(c1 + 1e-4f * fabsf(c1), c2 + 1e-4f * fabsf(c2), c1 - 1e-4f * fabsf(c1), c2 - 1e-4f * fabsf(c2));
+      w.sk[k] = make_float2(b.y, b.z);
     }
-    __syncwarp();
     const int anc = ev.a0 + ab * 32 + lane;
     const bool valid = anc < ev.a1;
-    float2 A = make_float2(0.0f, 0.0f);
-    int2 r3 = make_int2(0, 0), r5 = make_int2(0, 0);  // (first, count) of the anchor's T3s / T5s
+    float4 A = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    int4 at = make_int4(0, 0, 0, 0);
     if (valid) {
-      A = d.anc_axy[anc];
-      r3 = d.anc_t3[anc];
-      r5 = d.anc_t5[anc];
+      A = d.anc_a[anc];
+      at = d.anc_t[anc];
     }
-    // ---- phase 2: the exact cut list for one entry of the warp's list ----
-    auto phase2 = [&](int2 ent) {
+    w.anc[lane] = A;
+    w.at[lane] = at;
+    __syncwarp();
+    // ---- (3) the rest of the approximate cascade for one entry of w2; what survives goes to the queue ----
+    auto tail = [&](int2 ent, bool active) {
+      bool go = false;
+      const int t = ent.x & 0x7fffffff, ks = ent.y & 0xffff, src = (ent.y >> 16) & 31;
       const bool is5 = ent.x < 0;
-      const int t = ent.x & 0x7fffffff, ks = ent.y;
-      const int p = p0 + ks;
-      const float4 sd = s_seed[ks];
-      const Seed full = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p), __ldg(d.p_y0 + p),
-                                  __ldg(d.p_z0 + p), sd.x, sd.y, __ldg(d.p_z1 + p));
-      float score;
-      const unsigned r2 = is5 ? PtCand<true>::test(d, full, t, score) : PtCand<false>::test(d, full, t, score);
-      if (is5) near5 += (r2 >> 1) & 1u; else near3 += (r2 >> 1) & 1u;
-      if (r2 & ACC) {
-        const int slot = atomicAdd(&d.ctl->scratch_cur[is5 ? 3 : 2], 1);
-        if (slot < (is5 ? cap5 : cap3)) (is5 ? scratch5 : scratch3)[slot] = PtAccepted{p, t, score};
-        atomicAdd((is5 ? d.pls_pt5_cnt : d.pls_pt3_cnt) + p, 1);
+      if (active) {
+        const float4 s = w.sa[ks];
+        const float2 kt = w.sk[ks];
+        const float4 a = w.anc[src];
+        const float4 l = is5 ? d.t5_l[t] : d.t3_l[t];
+        bool ok;
+        const float kx = kx_approx(s.x, s.y, a.x, a.y, l.x, l.y, ok);
+        int c = pt_class_curv(kx, kt.x, kt.y, ok);
+        if (c == PT_PASS) {
+          if (is5) {
+            const float2 kio = d.t5_kio[t];
+            c = pt_class_curv(kx, kio.x, kt.y, ok);
+            if (c == PT_PASS) c = pt_class_curv(kx, kio.y, kt.y, ok);
+          } else {
+            c = pt_class_curv(kx, d.t3_k[t], kt.y, ok);
+          }
+        }
+        if (c == PT_PASS) {
+          const float z1 = d.seed_z1[p0 + ks], slope = d.seed_b[p0 + ks].w;
+          c = pt_class_rz(d.cuts, s.x, s.y, z1, slope, kx, a, ok);
+          if (c == PT_PASS) c = pt_class_rz(d.cuts, s.x, s.y, z1, slope, kx, l, ok);
+        }
+        go = c != PT_FAIL;  // all cuts surely pass, or one of them cannot be decided here: the exact cuts decide
       }
+      push_q(go, p0 + ks, ent.x);
     };
     int n2 = 0;
-    // pushes up to one entry per lane onto the warp's phase-2 list; runs phase 2 whenever 32 are waiting
-    auto push2 = [&](bool go, int cand, int ks) {
+    // pushes up to one entry per lane onto w2; runs the cascade whenever 32 are waiting
+    auto push2 = [&](bool go, int cand, int tag) {
       const unsigned m = __ballot_sync(kFull, go);
       if (m == 0u) return;
-      if (go) w.w2[n2 + __popc(m & ((1u << lane) - 1u))] = make_int2(cand, ks);
+      if (go) w.w2[n2 + __popc(m & ((1u << lane) - 1u))] = make_int2(cand, tag);
       n2 += __popc(m);
       if (n2 >= 32) {
         __syncwarp();
-        phase2(w.w2[lane]);
+        tail(w.w2[lane], true);
         const int2 rest = (32 + lane < n2) ? w.w2[32 + lane] : make_int2(0, 0);
         __syncwarp();
         w.w2[lane] = rest;
@@ -260,38 +287,29 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
         __syncwarp();
       }
     };
-    // The warp's 32 anchors, readable by every lane (a gate survivor is expanded by whichever lane is free).
-    w.axy[lane] = A;
-    w.r3[lane] = r3;
-    w.r5[lane] = r5;
-    __syncwarp();
-    // ---- expansion of up to 32 gate survivors (seed slot | anchor lane << 16 | gate-near << 31) into
-    // their (seed, T3) / (seed, T5) candidates, flattened over the lanes; the curvature pre-filter
-    // decides which go on to the exact cuts ----
+    // ---- (2) expansion of up to 32 gate survivors into their (seed, T3) / (seed, T5) candidates, flattened
+    // over the lanes; kx~ against the seed's curvature decides which go on ----
     auto expand = [&](int n_ent) {
       int n_c = 0;
       if (lane < n_ent) {
-        const unsigned ent = w.w1[lane];
-        const int src = (ent >> 16) & 31, ks = ent & 0xffff;
-        n_c = w.r3[src].y + w.r5[src].y;
-        const float kp = (-(float)__ldg(d.p_q + p0 + ks)) / (__ldg(d.p_pt + p0 + ks) * d.cuts.kr);
-        w.kp[lane] = kp;
-        w.tolk[lane] = d.cuts.pt_k_tol0 + d.cuts.pt_k_tol1 * fabsf(kp);
+        const int4 a = w.at[(w.w1[lane] >> 16) & 31];
+        n_c = a.y + a.w;
       }
       const int incl = warp_incl_scan(n_c);
-      w.pref[lane] = incl - n_c;
+      const int excl = incl - n_c;
+      w.pref[lane] = excl;
       const int T = __shfl_sync(kFull, incl, 31);
-      // item -> entry in O(1): one head bit per entry at the position of its first item; the entry of
-      // item `it` = number of head bits at or before it, minus one (falls back to bisection beyond 1024 items)
+      // item -> entry in O(1): one head bit per entry at the position of its first item; the entry of item
+      // `it` = number of head bits at or before it, minus one (bisection beyond 1024 items)
       w.heads[lane] = 0u;
       __syncwarp();
-      if (n_c > 0 && incl - n_c < 1024) atomicOr(&w.heads[(incl - n_c) >> 5], 1u << ((incl - n_c) & 31));
+      if (n_c > 0 && excl < 1024) atomicOr(&w.heads[excl >> 5], 1u << (excl & 31));
       __syncwarp();
       int heads_before = 0;
       for (int i0 = 0; i0 < T; i0 += 32) {
         const int it = i0 + lane;
-        bool go = false;
-        int cand = 0, ks = 0;
+        bool go = false, direct = false;
+        int cand = 0, tag = 0;
         const unsigned hw = i0 < 1024 ? w.heads[i0 >> 5] : 0u;
         if (it < T) {
           int lo;
@@ -307,20 +325,27 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
             }
           }
           const unsigned ent = w.w1[lo];
-          const int src = (ent >> 16) & 31, c = it - w.pref[lo];
-          ks = ent & 0xffff;
-          const int2 a3 = w.r3[src], a5 = w.r5[src];
-          const bool is5 = c >= a3.y;
-          const int t = is5 ? a5.x + (c - a3.y) : a3.x + c;
+          const int src = (ent >> 16) & 31, ks = ent & 0xffff, c = it - w.pref[lo];
+          const int4 a = w.at[src];
+          const bool is5 = c >= a.y;
+          const int t = is5 ? a.z + (c - a.y) : a.x + c;
           cand = t | (is5 ? 0x80000000 : 0);
-          go = true;
-          if (!(ent >> 31)) {
-            const float4 sd = s_seed[ks];
-            go = pt_curv_possible(w.kp[lo], w.tolk[lo], sd.x, sd.y, w.axy[src], is5 ? d.t5_lxy[t] : d.t3_lxy[t]);
+          tag = ks | (src << 16);
+          if (ent >> 31) {
+            direct = true;  // the gate was near its threshold: every candidate of the pair is flagged by the exact cuts
+          } else {
+            const float4 s = w.sa[ks];
+            const float2 kt = w.sk[ks];
+            const float4 an = w.anc[src];
+            const float2 l = *reinterpret_cast<const float2*>(is5 ? d.t5_l + t : d.t3_l + t);
+            bool ok;
+            const float kx = kx_approx(s.x, s.y, an.x, an.y, l.x, l.y, ok);
+            go = pt_class_curv(kx, kt.x, kt.y, ok) != PT_FAIL;
           }
         }
         heads_before += __popc(hw);
-        push2(go, cand, ks);
+        push_q(direct, p0 + (tag & 0xffff), cand);
+        push2(go, cand, tag);
       }
       __syncwarp();
     };
@@ -337,57 +362,54 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     const bool warp_has = bx0 <= bx1;
     const float bcx = 0.5f * (bx0 + bx1), bcy = 0.5f * (by0 + by1);
     const float bh = 0.5f * sqrtf((bx1 - bx0) * (bx1 - bx0) + (by1 - by0) * (by1 - by0)) * 1.001f + 1e-3f;
-    // ---- phase 1, 32 seeds at a time ----
+    // ---- (1) 32 seeds at a time ----
     for (int kb = 0; kb < n_seed && warp_has; kb += 32) {
-      // (a) one seed per lane against the circle: can its gate accept ANY point within bh of the centre?
-      //     gdot(A) <= v.wc + lv*bh and gcrs(A) >= |v x wc| - lv*bh, glim(A) <= glim at |wc| + bh; margins
-      //     1e-3 cover the rounding of both sides (~1e-6 relative).  Out of range: tested by every lane.
+      // (1a) one seed per lane against the circle: can its gate accept ANY point within bh of the centre?
+      //      gdot(A) <= v.wc + lv bh, gcrs(A) >= |v x wc| - lv bh, glim(A) <= glim at |wc| + bh (c1h, c2h >= 0
+      //      here); the 1e-4 inflation of c1h, c2h and the 1.001 factors cover the rounding of both sides.
+      //      Out of range: tested by every lane.
       bool maybe = false;
       if (kb + lane < n_seed) {
-        const float4 sd = s_seed[kb + lane];
-        const float lv = s_lv[kb + lane];
-        const float wx = bcx - sd.x, wy = bcy - sd.y;
+        const float4 s = w.sa[kb + lane];
+        const float4 g = w.sg[kb + lane];
+        const float wx = bcx - s.x, wy = bcy - s.y;
         const float lw2 = wx * wx + wy * wy;
-        float rl;
-        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
-        const float Lw = (lw2 * rl + bh) * 1.001f;
-        const float slack = lv * (bh * 1.001f + 1e-4f);
-        const float dotc = sd.z * wx + sd.w * wy;
-        const float crsc = fabsf(sd.z * wy - sd.w * wx);
-        const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f && lv <= 1e30f;
-        maybe = !in_range || (dotc + slack > 0.0f && crsc - slack <= (lv * Lw) * (Lw * inv_2rmin + gate_tol));
+        const float Lw = (lw2 * rsqrt_approx(lw2) + bh) * 1.001f;
+        const float lv2 = s.z * s.z + s.w * s.w;
+        const float lvh = lv2 * rsqrt_approx(lv2) * 1.001f;
+        const float slack = lvh * (bh * 1.001f + 1e-4f);
+        const float dotc = s.z * wx + s.w * wy;
+        const float crsc = fabsf(s.z * wy - s.w * wx);
+        const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f && lv2 >= 1e-30f && lv2 <= 1e30f;
+        maybe = !can_prune || !in_range || (dotc + slack > 0.0f && crsc - slack <= Lw * (Lw * g.x + g.y));
       }
       unsigned word = __ballot_sync(kFull, maybe);
-      // (b) the seeds that may match: every lane tests its own anchor
+      // (1b) the seeds that may match: every lane tests its own anchor
       while (word) {
         const int k = kb + __ffs(word) - 1;
         word &= word - 1;
         bool pass = false;
         unsigned ent = 0u;
         if (valid) {
-          const float4 sd = s_seed[k];
-          const float wx = A.x - sd.x, wy = A.y - sd.y;
-          const float gdot = sd.z * wx + sd.w * wy;
-          const float lw2 = wx * wx + wy * wy;
-          float rl;
-          asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rl) : "f"(lw2));
-          const float lw = lw2 * rl;
-          const float gcrs = fabsf(sd.z * wy - sd.w * wx);
-          const float lim = (s_lv[k] * lw) * (lw * inv_2rmin + gate_tol);
-          // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact
-          // gate is skipped), uncertain = within 2e-4 of the threshold or out of the approximation's
-          // range (the exact gate decides)
-          const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f;
-          pass = gdot > 0.0f && (!(gcrs > lim) || !in_range);
-          if (pass && !(in_range && gcrs <= lim * 0.9998f)) {
-            // phase 1b: the exact gate (CUTS.md section 7) decides and flags near-threshold
-            Seed s;
-            s.x1 = sd.x;  s.y1 = sd.y;  s.vx = sd.z;  s.vy = sd.w;  s.lv = s_lv[k];
-            const unsigned r = pt_gate(d.cuts, s, A.x, A.y);
+          const float4 s = w.sa[k];
+          const float4 g = w.sg[k];
+          const float wx = A.x - s.x, wy = A.y - s.y;
+          const float gdot = s.z * wx + s.w * wy;          // exactly the spec's gdot and gcrs (no FMA)
+          const float gcrs = fabsf(s.z * wy - s.w * wx);
+          const float lw2 = fmaf(wx, wx, wy * wy);
+          const float lw = lw2 * rsqrt_approx(lw2);
+          // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact gate
+          // is skipped), uncertain = within 1e-4 of the threshold or out of the approximation's range (NaN
+          // limits compare false both ways): the exact gate decides
+          pass = gdot > 0.0f && !(gcrs > lw * fmaf(lw, g.x, g.y));
+          if (pass && !(gcrs <= lw * fmaf(lw, g.z, g.w) && lw2 >= 1e-30f && lw2 <= 1e30f)) {
+            Seed sd;
+            sd.x1 = s.x;  sd.y1 = s.y;  sd.vx = s.z;  sd.vy = s.w;  sd.lv = d.seed_b[p0 + k].x;
+            const unsigned r = pt_gate(d.cuts, sd, A.x, A.y);
             pass = (r & ACC) != 0;
             if (!pass && (r & NEAR)) {  // every candidate of the anchor fails the gate near its threshold
-              near3 += (unsigned)r3.y;
-              near5 += (unsigned)r5.y;
+              near3 += (unsigned)at.y;
+              near5 += (unsigned)at.w;
             }
             if (r & NEAR) ent = 0x80000000u;
           }
@@ -411,7 +433,10 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     }
     __syncwarp();
     if (n1 > 0) expand(n1);
-    if (lane < n2) phase2(w.w2[lane]);
+    if (n2 > 0) {
+      __syncwarp();
+      tail(lane < n2 ? w.w2[lane] : make_int2(0, 0), lane < n2);
+    }
     if (__any_sync(kFull, (near3 | near5) != 0u)) {
       const int s3 = warp_sum((int)near3), s5 = warp_sum((int)near5);
       if (lane == 0) {
@@ -419,36 +444,52 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
         if (s5) atomicAdd(d.ev_cnt + (size_t)evi * kEvCnt + 5, (unsigned long long)s5);
       }
     }
-    __syncwarp();  // the seed tile is reused
+    __syncwarp();  // the tile's tables are reused
   }
 }
 
-// Groups the accepted pairs by seed: begin = exclusive scan of the per-seed counts (k_scan, before
-// this kernel); every scratch entry takes the next free slot of its seed.
-template <bool IS5>
-__global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
-  constexpr int kKind = IS5 ? K_PT5 : K_PT3;
-  const int n = d.ctl->scratch_cur[IS5 ? 3 : 2];
-  const int cap = d.cap[kKind];
-  const int* begin = IS5 ? d.pls_pt5_begin : d.pls_pt3_begin;
-  int* cur = IS5 ? d.pls_pt5_cur : d.pls_pt3_cur;
-  int2* out = IS5 ? d.pt5 : d.pt3;
-  float* out_s = IS5 ? d.pt5_score : d.pt3_score;
-  const PtAccepted* scratch = reinterpret_cast<const PtAccepted*>(IS5 ? d.ev_scratch2 : d.ev_scratch);
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    if (n > cap) {
-      atomicOr(&d.ctl->error, IS5 ? E_CAP_PT5 : E_CAP_PT3);
-      d.ctl->total[kKind] = 0;
-    } else {
-      d.ctl->total[kKind] = n;
-    }
+// The exact cut list of CUTS.md section 7 on the queue.  Accepted pairs go to scratch lists (one atomic per
+// accepted object) with a count per seed; near-threshold flags are counted here (and, for pairs failing the
+// gate near its threshold, in k_pt_eval).
+__global__ void __launch_bounds__(kBlock) k_pt_exact(Dev d) {
+  load_batch(d);
+  const int n_q = d.ctl->queue_cur;
+  const int cap3 = d.cap[K_PT3], cap5 = d.cap[K_PT5];
+  PtAccepted* scratch3 = reinterpret_cast<PtAccepted*>(d.ev_scratch);
+  PtAccepted* scratch5 = reinterpret_cast<PtAccepted*>(d.ev_scratch2);
+  if (n_q > d.cap_queue) {  // the queue holds the accepted pairs and the few undecided ones: capacity error
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(&d.ctl->error, E_CAP_PT3 | E_CAP_PT5);
+    return;
   }
-  if (n > cap) return;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    const PtAccepted a = scratch[i];
-    const int pos = begin[a.p] + atomicAdd(cur + a.p, 1);
-    out[pos] = make_int2(a.p, a.t);
-    out_s[pos] = a.score;
+  const int lane = threadIdx.x & 31;
+  for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; i0 < n_q; i0 += gridDim.x * blockDim.x) {
+    const int i = i0 + lane;  // whole warps stay in the loop: the scratch slots are taken with one atomic per warp and class
+    bool is5 = false;
+    unsigned r = 0;
+    PtAccepted acc{0, 0, 0.0f};
+    if (i < n_q) {
+      const int2 q = d.pt_queue[i];
+      acc.p = q.x;
+      acc.t = q.y & 0x7fffffff;
+      is5 = q.y < 0;
+      const Seed s = seed_from_table(d, acc.p);
+      r = is5 ? PtCand<true>::test(d, s, acc.t, acc.score) : PtCand<false>::test(d, s, acc.t, acc.score);
+      if (r & NEAR) count_near(d.ev_cnt, d.pls_event[acc.p], is5 ? 5 : 4);
+    }
+    const unsigned m3 = __ballot_sync(kFull, (r & ACC) && !is5), m5 = __ballot_sync(kFull, (r & ACC) && is5);
+    int b3 = 0, b5 = 0;
+    if (lane == 0) {
+      if (m3) b3 = atomicAdd(&d.ctl->scratch_cur[2], __popc(m3));
+      if (m5) b5 = atomicAdd(&d.ctl->scratch_cur[3], __popc(m5));
+    }
+    b3 = __shfl_sync(kFull, b3, 0);
+    b5 = __shfl_sync(kFull, b5, 0);
+    if (r & ACC) {
+      const unsigned below = (1u << lane) - 1u;
+      const int slot = is5 ? b5 + __popc(m5 & below) : b3 + __popc(m3 & below);
+      if (slot < (is5 ? cap5 : cap3)) (is5 ? scratch5 : scratch3)[slot] = acc;
+      atomicAdd((is5 ? d.pls_pt5_cnt : d.pls_pt3_cnt) + acc.p, 1);
+    }
   }
 }
 

@@ -1,9 +1,10 @@
 // lst_select.cuh -- step a6: duplicate removal and track-candidate selection (CUTS.md section 8,
-// PAPER.md:31-34, 56).  Set-defined rules; the candidates that can overlap an object are found
-// through an inverted index "objects containing MD m" (three lists per MD: T5, pT5, pT3), built
-// with one counting pass, the generic scan and one fill pass.  By the pigeonhole principle an
-// object sharing >= 3 of X's 5 MDs contains X.md[0], [2] or [4]; one sharing >= 2 of 5 contains one
-// of X.md[0..3]; one sharing >= 2 of X's 3 MDs contains X.md[0] or [1].
+// PAPER.md:31-34, 56), and the grouping of the accepted pT3 / pT5 by seed that precedes it.
+// Set-defined rules; the candidates that can overlap an object are found through an inverted index
+// "objects containing MD m": three linked lists per MD (T5, pT5, pT3), built in ONE pass with an atomic
+// exchange per (object, MD) -- node = object * 5 (or 3) + position, so no allocation, no counting pass and
+// no scan.  By the pigeonhole principle an object sharing >= 3 of X's 5 MDs contains X.md[0], [2] or [4];
+// one sharing >= 2 of 5 contains one of X.md[0..3]; one sharing >= 2 of X's 3 MDs contains X.md[0] or [1].
 #pragma once
 #include "lst_ls.cuh"
 #include "lst_pt.cuh"
@@ -12,66 +13,78 @@ namespace lst {
 
 __device__ __forceinline__ int ev_of_md(const Dev& d, int md) { return (d.md_info[md] >> 1) / d.n_mod; }
 
-// first object index of every event, per kind: ev_first[kind * (n_events + 1) + ev]
-__global__ void k_event_ranges(Dev d, int* ev_first) {
-  const int E1 = d.n_events + 1;
-  for (int ev = threadIdx.x; ev < E1; ev += blockDim.x) {
-    const int p = d.pls_ev_off[ev];
-    const int md = d.ctl->total[K_MD] > 0 ? d.mod_md_begin[min(ev, d.n_events) * d.n_mod] : 0;
-    const int ls = d.ctl->total[K_LS] > 0 ? d.md_ls_begin[md] : 0;
-    const int t3 = d.ctl->total[K_T3] > 0 ? d.ls_t3_begin[ls] : 0;
-    const int t5 = d.ctl->total[K_T5] > 0 ? d.t3_t5_begin[t3] : 0;
-    ev_first[K_MD * E1 + ev] = md;
-    ev_first[K_LS * E1 + ev] = ls;
-    ev_first[K_T3 * E1 + ev] = t3;
-    ev_first[K_T5 * E1 + ev] = t5;
-    ev_first[K_PT3 * E1 + ev] = d.ctl->total[K_PT3] > 0 ? d.pls_pt3_begin[p] : 0;
-    ev_first[K_PT5 * E1 + ev] = d.ctl->total[K_PT5] > 0 ? d.pls_pt5_begin[p] : 0;
-  }
+// offsets of the three node arrays inside idx_next
+__device__ __forceinline__ int node_base(const Dev& d, int kind) {
+  return kind == 0 ? 0 : (kind == 1 ? 5 * d.cap[K_T5] : 5 * d.cap[K_T5] + 5 * d.cap[K_PT5]);
+}
+__device__ __forceinline__ void idx_link(const Dev& d, int n_md, int kind, int md, int node) {
+  d.idx_next[node_base(d, kind) + node] = atomicExch(d.idx_head + kind * n_md + md, node + 1);
 }
 
-__global__ void __launch_bounds__(kBlock) k_sel_prepare(Dev d) {
+// After k_scan2 (per-seed counts -> begin offsets): every accepted (seed, T3) / (seed, T5) of the scratch
+// lists takes the next free slot of its seed (order inside a seed's range is arrival order: free by the
+// spec, reading S9) and is linked into the index of its MDs; the T5s are linked as well.
+// Block 0 also writes the first object of every event per kind (what the read-back slices by).
+__global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
+  load_batch(d);
+  const int n3 = d.ctl->scratch_cur[2], n5 = d.ctl->scratch_cur[3];
+  const int cap3 = d.cap[K_PT3], cap5 = d.cap[K_PT5];
+  const bool fit3 = n3 <= cap3, fit5 = n5 <= cap5;
+  const int n_t5 = d.ctl->total[K_T5], n_md = d.ctl->total[K_MD];
+  const bool sel = (d.cuts.stage_mask & 32) != 0 && fit3 && fit5;
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
-  const int n_slots = 3 * d.ctl->total[K_MD];
-  for (int i = i0; i <= n_slots; i += stride) {
-    d.idx_cnt[i] = 0;
-    d.idx_cur[i] = 0;
+  const PtAccepted* s3 = reinterpret_cast<const PtAccepted*>(d.ev_scratch);
+  const PtAccepted* s5 = reinterpret_cast<const PtAccepted*>(d.ev_scratch2);
+  if (i0 == 0) {
+    if (!fit3) atomicOr(&d.ctl->error, E_CAP_PT3);
+    if (!fit5) atomicOr(&d.ctl->error, E_CAP_PT5);
+    d.ctl->total[K_PT3] = fit3 ? n3 : 0;
+    d.ctl->total[K_PT5] = fit5 ? n5 : 0;
   }
-  for (int i = i0; i <= 4 * d.n_events; i += stride) {
-    d.tc_cnt[i] = 0;
-    d.tc_cur[i] = 0;
-  }
-  for (int i = i0; i < d.n_pls; i += stride) d.linked[i] = 0;
-}
-
-// FILL = false: count list lengths; FILL = true: write the lists (order inside a list is free)
-template <bool FILL>
-__global__ void __launch_bounds__(kBlock) k_index(Dev d) {
-  const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
-  const int n_md = d.ctl->total[K_MD];
-  const int n_t5 = d.ctl->total[K_T5], n_pt5 = d.ctl->total[K_PT5], n_pt3 = d.ctl->total[K_PT3];
-  for (int i = i0; i < n_t5 + n_pt5 + n_pt3; i += stride) {
-    int obj, base, nmd;
-    const int* md;
-    int tmp[3];
-    if (i < n_t5) {
-      obj = i; base = 0; nmd = 5; md = d.t5_md + 5 * (size_t)obj;
-    } else if (i < n_t5 + n_pt5) {
-      obj = i - n_t5; base = n_md; nmd = 5; md = d.t5_md + 5 * (size_t)d.pt5[obj].y;
-    } else {
-      obj = i - n_t5 - n_pt5; base = 2 * n_md; nmd = 3;
-      const int4 m = d.t3_md[d.pt3[obj].y];
-      tmp[0] = m.x; tmp[1] = m.y; tmp[2] = m.z;
-      md = tmp;
-    }
-    for (int k = 0; k < nmd; ++k) {
-      const int slot = base + md[k];
-      if (!FILL) {
-        atomicAdd(d.idx_cnt + slot, 1);
-      } else {
-        const int pos = d.idx_begin[slot] + atomicAdd(d.idx_cur + slot, 1);
-        if (pos < d.cap_idx) d.idx_list[pos] = obj;
+  const int n_a = fit3 ? n3 : 0, n_b = fit5 ? n5 : 0;
+  for (int i = i0; i < n_a + n_b + (sel ? n_t5 : 0); i += stride) {
+    if (i < n_a) {
+      const PtAccepted a = s3[i];
+      const int pos = d.pls_pt3_begin[a.p] + atomicAdd(d.pls_pt3_cur + a.p, 1);
+      d.pt3[pos] = make_int2(a.p, a.t);
+      d.pt3_score[pos] = a.score;
+      if (sel) {
+        const int4 m = d.t3_md[a.t];
+        idx_link(d, n_md, 2, m.x, 3 * pos);
+        idx_link(d, n_md, 2, m.y, 3 * pos + 1);
+        idx_link(d, n_md, 2, m.z, 3 * pos + 2);
       }
+    } else if (i < n_a + n_b) {
+      const PtAccepted a = s5[i - n_a];
+      const int pos = d.pls_pt5_begin[a.p] + atomicAdd(d.pls_pt5_cur + a.p, 1);
+      d.pt5[pos] = make_int2(a.p, a.t);
+      d.pt5_score[pos] = a.score;
+      if (sel) {
+        const int* md = d.t5_md + 5 * (size_t)a.t;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) idx_link(d, n_md, 1, md[k], 5 * pos + k);
+      }
+    } else {
+      const int t = i - n_a - n_b;
+      const int* md = d.t5_md + 5 * (size_t)t;
+#pragma unroll
+      for (int k = 0; k < 5; ++k) idx_link(d, n_md, 0, md[k], 5 * t + k);
+    }
+  }
+  if (blockIdx.x == 0) {
+    const int E1 = d.n_events + 1;
+    for (int ev = threadIdx.x; ev < E1; ev += blockDim.x) {
+      const int p = d.pls_ev_off[ev];
+      const int md = n_md > 0 ? d.mod_md_begin[ev * d.n_mod] : 0;
+      const int ls = d.ctl->total[K_LS] > 0 ? d.md_ls_begin[md] : 0;
+      const int t3 = d.ctl->total[K_T3] > 0 ? d.ls_t3_begin[ls] : 0;
+      const int t5 = n_t5 > 0 ? d.t3_t5_begin[t3] : 0;
+      d.ev_first[K_MD * E1 + ev] = md;
+      d.ev_first[K_LS * E1 + ev] = ls;
+      d.ev_first[K_T3 * E1 + ev] = t3;
+      d.ev_first[K_T5 * E1 + ev] = t5;
+      d.ev_first[K_PT3 * E1 + ev] = n_a > 0 ? d.pls_pt3_begin[p] : 0;
+      d.ev_first[K_PT5 * E1 + ev] = n_b > 0 ? d.pls_pt5_begin[p] : 0;
     }
   }
 }
@@ -107,8 +120,23 @@ __device__ __forceinline__ void load_t5_md(const Dev& d, int t5, int* m) {
   for (int k = 0; k < 5; ++k) m[k] = p[k];
 }
 
+// walks the list of objects of `kind` containing MD `md`: for (It it(d, n_md, kind, md); it.obj >= 0; it.next())
+struct IdxIt {
+  const int* next;
+  int node, per, obj;
+  __device__ IdxIt(const Dev& d, int n_md, int kind, int md)
+      : next(d.idx_next + node_base(d, kind)), node(d.idx_head[kind * n_md + md]), per(kind == 2 ? 3 : 5) {
+    obj = node ? (node - 1) / per : -1;
+  }
+  __device__ void advance() {
+    node = next[node - 1];
+    obj = node ? (node - 1) / per : -1;
+  }
+};
+
 // rule 1: pT5 vs pT5
 __global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
+  load_batch(d);
   const int stride = gridDim.x * blockDim.x;
   const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_PT5];
   for (int X = blockIdx.x * blockDim.x + threadIdx.x; X < n; X += stride) {
@@ -123,9 +151,8 @@ __global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
       if (better(d, d.pt5_score[Y], x.x, mY, sX, x.x, mX, 5)) keep = false;
     }
     for (int k = 0; k < 5 && keep; k += 2) {
-      const int slot = n_md + mX[k];
-      for (int j = d.idx_begin[slot]; j < d.idx_begin[slot + 1] && keep; ++j) {
-        const int Y = d.idx_list[j];
+      for (IdxIt it(d, n_md, 1, mX[k]); it.obj >= 0 && keep; it.advance()) {
+        const int Y = it.obj;
         if (Y == X) continue;
         const int2 y = d.pt5[Y];
         load_t5_md(d, y.y, mY);
@@ -134,7 +161,7 @@ __global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
     }
     d.keep5[X] = keep;
     if (keep) {
-      d.linked[x.x] = 1;  // one writer per value; pT3 survivors OR in 2 (rule 2)
+      d.linked[x.x] = 1;  // one writer per value; rule 4 (k_rule3) completes it with the surviving pT3s
       atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 0, 1);
     }
   }
@@ -142,6 +169,7 @@ __global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
 
 // rule 2: pT3 vs pT3, then vs surviving pT5
 __global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
+  load_batch(d);
   const int stride = gridDim.x * blockDim.x;
   const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_PT3], n_pt5 = d.ctl->total[K_PT5];
   for (int X = blockIdx.x * blockDim.x + threadIdx.x; X < n; X += stride) {
@@ -156,18 +184,16 @@ __global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
       if (better(d, d.pt3_score[Y], x.x, mY, sX, x.x, mX, 3)) keep = false;
     }
     for (int k = 0; k < 2 && keep; ++k) {
-      int slot = 2 * n_md + mX[k];
-      for (int j = d.idx_begin[slot]; j < d.idx_begin[slot + 1] && keep; ++j) {
-        const int Y = d.idx_list[j];
+      for (IdxIt it(d, n_md, 2, mX[k]); it.obj >= 0 && keep; it.advance()) {
+        const int Y = it.obj;
         if (Y == X) continue;
         const int2 y = d.pt3[Y];
         load_t3_md(d, y.y, mY);
         if (share(mY, 3, mX, 3) >= 2 && better(d, d.pt3_score[Y], y.x, mY, sX, x.x, mX, 3)) keep = false;
       }
       if (n_pt5 > 0) {
-        slot = n_md + mX[k];
-        for (int j = d.idx_begin[slot]; j < d.idx_begin[slot + 1] && keep; ++j) {
-          const int Z = d.idx_list[j];
+        for (IdxIt it(d, n_md, 1, mX[k]); it.obj >= 0 && keep; it.advance()) {
+          const int Z = it.obj;
           if (!d.keep5[Z]) continue;
           load_t5_md(d, d.pt5[Z].y, mY);
           if (share(mX, 3, mY, 5) >= 2) keep = false;
@@ -179,8 +205,13 @@ __global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
   }
 }
 
-// rule 3: T5 vs T5, vs surviving pT5, vs surviving pT3; rule 4: unlinked pLS
+// rule 3: T5 vs T5, vs surviving pT5, vs surviving pT3; rule 4: unlinked pLS.  The last block to finish
+// turns the per-(event, class) survivor counts into tc_begin (a scan of 4 * n_events + 1 numbers).
 __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
+  load_batch(d);
+  __shared__ int s_last;
+  __shared__ int s_carry;
+  __shared__ int s_warp[kWarps];
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_T5];
   const int n_pt5 = d.ctl->total[K_PT5], n_pt3 = d.ctl->total[K_PT3];
@@ -190,9 +221,8 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
     load_t5_md(d, X, mX);
     bool keep = true;
     for (int k = 0; k < 5 && keep; k += 2) {
-      const int slot = mX[k];
-      for (int j = d.idx_begin[slot]; j < d.idx_begin[slot + 1] && keep; ++j) {
-        const int Y = d.idx_list[j];
+      for (IdxIt it(d, n_md, 0, mX[k]); it.obj >= 0 && keep; it.advance()) {
+        const int Y = it.obj;
         if (Y == X) continue;
         load_t5_md(d, Y, mY);
         if (share(mY, 5, mX, 5) >= 3 && better(d, d.t5_score[Y], -1, mY, sX, -1, mX, 5)) keep = false;
@@ -200,18 +230,16 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
     }
     for (int k = 0; k < 4 && keep; ++k) {
       if (n_pt5 > 0) {
-        const int slot = n_md + mX[k];
-        for (int j = d.idx_begin[slot]; j < d.idx_begin[slot + 1] && keep; ++j) {
-          const int Z = d.idx_list[j];
+        for (IdxIt it(d, n_md, 1, mX[k]); it.obj >= 0 && keep; it.advance()) {
+          const int Z = it.obj;
           if (!d.keep5[Z]) continue;
           load_t5_md(d, d.pt5[Z].y, mY);
           if (share(mX, 5, mY, 5) >= 2) keep = false;
         }
       }
       if (n_pt3 > 0) {
-        const int slot = 2 * n_md + mX[k];
-        for (int j = d.idx_begin[slot]; j < d.idx_begin[slot + 1] && keep; ++j) {
-          const int Z = d.idx_list[j];
+        for (IdxIt it(d, n_md, 2, mX[k]); it.obj >= 0 && keep; it.advance()) {
+          const int Z = it.obj;
           if (!d.keep3[Z]) continue;
           load_t3_md(d, d.pt3[Z].y, mY);
           if (share(mX, 5, mY, 3) >= 2) keep = false;
@@ -229,20 +257,51 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
     d.linked[p] = lk;
     if (!lk) atomicAdd(d.tc_cnt + 4 * d.pls_event[p] + 3, 1);
   }
+  // ---- last block: tc_begin = exclusive scan of tc_cnt, in chunks of kBlock ----
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    s_last = atomicAdd(&d.ctl->done_rule3, 1) == (int)gridDim.x - 1;
+    s_carry = 0;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const int m = 4 * d.n_events;  // tc_begin[0 .. m], tc_begin[m] = total
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int c0 = 0; c0 < m; c0 += kBlock) {
+    const int i = c0 + threadIdx.x;
+    const int v = i < m ? __ldcg(d.tc_cnt + i) : 0;
+    const int incl = warp_incl_scan(v);
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int base = s_carry;
+    for (int w = 0; w < warp; ++w) base += s_warp[w];
+    if (i < m) d.tc_begin[i] = base + incl - v;
+    __syncthreads();
+    if (threadIdx.x == kBlock - 1) s_carry = base + incl;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const int total = s_carry;
+    d.tc_begin[m] = total;
+    if (total > d.cap[K_TC]) {
+      atomicOr(&d.ctl->error, E_CAP_TC);
+      d.ctl->total[K_TC] = 0;
+    } else {
+      d.ctl->total[K_TC] = total;
+    }
+  }
 }
 
 // track candidates: (type, pls, t5, t3, hit_idx[12]) per event in class order; event-local indices
-__global__ void __launch_bounds__(kBlock) k_tc_emit(Dev d, const int* __restrict__ ev_first) {
+__global__ void __launch_bounds__(kBlock) k_tc_emit(Dev d) {
+  load_batch(d);
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int E1 = d.n_events + 1;
   const int n_pt5 = d.ctl->total[K_PT5], n_pt3 = d.ctl->total[K_PT3], n_t5 = d.ctl->total[K_T5];
-  const int total = d.tc_begin[4 * d.n_events];
-  const bool fits = total <= d.cap[K_TC];
-  if (i0 == 0) {
-    if (!fits) atomicOr(&d.ctl->error, E_CAP_TC);
-    d.ctl->total[K_TC] = fits ? total : 0;
-  }
-  if (!fits) return;
+  const int* __restrict__ ev_first = d.ev_first;
+  if (d.tc_begin[4 * d.n_events] > d.cap[K_TC]) return;  // flagged by k_rule3
   for (int i = i0; i < n_pt5 + n_pt3 + n_t5 + d.n_pls; i += stride) {
     int cls, ev, pls = -1, t5 = -1, t3 = -1, nmd = 0;
     int md[5];

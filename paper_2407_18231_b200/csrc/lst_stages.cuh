@@ -9,10 +9,12 @@ namespace lst {
 
 template <class Stage>
 __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
+  load_batch(d);
   __shared__ int s_tile;
   __shared__ int s_scan[kWarps + 2];
   __shared__ unsigned long long s_tests[kEvSmem];
   Stage st(d);
+  st.prologue();
   const int n = st.n_owners();
   const int n_tiles = n > 0 ? (n + kBlock - 1) / kBlock : 1;
   EvTests tbl;
@@ -48,6 +50,28 @@ __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
   tbl.flush();
 }
 
+// position (x, y, z, r) of an MD with its endcap flag in the sign bit of r (r >= 0): what the seed linking reads
+__device__ __forceinline__ float4 pack_flag(float4 a, int endcap) {
+  a.w = __int_as_float(__float_as_int(a.w) | (endcap ? 0x80000000 : 0));
+  return a;
+}
+
+// ---- anchors of the seed linking (lst_pt.cuh): the MDs that start at least one T3 ----
+// The anchors of an event are sorted into kAncBins = 8 radial classes x 64 azimuthal sectors (counting sort:
+// the T5 kernel's prologue counts and keeps the arrival rank, k_anchor_sort scans the event's bins and
+// places), so the 32 anchors of a warp of k_pt_eval sit within a few cm of each other.
+constexpr int kAncBins = 512;
+
+__device__ __forceinline__ int anchor_bin(float x, float y, float r) {
+  const int rc = (r >= 29.5f) + (r >= 43.5f) + (r >= 59.5f) + (r >= 78.0f) + (r >= 98.0f) + (r >= 125.0f);
+  const float a = fabsf(x) + fabsf(y);
+  const float t = a > 0.0f ? y / a : 0.0f;                                  // diamond angle, monotone in azimuth
+  const float ps = x >= 0.0f ? (y >= 0.0f ? t : 4.0f + t) : 2.0f - t;      // [0, 4)
+  int sec = (int)(ps * 16.0f);
+  sec = sec < 0 ? 0 : (sec > 63 ? 63 : sec);
+  return rc * 64 + sec;  // any finite or non-finite input lands in [0, 512): binning never affects results
+}
+
 // ---- a1: Mini-Doublets: lst_md.cuh ----
 // ---- a2: Line Segments: lst_ls.cuh ----
 
@@ -56,6 +80,7 @@ struct StageT3 {
   static constexpr int kTicket = T_T3, kKind = K_T3, kErr = E_CAP_T3, kStage = 2;
   const Dev& d;
   __device__ explicit StageT3(const Dev& dd) : d(dd) {}
+  __device__ void prologue() const {}
   __device__ int n_owners() const { return (d.cuts.stage_mask & 4) ? d.ctl->total[K_LS] : 0; }
   __device__ int* begin() const { return d.ls_t3_begin; }
   template <bool FILL>
@@ -84,8 +109,7 @@ struct StageT3 {
           d.t3_ls[pos] = make_int2(l, l2);
           d.t3_md[pos] = make_int4(ab.x, ab.y, C, eAB | (eC << 2));
           d.t3_k[pos] = k3;
-          d.t3_axy[pos] = make_float2(a.x, a.y);
-          d.t3_lxy[pos] = make_float2(c.x, c.y);
+          d.t3_l[pos] = pack_flag(c, eC);
         }
         ++pos;
         ++cnt;
@@ -101,6 +125,23 @@ struct StageT5 {
   static constexpr int kTicket = T_T5, kKind = K_T5, kErr = E_CAP_T5, kStage = 3;
   const Dev& d;
   __device__ explicit StageT5(const Dev& dd) : d(dd) {}
+  // Rides along (needs the finished T3s only): which MDs are anchors of the seed linking, their bin and
+  // their arrival rank in it.
+  __device__ void prologue() const {
+    const bool on = (d.cuts.stage_mask & 16) && d.ctl->total[K_T3] > 0 && d.n_pls > 0;
+    const int n = d.ctl->total[K_MD];
+    for (int A = blockIdx.x * blockDim.x + threadIdx.x; A < n; A += gridDim.x * blockDim.x) {
+      int bin = -1, rank = 0;
+      if (on && d.ls_t3_begin[d.md_ls_begin[A + 1]] > d.ls_t3_begin[d.md_ls_begin[A]]) {
+        const float4 a = d.md_a[A];
+        const int ev = (d.md_info[A] >> 1) / d.n_mod;
+        bin = anchor_bin(a.x, a.y, a.w);
+        rank = atomicAdd(d.anc_bin_cnt + ev * kAncBins + bin, 1);
+      }
+      d.anc_bin[A] = bin;
+      d.anc_rank[A] = rank;
+    }
+  }
   __device__ int n_owners() const { return (d.cuts.stage_mask & 8) ? d.ctl->total[K_T3] : 0; }
   __device__ int* begin() const { return d.t3_t5_begin; }
   template <bool FILL>
@@ -127,8 +168,8 @@ struct StageT5 {
           int* md = d.t5_md + 5 * (size_t)pos;
           md[0] = m1.x; md[1] = m1.y; md[2] = m1.z; md[3] = m2.y; md[4] = m2.z;
           d.t5_score[pos] = score;
-          d.t5_axy[pos] = d.t3_axy[t1];
-          d.t5_lxy[pos] = d.t3_lxy[t2];
+          d.t5_l[pos] = d.t3_l[t2];
+          d.t5_kio[pos] = make_float2(ki, d.t3_k[t2]);
         }
         ++pos;
         ++cnt;

@@ -15,7 +15,7 @@ namespace lst {
 struct PtEvent;  // lst_pt.cuh
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT3, T_PT5, T_IDX, T_TC, T_PP3, T_PP5, T_ANC, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT, T_PP3, T_PP5, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
@@ -28,11 +28,24 @@ struct Ctl {
   int ticket[T_N];
   int total[K_NKINDS];
   int error;
-  int pad;
+  int done_rule3;                    // blocks of k_rule3 that have finished (the last one scans tc_cnt)
   int scratch_cur[4];                // accepted objects in the scratch lists: [1] LS, [2] pT3, [3] pT5
+  int queue_cur;                     // entries of the exact-evaluation queue of the seed linking
+  int pad[3];
+};
+
+// What changes from batch to batch: sizes and input pointers.  Lives in device memory (copied in front of
+// every launch sequence), so the kernel arguments -- and with them the CUDA graph of a context -- never change.
+struct Batch {
+  int n_events, n_hits, n_pls, pad;
+  const float *in_x, *in_y, *in_z;
+  const int* in_sensor;
+  const float *p_pt, *p_x0, *p_y0, *p_z0, *p_x1, *p_y1, *p_z1;
+  const int* p_q;
 };
 
 struct Dev {
+  const Batch* batch;  // device copy; load_batch() fills the batch fields below at the top of every kernel
   // ---- geometry (immutable, shared) ----
   int n_mod;
   const int* subdet;    // [n_mod]
@@ -63,7 +76,6 @@ struct Dev {
   // ---- a1: MD (grouped by global module) ----
   int* md_cnt;        // [n_hits] MDs owned by a sorted hit (upper-sensor hits only)
   int* md_stash;      // [n_hits][4] sorted positions of the first accepted lower hits
-  int* hit_md_begin;  // [n_hits + 1] exclusive scan of md_cnt
   int* mod_md_begin;  // [n_events * n_mod + 1] first MD of a global module
   int2* md_hit;       // (h_lo, h_hi) event-local input indices
   int* md_info;       // 2 * gm + endcap
@@ -79,21 +91,24 @@ struct Dev {
   int2* t3_ls;
   int4* t3_md;  // (A, B, C, endcap flags bit0 A, bit1 B, bit2 C)
   float* t3_k;
-  float2* t3_axy;  // anchor of the first MD (coalesced operand of the pLS gate)
-  float2* t3_lxy;  // anchor of the last MD (curvature pre-filter of the pLS linking)
+  float4* t3_l;  // last MD (x, y, z, r | endcap << 31): the operand of the seed linking's pre-filters
   // ---- a4: T5 (owner = first T3) ----
   int* t3_t5_begin;  // [n_t3 + 1]
   int2* t5_t3;
   int* t5_md;  // [n_t5][5]
   float* t5_score;
-  float2* t5_axy;
-  float2* t5_lxy;
+  float4* t5_l;    // last MD, as t3_l
+  float2* t5_kio;  // (ki, ko) = k3 of the two T3s
   // ---- a5: pT3 / pT5 (owner = pLS) ----
+  float4* seed_a;      // [n_pls] x1, y1, vx, vy           (CUTS.md section 7, computed once per seed)
+  float4* seed_b;      // [n_pls] lv, kp, tolk, slope
+  float* seed_z1;      // [n_pls]
   PtEvent* pt_ev;      // [n_events + 1] anchor / seed ranges and first tile of every event
-  int *anc_bin, *anc_rank;  // [n_md] bin (event * 256 + radial class * 32 + sector, -1 = no anchor) and arrival rank
-  int *anc_bin_cnt, *anc_bin_begin;  // [n_events * 256 + 1] (counts zeroed per batch)
-  float2* anc_axy;     // [n_anchor] anchor position
-  int2 *anc_t3, *anc_t5;  // [n_anchor] (first, count) of the T3s / T5s starting at the anchor
+  int *anc_bin, *anc_rank;  // [n_md] bin (radial class * 64 + sector, -1 = no anchor) and arrival rank in the event's bin
+  int* anc_bin_cnt;    // [n_events * 512] anchors per (event, bin) (zeroed per batch)
+  float4* anc_a;       // [n_md] anchor (x, y, z, r | endcap << 31), the anchors of event e from mod_md_begin[e * n_mod] on
+  int4* anc_t;         // [n_md] (first T3, number of T3s, first T5, number of T5s) starting at the anchor
+  int2* pt_queue;      // candidates for the exact cuts: (seed, T3 / T5 index | T5 flag << 31)
   int *pls_pt3_cnt, *pls_pt5_cnt;  // [n_pls + 1] accepted per seed (zeroed per batch)
   int *pls_pt3_cur, *pls_pt5_cur;  // [n_pls] next free slot of a seed's range (zeroed per batch)
   int* pls_event;      // [n_pls]
@@ -104,19 +119,28 @@ struct Dev {
   int2* pt5;
   float* pt5_score;
   // ---- a6: duplicate removal + track candidates ----
-  int* idx_cnt;    // [3 * n_md + 1] objects containing MD m: kind 0 T5, 1 pT5, 2 pT3
-  int* idx_begin;  // [3 * n_md + 1]
-  int* idx_cur;    // [3 * n_md]
-  int* idx_list;   // [5 * n_t5 + 5 * n_pt5 + 3 * n_pt3]
+  int* idx_head;   // [3 * n_md] objects containing MD m, as linked lists: kind 0 T5, 1 pT5, 2 pT3; 0 = end, else node + 1
+  int* idx_next;   // [5 * cap T5 | 5 * cap pT5 | 3 * cap pT3] node = object * (5 or 3) + position of the MD in it
   unsigned char *keep5, *keep3, *keepT, *linked;
-  int* tc_cnt;    // [n_events * 4 + 1] survivors per (event, class)
+  int* tc_cnt;    // [n_events * 4 + 1] survivors per (event, class) (zeroed per batch)
   int* tc_begin;  // [n_events * 4 + 1]
-  int* tc_cur;    // [n_events * 4]
+  int* tc_cur;    // [n_events * 4] (zeroed per batch)
   int* tc;        // [n_tc][16]
+  int* ev_first;  // [K_PT5 + 1][n_events + 1] first object of every event, per kind
   // ---- capacities ----
   int cap[K_NKINDS];
-  int cap_idx;
+  int cap_queue;
   Cuts cuts;
 };
+
+// first statement of every kernel: the batch fields of the by-value argument come from device memory
+__device__ __forceinline__ void load_batch(Dev& d) {
+  const Batch* __restrict__ b = d.batch;
+  d.n_events = b->n_events;  d.n_hits = b->n_hits;  d.n_pls = b->n_pls;
+  d.in_x = b->in_x;  d.in_y = b->in_y;  d.in_z = b->in_z;  d.in_sensor = b->in_sensor;
+  d.p_pt = b->p_pt;  d.p_q = b->p_q;
+  d.p_x0 = b->p_x0;  d.p_y0 = b->p_y0;  d.p_z0 = b->p_z0;
+  d.p_x1 = b->p_x1;  d.p_y1 = b->p_y1;  d.p_z1 = b->p_z1;
+}
 
 }  // namespace lst
