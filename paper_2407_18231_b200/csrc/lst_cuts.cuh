@@ -173,4 +173,101 @@ __device__ __forceinline__ unsigned t5_test(const Cuts& c, float ki, float ko, f
   return res | ACC;
 }
 
+// ---- approximate classification of a cut v <= t (used by the pre-filters of MD, LS and the seed linking) ----
+// A pre-filter evaluates a cut with cheaper arithmetic (rsqrt.approx, approximate division, FMA) and a band
+// b >= |v~ - v| + |t~ - t| + 1e-5 |t| (the near-threshold window of CUTS.md section 0):
+//   v~ > t~ + b  =>  the exact cut fails and is not near     (PT_FAIL)
+//   v~ < t~ - b  =>  the exact cut passes and is not near    (PT_PASS)
+//   otherwise, or when an operand is NaN / outside the range where the error bound holds: PT_UNSURE,
+//   and the exact arithmetic of the spec decides.
+// A candidate is dropped only at a cut that surely fails AFTER cuts that surely pass: the spec rejects it at
+// that cut without a near flag (evaluation stops at the first failed cut), so objects AND counters are unchanged.
+enum PtClass : int { PT_FAIL = 0, PT_PASS = 1, PT_UNSURE = 2 };
+
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+__device__ __forceinline__ int classify(float v, float t, float band, bool ok) {
+  if (ok && v > t + band) return PT_FAIL;
+  if (ok && v < t - band) return PT_PASS;
+  return PT_UNSURE;  // includes every NaN
+}
+
+// CUTS.md section 3 without sqrt or division.  Barrel: crs, dot, K = ra INV_2RMIN + tol, zv, zl are formed
+// exactly as in the spec; only lim = (ra dd) K is replaced by lim^2 ~ ((ra ra)(dx^2 + dy^2))(K K) (relative
+// error < 5e-7), compared with crs^2 at +-1e-4 (= +-5e-5 on |crs| / lim, 5x the near window).  The second
+// cut is the spec's own arithmetic.  Endcap: bend / den by approximate division (2^-22), band 3e-5.
+__device__ __forceinline__ int md_class(const Cuts& c, bool endcap, float4 a, float4 b) {
+  if (!endcap) {
+    const float dx = b.x - a.x, dy = b.y - a.y;
+    const float dot = a.x * dx + a.y * dy;
+    const float crs = a.x * dy - a.y * dx;
+    if (!(dot > 0.0f)) return PT_FAIL;  // strict cut, never flagged (a NaN fails it, as in the spec)
+    const float K = a.w * c.inv_2rmin + c.md_b_phi_tol;
+    const float lim2 = ((a.w * a.w) * fmaf(dx, dx, dy * dy)) * (K * K);
+    const float c2 = crs * crs;
+    const bool ok = K >= 0.0f && lim2 >= 1e-30f && lim2 <= 1e30f;
+    if (ok && c2 > lim2 * 1.0001f) return PT_FAIL;
+    if (!(ok && c2 < lim2 * 0.9999f)) return PT_UNSURE;
+    const float zv = fabsf(b.z * a.w - a.z * b.w);
+    const float zl = c.z0_max * (b.w - a.w) + c.md_z_tol * a.w;
+    if (near_thr(c, zv, zl) || !(zl == zl)) return PT_UNSURE;
+    return zv <= zl ? PT_PASS : PT_FAIL;
+  }
+  const float crs = a.x * b.y - a.y * b.x;
+  const float dz = fabsf(b.z - a.z);
+  const float den = fabsf(a.z) - c.z0_max;
+  const float q = __fdividef((((a.w * a.w) * dz) * c.inv_2rmin) * c.md_e_slope, den);
+  const float lim = b.w * (q + c.md_e_tol);
+  const float band = 3e-5f * (fabsf(lim) + fabsf(b.w * q));
+  const int c1 = classify(fabsf(crs), lim, band, fabsf(den) >= 1e-30f && fabsf(den) <= 1e30f);
+  if (c1 != PT_PASS) return c1;
+  const float rv = fabsf(b.w * a.z - a.w * b.z);
+  const float rl = c.z0_max * fabsf(b.w - a.w) + c.md_z_tol * fabsf(a.z);
+  if (near_thr(c, rv, rl) || !(rl == rl)) return PT_UNSURE;
+  return rv <= rl ? PT_PASS : PT_FAIL;
+}
+
+// CUTS.md section 4 with one rsqrt.approx per length and approximate divisions.  PT_FAIL = surely rejected and
+// not near; anything else needs the exact cut list (an accepted LS needs its exact kappa anyway).
+// Errors against the spec's binary32 values: kappa 1e-6 relative (crs exact); g(t^2) 1e-6 (u g'/g <= 0.43 for
+// u <= 1, same polynomial); rho 3e-6; c and 1/c 4e-7.
+__device__ __forceinline__ int ls_class(const Cuts& c, float4 A, float2 uA, bool eA, float4 B, float2 uB, bool eB) {
+  const float ex = B.x - A.x, ey = B.y - A.y;
+  const float c2 = fmaf(ex, ex, ey * ey);
+  const float crs = A.x * B.y - A.y * B.x;
+  const float rr = A.w * B.w;
+  const float den2 = (rr * rr) * c2;
+  bool ok = den2 >= 1e-30f && den2 <= 1e30f && c2 >= 1e-30f && c2 <= 1e30f && rr >= 0.0f;
+  const float kappa = (2.0f * crs) * rsqrt_approx(den2);  // rA, rB >= 0 (square roots) or NaN (-> not ok)
+  const float kv = fabsf(kappa) * c.r_min;
+  int cl = classify(kv, c.ls_kappa_max, 2e-5f * fabsf(c.ls_kappa_max) + 3e-6f * kv, ok);
+  if (cl != PT_PASS) return cl;
+  const float tA = (A.w * kappa) * 0.5f, tB = (B.w * kappa) * 0.5f;
+  ok = ok && fabsf(tA) <= 1.0f && fabsf(tB) <= 1.0f;
+  const float rho = __fdividef(B.w * g_poly(tB * tB), A.w * g_poly(tA * tA));
+  const float ztol = (eA || eB) ? c.ls_z_tol * (1.0f + __fdividef(fabsf(B.z), B.w)) : c.ls_z_tol;
+  const float zar = A.z * rho;
+  const float zv = fabsf(B.z - zar);
+  const float zl = c.z0_max * (rho - 1.0f) + ztol;
+  cl = classify(zv, zl, 1.2e-5f * fabsf(zl) + 5e-6f * (fabsf(zar) + fabsf(c.z0_max * rho)) + 1e-6f * (fabsf(B.z) + fabsf(ztol)), ok);
+  if (cl != PT_PASS) return cl;
+  const float icc = rsqrt_approx(c2);
+  const float half = ((c2 * icc) * kappa) * 0.5f;
+  if (!eA) {
+    const float sA = (uA.x * ey - uA.y * ex) * icc;
+    cl = classify(fabsf(sA - half), c.ls_dir_tol, 1.2e-5f * fabsf(c.ls_dir_tol) + 3e-6f * (fabsf(sA) + fabsf(half)), ok);
+    if (cl != PT_PASS) return cl;
+  }
+  if (!eB) {
+    const float sB = (uB.x * ey - uB.y * ex) * icc;
+    cl = classify(fabsf(sB + half), c.ls_dir_tol, 1.2e-5f * fabsf(c.ls_dir_tol) + 3e-6f * (fabsf(sB) + fabsf(half)), ok);
+    if (cl != PT_PASS) return cl;
+  }
+  return PT_PASS;
+}
+
 }  // namespace lst

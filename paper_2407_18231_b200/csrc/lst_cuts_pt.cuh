@@ -103,14 +103,6 @@ __device__ __forceinline__ unsigned pt_after_gate(const Cuts& c, const Seed& s, 
 //        r-z cuts      b = 1.2e-5 zt + 8e-6 |slope sq~| + 1e-6 (|z1| + |zQ|)
 //        (sq = lq g((lq kx / 2)^2): rel. error <= 3 ulp (lq) + 0.43 * 2 (d + 5 ulp) (g, u g'/g <= 0.43 on
 //        u <= 1) + polynomial rounding < 5e-6; the last term covers the roundings of the sum).
-enum PtClass : int { PT_FAIL = 0, PT_PASS = 1, PT_UNSURE = 2 };
-
-__device__ __forceinline__ float rsqrt_approx(float x) {
-  float r;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-  return r;
-}
-
 // kx~; ok = false when the product of the squared lengths leaves the range where the bound holds
 __device__ __forceinline__ float kx_approx(float x1, float y1, float xa, float ya, float xl, float yl, bool& ok) {
   const float ax = xa - x1, ay = ya - y1;
@@ -120,12 +112,6 @@ __device__ __forceinline__ float kx_approx(float x1, float y1, float xa, float y
   const float prod = (fmaf(ax, ax, ay * ay) * fmaf(bx, bx, by * by)) * fmaf(cx, cx, cy * cy);
   ok = prod >= 1e-30f && prod <= 1e30f;
   return (2.0f * crs) * rsqrt_approx(prod);
-}
-
-__device__ __forceinline__ int classify(float v, float t, float band, bool ok) {
-  if (ok && v > t + band) return PT_FAIL;
-  if (ok && v < t - band) return PT_PASS;
-  return PT_UNSURE;  // includes every NaN
 }
 
 __device__ __forceinline__ int pt_class_curv(float kx, float kref, float tolk, bool ok) {

@@ -42,13 +42,14 @@ struct LsWarp {  // per-warp scratch in shared memory
   int pref[kLsRanges + 1];  // exclusive prefix of the list lengths
   int b0[kLsRanges];        // first MD of the list | endcap(target) << 27 | owner slot << 28
   unsigned heads[kLsHeadWords];  // bit p set = a list starts at pair p (pairs below 32 * kLsHeadWords)
+  int2 cq[64];                   // pairs the pre-filter could not reject: (B, owner slot | endcap(B) << 8), in pair order
   LsAccepted stage[kLsStage];
 };
 
 __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
   load_batch(d);
   __shared__ LsWarp s_w[kWarps];
-  __shared__ unsigned long long s_tests[kEvSmem];
+  __shared__ unsigned s_tests[2 * kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   LsWarp& w = s_w[warp];
   EvTests tbl;
@@ -107,7 +108,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
           const int B0 = d.mod_md_begin[gb + m2];
           n_t = d.mod_md_begin[gb + m2 + 1] - B0;
           ent = B0 | ((__ldg(d.subdet + m2) != 0) << 27) | (o << 28);
-          if (!one_event) tbl.add(gb / d.n_mod, (unsigned long long)n_t);
+          if (!one_event) tbl.add(gb / d.n_mod, (unsigned)n_t);
         }
         const int incl = warp_incl_scan(n_t);
         const unsigned nz = __ballot_sync(kFull, n_t > 0);
@@ -124,17 +125,41 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
       const int P = carry;
       if (lane == 0) w.pref[Rn] = P;
       __syncwarp();
-      if (one_event && lane == 0) tbl.add(w.gb[first] / d.n_mod, (unsigned long long)P);
-      // ---- pairs of the pass, 32 at a time; pass 1 only if the stage overflowed ----
+      if (one_event && lane == 0) tbl.add(w.gb[first] / d.n_mod, (unsigned)P);
+      // ---- pairs of the pass, 32 at a time: the approximate cut list (ls_class) drops 95 % of them; the rest
+      // queue up in pair order and take the exact cuts of CUTS.md section 4 on full warps.  Pass 1 runs only
+      // if the stage overflowed: it evaluates the pairs again and writes straight to the scratch list. ----
       int base = 0, run = 0;
       for (int pass = 0; pass < 2; ++pass) {
         run = 0;
-        int heads_before = 0;
-        for (int p0 = 0; p0 < P; p0 += 32) {
-          const int p = p0 + lane;
+        int heads_before = 0, n_c = 0;
+        auto exact = [&](int n_now) {  // lanes below n_now take one queued pair each
           unsigned res = 0;
           LsAccepted acc;
           int o = 0;
+          if (lane < n_now) {
+            const int2 q = w.cq[lane];
+            o = q.y & 0xff;
+            acc.B = q.x;
+            res = ls_test(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[acc.B], d.md_u[acc.B], (q.y >> 8) & 1, acc.kappa);
+          }
+          if (pass == 0 && (res & NEAR)) count_near(d.ev_cnt, w.gb[o] / d.n_mod, 1);
+          const unsigned m = __ballot_sync(kFull, res & ACC);
+          if (res & ACC) {
+            const int pos = run + __popc(m & ((1u << lane) - 1u));
+            if (pass == 0) {
+              if (pos < kLsStage) w.stage[pos] = acc;
+              atomicAdd(&w.cnt[o], 1);
+            } else if (base + pos < cap) {
+              scratch[base + pos] = acc;
+            }
+          }
+          run += __popc(m);
+        };
+        for (int p0 = 0; p0 < P; p0 += 32) {
+          const int p = p0 + lane;
+          bool go = false;
+          int2 q = make_int2(0, 0);
           const unsigned hw = p0 < 32 * kLsHeadWords ? w.heads[p0 >> 5] : 0u;
           if (p < P) {
             int lo;  // list of pair p: the last list starting at or before p
@@ -149,23 +174,29 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
               }
             }
             const int ent = w.b0[lo];
-            o = (unsigned)ent >> 28;
-            acc.B = (ent & 0x7ffffff) + (p - w.pref[lo]);
-            res = ls_test(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[acc.B], d.md_u[acc.B], (ent >> 27) & 1, acc.kappa);
+            const int o = (unsigned)ent >> 28, eB = (ent >> 27) & 1;
+            q.x = (ent & 0x7ffffff) + (p - w.pref[lo]);
+            q.y = o | (eB << 8);
+            go = ls_class(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[q.x], d.md_u[q.x], eB != 0) != PT_FAIL;
           }
-          if (pass == 0 && (res & NEAR)) count_near(d.ev_cnt, w.gb[o] / d.n_mod, 1);
-          const unsigned m = __ballot_sync(kFull, res & ACC);
-          if (res & ACC) {
-            const int pos = run + __popc(m & ((1u << lane) - 1u));
-            if (pass == 0) {
-              if (pos < kLsStage) w.stage[pos] = acc;
-              atomicAdd(&w.cnt[o], 1);
-            } else if (base + pos < cap) {
-              scratch[base + pos] = acc;
-            }
-          }
-          run += __popc(m);
           heads_before += __popc(hw);
+          const unsigned m = __ballot_sync(kFull, go);
+          if (m == 0u) continue;
+          if (go) w.cq[n_c + __popc(m & ((1u << lane) - 1u))] = q;
+          n_c += __popc(m);
+          if (n_c >= 32) {
+            __syncwarp();
+            exact(32);
+            const int2 rest = (32 + lane < n_c) ? w.cq[32 + lane] : make_int2(0, 0);
+            __syncwarp();
+            w.cq[lane] = rest;
+            n_c -= 32;
+            __syncwarp();
+          }
+        }
+        if (n_c > 0) {
+          __syncwarp();
+          exact(n_c);
         }
         if (pass == 1) break;
         // ---- one atomic for the pass; per-MD count and scratch position ----

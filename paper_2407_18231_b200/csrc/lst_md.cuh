@@ -22,11 +22,30 @@ constexpr int kMdStash = 4;  // stashed MDs per upper hit
 __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
   load_batch(d);
   __shared__ int s_own[kWarps][96];
-  __shared__ unsigned long long s_tests[kEvSmem];
+  __shared__ unsigned s_tests[2 * kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int n = (d.cuts.stage_mask & 1) ? d.n_hits : 0;
   EvTests tbl;
   tbl.init(s_tests, d.ev_cnt, 0, d.n_events);
+  // candidates of CUTS.md section 3 per event: (lower hits) x (upper hits) of every module (consecutive
+  // threads take consecutive modules, i.e. one event: one shared-memory update per warp)
+  if (n > 0) {
+    const int n_gm = d.n_events * d.n_mod;
+    for (int g0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; g0 < n_gm; g0 += gridDim.x * blockDim.x) {
+      const int gm = g0 + lane;
+      unsigned t = 0u;
+      if (gm < n_gm) {
+        const int s0 = __ldg(d.sens_begin + 2 * gm), s1 = __ldg(d.sens_begin + 2 * gm + 1), s2 = __ldg(d.sens_begin + 2 * gm + 2);
+        const unsigned long long t64 = (unsigned long long)(s1 - s0) * (unsigned long long)(s2 - s1);
+        if (t64 < (1ull << 26)) {
+          t = (unsigned)t64;
+        } else {  // a module with > 6.7e7 hit pairs: straight to global memory (the warp sum above stays < 2^32)
+          atomicAdd(d.ev_cnt + (size_t)(gm / d.n_mod) * kEvCnt + 6, t64);
+        }
+      }
+      tbl.warp_add(min(gm, n_gm - 1) / d.n_mod, t);
+    }
+  }
   // one round: up to 32 queued upper hits, one per lane, each against its module's lower hits
   auto round = [&](int n_now) {
     int i = -1, a = 0, a1 = 0, endcap = 0, ev = 0;
@@ -41,22 +60,27 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
       endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
       hb = d.hit[i];
     }
-    tbl.warp_add(ev, (unsigned long long)(a1 - a));
-    int cnt = 0;
+    int cnt = 0, near = 0;
     int stash[kMdStash];
 #pragma unroll
     for (int k = 0; k < kMdStash; ++k) stash[k] = 0;
     for (; a < a1; ++a) {
-      float ux, uy;
-      const unsigned r = md_test(d.cuts, endcap, d.hit[a], hb, ux, uy);
-      if (r & NEAR) count_near(d.ev_cnt, ev, 0);
-      if (r & ACC) {
+      const float4 ha = d.hit[a];
+      int cl = md_class(d.cuts, endcap, ha, hb);  // sqrt- and division-free; the exact cuts only where it cannot decide
+      if (cl == PT_UNSURE) {
+        float ux, uy;
+        const unsigned r = md_test(d.cuts, endcap, ha, hb, ux, uy);
+        near += (r >> 1) & 1u;
+        cl = (r & ACC) ? PT_PASS : PT_FAIL;
+      }
+      if (cl == PT_PASS) {
 #pragma unroll
         for (int k = 0; k < kMdStash; ++k)
           if (cnt == k) stash[k] = a;
         ++cnt;
       }
     }
+    if (near) atomicAdd(d.ev_cnt + (size_t)ev * kEvCnt + 0, (unsigned long long)near);
     if (i >= 0) {
       d.md_cnt[i] = cnt;
       reinterpret_cast<int4*>(d.md_stash)[i] = make_int4(stash[0], stash[1], stash[2], stash[3]);

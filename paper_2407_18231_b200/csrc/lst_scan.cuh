@@ -46,36 +46,46 @@ __device__ __forceinline__ void count_near(unsigned long long* ev_cnt, int ev, i
 }
 
 // Candidate counts are accumulated per block in a shared-memory table indexed by event (events beyond
-// the table go straight to global memory) and flushed once at the end of the kernel.
+// the table go straight to global memory) and flushed once at the end of the kernel.  The table holds
+// 64-bit counts as two 32-bit words (shared-memory atomics are native for 32 bits only; a 64-bit add is a
+// compare-and-swap loop): the low word is added atomically, a wrap-around carries into the high word.
 struct EvTests {
-  unsigned long long* s;  // [64] shared
+  unsigned* s;            // [2][64] shared: low words, high words
   unsigned long long* g;  // ev_cnt
   int stage, n_events;
-  __device__ __forceinline__ void init(unsigned long long* smem, unsigned long long* ev_cnt, int st, int n_ev) {
+  __device__ __forceinline__ void init(unsigned* smem, unsigned long long* ev_cnt, int st, int n_ev) {
     s = smem;  g = ev_cnt;  stage = st;  n_events = n_ev;
-    for (int i = threadIdx.x; i < 64; i += blockDim.x) smem[i] = 0ull;
+    for (int i = threadIdx.x; i < 128; i += blockDim.x) smem[i] = 0u;
     __syncthreads();
   }
-  __device__ __forceinline__ void add(int ev, unsigned long long n) const {
-    if (n == 0ull) return;
-    if (ev < 64) atomicAdd(s + ev, n); else atomicAdd(g + (size_t)ev * 12 + 6 + stage, n);
+  // n < 2^32 per call
+  __device__ __forceinline__ void add(int ev, unsigned n) const {
+    if (n == 0u) return;
+    if (ev < 64) {
+      const unsigned old = atomicAdd(s + ev, n);
+      if (old + n < old) atomicAdd(s + 64 + ev, 1u);
+    } else {
+      atomicAdd(g + (size_t)ev * 12 + 6 + stage, (unsigned long long)n);
+    }
   }
   // called by all 32 lanes: lanes of the leader's event are summed into one update (the common case:
-  // consecutive work items belong to one event), the others add their own
-  __device__ __forceinline__ void warp_add(int ev, unsigned long long n) const {
-    const unsigned act = __ballot_sync(kFull, n != 0ull);
+  // consecutive work items belong to one event), the others add their own.  Sum over the warp < 2^32.
+  __device__ __forceinline__ void warp_add(int ev, unsigned n) const {
+    const unsigned act = __ballot_sync(kFull, n != 0u);
     if (act == 0u) return;
     const int lane = threadIdx.x & 31, lead = __ffs(act) - 1;
     const int ev0 = __shfl_sync(kFull, ev, lead);
-    const bool same = n != 0ull && ev == ev0;
-    const unsigned long long sum = warp_sum_u64(same ? n : 0ull);
+    const bool same = n != 0u && ev == ev0;
+    const unsigned sum = (unsigned)warp_sum((int)(same ? n : 0u));
     if (lane == lead) add(ev0, sum);
-    else if (n != 0ull && !same) add(ev, n);
+    else if (n != 0u && !same) add(ev, n);
   }
   __device__ __forceinline__ void flush() const {  // all threads of the block
     __syncthreads();
-    for (int e = threadIdx.x; e < 64 && e < n_events; e += blockDim.x)
-      if (s[e]) atomicAdd(g + (size_t)e * 12 + 6 + stage, s[e]);
+    for (int e = threadIdx.x; e < 64 && e < n_events; e += blockDim.x) {
+      const unsigned long long v = ((unsigned long long)s[64 + e] << 32) | s[e];
+      if (v) atomicAdd(g + (size_t)e * 12 + 6 + stage, v);
+    }
   }
 };
 

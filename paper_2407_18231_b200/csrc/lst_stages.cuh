@@ -12,7 +12,7 @@ __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
   load_batch(d);
   __shared__ int s_tile;
   __shared__ int s_scan[kWarps + 2];
-  __shared__ unsigned long long s_tests[kEvSmem];
+  __shared__ unsigned s_tests[2 * kEvSmem];
   Stage st(d);
   st.prologue();
   const int n = st.n_owners();
@@ -26,14 +26,14 @@ __global__ void __launch_bounds__(kBlock) k_stage(Dev d) {
     if (tile >= n_tiles) break;
     const int owner = tile * kBlock + threadIdx.x;
     int cnt = 0, ev = 0;
-    unsigned long long tests = 0;
+    unsigned tests = 0;
     if (owner < n) cnt = st.template visit<false>(owner, 0, ev, tests);
     tbl.warp_add(ev, tests);
     int tb, tt;
     const int off = tile_alloc(cnt, d.tstate[Stage::kTicket], tile, s_scan, tb, tt);
     if (owner < n) st.begin()[owner] = off;
     if (cnt > 0) {
-      unsigned long long t0 = 0;
+      unsigned t0 = 0;
       st.template visit<true>(owner, off, ev, t0);
     }
     if (tile == n_tiles - 1 && threadIdx.x == 0) {
@@ -84,7 +84,7 @@ struct StageT3 {
   __device__ int n_owners() const { return (d.cuts.stage_mask & 4) ? d.ctl->total[K_LS] : 0; }
   __device__ int* begin() const { return d.ls_t3_begin; }
   template <bool FILL>
-  __device__ int visit(int l, int pos, int& ev, unsigned long long& tests) const {
+  __device__ int visit(int l, int pos, int& ev, unsigned& tests) const {
     const int2 ab = d.ls_md[l];
     const int l0 = d.md_ls_begin[ab.y], l1 = d.md_ls_begin[ab.y + 1];
     if (l0 == l1) return 0;
@@ -93,7 +93,7 @@ struct StageT3 {
     const int eAB = (infoA & 1) | ((d.md_info[ab.y] & 1) << 1);
     if (!FILL) {
       ev = (infoA >> 1) / d.n_mod;
-      tests = (unsigned long long)(l1 - l0);
+      tests = (unsigned)(l1 - l0);
     }
     const int cap = d.cap[K_T3];
     int cnt = 0;
@@ -145,13 +145,13 @@ struct StageT5 {
   __device__ int n_owners() const { return (d.cuts.stage_mask & 8) ? d.ctl->total[K_T3] : 0; }
   __device__ int* begin() const { return d.t3_t5_begin; }
   template <bool FILL>
-  __device__ int visit(int t1, int pos, int& ev, unsigned long long& tests) const {
+  __device__ int visit(int t1, int pos, int& ev, unsigned& tests) const {
     const int4 m1 = d.t3_md[t1];
     const int u0 = d.ls_t3_begin[d.md_ls_begin[m1.z]], u1 = d.ls_t3_begin[d.md_ls_begin[m1.z + 1]];
     if (u0 == u1) return 0;
     if (!FILL) {
       ev = (d.md_info[m1.x] >> 1) / d.n_mod;
-      tests = (unsigned long long)(u1 - u0);
+      tests = (unsigned)(u1 - u0);
     }
     const float ki = d.t3_k[t1];
     const float4 b = d.md_a[m1.y], c = d.md_a[m1.z];
