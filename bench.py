@@ -45,6 +45,12 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=("b200", "reference"), default="b200")
     ap.add_argument("--pu", type=int, default=200)
+    ap.add_argument("--workload", choices=("C5", "C6"), default="C5",
+                    help="C5 = BASELINE.json configs[4] (the metric's workload); C6 = the strip-like second workload "
+                         "of SURVEY.md 8(f)2 (lst_inputs.configs)")
+    ap.add_argument("--truth-report", action="store_true",
+                    help="run C4 and one batch of the workload through the CUDA path and print the synthetic-truth "
+                         "metrics (PAPER.md:54-58, Figs. 3-4 in form) as JSON")
     ap.add_argument("--events", type=int, default=16, help="events per batch (= per step)")
     ap.add_argument("--streams", type=int, default=8, help="contexts / CUDA streams in flight")
     ap.add_argument("--batches", type=int, default=6, help="distinct input batches rotated through")
@@ -64,7 +70,7 @@ def dist_env():
 # ---------------------------------------------------------------------------------------------
 # inputs
 # ---------------------------------------------------------------------------------------------
-def make_batches(pu, n_events, n_batches, rank=0, world=1):
+def make_batches(pu, n_events, n_batches, rank=0, world=1, config="C5"):
     """n_batches distinct batches of n_events C5 events (lst_inputs recipe); every rank
     takes its own event numbers (paper_2407_18231_b200.replicas: replicas only, no collective)."""
     from lst_inputs import make_config_event
@@ -73,7 +79,7 @@ def make_batches(pu, n_events, n_batches, rank=0, world=1):
 
     out = []
     for idx in event_indices(rank, world, n_batches, n_events):
-        evs = [make_config_event("C5", pu=pu, index=i, seeds=True) for i in idx]
+        evs = [make_config_event(config, pu=pu, index=i, seeds=True) for i in idx]
         out.append((evs, concat_events(evs)))
     return out
 
@@ -172,6 +178,34 @@ def algorithmic_work(name, s, n_sens):
     return table.get(name, 0), flops
 
 
+def workload_string(args):
+    """config.workload: the same string from both arms (the driver compares them)."""
+    if args.workload == "C6":
+        return ("C6 PU%d: batches of %d strip-like events (SURVEY.md 8(f)2: C5's generator, 5 cm strips in the outer "
+                "layers, r-z windows of lst_inputs.configs.C6_PARAMS), %d streams" % (args.pu, args.events, args.streams))
+    return ("C5 PU%d: batches of %d PU200-like events (BASELINE.json configs[4]; generator of configs[2] with pLS "
+            "seeds), %d streams" % (args.pu, args.events, args.streams))
+
+
+def oracle_params(workload):
+    import oracle
+
+    if workload == "C6":
+        from lst_inputs.configs import C6_PARAMS
+
+        return oracle.default_params(**C6_PARAMS)
+    return None
+
+
+def workload_params(lst, workload):
+    """Cut constants of the workload: CUTS.md defaults for C5; C6 opens the r-z windows to the strip length."""
+    if workload == "C6":
+        from lst_inputs.configs import C6_PARAMS
+
+        return lst.lst_default_params(**C6_PARAMS)
+    return None
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -204,13 +238,13 @@ def run_b200(args):
             dist.barrier()
 
     E, S, NB = args.events, max(1, args.streams), max(1, args.batches)
-    geom, off, tgt = make_config_geometry("C5")
+    geom, off, tgt = make_config_geometry(args.workload)
     n_sens = E * 2 * geom.n_modules
     t0 = time.time()
-    batches = make_batches(args.pu, E, NB, rank, world)
+    batches = make_batches(args.pu, E, NB, rank, world, args.workload)
     gen_s = time.time() - t0
 
-    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt, workload_params(lst, args.workload))
     caps = lst.lst_default_caps(max_events=E)
     streams = [torch.cuda.Stream() for _ in range(S)]
     ctxs = [lst.lst_ctx_create(g, caps, st.cuda_stream) for st in streams]
@@ -339,10 +373,23 @@ def run_b200(args):
     else:
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": top["gbs"], "peak": hbm_gbs, "unit": "GB/s",
                 "frac": top["hbm_frac"], "traffic": None, "peak_source": peak_src + " copy bandwidth"}
-    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")  # from the committed ncu --set full capture
+    # DRAM traffic and executed warp instructions of the dominant kernel cannot be measured without a profiler:
+    # they come from the committed ncu --set full capture (profiles/traffic.json), and only when that capture was
+    # taken on this workload; the field says so
+    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
+    roof["traffic_source"] = None
     if os.path.exists(traffic_path):
         with open(traffic_path) as f:
-            roof["traffic"] = json.load(f).get(top["name"])
+            cap = json.load(f)
+        if cap.get("workload") == args.workload and cap.get("pu") == args.pu and cap.get("events") == E \
+                and top["name"] in cap.get("kernels", {}):
+            k = cap["kernels"][top["name"]]
+            roof["traffic"] = k.get("dram_bytes")
+            roof["traffic_source"] = "ncu capture %s (stored, not measured in this run)" % cap.get("capture", "?")
+            if k.get("warp_inst"):  # issue-rate roofline: 148 SMs x 4 schedulers x clock
+                issue_peak = 148 * 4 * sm_max_mhz * 1e6
+                roof["issue_frac"] = round(k["warp_inst"] / (top["ms"] * 1e-3) / issue_peak, 4)
+                roof["warp_inst"] = k["warp_inst"]
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -357,16 +404,16 @@ def run_b200(args):
     # ---- CPU baseline (rank 0, N = 1 only) -------------------------------------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = oracle_rate(batches[0][0][:E], geom, off, tgt)
+        cpu = oracle_rate(batches[0][0][:E], geom, off, tgt, params=oracle_params(args.workload))
 
     n_hits = [int(b["x"].shape[0]) for _, b in batches]
     line = {
         "metric": METRIC, "value": round(world * args.steps * E / (ms * 1e-3), 1), "unit": UNIT,
-        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, S), "ms_per_step": round(ms / args.steps, 5),
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "warmup_effective": max(args.warmup, S),
+        "ms_per_step": round(ms / args.steps, 5),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {
-            "workload": "C5 PU%d: batches of %d PU200-like events (BASELINE.json configs[4]; generator of "
-                        "configs[2] with pLS seeds), %d streams" % (args.pu, E, S),
+            "workload": workload_string(args),
             "events_per_step": E, "hits_per_event": int(np.mean(n_hits) / E), "pls_per_event": ksum["n_pls"] // E,
             "modules": int(geom.n_modules), "parallelism": "replicas x%d, no collective" % world,
             "l2": "inputs rotate over %d distinct batches + %d context workspaces (> 126 MB L2); per-kernel "
@@ -374,6 +421,11 @@ def run_b200(args):
             "objects_per_step": {k: ksum["n_" + k] for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
             "tests_per_step": dict(zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["n_tests"])),
             "near_threshold_per_step": dict(zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["near"])),
+            # north_star states the 0.01 % bar against objects; reading N2 checks it against candidates
+            "near_frac_of_candidates": {k: (round(n / t, 9) if t else None) for k, n, t in
+                                        zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["near"], ksum["n_tests"])},
+            "near_frac_of_objects": {k: (round(n / ksum["n_" + k], 9) if ksum["n_" + k] else None) for k, n in
+                                     zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["near"])},
             "generation_s": round(gen_s, 1),
         },
         "e2e": {"value": round(world * args.steps * E / (ms_e2e * 1e-3), 1), "unit": UNIT,
@@ -399,7 +451,7 @@ def run_b200(args):
 # ---------------------------------------------------------------------------------------------
 # the CPU oracle: cpu_baseline leg and --impl reference
 # ---------------------------------------------------------------------------------------------
-def oracle_rate(events, geom, off, tgt, single=True):
+def oracle_rate(events, geom, off, tgt, single=True, params=None):
     """Times oracle.run_event (as it stands, one thread per event) over `events` on the host cores."""
     from concurrent.futures import ThreadPoolExecutor
 
@@ -414,7 +466,7 @@ def oracle_rate(events, geom, off, tgt, single=True):
     threads = max(1, min(cores, len(events)))
 
     def one(ev):
-        r = oracle.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+        r = oracle.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls, params)
         return len(r["tc"])
 
     t_single = float("nan")
@@ -440,33 +492,34 @@ def run_reference(args):
         return
     from lst_inputs import make_config_geometry
 
-    geom, off, tgt = make_config_geometry("C5")
+    geom, off, tgt = make_config_geometry(args.workload)
     cores = os.cpu_count() or 1
     try:
         cores = len(os.sched_getaffinity(0))
     except AttributeError:
         pass
     per_step = max(1, min(cores, args.events))
+    oparams = oracle_params(args.workload)
     # keep the whole run within a few minutes: ~1.5 s of one core per PU200 event
     steps = max(1, min(args.steps, 20))
     warm = max(0, min(args.warmup, 1))
-    batches = make_batches(args.pu, per_step, 2)
+    batches = make_batches(args.pu, per_step, 2, config=args.workload)
     for _ in range(warm):
-        oracle_rate(batches[0][0], geom, off, tgt, single=False)
+        oracle_rate(batches[0][0], geom, off, tgt, single=False, params=oparams)
     t0 = time.perf_counter()
     res = None
     for i in range(steps):
-        res = oracle_rate(batches[i % 2][0], geom, off, tgt, single=False)
+        res = oracle_rate(batches[i % 2][0], geom, off, tgt, single=False, params=oparams)
     wall = time.perf_counter() - t0
     n_ev = steps * per_step
     value = round(n_ev / wall, 3)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": steps, "warmup": warm, "ms_per_step": round(wall / steps * 1e3, 3), "higher_is_better": True,
+        "steps": steps, "warmup": args.warmup, "warmup_effective": warm, "steps_requested": args.steps,
+        "ms_per_step": round(wall / steps * 1e3, 3), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "C5 PU%d: batches of %d PU200-like events (BASELINE.json configs[4]); each step "
-                               "a bounded sample of %d events" % (args.pu, args.events, per_step),
-                   "events_per_step": per_step},
+        "config": {"workload": workload_string(args), "events_per_step": per_step,
+                   "note": "each step is a bounded sample of %d events of the step's batch" % per_step},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": res["cores"], "kind": "oracle",
                          "sample": "%d steps x %d events, oracle.run_event, %d threads" % (steps, per_step,
                                                                                            res["cores"])},
@@ -476,9 +529,52 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_truth_report(args):
+    """synthetic-truth metrics of the track candidates the CUDA path returns (PAPER.md:54-58,
+    Figs. 3-4 in form, not in values): C4 (prompt + displaced tracks) and one batch of the workload."""
+    import torch
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    from paper_2407_18231_b200 import build as lst_build
+
+    lst_build.build()
+    import paper_2407_18231_b200 as lst
+    from lst_inputs import make_config_event, make_config_geometry
+    from lst_inputs.events import concat_events
+    from lst_inputs.truth_metrics import merge_metrics, track_candidate_metrics
+
+    out = {}
+    geom, off, tgt = make_config_geometry("C4")
+    ev = make_config_event("C4")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    res = lst.lst_run_event(g, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+    lst.lst_free(g)
+    out["C4"] = {"all": track_candidate_metrics(res, ev), "with_outer_tracker_hits": track_candidate_metrics(res, ev, classes=(0, 1, 2)),
+                 "T5_only": track_candidate_metrics(res, ev, classes=(2,))}
+    geom, off, tgt = make_config_geometry(args.workload)
+    evs = [make_config_event(args.workload, pu=args.pu, index=i, seeds=True) for i in range(args.events)]
+    b = concat_events(evs)
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt, workload_params(lst, args.workload))
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=args.events), torch.cuda.Stream().cuda_stream)
+    h, keep = lst.make_hits(b["x"], b["y"], b["z"], b["sensor"], b["hit_offsets"])
+    s, keep = lst.make_pls(b["pls"], b["pls_offsets"], keep)
+    lst.lst_ctx_run(ctx, len(evs), h, s)
+    lst.lst_ctx_sync(ctx)
+    per_ev = [lst.lst_ctx_fetch_event(ctx, i) for i in range(len(evs))]
+    lst.lst_free(ctx)
+    lst.lst_free(g)
+    key = "%s_PU%d_x%d" % (args.workload, args.pu, len(evs))
+    out[key] = {"all": merge_metrics([track_candidate_metrics(r, e) for r, e in zip(per_ev, evs)]),
+                "with_outer_tracker_hits": merge_metrics([track_candidate_metrics(r, e, classes=(0, 1, 2))
+                                                          for r, e in zip(per_ev, evs)])}
+    print(json.dumps({"truth_report": out, "source": "track candidates fetched through the C ABI (CUDA path)"}))
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.truth_report:
+        run_truth_report(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_b200(args)

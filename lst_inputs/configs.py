@@ -5,6 +5,9 @@ C2 barrel, 500 helices + noise + 5%  -> full chain + duplicate removal
 C3 PU200-like single event (barrel + endcap, ~7000 helices)
 C4 C2 + pLS seeds + 50 displaced helices
 C5 batches of 16 C3-like events at PU 50/100/140/200/250 (35 tracks per PU unit)
+C6 (not a BASELINE.json config) C5's generator with strip-like sensors: 5 cm strips along z on
+   the three outer barrel layers and two strip rows per endcap ring beyond r = 60 cm, with the z windows of the
+   cuts opened to the strip length (C6_PARAMS) -- the combinatorics-heavier second workload
 """
 from __future__ import annotations
 
@@ -15,11 +18,15 @@ from .events import Event, EventSpec, generate_event
 from .geometry import Geometry, make_geometry
 
 CONFIG_NAMES = ("C1", "C2", "C3", "C4", "C5")
+# cut constants of the strip-like workload: the r-z windows must hold a strip (pitch 5 cm, i.e. +-2.5 cm of
+# quantisation per hit); everything else as in CUTS.md section 1
+STRIP_PITCH = 5.0
+C6_PARAMS = {"md_z_tol": 5.5, "ls_z_tol": 4.0, "t3_z_tol0": 4.0, "t3_z_tol1": 1.0, "pt_z_tol": 5.0}
 PU_POINTS = (50, 100, 140, 200, 250)
 TRACKS_PER_PU = 35
 
 _GEOM_OF = {"C1": "barrel_z60", "C2": "barrel_z60", "C3": "barrel_z120_endcap",
-            "C4": "barrel_z60", "C5": "barrel_z120_endcap"}
+            "C4": "barrel_z60", "C5": "barrel_z120_endcap", "C6": "barrel_z120_endcap"}
 
 
 @lru_cache(maxsize=None)
@@ -43,6 +50,9 @@ def spec_of(config: str, pu: int = 200, seeds: bool | None = None) -> EventSpec:
     if config == "C3" or config == "C5":
         return EventSpec(n_tracks=TRACKS_PER_PU * pu, pt_dist=("power3", 0.3), eta_max=2.5,
                          noise=("frac", 0.01), seeds=bool(seeds))
+    if config == "C6":
+        return EventSpec(n_tracks=TRACKS_PER_PU * pu, pt_dist=("power3", 0.3), eta_max=2.5,
+                         noise=("frac", 0.01), seeds=bool(seeds), strip_pitch=STRIP_PITCH)
     if config == "C4":
         return EventSpec(n_tracks=500, pt_dist=("loguniform", 0.8, 20.0), eta_max=1.0,
                          noise=("count", 2000), inefficiency=0.05, seeds=True, n_displaced=50)
@@ -52,7 +62,7 @@ def spec_of(config: str, pu: int = 200, seeds: bool | None = None) -> EventSpec:
 def make_config_event(config: str, pu: int = 200, index: int = 0, seeds: bool | None = None) -> Event:
     """Seed = config number (C1..C4); C5: 1000*PU + event index (G7)."""
     geom, _, _ = make_config_geometry(config)
-    if config == "C5":
+    if config in ("C5", "C6"):
         seed = 1000 * pu + index
     else:
         seed = int(config[1])
@@ -60,5 +70,5 @@ def make_config_event(config: str, pu: int = 200, index: int = 0, seeds: bool | 
     return generate_event(geom, spec_of(config, pu, seeds), seed)
 
 
-def c5_batch(pu: int = 200, n_events: int = 16, seeds: bool = True, first: int = 0):
-    return [make_config_event("C5", pu=pu, index=first + i, seeds=seeds) for i in range(n_events)]
+def c5_batch(pu: int = 200, n_events: int = 16, seeds: bool = True, first: int = 0, config: str = "C5"):
+    return [make_config_event(config, pu=pu, index=first + i, seeds=seeds) for i in range(n_events)]

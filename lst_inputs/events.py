@@ -44,6 +44,12 @@ class EventSpec:
     d0_max: float = 20.0
     sigma_vz: float = 5.0
     phi_range: tuple = (0.0, TWO_PI)  # azimuth window of the generated helices
+    # strip-like sensors (Fig. 1): on the barrel layers listed here (1-based) a hit's
+    # z is the centre of its strip of length strip_pitch; on endcap rings starting at r >= strip_endcap_rmin
+    # its r is the centre of one of the two strip rows of the ring.  0 = the default pixel-like sensors.
+    strip_pitch: float = 0.0
+    strip_layers: tuple = (4, 5, 6)
+    strip_endcap_rmin: float = 60.0
 
 
 @dataclass
@@ -98,6 +104,21 @@ def _make_tracks(rng, spec: EventSpec):
     return Tracks(xs, ys, z0, phi0, eta, pt, q), d0
 
 
+def _strip_z(z, pitch):
+    """Centre of the strip (length ``pitch``, edges at multiples of it) that holds z."""
+    return (np.floor(z / pitch) + 0.5) * pitch
+
+
+def _strip_r(r):
+    """Centre of the strip row of an endcap ring that holds r (two rows per ring)."""
+    w = (ENDCAP_RMAX - ENDCAP_RMIN) / ENDCAP_NRINGS
+    ir = np.clip(np.floor((r - ENDCAP_RMIN) / w), 0, ENDCAP_NRINGS - 1)
+    r1 = ENDCAP_RMIN + ir * w
+    half = 0.5 * w
+    row = np.clip(np.floor((r - r1) / half), 0, 1)
+    return r1 + (row + 0.5) * half, r1
+
+
 def _signal_hits(rng, geom: Geometry, trk: Tracks, spec: EventSpec):
     n = len(trk)
     n_turns = int(np.ceil(spec.max_turns))
@@ -114,6 +135,8 @@ def _signal_hits(rng, geom: Geometry, trk: Tracks, spec: EventSpec):
             continue
         phi = np.arctan2(y[ii, jj], x[ii, jj]) + rng.normal(0.0, SIGMA_RPHI, ii.size) / rho
         zz = z[ii, jj] + rng.normal(0.0, SIGMA_Z, ii.size)
+        if spec.strip_pitch > 0.0 and (il + 1) in spec.strip_layers:
+            zz = _strip_z(zz, spec.strip_pitch)
         m = geom.barrel_module(np.full(ii.size, il), phi, zz)
         xs.append(rho * np.cos(phi))
         ys.append(rho * np.sin(phi))
@@ -130,6 +153,9 @@ def _signal_hits(rng, geom: Geometry, trk: Tracks, spec: EventSpec):
         if ii.size == 0:
             continue
         rr = r[ii] + rng.normal(0.0, SIGMA_Z, ii.size)
+        if spec.strip_pitch > 0.0:
+            rq, r1 = _strip_r(rr)
+            rr = np.where(r1 >= spec.strip_endcap_rmin, rq, rr)
         phi = np.arctan2(y[ii], x[ii]) + rng.normal(0.0, SIGMA_RPHI, ii.size) / r[ii]
         m = geom.endcap_module(np.full(ii.size, iside), np.full(ii.size, idisk), rr, phi)
         xs.append(rr * np.cos(phi))
@@ -145,8 +171,8 @@ def _signal_hits(rng, geom: Geometry, trk: Tracks, spec: EventSpec):
             np.concatenate(sens).astype(np.int64), np.concatenate(truth).astype(np.int64))
 
 
-def _noise_hits(rng, geom: Geometry, n: int):
-    """``n`` hits, each on a uniformly chosen sensor, uniform over that sensor's area."""
+def _noise_hits(rng, geom: Geometry, n: int, spec: EventSpec | None = None):
+    """``n`` hits, each on a uniformly chosen sensor, uniform over that sensor's area (strip sensors: on a strip centre)."""
     sensor = rng.integers(0, geom.n_sensors, n)
     m = sensor // 2
     s = sensor % 2
@@ -167,7 +193,10 @@ def _noise_hits(rng, geom: Geometry, n: int):
         phi = (iphi + u1[bar]) / nphi * TWO_PI
         x[bar] = rho * np.cos(phi)
         y[bar] = rho * np.sin(phi)
-        z[bar] = -geom.barrel_zmax + (iz + u2[bar]) * TILE
+        zb = -geom.barrel_zmax + (iz + u2[bar]) * TILE
+        if spec is not None and spec.strip_pitch > 0.0:
+            zb = np.where(np.isin(il + 1, spec.strip_layers), _strip_z(zb, spec.strip_pitch), zb)
+        z[bar] = zb
     end = ~bar
     if end.any():
         me = m[end]
@@ -180,6 +209,8 @@ def _noise_hits(rng, geom: Geometry, n: int):
         r1 = ENDCAP_RMIN + ir * w
         r2 = r1 + w
         r = np.sqrt(r1 * r1 + u2[end] * (r2 * r2 - r1 * r1))
+        if spec is not None and spec.strip_pitch > 0.0:
+            r = np.where(r1 >= spec.strip_endcap_rmin, _strip_r(r)[0], r)
         phi = (iphi + u1[end]) / nphi * TWO_PI
         x[end] = r * np.cos(phi)
         y[end] = r * np.sin(phi)
@@ -243,7 +274,7 @@ def generate_event(geom: Geometry, spec: EventSpec, seed: int) -> Event:
         x, y, z, sensor, truth = x[keep], y[keep], z[keep], sensor[keep], truth[keep]
     if spec.noise is not None:
         n_noise = int(spec.noise[1]) if spec.noise[0] == "count" else int(round(spec.noise[1] * x.shape[0]))
-        nx, ny, nz, ns = _noise_hits(rng, geom, n_noise)
+        nx, ny, nz, ns = _noise_hits(rng, geom, n_noise, spec)
         x = np.concatenate([x, nx])
         y = np.concatenate([y, ny])
         z = np.concatenate([z, nz])

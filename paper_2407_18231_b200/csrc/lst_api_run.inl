@@ -70,11 +70,11 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   k_pt_place<<<gp, kBlock, 0, st>>>(d);
   if (mask & 32) {
     L.mark("rule1_pt5");
-    k_rule1<<<gp, kBlock, 0, st>>>(d);
+    k_rule1<<<gw, kBlock, 0, st>>>(d);
     L.mark("rule2_pt3");
-    k_rule2<<<gp, kBlock, 0, st>>>(d);
+    k_rule2<<<gw, kBlock, 0, st>>>(d);
     L.mark("rule3_t5");
-    k_rule3<<<gp, kBlock, 0, st>>>(d);
+    k_rule3<<<gw, kBlock, 0, st>>>(d);
     L.mark("tc_emit");
     k_tc_emit<<<gp, kBlock, 0, st>>>(d);
   }

@@ -134,120 +134,161 @@ struct IdxIt {
   }
 };
 
-// rule 1: pT5 vs pT5
-__global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
-  load_batch(d);
-  const int stride = gridDim.x * blockDim.x;
-  const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_PT5];
-  for (int X = blockIdx.x * blockDim.x + threadIdx.x; X < n; X += stride) {
-    const int2 x = d.pt5[X];
-    const float sX = d.pt5_score[X];
-    int mX[5], mY[5];
-    load_t5_md(d, x.y, mX);
-    bool keep = true;
-    for (int Y = d.pls_pt5_begin[x.x]; Y < d.pls_pt5_begin[x.x + 1] && keep; ++Y) {
-      if (Y == X) continue;
-      load_t5_md(d, d.pt5[Y].y, mY);
-      if (better(d, d.pt5_score[Y], x.x, mY, sX, x.x, mX, 5)) keep = false;
-    }
-    for (int k = 0; k < 5 && keep; k += 2) {
-      for (IdxIt it(d, n_md, 1, mX[k]); it.obj >= 0 && keep; it.advance()) {
-        const int Y = it.obj;
-        if (Y == X) continue;
-        const int2 y = d.pt5[Y];
-        load_t5_md(d, y.y, mY);
-        if (share(mY, 5, mX, 5) >= 3 && better(d, d.pt5_score[Y], y.x, mY, sX, x.x, mX, 5)) keep = false;
-      }
-    }
-    d.keep5[X] = keep;
-    if (keep) {
-      d.linked[x.x] = 1;  // one writer per value; rule 4 (k_rule3) completes it with the surviving pT3s
-      atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 0, 1);
-    }
-  }
+// The three rules are latency-bound: an object walks a handful of short linked lists, every element a chain of
+// dependent loads.  Each object is therefore given a group of 4, 8 or 16 lanes, one list (or the same-seed
+// range) per lane; a ballot over the group decides.  Groups are aligned sub-warps.
+template <int LANES>
+__device__ __forceinline__ bool group_any(bool pred) {
+  const unsigned m = __ballot_sync(kFull, pred);
+  const int lane = threadIdx.x & 31;
+  return ((m >> (lane & ~(LANES - 1))) & ((1u << LANES) - 1u)) != 0u;
 }
 
-// rule 2: pT3 vs pT3, then vs surviving pT5
-__global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
+// rule 1: pT5 X is removed by a better pT5 of the same seed (task 0) or sharing >= 3 MDs (tasks 1..3: the
+// lists of X.md[0], [2], [4])
+__global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
   load_batch(d);
-  const int stride = gridDim.x * blockDim.x;
-  const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_PT3], n_pt5 = d.ctl->total[K_PT5];
-  for (int X = blockIdx.x * blockDim.x + threadIdx.x; X < n; X += stride) {
-    const int2 x = d.pt3[X];
-    const float sX = d.pt3_score[X];
-    int mX[3], mY[5];
-    load_t3_md(d, x.y, mX);
-    bool keep = !(d.linked[x.x] & 1);  // rule 2b: seed already in a surviving pT5
-    for (int Y = d.pls_pt3_begin[x.x]; Y < d.pls_pt3_begin[x.x + 1] && keep; ++Y) {
-      if (Y == X) continue;
-      load_t3_md(d, d.pt3[Y].y, mY);
-      if (better(d, d.pt3_score[Y], x.x, mY, sX, x.x, mX, 3)) keep = false;
-    }
-    for (int k = 0; k < 2 && keep; ++k) {
-      for (IdxIt it(d, n_md, 2, mX[k]); it.obj >= 0 && keep; it.advance()) {
-        const int Y = it.obj;
-        if (Y == X) continue;
-        const int2 y = d.pt3[Y];
-        load_t3_md(d, y.y, mY);
-        if (share(mY, 3, mX, 3) >= 2 && better(d, d.pt3_score[Y], y.x, mY, sX, x.x, mX, 3)) keep = false;
-      }
-      if (n_pt5 > 0) {
-        for (IdxIt it(d, n_md, 1, mX[k]); it.obj >= 0 && keep; it.advance()) {
-          const int Z = it.obj;
-          if (!d.keep5[Z]) continue;
-          load_t5_md(d, d.pt5[Z].y, mY);
-          if (share(mX, 3, mY, 5) >= 2) keep = false;
+  constexpr int kRuleLanes = 4;
+  const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_PT5];
+  const int task = threadIdx.x & (kRuleLanes - 1);
+  const int n_groups = gridDim.x * blockDim.x / kRuleLanes, g0 = (blockIdx.x * blockDim.x + threadIdx.x) / kRuleLanes;
+  for (int X0 = 0; X0 < n; X0 += n_groups) {  // all lanes of a warp stay in the loop (ballot)
+    const int X = X0 + g0;
+    bool rem = false;
+    int2 x = make_int2(0, 0);
+    if (X < n && task < 4) {
+      x = d.pt5[X];
+      const float sX = d.pt5_score[X];
+      int mX[5], mY[5];
+      load_t5_md(d, x.y, mX);
+      if (task == 0) {
+        for (int Y = d.pls_pt5_begin[x.x]; Y < d.pls_pt5_begin[x.x + 1] && !rem; ++Y) {
+          if (Y == X) continue;
+          load_t5_md(d, d.pt5[Y].y, mY);
+          rem = better(d, d.pt5_score[Y], x.x, mY, sX, x.x, mX, 5);
+        }
+      } else {
+        for (IdxIt it(d, n_md, 1, mX[2 * (task - 1)]); it.obj >= 0 && !rem; it.advance()) {
+          const int Y = it.obj;
+          if (Y == X) continue;
+          const int2 y = d.pt5[Y];
+          load_t5_md(d, y.y, mY);
+          rem = share(mY, 5, mX, 5) >= 3 && better(d, d.pt5_score[Y], y.x, mY, sX, x.x, mX, 5);
         }
       }
     }
-    d.keep3[X] = keep;
-    if (keep) atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 1, 1);
+    const bool keep = !group_any<kRuleLanes>(rem);
+    if (X < n && task == 0) {
+      d.keep5[X] = keep;
+      if (keep) {
+        d.linked[x.x] = 1;  // one writer per value; rule 4 (k_rule3) completes it with the surviving pT3s
+        atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 0, 1);
+      }
+    }
   }
 }
 
-// rule 3: T5 vs T5, vs surviving pT5, vs surviving pT3; rule 4: unlinked pLS.  The last block to finish
-// turns the per-(event, class) survivor counts into tc_begin (a scan of 4 * n_events + 1 numbers).
+// rule 2: pT3 X is removed by a better pT3 of the same seed (task 0) or sharing >= 2 MDs (tasks 1, 2: lists of
+// X.md[0], [1]), or by a SURVIVING pT5 of its seed (task 0) or sharing >= 2 MDs (tasks 3, 4)
+__global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
+  load_batch(d);
+  constexpr int kRuleLanes = 8;
+  const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_PT3], n_pt5 = d.ctl->total[K_PT5];
+  const int task = threadIdx.x & (kRuleLanes - 1);
+  const int n_groups = gridDim.x * blockDim.x / kRuleLanes, g0 = (blockIdx.x * blockDim.x + threadIdx.x) / kRuleLanes;
+  for (int X0 = 0; X0 < n; X0 += n_groups) {
+    const int X = X0 + g0;
+    bool rem = false;
+    int2 x = make_int2(0, 0);
+    if (X < n && task < 5) {
+      x = d.pt3[X];
+      const float sX = d.pt3_score[X];
+      int mX[3], mY[5];
+      load_t3_md(d, x.y, mX);
+      if (task == 0) {
+        rem = d.linked[x.x] & 1;  // rule 2b: seed already in a surviving pT5
+        for (int Y = d.pls_pt3_begin[x.x]; Y < d.pls_pt3_begin[x.x + 1] && !rem; ++Y) {
+          if (Y == X) continue;
+          load_t3_md(d, d.pt3[Y].y, mY);
+          rem = better(d, d.pt3_score[Y], x.x, mY, sX, x.x, mX, 3);
+        }
+      } else if (task <= 2) {
+        for (IdxIt it(d, n_md, 2, mX[task - 1]); it.obj >= 0 && !rem; it.advance()) {
+          const int Y = it.obj;
+          if (Y == X) continue;
+          const int2 y = d.pt3[Y];
+          load_t3_md(d, y.y, mY);
+          rem = share(mY, 3, mX, 3) >= 2 && better(d, d.pt3_score[Y], y.x, mY, sX, x.x, mX, 3);
+        }
+      } else if (n_pt5 > 0) {
+        for (IdxIt it(d, n_md, 1, mX[task - 3]); it.obj >= 0 && !rem; it.advance()) {
+          const int Z = it.obj;
+          if (!d.keep5[Z]) continue;
+          load_t5_md(d, d.pt5[Z].y, mY);
+          rem = share(mX, 3, mY, 5) >= 2;
+        }
+      }
+    }
+    const bool keep = !group_any<kRuleLanes>(rem);
+    if (X < n && task == 0) {
+      d.keep3[X] = keep;
+      if (keep) atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 1, 1);
+    }
+  }
+}
+
+// rule 3: T5 X is removed by a better T5 sharing >= 3 MDs (tasks 0..2: lists of X.md[0], [2], [4]), by a surviving
+// pT5 (tasks 3..6) or pT3 (tasks 7..10) sharing >= 2 MDs (lists of X.md[0..3]); rule 4: unlinked pLS.  The last
+// block to finish turns the per-(event, class) survivor counts into tc_begin (a scan of 4 * n_events + 1 numbers).
 __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
   load_batch(d);
+  constexpr int kRuleLanes = 16;
   __shared__ int s_last;
   __shared__ int s_carry;
   __shared__ int s_warp[kWarps];
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_T5];
   const int n_pt5 = d.ctl->total[K_PT5], n_pt3 = d.ctl->total[K_PT3];
-  for (int X = i0; X < n; X += stride) {
-    const float sX = d.t5_score[X];
-    int mX[5], mY[5];
-    load_t5_md(d, X, mX);
-    bool keep = true;
-    for (int k = 0; k < 5 && keep; k += 2) {
-      for (IdxIt it(d, n_md, 0, mX[k]); it.obj >= 0 && keep; it.advance()) {
-        const int Y = it.obj;
-        if (Y == X) continue;
-        load_t5_md(d, Y, mY);
-        if (share(mY, 5, mX, 5) >= 3 && better(d, d.t5_score[Y], -1, mY, sX, -1, mX, 5)) keep = false;
-      }
-    }
-    for (int k = 0; k < 4 && keep; ++k) {
-      if (n_pt5 > 0) {
-        for (IdxIt it(d, n_md, 1, mX[k]); it.obj >= 0 && keep; it.advance()) {
-          const int Z = it.obj;
-          if (!d.keep5[Z]) continue;
-          load_t5_md(d, d.pt5[Z].y, mY);
-          if (share(mX, 5, mY, 5) >= 2) keep = false;
+  const int task = threadIdx.x & (kRuleLanes - 1);
+  const int n_groups = stride / kRuleLanes, g0 = i0 / kRuleLanes;
+  for (int X0 = 0; X0 < n; X0 += n_groups) {
+    const int X = X0 + g0;
+    bool rem = false;
+    int md0 = 0;
+    if (X < n && task < 11) {
+      const float sX = d.t5_score[X];
+      int mX[5], mY[5];
+      load_t5_md(d, X, mX);
+      md0 = mX[0];
+      if (task < 3) {
+        for (IdxIt it(d, n_md, 0, mX[2 * task]); it.obj >= 0 && !rem; it.advance()) {
+          const int Y = it.obj;
+          if (Y == X) continue;
+          load_t5_md(d, Y, mY);
+          rem = share(mY, 5, mX, 5) >= 3 && better(d, d.t5_score[Y], -1, mY, sX, -1, mX, 5);
         }
-      }
-      if (n_pt3 > 0) {
-        for (IdxIt it(d, n_md, 2, mX[k]); it.obj >= 0 && keep; it.advance()) {
+      } else if (task < 7) {
+        if (n_pt5 > 0)
+          for (IdxIt it(d, n_md, 1, mX[task - 3]); it.obj >= 0 && !rem; it.advance()) {
+            const int Z = it.obj;
+            if (!d.keep5[Z]) continue;
+            load_t5_md(d, d.pt5[Z].y, mY);
+            rem = share(mX, 5, mY, 5) >= 2;
+          }
+      } else if (n_pt3 > 0) {
+        for (IdxIt it(d, n_md, 2, mX[task - 7]); it.obj >= 0 && !rem; it.advance()) {
           const int Z = it.obj;
           if (!d.keep3[Z]) continue;
           load_t3_md(d, d.pt3[Z].y, mY);
-          if (share(mX, 5, mY, 3) >= 2) keep = false;
+          rem = share(mX, 5, mY, 3) >= 2;
         }
       }
     }
-    d.keepT[X] = keep;
-    if (keep) atomicAdd(d.tc_cnt + 4 * ev_of_md(d, mX[0]) + 2, 1);
+    const bool keep = !group_any<kRuleLanes>(rem);
+    if (X < n && task == 0) {
+      d.keepT[X] = keep;
+      if (keep) atomicAdd(d.tc_cnt + 4 * ev_of_md(d, md0) + 2, 1);
+    }
   }
   // rule 4: a pLS is linked if it seeds a surviving pT5 (flag set by rule 1) or pT3
   for (int p = i0; p < d.n_pls; p += stride) {

@@ -145,3 +145,27 @@ def test_ragged_batch_with_empty_events(lst, oracle_mod):
     finally:
         lst.lst_free(ctx)
         lst.lst_free(g)
+
+
+def test_strip_like_workload(lst, oracle_mod):
+    """the second workload -- strip-like sensors in the outer layers, r-z windows opened to the
+    strip length (lst_inputs.configs.C6_PARAMS): 3-5 x the MD / LS / T3 candidates of C5 at the same pileup.
+    Two PU140 events in one launch sequence, every object and both counters equal to the oracle's."""
+    from lst_inputs import c5_batch
+    from lst_inputs.configs import C6_PARAMS
+
+    geom, off, tgt = make_config_geometry("C6")
+    evs = c5_batch(pu=140, n_events=2, config="C6")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt, lst.lst_default_params(**C6_PARAMS))
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=2))
+    try:
+        run_batch(lst, ctx, evs)
+        for i, ev in enumerate(evs):
+            want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls,
+                                        oracle_mod.default_params(**C6_PARAMS))
+            ref = _oracle(oracle_mod, geom, off, tgt, make_config_event("C5", pu=140, index=i, seeds=True))
+            assert len(want["ls_md"]) > 2 * len(ref["ls_md"]) and len(want["t3_md"]) > 3 * len(ref["t3_md"])
+            assert_same(canon(lst.lst_ctx_fetch_event(ctx, i)), canon(want), f"C6 event {i}: ")
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)

@@ -72,3 +72,32 @@ def test_concat_events_offsets():
     assert b["hit_offsets"].tolist() == np.concatenate([[0], np.cumsum([e.n_hits for e in evs])]).tolist()
     assert b["pls_offsets"][-1] == sum(e.n_pls for e in evs) == len(b["pls"]["pt"])
     assert len(b["x"]) == b["hit_offsets"][-1]
+
+
+def test_strip_like_sensors_quantise_z_and_r():
+    """SURVEY.md 8(f)2 / PAPER.md:23, Fig. 1: on the three outer barrel layers a hit sits on the centre of a 5 cm
+    strip, on the outer endcap rings on the centre of one of two strip rows; the inner layers keep their resolution.
+    Same tracks, same hit count and module assignment as the pixel-like event of the same seed."""
+    from lst_inputs.configs import STRIP_PITCH
+    from lst_inputs.geometry import ENDCAP_NRINGS, ENDCAP_RMAX, ENDCAP_RMIN
+
+    geom, off, tgt = make_config_geometry("C6")
+    a = make_config_event("C5", pu=50, index=1, seeds=True)
+    b = make_config_event("C6", pu=50, index=1, seeds=True)
+    assert a.n_hits == b.n_hits and np.array_equal(a.sensor, b.sensor) and np.array_equal(a.truth, b.truth)
+    m = b.sensor // 2
+    bar = geom.subdet[m] == 0
+    outer = bar & (geom.layer[m] >= 4)
+    zq = b.z[outer] / STRIP_PITCH - 0.5
+    assert outer.sum() > 1000 and np.allclose(zq, np.round(zq), atol=1e-4)
+    inner = bar & (geom.layer[m] <= 3)
+    assert np.array_equal(b.z[inner], a.z[inner]) and np.array_equal(b.x[bar], a.x[bar])
+    zi = b.z[inner] / STRIP_PITCH - 0.5
+    assert np.mean(np.abs(zi - np.round(zi)) < 1e-3) < 0.01
+    end = ~bar
+    w = (ENDCAP_RMAX - ENDCAP_RMIN) / ENDCAP_NRINGS
+    r = np.hypot(b.x[end].astype(np.float64), b.y[end].astype(np.float64))
+    far = r > 62.0
+    rq = (r[far] - ENDCAP_RMIN) / (0.5 * w) - 0.5
+    assert far.sum() > 100 and np.allclose(rq, np.round(rq), atol=2e-3)
+    assert np.abs(np.hypot(a.x[end], a.y[end]) - np.hypot(b.x[end], b.y[end])).max() < 0.5 * w + 1e-3
