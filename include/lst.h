@@ -59,7 +59,11 @@ typedef struct lst_params {
   float t5_tol0, t5_tol1;
   float pt_gate_tol, pt_k_tol0, pt_k_tol1, pt_z_tol;
   float near_rel;
-  int32_t stage_mask; /* bit0 MD, 1 LS, 2 T3, 3 T5, 4 pT3/pT5, 5 duplicate removal + TC */
+  int32_t stage_mask; /* bit0 MD, 1 LS, 2 T3, 3 T5, 4 pT3/pT5, 5 duplicate removal + TC, 6 T4, 7 learned T5 */
+  /* extensions of CUTS.md sections 10 and 11, used only with stage_mask bits 6 / 7 */
+  float t4_tol0, t4_tol1;
+  float t5_mlp_scale, t5_mlp_thr;
+  float t5_mlp[65]; /* W1[8][6] row-major, b1[8], W2[8], b2 */
 } lst_params;
 
 /* Fills *p with the defaults of CUTS.md section 1 (stage_mask = 0x3f). */
@@ -72,6 +76,7 @@ typedef struct lst_caps {
   int32_t max_events;
   int32_t max_hits, max_pls;
   int32_t max_md, max_ls, max_t3, max_t5, max_pt3, max_pt5, max_tc;
+  int32_t max_t4; /* T4 objects (CUTS.md section 10; only used with stage_mask bit 6) */
 } lst_caps;
 
 /* Defaults sized for 16 PU250-like events (a few hundred MB; the B200 has 180 GB). */
@@ -105,7 +110,7 @@ typedef struct lst_pls {
 typedef struct lst_geometry lst_geometry;
 typedef struct lst_ctx lst_ctx;
 
-enum { LST_ST_MD = 0, LST_ST_LS, LST_ST_T3, LST_ST_T5, LST_ST_PT3, LST_ST_PT5, LST_N_STAGES };
+enum { LST_ST_MD = 0, LST_ST_LS, LST_ST_T3, LST_ST_T5, LST_ST_PT3, LST_ST_PT5, LST_ST_T4, LST_N_STAGES };
 
 /* Result of one event, host memory, library-owned (lst_free).  Layouts as in CUTS.md. */
 typedef struct lst_event_out {
@@ -128,7 +133,12 @@ typedef struct lst_event_out {
   float* pt3_score;
   int32_t* pt5;       /* [n_pt5][2] pls, t5 */
   float* pt5_score;
-  int32_t* tc;        /* [n_tc][16] type, pls, t5, t3, hit_idx[12]; classes in order pT5, pT3, T5, pLS */
+  int32_t* tc;        /* [n_tc][16] type, pls, t5, t3, hit_idx[12]; classes in order pT5, pT3, T5, pLS (, T4) */
+  /* extension (CUTS.md section 10): 4-MD objects, empty unless stage_mask bit 6 is set */
+  int32_t n_t4;
+  int32_t* t4_t3;     /* [n_t4][2] */
+  int32_t* t4_md;     /* [n_t4][4] */
+  float* t4_score;    /* [n_t4] */
 } lst_event_out;
 
 /* Totals of the last batch of a context (host struct filled by lst_ctx_sync); near / n_tests are the
@@ -136,7 +146,7 @@ typedef struct lst_event_out {
 typedef struct lst_batch_summary {
   int32_t n_events;
   int32_t n_hits, n_pls;
-  int32_t n_md, n_ls, n_t3, n_t5, n_pt3, n_pt5, n_tc;
+  int32_t n_md, n_ls, n_t3, n_t5, n_pt3, n_pt5, n_tc, n_t4;
   int64_t near[LST_N_STAGES];
   int64_t n_tests[LST_N_STAGES];
 } lst_batch_summary;

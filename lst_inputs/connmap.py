@@ -4,7 +4,9 @@ Edges m -> m' where m' is the NEXT module crossed (lower-sensor surfaces, in
 path order) by a pT >= 0.8 GeV helix leaving the beam line at |z0| <= 15 cm.
 Built by a seeded Monte-Carlo scan over (phi, eta, z0, signed 1/pT); the map
 is an INPUT of the method: oracle and CUDA path read the same CSR arrays.
-No skip-layer edges.  The scan is cached under ``lst_inputs/_cache`` (a pure
+No skip-layer edges by default; ``skip=True`` adds the edges
+m -> m'' to the module crossed AFTER the next one, so that a Line Segment can bridge a layer
+that has no hit.  The scan is cached under ``lst_inputs/_cache`` (a pure
 speed-up: the same seed regenerates the same map).
 """
 from __future__ import annotations
@@ -22,7 +24,7 @@ _CACHE_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "_cache")
 _CACHE_VERSION = 2
 
 
-def _scan_chunk(geom: Geometry, rng: np.random.Generator, n: int, eta_max: float):
+def _scan_chunk(geom: Geometry, rng: np.random.Generator, n: int, eta_max: float, skip: bool = False):
     phi0 = rng.uniform(0.0, 2.0 * np.pi, n)
     eta = rng.uniform(-eta_max, eta_max, n)
     z0 = rng.uniform(-Z0_MAX_MAP, Z0_MAX_MAP, n)
@@ -57,15 +59,19 @@ def _scan_chunk(geom: Geometry, rng: np.random.Generator, n: int, eta_max: float
     mods = np.take_along_axis(mods, order, axis=1)
     a = mods[:, :-1].ravel()
     b = mods[:, 1:].ravel()
+    if skip:  # also the crossing after the next one (invalid crossings sort last: t = inf)
+        a = np.concatenate([a, mods[:, :-2].ravel()])
+        b = np.concatenate([b, mods[:, 2:].ravel()])
     keep = (a >= 0) & (b >= 0)
     return a[keep], b[keep]
 
 
-def build_connection_map(geom: Geometry, n_samples: int | None = None, seed: int = 12345, cache: bool = True):
+def build_connection_map(geom: Geometry, n_samples: int | None = None, seed: int = 12345, cache: bool = True,
+                         skip: bool = False):
     """Return CSR ``(offsets int32[n_modules+1], targets int32[n_edges])``, targets sorted per row."""
     if n_samples is None:
         n_samples = 3_000_000 if geom.has_endcap else 1_000_000
-    tag = f"{geom.name}_n{n_samples}_s{seed}_v{_CACHE_VERSION}.npz"
+    tag = f"{geom.name}_n{n_samples}_s{seed}_v{_CACHE_VERSION}{'_skip' if skip else ''}.npz"
     path = os.path.join(_CACHE_DIR, tag)
     if cache and os.path.exists(path):
         with np.load(path) as f:
@@ -79,7 +85,7 @@ def build_connection_map(geom: Geometry, n_samples: int | None = None, seed: int
     done = 0
     while done < n_samples:
         n = min(chunk, n_samples - done)
-        a, b = _scan_chunk(geom, rng, n, eta_max)
+        a, b = _scan_chunk(geom, rng, n, eta_max, skip)
         keys = np.union1d(keys, np.unique(a.astype(np.int64) * nm + b.astype(np.int64)))
         done += n
     src = (keys // nm).astype(np.int64)

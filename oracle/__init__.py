@@ -17,6 +17,8 @@ from .binding import (  # noqa: F401
     ls_test,
     t3_test,
     t5_test,
+    t4_test,
+    dedup_t4,
     pt_test,
     run_event,
     dedup,

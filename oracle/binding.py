@@ -12,10 +12,12 @@ _SRC = os.path.join(_HERE, "lst_oracle.c")
 _HDR = os.path.join(_HERE, "lst_oracle.h")
 _SO = os.path.join(_HERE, "liblst_oracle.so")
 
-STAGES = ("md", "ls", "t3", "t5", "pt3", "pt5")
-KINDS = ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")
-_KIND_W = (3, 2, 5, 7, 2, 2, 16)
-_KIND_FW = (6, 1, 1, 1, 1, 1, 0)
+STAGES = ("md", "ls", "t3", "t5", "pt3", "pt5", "t4")
+KINDS = ("md", "ls", "t3", "t5", "pt3", "pt5", "tc", "t4")
+_KIND_W = (3, 2, 5, 7, 2, 2, 16, 6)
+_KIND_FW = (6, 1, 1, 1, 1, 1, 0, 1)
+N_STAGES = len(STAGES)
+_EXT_FIELDS = ("t4_tol0", "t4_tol1", "t5_mlp_scale", "t5_mlp_thr")
 
 _FLOAT_FIELDS = (
     "b_field", "pt_min", "z0_max", "md_b_phi_tol", "md_z_tol", "md_e_slope", "md_e_tol",
@@ -25,10 +27,11 @@ _FLOAT_FIELDS = (
 
 
 class Params(C.Structure):
-    _fields_ = [(f, C.c_float) for f in _FLOAT_FIELDS] + [("stage_mask", C.c_int)]
+    _fields_ = [(f, C.c_float) for f in _FLOAT_FIELDS] + [("stage_mask", C.c_int)] + \
+               [(f, C.c_float) for f in _EXT_FIELDS] + [("t5_mlp", C.c_float * 65)]
 
     def as_dict(self):
-        d = {f: float(np.float32(getattr(self, f))) for f in _FLOAT_FIELDS}
+        d = {f: float(np.float32(getattr(self, f))) for f in _FLOAT_FIELDS + _EXT_FIELDS}
         d["stage_mask"] = int(self.stage_mask)
         return d
 
@@ -67,10 +70,12 @@ def _load():
     lib.orc_ls_test.argtypes = [pp, fp, C.c_int, fp, C.c_int, fp, ip]
     lib.orc_t3_test.argtypes = [pp, fp, C.c_int, fp, C.c_int, fp, C.c_int, fp, ip]
     lib.orc_t5_test.argtypes = [pp, C.c_float, C.c_float, fp, fp, fp, fp, ip]
+    lib.orc_t4_test.argtypes = [pp, C.c_float, C.c_float, fp, ip]
     lib.orc_pt_test.argtypes = [pp, fp, fp, C.c_int, fp, C.c_int, fp, C.c_int, C.c_float, fp, ip]
     cp = C.POINTER(C.c_char)
     lib.orc_dedup.argtypes = [ip, ip, C.c_int, ip, C.c_int, fp, ip, C.c_int, fp, ip, C.c_int, fp, C.c_int,
                               cp, cp, cp, cp]
+    lib.orc_dedup_t4.argtypes = [ip, ip, ip, C.c_int, ip, C.c_int, ip, C.c_int, cp, cp, cp, ip, C.c_int, fp, cp]
     lib.orc_run_event.restype = C.c_void_p
     lib.orc_run_event.argtypes = [pp, C.c_int, ip, ip, ip, C.c_int, fp, fp, fp, ip, C.c_int, fp, ip,
                                   fp, fp, fp, fp, fp, fp]
@@ -89,7 +94,13 @@ def default_params(**overrides) -> Params:
     for k, v in overrides.items():
         if not hasattr(p, k):
             raise KeyError(k)
-        setattr(p, k, v)
+        if k == "t5_mlp":
+            w = np.asarray(v, dtype=np.float32).ravel()
+            assert w.shape[0] == 65
+            for i in range(65):
+                p.t5_mlp[i] = float(w[i])
+        else:
+            setattr(p, k, v)
     return p
 
 
@@ -162,8 +173,17 @@ def t5_test(ki, ko, mdB, mdC, mdD, p: Params | None = None):
     d, pd = _fa(mdD, 2)
     acc = _load().orc_t5_test(C.byref(_params(p)), C.c_float(float(np.float32(ki))),
                               C.c_float(float(np.float32(ko))), pb, pc, pd, vals, C.byref(near))
-    names = ("kb", "tol", "score")
-    return bool(acc), bool(near.value), dict(zip(names, np.array(vals[:3], dtype=np.float32)))
+    names = ("kb", "tol", "score", "s")
+    return bool(acc), bool(near.value), dict(zip(names, np.array(vals[:4], dtype=np.float32)))
+
+
+def t4_test(k1, k2, p: Params | None = None):
+    """CUTS.md section 10: two T3 curvatures -> (accept, near, {d, tol, score})."""
+    vals = (C.c_float * 4)()
+    near = C.c_int(0)
+    acc = _load().orc_t4_test(C.byref(_params(p)), C.c_float(float(np.float32(k1))), C.c_float(float(np.float32(k2))),
+                              vals, C.byref(near))
+    return bool(acc), bool(near.value), dict(zip(("d", "tol", "score"), np.array(vals[:3], dtype=np.float32)))
 
 
 def pt_test(pls, mdA, eA, mdL, eL, kt, base_score=0.0, p: Params | None = None):
@@ -205,6 +225,26 @@ def dedup(md_hits, t3_md, t5_md, t5_score, pt3, pt3_score, pt5, pt5_score, n_pls
                       int(n_pls), keep5.ctypes.data_as(cp), keep3.ctypes.data_as(cp), keepT.ctypes.data_as(cp),
                       linked.ctypes.data_as(cp))
     return keep5[:-1].astype(bool), keep3[:-1].astype(bool), keepT[:-1].astype(bool), linked[:-1].astype(bool)
+
+
+def dedup_t4(md_hits, t3_md, t5_md, pt3, pt5, keep5, keep3, keepT, t4_md, t4_score):
+    """CUTS.md section 10 rule 5; returns keep4 as a bool array."""
+    ip = C.POINTER(C.c_int)
+    fp = C.POINTER(C.c_float)
+    cp = C.POINTER(C.c_char)
+
+    def i32(a, w):
+        return np.ascontiguousarray(np.asarray(a, dtype=np.int32).reshape(-1, w))
+
+    md_hits, t3_md, t5_md, pt3, pt5, t4_md = i32(md_hits, 2), i32(t3_md, 3), i32(t5_md, 5), i32(pt3, 2), i32(pt5, 2), i32(t4_md, 4)
+    t4_score = np.ascontiguousarray(np.asarray(t4_score, dtype=np.float32).ravel())
+    k5, k3, kT = (np.ascontiguousarray(np.append(np.asarray(k, dtype=np.uint8), 0)) for k in (keep5, keep3, keepT))
+    keep4 = np.zeros(len(t4_md) + 1, dtype=np.uint8)
+    _load().orc_dedup_t4(md_hits.ctypes.data_as(ip), t3_md.ctypes.data_as(ip), t5_md.ctypes.data_as(ip), len(t5_md),
+                         pt3.ctypes.data_as(ip), len(pt3), pt5.ctypes.data_as(ip), len(pt5), k5.ctypes.data_as(cp),
+                         k3.ctypes.data_as(cp), kT.ctypes.data_as(cp), t4_md.ctypes.data_as(ip), len(t4_md),
+                         t4_score.ctypes.data_as(fp), keep4.ctypes.data_as(cp))
+    return keep4[:-1].astype(bool)
 
 
 def run_event(subdet, conn_off, conn_tgt, x, y, z, sensor, pls: dict | None = None, params: Params | None = None):
@@ -250,8 +290,8 @@ def run_event(subdet, conn_off, conn_tgt, x, y, z, sensor, pls: dict | None = No
             if n and _KIND_FW[k]:
                 lib.orc_copy_f32(h, k, af.ctypes.data_as(fp))
             raw_f[name] = af
-        near = (C.c_longlong * 6)()
-        nt = (C.c_longlong * 6)()
+        near = (C.c_longlong * N_STAGES)()
+        nt = (C.c_longlong * N_STAGES)()
         lib.orc_counters(h, near, nt)
     finally:
         lib.orc_free_event(h)
@@ -264,5 +304,6 @@ def run_event(subdet, conn_off, conn_tgt, x, y, z, sensor, pls: dict | None = No
         "pt3": raw_i["pt3"], "pt3_score": raw_f["pt3"][:, 0].copy(),
         "pt5": raw_i["pt5"], "pt5_score": raw_f["pt5"][:, 0].copy(),
         "tc": raw_i["tc"],
+        "t4_t3": raw_i["t4"][:, 0:2].copy(), "t4_md": raw_i["t4"][:, 2:6].copy(), "t4_score": raw_f["t4"][:, 0].copy(),
         "near": np.array(near[:], dtype=np.int64), "n_tests": np.array(nt[:], dtype=np.int64),
     }

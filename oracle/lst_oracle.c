@@ -33,6 +33,11 @@ void orc_default_params(orc_params* p) {
   p->pt_z_tol = 2.0f;
   p->near_rel = 1e-5f;
   p->stage_mask = 0x3f;
+  p->t4_tol0 = 4e-4f;
+  p->t4_tol1 = 0.05f;
+  p->t5_mlp_scale = 100.0f;
+  p->t5_mlp_thr = 1.0f;
+  for (int i = 0; i < 65; ++i) p->t5_mlp[i] = 0.0f;
 }
 
 void orc_derived(const orc_params* p, float out[3]) {
@@ -224,16 +229,49 @@ int orc_t5_test(const orc_params* p, float ki, float ko, const float* B, const f
   float tol = p->t5_tol0 + p->t5_tol1 * fmaxf(fabsf(ki), fabsf(ko));
   float d1 = ki - kb, d2 = kb - ko, d3 = ki - ko;
   int nr = 0, acc = 0;
-  nr |= near_thr(p, fabsf(d1), tol);
-  if (fabsf(d1) <= tol) {
-    nr |= near_thr(p, fabsf(d2), tol);
-    if (fabsf(d2) <= tol) {
-      nr |= near_thr(p, fabsf(d3), tol);
-      if (fabsf(d3) <= tol) acc = 1;
+  float s = 0.0f;
+  if (p->stage_mask & 128) {
+    /* CUTS.md section 11: one cut on a 6-8-1 rectifier perceptron */
+    const float* W1 = p->t5_mlp;
+    const float* b1 = p->t5_mlp + 48;
+    const float* W2 = p->t5_mlp + 56;
+    float S = p->t5_mlp_scale;
+    float f[6] = {fabsf(ki) * S, fabsf(kb) * S, fabsf(ko) * S, fabsf(d1) * S, fabsf(d2) * S, fabsf(d3) * S};
+    float h[8];
+    for (int j = 0; j < 8; ++j) {
+      float a = b1[j];
+      for (int i = 0; i < 6; ++i) a = a + W1[6 * j + i] * f[i];
+      h[j] = fmaxf(a, 0.0f);
+    }
+    s = p->t5_mlp[64];
+    for (int j = 0; j < 8; ++j) s = s + W2[j] * h[j];
+    nr |= near_thr(p, s, p->t5_mlp_thr);
+    if (s <= p->t5_mlp_thr) acc = 1;
+  } else {
+    nr |= near_thr(p, fabsf(d1), tol);
+    if (fabsf(d1) <= tol) {
+      nr |= near_thr(p, fabsf(d2), tol);
+      if (fabsf(d2) <= tol) {
+        nr |= near_thr(p, fabsf(d3), tol);
+        if (fabsf(d3) <= tol) acc = 1;
+      }
     }
   }
   if (vals) {
-    vals[0] = kb; vals[1] = tol; vals[2] = (d1 * d1 + d2 * d2) + d3 * d3; vals[3] = 0.0f;
+    vals[0] = kb; vals[1] = tol; vals[2] = (d1 * d1 + d2 * d2) + d3 * d3; vals[3] = s;
+  }
+  if (near) *near = nr;
+  return acc;
+}
+
+/* CUTS.md section 10 ("more objects": a 4-MD object from two T3s sharing two MDs) */
+int orc_t4_test(const orc_params* p, float k1, float k2, float* vals, int* near) {
+  float tol = p->t4_tol0 + p->t4_tol1 * fmaxf(fabsf(k1), fabsf(k2));
+  float d = k1 - k2;
+  int nr = near_thr(p, fabsf(d), tol);
+  int acc = fabsf(d) <= tol;
+  if (vals) {
+    vals[0] = d; vals[1] = tol; vals[2] = d * d; vals[3] = 0.0f;
   }
   if (near) *near = nr;
   return acc;
@@ -333,8 +371,8 @@ struct orc_event {
   long long n_tests[ORC_N_STAGES];
 };
 
-static const int KIND_W[ORC_N_KINDS] = {3, 2, 5, 7, 2, 2, 16};
-static const int KIND_FW[ORC_N_KINDS] = {6, 1, 1, 1, 1, 1, 0};
+static const int KIND_W[ORC_N_KINDS] = {3, 2, 5, 7, 2, 2, 16, 6};
+static const int KIND_FW[ORC_N_KINDS] = {6, 1, 1, 1, 1, 1, 0, 1};
 
 int orc_count(const orc_event* ev, int kind) { return ev->n[kind]; }
 void orc_copy_i32(const orc_event* ev, int kind, int* dst) {
@@ -366,6 +404,7 @@ void orc_free_event(orc_event* ev) {
 #define T5_I(ev, i) ((ev)->i32[ORC_K_T5].v + 7 * (i))
 #define PT3_I(ev, i) ((ev)->i32[ORC_K_PT3].v + 2 * (i))
 #define PT5_I(ev, i) ((ev)->i32[ORC_K_PT5].v + 2 * (i))
+#define T4_I(ev, i) ((ev)->i32[ORC_K_T4].v + 6 * (i))
 
 /* CUTS.md section 8: number of MDs common to two MD lists */
 static int share(const int* a, int na, const int* b, int nb) {
@@ -461,6 +500,27 @@ void orc_dedup(const int* md_hits, const int* t3_md, int n_t3, const int* t5_md,
     if (keep5[X]) linked[pt5[2 * X]] = 1;
   for (int X = 0; X < n_pt3; ++X)
     if (keep3[X]) linked[pt3[2 * X]] = 1;
+}
+
+/* CUTS.md section 10, rule 5: T4 against better T4s (unfiltered set) and against the survivors of rules 1-3 */
+void orc_dedup_t4(const int* md_hits, const int* t3_md, const int* t5_md, int n_t5, const int* pt3, int n_pt3,
+                  const int* pt5, int n_pt5, const char* keep5, const char* keep3, const char* keepT,
+                  const int* t4_md, int n_t4, const float* t4_score, char* keep4) {
+  for (int X = 0; X < n_t4; ++X) {
+    const int* mX = t4_md + 4 * X;
+    keep4[X] = 1;
+    for (int Y = 0; Y < n_t4; ++Y) {
+      if (Y == X) continue;
+      const int* mY = t4_md + 4 * Y;
+      if (share(mY, 4, mX, 4) >= 3 && better(md_hits, t4_score[Y], -1, mY, t4_score[X], -1, mX, 4)) keep4[X] = 0;
+    }
+    for (int Z = 0; Z < n_pt5; ++Z)
+      if (keep5[Z] && share(mX, 4, t5_md + 5 * pt5[2 * Z + 1], 5) >= 2) keep4[X] = 0;
+    for (int Z = 0; Z < n_pt3; ++Z)
+      if (keep3[Z] && share(mX, 4, t3_md + 3 * pt3[2 * Z + 1], 3) >= 2) keep4[X] = 0;
+    for (int Z = 0; Z < n_t5; ++Z)
+      if (keepT[Z] && share(mX, 4, t5_md + 5 * Z, 5) >= 2) keep4[X] = 0;
+  }
 }
 
 static void push_tc(orc_event* ev, int type, int pls, int t5, int t3, const int* md, int nmd) {
@@ -632,6 +692,38 @@ orc_event* orc_run_event(const orc_params* p, int n_modules, const int* subdet, 
   }
   const int n_t5 = ev->n[ORC_K_T5];
 
+  /* ---- stage 6 (extension): T4 (CUTS.md section 10) ---- */
+  if (mask & 64) {
+    /* T3s whose FIRST LS is l: T3s are pushed in order of their first LS */
+    int* t3_of_ls = (int*)calloc((size_t)(n_ls + 2), sizeof(int));
+    for (int t = 0; t < n_t3; ++t) t3_of_ls[T3_I(ev, t)[0] + 1]++;
+    for (int l = 0; l < n_ls; ++l) t3_of_ls[l + 1] += t3_of_ls[l];
+    for (int t1 = 0; t1 < n_t3; ++t1) {
+      const int* a1 = T3_I(ev, t1);
+      int l2 = a1[1];
+      for (int t2 = t3_of_ls[l2]; t2 < t3_of_ls[l2 + 1]; ++t2) {
+        const int* a2 = T3_I(ev, t2);
+        float vals[4];
+        int nr;
+        ev->n_tests[ORC_ST_T4]++;
+        int acc = orc_t4_test(p, ev->f32[ORC_K_T3].v[t1], ev->f32[ORC_K_T3].v[t2], vals, &nr);
+        ev->near[ORC_ST_T4] += nr;
+        if (!acc) continue;
+        ivec* a = &ev->i32[ORC_K_T4];
+        ipush(a, t1);
+        ipush(a, t2);
+        ipush(a, a1[2]);
+        ipush(a, a1[3]);
+        ipush(a, a1[4]);
+        ipush(a, a2[4]);
+        fpush(&ev->f32[ORC_K_T4], vals[2]);
+        ev->n[ORC_K_T4]++;
+      }
+    }
+    free(t3_of_ls);
+  }
+  const int n_t4 = ev->n[ORC_K_T4];
+
   /* ---- stages 4, 5: pT3 / pT5 (CUTS.md section 7) ---- */
   if ((mask & 16) && n_pls > 0) {
     for (int ip = 0; ip < n_pls; ++ip) {
@@ -704,6 +796,18 @@ orc_event* orc_run_event(const orc_params* p, int n_modules, const int* subdet, 
       if (keepT[X]) push_tc(ev, 2, -1, X, -1, T5_I(ev, X) + 2, 5);
     for (int ip = 0; ip < n_pls; ++ip)
       if (!linked[ip]) push_tc(ev, 3, ip, -1, -1, 0, 0);
+    if (n_t4 > 0) { /* CUTS.md section 10, rule 5 and TC class 4 */
+      char* keep4 = (char*)malloc((size_t)n_t4);
+      int* t4_md = (int*)malloc(sizeof(int) * (size_t)(4 * n_t4));
+      for (int i = 0; i < n_t4; ++i)
+        for (int k = 0; k < 4; ++k) t4_md[4 * i + k] = T4_I(ev, i)[2 + k];
+      orc_dedup_t4(md_hits, t3_md, t5_md, n_t5, ev->i32[ORC_K_PT3].v, n_pt3, ev->i32[ORC_K_PT5].v, n_pt5, keep5,
+                   keep3, keepT, t4_md, n_t4, ev->f32[ORC_K_T4].v, keep4);
+      for (int X = 0; X < n_t4; ++X)
+        if (keep4[X]) push_tc(ev, 4, -1, -1, T4_I(ev, X)[0], t4_md + 4 * X, 4);
+      free(keep4);
+      free(t4_md);
+    }
     free(keep5);
     free(keep3);
     free(keepT);

@@ -31,9 +31,13 @@ typedef struct orc_params {
   float pt_gate_tol, pt_k_tol0, pt_k_tol1, pt_z_tol;
   float near_rel;
   int stage_mask;
+  /* extensions (CUTS.md sections 10, 11), off unless stage_mask bits 6 / 7 are set */
+  float t4_tol0, t4_tol1;
+  float t5_mlp_scale, t5_mlp_thr;
+  float t5_mlp[65]; /* W1[8][6], b1[8], W2[8], b2 */
 } orc_params;
 
-enum { ORC_ST_MD = 0, ORC_ST_LS, ORC_ST_T3, ORC_ST_T5, ORC_ST_PT3, ORC_ST_PT5, ORC_N_STAGES };
+enum { ORC_ST_MD = 0, ORC_ST_LS, ORC_ST_T3, ORC_ST_T5, ORC_ST_PT3, ORC_ST_PT5, ORC_ST_T4, ORC_N_STAGES };
 
 /* CUTS.md section 1 defaults. */
 void orc_default_params(orc_params* p);
@@ -58,9 +62,11 @@ int orc_ls_test(const orc_params* p, const float* mdA, int endcapA, const float*
 /* CUTS.md section 5.  md = x, y, z, r.  vals[4] = k3, ratio, zv, tol. */
 int orc_t3_test(const orc_params* p, const float* mdA, int eA, const float* mdB, int eB,
                 const float* mdC, int eC, float* vals, int* near);
-/* CUTS.md section 6.  vals[4] = kb, tol, score, 0. */
+/* CUTS.md section 6 (section 11 when stage_mask bit 7 is set).  vals[4] = kb, tol, score, s (MLP output, else 0). */
 int orc_t5_test(const orc_params* p, float ki, float ko, const float* mdB, const float* mdC,
                 const float* mdD, float* vals, int* near);
+/* CUTS.md section 10.  vals[4] = d, tol, score, 0. */
+int orc_t4_test(const orc_params* p, float k1, float k2, float* vals, int* near);
 /* CUTS.md section 7.  pls = pt, q, x0, y0, z0, x1, y1, z1.  kt[0..n_kt) = the stored curvatures
  * compared with kx (1 for a T3, 2 for a T5); base_score added to the score (0 / T5 score).
  * vals[8] = kp, gdot, gcrs, glim, kx, zqA, zqL, score. */
@@ -73,6 +79,10 @@ void orc_dedup(const int* md_hits, const int* t3_md, int n_t3, const int* t5_md,
                const float* t5_score, const int* pt3, int n_pt3, const float* pt3_score,
                const int* pt5, int n_pt5, const float* pt5_score, int n_pls, char* keep5,
                char* keep3, char* keepT, char* linked);
+/* CUTS.md section 10 rule 5, after orc_dedup: t4_md [n_t4][4]; output keep4[n_t4]. */
+void orc_dedup_t4(const int* md_hits, const int* t3_md, const int* t5_md, int n_t5, const int* pt3, int n_pt3,
+                  const int* pt5, int n_pt5, const char* keep5, const char* keep3, const char* keepT,
+                  const int* t4_md, int n_t4, const float* t4_score, char* keep4);
 
 /* ---- whole event ------------------------------------------------------------------------------ */
 typedef struct orc_event orc_event;
@@ -94,13 +104,14 @@ enum {
   ORC_K_PT3,    /* i32 [n][2]  pls, t3 */
   ORC_K_PT5,    /* i32 [n][2]  pls, t5 */
   ORC_K_TC,     /* i32 [n][16] type, pls, t5, t3, hit_idx[12] */
+  ORC_K_T4,     /* i32 [n][6]  t3_0, t3_1, md x4 (CUTS.md section 10) */
   ORC_N_KINDS
 };
 int orc_count(const orc_event* ev, int kind);
 void orc_copy_i32(const orc_event* ev, int kind, int* dst);
-/* f32 payload per object: MD [n][6] x,y,z,r,ux,uy; LS [n] kappa; T3 [n] k3; T5/PT3/PT5 [n] score. */
+/* f32 payload per object: MD [n][6] x,y,z,r,ux,uy; LS [n] kappa; T3 [n] k3; T5/PT3/PT5/T4 [n] score. */
 void orc_copy_f32(const orc_event* ev, int kind, float* dst);
-/* per-stage counters: near[6], n_tests[6] (candidates evaluated). */
+/* per-stage counters: near[ORC_N_STAGES], n_tests[ORC_N_STAGES] (candidates evaluated). */
 void orc_counters(const orc_event* ev, long long* near, long long* n_tests);
 
 #ifdef __cplusplus

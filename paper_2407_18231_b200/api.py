@@ -101,6 +101,8 @@ def event_out_to_dict(o: lst_event_out) -> dict:
         "pt3": _np(o.pt3, (o.n_pt3, 2), np.int32), "pt3_score": _np(o.pt3_score, (o.n_pt3,), np.float32),
         "pt5": _np(o.pt5, (o.n_pt5, 2), np.int32), "pt5_score": _np(o.pt5_score, (o.n_pt5,), np.float32),
         "tc": _np(o.tc, (o.n_tc, 16), np.int32),
+        "t4_t3": _np(o.t4_t3, (o.n_t4, 2), np.int32), "t4_md": _np(o.t4_md, (o.n_t4, 4), np.int32),
+        "t4_score": _np(o.t4_score, (o.n_t4,), np.float32),
         "near": np.array([o.near[i] for i in range(N_STAGES)], dtype=np.int64),
         "n_tests": np.array([o.n_tests[i] for i in range(N_STAGES)], dtype=np.int64),
     }

@@ -14,8 +14,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liblst_b200.so")
 
 LST_OK, LST_ERR_ARG, LST_ERR_CUDA, LST_ERR_CAPACITY, LST_ERR_GEOMETRY = 0, -1, -2, -3, -4
-N_STAGES = 6
-STAGES = ("md", "ls", "t3", "t5", "pt3", "pt5")
+N_STAGES = 7
+STAGES = ("md", "ls", "t3", "t5", "pt3", "pt5", "t4")
+_EXT_FIELDS = ("t4_tol0", "t4_tol1", "t5_mlp_scale", "t5_mlp_thr")
 
 _FLOAT_FIELDS = (
     "b_field", "pt_min", "z0_max", "md_b_phi_tol", "md_z_tol", "md_e_slope", "md_e_tol",
@@ -38,17 +39,18 @@ class lst_module(C.Structure):
 
 
 class lst_params(C.Structure):
-    _fields_ = [(f, C.c_float) for f in _FLOAT_FIELDS] + [("stage_mask", C.c_int32)]
+    _fields_ = [(f, C.c_float) for f in _FLOAT_FIELDS] + [("stage_mask", C.c_int32)] + \
+               [(f, C.c_float) for f in _EXT_FIELDS] + [("t5_mlp", C.c_float * 65)]
 
     def as_dict(self):
-        d = {f: float(np.float32(getattr(self, f))) for f in _FLOAT_FIELDS}
+        d = {f: float(np.float32(getattr(self, f))) for f in _FLOAT_FIELDS + _EXT_FIELDS}
         d["stage_mask"] = int(self.stage_mask)
         return d
 
 
 class lst_caps(C.Structure):
     _fields_ = [(f, C.c_int32) for f in ("max_events", "max_hits", "max_pls", "max_md", "max_ls", "max_t3",
-                                          "max_t5", "max_pt3", "max_pt5", "max_tc")]
+                                          "max_t5", "max_pt3", "max_pt5", "max_tc", "max_t4")]
 
 
 class lst_hits(C.Structure):
@@ -68,16 +70,17 @@ class lst_event_out(C.Structure):
         [("near", C.c_int64 * N_STAGES), ("n_tests", C.c_int64 * N_STAGES),
          ("md_hits", _ip), ("md_module", _ip), ("md_f", _fp), ("ls_md", _ip), ("ls_kappa", _fp),
          ("t3_ls", _ip), ("t3_md", _ip), ("t3_k", _fp), ("t5_t3", _ip), ("t5_md", _ip), ("t5_score", _fp),
-         ("pt3", _ip), ("pt3_score", _fp), ("pt5", _ip), ("pt5_score", _fp), ("tc", _ip)]
+         ("pt3", _ip), ("pt3_score", _fp), ("pt5", _ip), ("pt5_score", _fp), ("tc", _ip),
+         ("n_t4", C.c_int32), ("t4_t3", _ip), ("t4_md", _ip), ("t4_score", _fp)]
 
 
 class lst_batch_summary(C.Structure):
     _fields_ = [(f, C.c_int32) for f in ("n_events", "n_hits", "n_pls", "n_md", "n_ls", "n_t3", "n_t5", "n_pt3",
-                                          "n_pt5", "n_tc")] + \
+                                          "n_pt5", "n_tc", "n_t4")] + \
         [("near", C.c_int64 * N_STAGES), ("n_tests", C.c_int64 * N_STAGES)]
 
     def as_dict(self):
-        d = {f: int(getattr(self, f)) for f, _ in self._fields_[:10]}
+        d = {f: int(getattr(self, f)) for f, _ in self._fields_[:11]}
         d["near"] = [int(v) for v in self.near]
         d["n_tests"] = [int(v) for v in self.n_tests]
         return d
@@ -144,7 +147,14 @@ def lst_default_params(**overrides) -> lst_params:
     for k, v in overrides.items():
         if not hasattr(p, k):
             raise KeyError(k)
-        setattr(p, k, v)
+        if k == "t5_mlp":
+            w = np.asarray(v, dtype=np.float32).ravel()
+            if w.shape[0] != 65:
+                raise ValueError("t5_mlp holds 65 weights (CUTS.md section 11)")
+            for i in range(65):
+                p.t5_mlp[i] = float(w[i])
+        else:
+            setattr(p, k, v)
     return p
 
 

@@ -64,8 +64,8 @@ struct lst_ctx {
   // pinned host mirrors
   Ctl* h_ctl;
   unsigned long long* h_ev_cnt;  // [max_events][kEvCnt]
-  int* h_ev_first;  // [K_PT5 + 1][max_events + 1]
-  int* h_tc_begin;  // [4 * max_events + 1] first track candidate of every (event, class)
+  int* h_ev_first;  // [K_NKINDS][max_events + 1]
+  int* h_tc_begin;  // [kTcClasses * max_events + 1] first track candidate of every (event, class)
   int h_pls_off[2];
   std::vector<int> last_hit_off, last_pls_off;
   int last_n_events;
@@ -99,6 +99,9 @@ extern "C" void lst_default_params(lst_params* p) {  // CUTS.md section 1
   p->pt_gate_tol = 0.05f;  p->pt_k_tol0 = 5e-4f;  p->pt_k_tol1 = 0.10f;  p->pt_z_tol = 2.0f;
   p->near_rel = 1e-5f;
   p->stage_mask = 0x3f;
+  p->t4_tol0 = 4e-4f;  p->t4_tol1 = 0.05f;              // CUTS.md section 10
+  p->t5_mlp_scale = 100.0f;  p->t5_mlp_thr = 1.0f;      // CUTS.md section 11; the weights are inputs (default 0)
+  for (int i = 0; i < 65; ++i) p->t5_mlp[i] = 0.0f;
 }
 
 extern "C" void lst_default_caps(lst_caps* c) {
@@ -113,6 +116,7 @@ extern "C" void lst_default_caps(lst_caps* c) {
   c->max_pt3 = 1 << 20;
   c->max_pt5 = 1 << 20;
   c->max_tc = 256 << 10;
+  c->max_t4 = 2 << 20;
 }
 
 static Cuts make_cuts(const lst_params& p) {  // CUTS.md section 1, derived constants in binary32
@@ -131,6 +135,9 @@ static Cuts make_cuts(const lst_params& p) {  // CUTS.md section 1, derived cons
   volatile float inv = 1.0f / (2.0f * r_min);
   c.kr = kr;  c.r_min = r_min;  c.inv_2rmin = inv;
   c.stage_mask = p.stage_mask;
+  c.t4_tol0 = p.t4_tol0;  c.t4_tol1 = p.t4_tol1;
+  c.t5_mlp_scale = p.t5_mlp_scale;  c.t5_mlp_thr = p.t5_mlp_thr;
+  for (int i = 0; i < 65; ++i) c.t5_mlp[i] = p.t5_mlp[i];
   return c;
 }
 
@@ -219,14 +226,15 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.tstate[T_PT] = nullptr;  // ticket only
   d.tstate[T_PP3] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
+  d.tstate[T_T4] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
   d.sens_cnt = b.take<int>(n_sens + 1);
   d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins);
   d.pls_pt3_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt3_cur = b.take<int>(c.max_pls);
   d.pls_pt5_cur = b.take<int>(c.max_pls);
-  d.tc_cnt = b.take<int>(4 * (size_t)c.max_events + 1);
-  d.tc_cur = b.take<int>(4 * (size_t)c.max_events + 1);
+  d.tc_cnt = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
+  d.tc_cur = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
   d.linked = b.take<unsigned char>(c.max_pls);
   b.off = (b.off + 255) & ~size_t(255);
   if (zero_bytes) *zero_bytes = b.off;
@@ -267,6 +275,10 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.t5_score = b.take<float>(c.max_t5);
   d.t5_l = b.take<float4>(c.max_t5);
   d.t5_kio = b.take<float2>(c.max_t5);
+  d.t3_t4_begin = b.take<int>((size_t)c.max_t3 + 1);
+  d.t4_t3 = b.take<int2>(c.max_t4);
+  d.t4_md = b.take<int4>(c.max_t4);
+  d.t4_score = b.take<float>(c.max_t4);
   // --- a5 ---
   d.seed_a = b.take<float4>(c.max_pls);
   d.seed_b = b.take<float4>(c.max_pls);
@@ -287,14 +299,15 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.pt5 = b.take<int2>(c.max_pt5);
   d.pt5_score = b.take<float>(c.max_pt5);
   // --- a6 ---
-  d.idx_head = b.take<int>(3 * (size_t)c.max_md);
-  d.idx_next = b.take<int>(5 * (size_t)c.max_t5 + 5 * (size_t)c.max_pt5 + 3 * (size_t)c.max_pt3);
+  d.idx_head = b.take<int>(4 * (size_t)c.max_md);
+  d.idx_next = b.take<int>(5 * (size_t)c.max_t5 + 5 * (size_t)c.max_pt5 + 3 * (size_t)c.max_pt3 + 4 * (size_t)c.max_t4);
+  d.keep4 = b.take<unsigned char>(c.max_t4);
   d.keep5 = b.take<unsigned char>(c.max_pt5);
   d.keep3 = b.take<unsigned char>(c.max_pt3);
   d.keepT = b.take<unsigned char>(c.max_t5);
-  d.tc_begin = b.take<int>(4 * (size_t)c.max_events + 1);
+  d.tc_begin = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
   d.tc = b.take<int>(16 * (size_t)c.max_tc);
-  d.ev_first = b.take<int>((size_t)(K_PT5 + 1) * (c.max_events + 1));
+  d.ev_first = b.take<int>((size_t)K_NKINDS * (c.max_events + 1));
   // --- staging of host inputs + per-event tables + the batch record ---
   float* fx = b.take<float>(c.max_hits);
   float* fy = b.take<float>(c.max_hits);
@@ -316,15 +329,16 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
     ctx->d_hit_ev_off = ho;  ctx->d_pls_ev_off = po;  ctx->d_batch = bt;
   }
   d.cap[K_MD] = c.max_md;  d.cap[K_LS] = c.max_ls;  d.cap[K_T3] = c.max_t3;  d.cap[K_T5] = c.max_t5;
-  d.cap[K_PT3] = c.max_pt3;  d.cap[K_PT5] = c.max_pt5;  d.cap[K_TC] = c.max_tc;
+  d.cap[K_PT3] = c.max_pt3;  d.cap[K_PT5] = c.max_pt5;  d.cap[K_TC] = c.max_tc;  d.cap[K_T4] = c.max_t4;
   return (b.off + 255) & ~size_t(255);
 }
 
 bool caps_ok(const lst_caps& c) {
   // max_md: the LS stage packs an MD index into 27 bits (lst_ls.cuh); max_pls: a seed slot into 16 bits per tile
   return c.max_events > 0 && c.max_hits > 0 && c.max_pls > 0 && c.max_md > 0 && c.max_ls > 0 && c.max_t3 > 0 &&
-         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_md <= LST_MAX_MD &&
-         5LL * c.max_t5 + 5LL * c.max_pt5 + 3LL * c.max_pt3 < 0x7fffffffLL && 16LL * c.max_tc < 0x7fffffffLL;
+         c.max_t5 > 0 && c.max_pt3 > 0 && c.max_pt5 > 0 && c.max_tc > 0 && c.max_t4 > 0 && c.max_md <= LST_MAX_MD &&
+         5LL * c.max_t5 + 5LL * c.max_pt5 + 3LL * c.max_pt3 + 4LL * c.max_t4 < 0x7fffffffLL &&
+         16LL * c.max_tc < 0x7fffffffLL;
 }
 
 }  // namespace
@@ -400,8 +414,8 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   ctx->dev.cuts = g->cuts;
   bool ok = cudaMallocHost(&ctx->h_ctl, sizeof(Ctl)) == cudaSuccess &&
             cudaMallocHost(&ctx->h_ev_cnt, sizeof(unsigned long long) * kEvCnt * c.max_events) == cudaSuccess &&
-            cudaMallocHost(&ctx->h_ev_first, sizeof(int) * (K_PT5 + 1) * (c.max_events + 1)) == cudaSuccess &&
-            cudaMallocHost(&ctx->h_tc_begin, sizeof(int) * (4 * (size_t)c.max_events + 1)) == cudaSuccess;
+            cudaMallocHost(&ctx->h_ev_first, sizeof(int) * K_NKINDS * (c.max_events + 1)) == cudaSuccess &&
+            cudaMallocHost(&ctx->h_tc_begin, sizeof(int) * (kTcClasses * (size_t)c.max_events + 1)) == cudaSuccess;
   for (int i = 0; ok && i <= kMaxKernels; ++i) ok = cudaEventCreate(&ctx->ev[i]) == cudaSuccess;
   if (!ok) {
     ctx_destroy(ctx);

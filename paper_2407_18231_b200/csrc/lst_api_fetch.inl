@@ -10,6 +10,7 @@ void out_destroy(lst_event_out* o) {
   free(o->t5_t3);  free(o->t5_md);  free(o->t5_score);
   free(o->pt3);  free(o->pt3_score);  free(o->pt5);  free(o->pt5_score);
   free(o->tc);
+  free(o->t4_t3);  free(o->t4_md);  free(o->t4_score);
   o->magic = 0;
   free(o);
 }
@@ -53,11 +54,14 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
   o->n_pt3 = first(K_PT3, ev + 1) - f_p3;
   o->n_pt5 = first(K_PT5, ev + 1) - f_p5;
   const bool has_tc = (ctx->g->cuts.stage_mask & 32) != 0;
-  const int tc0 = has_tc ? ctx->h_tc_begin[4 * (size_t)ev] : 0;
-  o->n_tc = has_tc ? ctx->h_tc_begin[4 * (size_t)(ev + 1)] - tc0 : 0;
+  const int tc0 = has_tc ? ctx->h_tc_begin[kTcClasses * (size_t)ev] : 0;
+  o->n_tc = has_tc ? ctx->h_tc_begin[kTcClasses * (size_t)(ev + 1)] - tc0 : 0;
+  const bool has_t4 = (ctx->g->cuts.stage_mask & 64) != 0;
+  const int f_t4 = has_t4 ? first(K_T4, ev) : 0;
+  o->n_t4 = has_t4 ? first(K_T4, ev + 1) - f_t4 : 0;
   for (int k = 0; k < LST_N_STAGES; ++k) {  // counters of THIS event
     o->near[k] = (int64_t)ctx->h_ev_cnt[(size_t)ev * kEvCnt + k];
-    o->n_tests[k] = (int64_t)ctx->h_ev_cnt[(size_t)ev * kEvCnt + 6 + k];
+    o->n_tests[k] = (int64_t)ctx->h_ev_cnt[(size_t)ev * kEvCnt + kStages + k];
   }
   const int n_md = o->n_md, n_ls = o->n_ls, n_t3 = o->n_t3, n_t5 = o->n_t5;
   o->md_hits = halloc<int32_t>(2 * (size_t)n_md);
@@ -76,6 +80,9 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
   o->pt5 = halloc<int32_t>(2 * (size_t)o->n_pt5);
   o->pt5_score = halloc<float>(o->n_pt5);
   o->tc = halloc<int32_t>(16 * (size_t)o->n_tc);
+  o->t4_t3 = halloc<int32_t>(2 * (size_t)o->n_t4);
+  o->t4_md = halloc<int32_t>(4 * (size_t)o->n_t4);
+  o->t4_score = halloc<float>(o->n_t4);
   std::vector<int> info(n_md);
   std::vector<float4> a(n_md);
   std::vector<float2> u(n_md);
@@ -93,7 +100,9 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
             d2h(o->pt3_score, d.pt3_score, f_p3, o->n_pt3) &&
             d2h(reinterpret_cast<int2*>(o->pt5), d.pt5, f_p5, o->n_pt5) &&
             d2h(o->pt5_score, d.pt5_score, f_p5, o->n_pt5) &&
-            d2h(o->tc, d.tc, 16 * (size_t)tc0, 16 * (size_t)o->n_tc);
+            d2h(o->tc, d.tc, 16 * (size_t)tc0, 16 * (size_t)o->n_tc) &&
+            d2h(reinterpret_cast<int2*>(o->t4_t3), d.t4_t3, f_t4, o->n_t4) &&
+            d2h(reinterpret_cast<int4*>(o->t4_md), d.t4_md, f_t4, o->n_t4) && d2h(o->t4_score, d.t4_score, f_t4, o->n_t4);
   ok = (cudaStreamSynchronize(ctx->stream) == cudaSuccess) && ok;
   if (!ok) {
     out_destroy(o);
@@ -113,6 +122,8 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
   for (size_t i = 0; i < 5 * (size_t)n_t5; ++i) o->t5_md[i] -= f_md;
   for (int i = 0; i < o->n_pt3; ++i) { o->pt3[2 * i] -= f_pls;  o->pt3[2 * i + 1] -= f_t3; }
   for (int i = 0; i < o->n_pt5; ++i) { o->pt5[2 * i] -= f_pls;  o->pt5[2 * i + 1] -= f_t5; }
+  for (size_t i = 0; i < 2 * (size_t)o->n_t4; ++i) o->t4_t3[i] -= f_t3;
+  for (size_t i = 0; i < 4 * (size_t)o->n_t4; ++i) o->t4_md[i] -= f_md;
   *out = o;
   return LST_OK;
 }
@@ -131,7 +142,7 @@ extern "C" int lst_ctx_fetch_tc(lst_ctx* ctx, int32_t* tc, int32_t cap_tc, int32
     CK(cudaMemcpyAsync(tc, ctx->dev.tc, sizeof(int) * 16 * (size_t)n, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
   }
-  for (int e = 0; e <= E; ++e) tc_event_offsets[e] = ctx->h_tc_begin[4 * (size_t)e];  // read back by lst_ctx_run
+  for (int e = 0; e <= E; ++e) tc_event_offsets[e] = ctx->h_tc_begin[kTcClasses * (size_t)e];  // read back by lst_ctx_run
   return LST_OK;
 }
 

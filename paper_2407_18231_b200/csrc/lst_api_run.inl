@@ -56,6 +56,10 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   k_stage<StageT3><<<gp, kBlock, 0, st>>>(d);
   L.mark("t5");
   k_stage<StageT5><<<gp, kBlock, 0, st>>>(d);
+  if (mask & 64) {  // extension: T4 (CUTS.md section 10)
+    L.mark("t4");
+    k_stage<StageT4><<<gp, kBlock, 0, st>>>(d);
+  }
   L.mark("anchor_sort");
   k_anchor_sort<<<ctx->caps.max_events * kAncBlocksPerEvent, kBlock, 0, st>>>(d);
   L.mark("pt");
@@ -74,7 +78,13 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
     L.mark("rule2_pt3");
     k_rule2<<<gw, kBlock, 0, st>>>(d);
     L.mark("rule3_t5");
-    k_rule3<<<gw, kBlock, 0, st>>>(d);
+    if (mask & 64) {
+      k_rule3<false><<<gw, kBlock, 0, st>>>(d);
+      L.mark("rule_t4");
+      k_rule_t4<<<gw, kBlock, 0, st>>>(d);
+    } else {
+      k_rule3<true><<<gw, kBlock, 0, st>>>(d);
+    }
     L.mark("tc_emit");
     k_tc_emit<<<gp, kBlock, 0, st>>>(d);
   }
@@ -194,10 +204,10 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   const Dev& d = ctx->dev;
   CK(cudaMemcpyAsync(ctx->h_ctl, d.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st));
   CK(cudaMemcpyAsync(ctx->h_ev_cnt, d.ev_cnt, sizeof(unsigned long long) * kEvCnt * n_events, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(ctx->h_ev_first, d.ev_first, sizeof(int) * (K_PT5 + 1) * (n_events + 1),
-                     cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(ctx->h_ev_first, d.ev_first, sizeof(int) * K_NKINDS * (n_events + 1), cudaMemcpyDeviceToHost, st));
   if (mask & 32)
-    CK(cudaMemcpyAsync(ctx->h_tc_begin, d.tc_begin, sizeof(int) * (4 * (size_t)n_events + 1), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(ctx->h_tc_begin, d.tc_begin, sizeof(int) * (kTcClasses * (size_t)n_events + 1),
+                       cudaMemcpyDeviceToHost, st));
   ctx->dev.n_events = n_events;
   ctx->dev.n_hits = hits->n;
   ctx->dev.n_pls = n_pls;
@@ -218,12 +228,13 @@ extern "C" int lst_ctx_sync(lst_ctx* ctx, lst_batch_summary* s) {
     s->n_pls = ctx->dev.n_pls;
     s->n_md = h.total[K_MD];  s->n_ls = h.total[K_LS];  s->n_t3 = h.total[K_T3];  s->n_t5 = h.total[K_T5];
     s->n_pt3 = h.total[K_PT3];  s->n_pt5 = h.total[K_PT5];  s->n_tc = h.total[K_TC];
+    s->n_t4 = (ctx->g->cuts.stage_mask & 64) ? h.total[K_T4] : 0;
     for (int k = 0; k < LST_N_STAGES; ++k) {  // batch totals = sums of the per-event counters
       s->near[k] = 0;
       s->n_tests[k] = 0;
       for (int e = 0; e < ctx->last_n_events; ++e) {
         s->near[k] += (int64_t)ctx->h_ev_cnt[(size_t)e * kEvCnt + k];
-        s->n_tests[k] += (int64_t)ctx->h_ev_cnt[(size_t)e * kEvCnt + 6 + k];
+        s->n_tests[k] += (int64_t)ctx->h_ev_cnt[(size_t)e * kEvCnt + kStages + k];
       }
     }
   }

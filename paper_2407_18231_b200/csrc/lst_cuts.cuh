@@ -17,6 +17,10 @@ struct Cuts {  // CUTS.md section 1: primary constants + derived (computed on th
   float near_rel;
   float kr, r_min, inv_2rmin;
   int stage_mask;
+  // extensions: CUTS.md section 10 (T4) and section 11 (learned T5 selection)
+  float t4_tol0, t4_tol1;
+  float t5_mlp_scale, t5_mlp_thr;
+  float t5_mlp[65];  // W1[8][6] row-major, b1[8], W2[8], b2
 };
 
 // CUTS.md section 0: near-threshold flag of a cut v <= t
@@ -155,21 +159,47 @@ __device__ __forceinline__ unsigned t3_test(const Cuts& c, float4 A, float4 B, f
   return res | ACC;
 }
 
-// CUTS.md section 6 (reading S3).  B, C, D = anchors of the bridge MDs.
+// CUTS.md section 6 (reading S3).  B, C, D = anchors of the bridge MDs.  With stage-mask bit 7
+// the three pairwise cuts are replaced by the one cut of CUTS.md section 11.
 __device__ __forceinline__ unsigned t5_test(const Cuts& c, float ki, float ko, float4 B, float4 C,
                                             float4 D, float& score_out) {
   float l0, l1;
   float kb = kappa3(B.x, B.y, C.x, C.y, D.x, D.y, l0, l1);
-  float tol = c.t5_tol0 + c.t5_tol1 * fmaxf(fabsf(ki), fabsf(ko));
   float d1 = ki - kb, d2 = kb - ko, d3 = ki - ko;
   unsigned res = 0;
-  if (near_thr(c, fabsf(d1), tol)) res |= NEAR;
-  if (!(fabsf(d1) <= tol)) return res;
-  if (near_thr(c, fabsf(d2), tol)) res |= NEAR;
-  if (!(fabsf(d2) <= tol)) return res;
-  if (near_thr(c, fabsf(d3), tol)) res |= NEAR;
-  if (!(fabsf(d3) <= tol)) return res;
+  if (c.stage_mask & 128) {
+    const float S = c.t5_mlp_scale;
+    const float f[6] = {fabsf(ki) * S, fabsf(kb) * S, fabsf(ko) * S, fabsf(d1) * S, fabsf(d2) * S, fabsf(d3) * S};
+    float s = c.t5_mlp[64];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      float a = c.t5_mlp[48 + j];
+#pragma unroll
+      for (int i = 0; i < 6; ++i) a = a + c.t5_mlp[6 * j + i] * f[i];
+      s = s + c.t5_mlp[56 + j] * fmaxf(a, 0.0f);
+    }
+    if (near_thr(c, s, c.t5_mlp_thr)) res |= NEAR;
+    if (!(s <= c.t5_mlp_thr)) return res;
+  } else {
+    float tol = c.t5_tol0 + c.t5_tol1 * fmaxf(fabsf(ki), fabsf(ko));
+    if (near_thr(c, fabsf(d1), tol)) res |= NEAR;
+    if (!(fabsf(d1) <= tol)) return res;
+    if (near_thr(c, fabsf(d2), tol)) res |= NEAR;
+    if (!(fabsf(d2) <= tol)) return res;
+    if (near_thr(c, fabsf(d3), tol)) res |= NEAR;
+    if (!(fabsf(d3) <= tol)) return res;
+  }
   score_out = (d1 * d1 + d2 * d2) + d3 * d3;
+  return res | ACC;
+}
+
+// CUTS.md section 10: T4 = two T3s sharing two MDs; k1, k2 = their stored curvatures
+__device__ __forceinline__ unsigned t4_test(const Cuts& c, float k1, float k2, float& score_out) {
+  const float tol = c.t4_tol0 + c.t4_tol1 * fmaxf(fabsf(k1), fabsf(k2));
+  const float dd = k1 - k2;
+  unsigned res = near_thr(c, fabsf(dd), tol) ? NEAR : 0u;
+  if (!(fabsf(dd) <= tol)) return res;
+  score_out = dd * dd;
   return res | ACC;
 }
 

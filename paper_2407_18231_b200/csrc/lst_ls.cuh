@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
 
 // Placement with the exclusive scan of ls_cnt fused in (tiles of kBlock inner MDs by ticket, block scan +
 // look-back): every MD's LSs go from the scratch list to their final slot, md_ls_begin is written on the
-// way.  Rides along: the three list heads of every MD of the duplicate-removal index are cleared.
+// way.  Rides along: the four list heads of every MD of the duplicate-removal index are cleared.
 __global__ void __launch_bounds__(kBlock) k_ls_place(Dev d) {
   load_batch(d);
   __shared__ int s_tile;
@@ -249,6 +249,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_place(Dev d) {
       d.idx_head[A] = 0;
       d.idx_head[n_md + A] = 0;
       d.idx_head[2 * n_md + A] = 0;
+      d.idx_head[3 * n_md + A] = 0;
       const int src = d.ls_sbase[A];
       for (int k = 0; k < n; ++k) {
         const LsAccepted s = scratch[src + k];

@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
         if (t64 < (1ull << 26)) {
           t = (unsigned)t64;
         } else {  // a module with > 6.7e7 hit pairs: straight to global memory (the warp sum above stays < 2^32)
-          atomicAdd(d.ev_cnt + (size_t)(gm / d.n_mod) * kEvCnt + 6, t64);
+          atomicAdd(d.ev_cnt + (size_t)(gm / d.n_mod) * kEvCnt + kStages, t64);
         }
       }
       tbl.warp_add(min(gm, n_gm - 1) / d.n_mod, t);

@@ -140,10 +140,10 @@ __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
       int c0 = 0, c1 = 0;
       if (on) {  // candidates of CUTS.md section 7: every (seed, T3) and (seed, T5) of the event
         event_cands<false>(d, ev, c0, c1);
-        d.ev_cnt[(size_t)ev * kEvCnt + 6 + 4] = (unsigned long long)ns * (c1 - c0);
+        d.ev_cnt[(size_t)ev * kEvCnt + kStages + 4] = (unsigned long long)ns * (c1 - c0);
         if (on5) {
           event_cands<true>(d, ev, c0, c1);
-          d.ev_cnt[(size_t)ev * kEvCnt + 6 + 5] = (unsigned long long)ns * (c1 - c0);
+          d.ev_cnt[(size_t)ev * kEvCnt + kStages + 5] = (unsigned long long)ns * (c1 - c0);
         }
       }
     }

@@ -42,7 +42,7 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
 // ---- per-event counters (CUTS.md section 0: near-threshold candidates and candidates per stage) ----
 // Near-threshold candidates are rare (a few per million): one global atomic where it happens.
 __device__ __forceinline__ void count_near(unsigned long long* ev_cnt, int ev, int stage) {
-  atomicAdd(ev_cnt + (size_t)ev * 12 + stage, 1ull);
+  atomicAdd(ev_cnt + (size_t)ev * 14 + stage, 1ull);  // 14 = kEvCnt (lst_types.cuh)
 }
 
 // Candidate counts are accumulated per block in a shared-memory table indexed by event (events beyond
@@ -65,7 +65,7 @@ struct EvTests {
       const unsigned old = atomicAdd(s + ev, n);
       if (old + n < old) atomicAdd(s + 64 + ev, 1u);
     } else {
-      atomicAdd(g + (size_t)ev * 12 + 6 + stage, (unsigned long long)n);
+      atomicAdd(g + (size_t)ev * 14 + 7 + stage, (unsigned long long)n);
     }
   }
   // called by all 32 lanes: lanes of the leader's event are summed into one update (the common case:
@@ -84,7 +84,7 @@ struct EvTests {
     __syncthreads();
     for (int e = threadIdx.x; e < 64 && e < n_events; e += blockDim.x) {
       const unsigned long long v = ((unsigned long long)s[64 + e] << 32) | s[e];
-      if (v) atomicAdd(g + (size_t)e * 12 + 6 + stage, v);
+      if (v) atomicAdd(g + (size_t)e * 14 + 7 + stage, v);
     }
   }
 };

@@ -15,7 +15,8 @@ __device__ __forceinline__ int ev_of_md(const Dev& d, int md) { return (d.md_inf
 
 // offsets of the three node arrays inside idx_next
 __device__ __forceinline__ int node_base(const Dev& d, int kind) {
-  return kind == 0 ? 0 : (kind == 1 ? 5 * d.cap[K_T5] : 5 * d.cap[K_T5] + 5 * d.cap[K_PT5]);
+  return kind == 0 ? 0 : (kind == 1 ? 5 * d.cap[K_T5] : (kind == 2 ? 5 * d.cap[K_T5] + 5 * d.cap[K_PT5]
+                                                                   : 5 * d.cap[K_T5] + 5 * d.cap[K_PT5] + 3 * d.cap[K_PT3]));
 }
 __device__ __forceinline__ void idx_link(const Dev& d, int n_md, int kind, int md, int node) {
   d.idx_next[node_base(d, kind) + node] = atomicExch(d.idx_head + kind * n_md + md, node + 1);
@@ -32,6 +33,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
   const bool fit3 = n3 <= cap3, fit5 = n5 <= cap5;
   const int n_t5 = d.ctl->total[K_T5], n_md = d.ctl->total[K_MD];
   const bool sel = (d.cuts.stage_mask & 32) != 0 && fit3 && fit5;
+  const int n_t4 = sel ? d.ctl->total[K_T4] : 0;
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const PtAccepted* s3 = reinterpret_cast<const PtAccepted*>(d.ev_scratch);
   const PtAccepted* s5 = reinterpret_cast<const PtAccepted*>(d.ev_scratch2);
@@ -42,7 +44,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
     d.ctl->total[K_PT5] = fit5 ? n5 : 0;
   }
   const int n_a = fit3 ? n3 : 0, n_b = fit5 ? n5 : 0;
-  for (int i = i0; i < n_a + n_b + (sel ? n_t5 : 0); i += stride) {
+  for (int i = i0; i < n_a + n_b + (sel ? n_t5 : 0) + n_t4; i += stride) {
     if (i < n_a) {
       const PtAccepted a = s3[i];
       const int pos = d.pls_pt3_begin[a.p] + atomicAdd(d.pls_pt3_cur + a.p, 1);
@@ -64,11 +66,18 @@ __global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
 #pragma unroll
         for (int k = 0; k < 5; ++k) idx_link(d, n_md, 1, md[k], 5 * pos + k);
       }
-    } else {
+    } else if (i < n_a + n_b + n_t5) {
       const int t = i - n_a - n_b;
       const int* md = d.t5_md + 5 * (size_t)t;
 #pragma unroll
       for (int k = 0; k < 5; ++k) idx_link(d, n_md, 0, md[k], 5 * t + k);
+    } else {
+      const int t = i - n_a - n_b - n_t5;
+      const int4 m = d.t4_md[t];
+      idx_link(d, n_md, 3, m.x, 4 * t);
+      idx_link(d, n_md, 3, m.y, 4 * t + 1);
+      idx_link(d, n_md, 3, m.z, 4 * t + 2);
+      idx_link(d, n_md, 3, m.w, 4 * t + 3);
     }
   }
   if (blockIdx.x == 0) {
@@ -85,6 +94,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_place(Dev d) {
       d.ev_first[K_T5 * E1 + ev] = t5;
       d.ev_first[K_PT3 * E1 + ev] = n_a > 0 ? d.pls_pt3_begin[p] : 0;
       d.ev_first[K_PT5 * E1 + ev] = n_b > 0 ? d.pls_pt5_begin[p] : 0;
+      d.ev_first[K_T4 * E1 + ev] = d.ctl->total[K_T4] > 0 ? d.t3_t4_begin[t3] : 0;
     }
   }
 }
@@ -125,7 +135,7 @@ struct IdxIt {
   const int* next;
   int node, per, obj;
   __device__ IdxIt(const Dev& d, int n_md, int kind, int md)
-      : next(d.idx_next + node_base(d, kind)), node(d.idx_head[kind * n_md + md]), per(kind == 2 ? 3 : 5) {
+      : next(d.idx_next + node_base(d, kind)), node(d.idx_head[kind * n_md + md]), per(kind == 2 ? 3 : (kind == 3 ? 4 : 5)) {
     obj = node ? (node - 1) / per : -1;
   }
   __device__ void advance() {
@@ -182,7 +192,7 @@ __global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
       d.keep5[X] = keep;
       if (keep) {
         d.linked[x.x] = 1;  // one writer per value; rule 4 (k_rule3) completes it with the surviving pT3s
-        atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 0, 1);
+        atomicAdd(d.tc_cnt + kTcClasses * d.pls_event[x.x] + 0, 1);
       }
     }
   }
@@ -232,7 +242,49 @@ __global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
     const bool keep = !group_any<kRuleLanes>(rem);
     if (X < n && task == 0) {
       d.keep3[X] = keep;
-      if (keep) atomicAdd(d.tc_cnt + 4 * d.pls_event[x.x] + 1, 1);
+      if (keep) atomicAdd(d.tc_cnt + kTcClasses * d.pls_event[x.x] + 1, 1);
+    }
+  }
+}
+
+// Called by every block at the end of the last rule kernel: the last block to arrive turns the per-(event, class)
+// survivor counts into tc_begin (a scan of kTcClasses * n_events + 1 numbers, in chunks of kBlock).
+__device__ __forceinline__ void tc_scan_by_last_block(const Dev& d) {
+  __shared__ int s_last;
+  __shared__ int s_carry;
+  __shared__ int s_warp[kWarps];
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    s_last = atomicAdd(&d.ctl->done_rule, 1) == (int)gridDim.x - 1;
+    s_carry = 0;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const int m = kTcClasses * d.n_events;  // tc_begin[0 .. m], tc_begin[m] = total
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int c0 = 0; c0 < m; c0 += kBlock) {
+    const int i = c0 + threadIdx.x;
+    const int v = i < m ? __ldcg(d.tc_cnt + i) : 0;
+    const int incl = warp_incl_scan(v);
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int base = s_carry;
+    for (int w = 0; w < warp; ++w) base += s_warp[w];
+    if (i < m) d.tc_begin[i] = base + incl - v;
+    __syncthreads();
+    if (threadIdx.x == kBlock - 1) s_carry = base + incl;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const int total = s_carry;
+    d.tc_begin[m] = total;
+    if (total > d.cap[K_TC]) {
+      atomicOr(&d.ctl->error, E_CAP_TC);
+      d.ctl->total[K_TC] = 0;
+    } else {
+      d.ctl->total[K_TC] = total;
     }
   }
 }
@@ -240,12 +292,10 @@ __global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
 // rule 3: T5 X is removed by a better T5 sharing >= 3 MDs (tasks 0..2: lists of X.md[0], [2], [4]), by a surviving
 // pT5 (tasks 3..6) or pT3 (tasks 7..10) sharing >= 2 MDs (lists of X.md[0..3]); rule 4: unlinked pLS.  The last
 // block to finish turns the per-(event, class) survivor counts into tc_begin (a scan of 4 * n_events + 1 numbers).
+template <bool SCAN>
 __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
   load_batch(d);
   constexpr int kRuleLanes = 16;
-  __shared__ int s_last;
-  __shared__ int s_carry;
-  __shared__ int s_warp[kWarps];
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_T5];
   const int n_pt5 = d.ctl->total[K_PT5], n_pt3 = d.ctl->total[K_PT3];
@@ -287,7 +337,7 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
     const bool keep = !group_any<kRuleLanes>(rem);
     if (X < n && task == 0) {
       d.keepT[X] = keep;
-      if (keep) atomicAdd(d.tc_cnt + 4 * ev_of_md(d, md0) + 2, 1);
+      if (keep) atomicAdd(d.tc_cnt + kTcClasses * ev_of_md(d, md0) + 2, 1);
     }
   }
   // rule 4: a pLS is linked if it seeds a surviving pT5 (flag set by rule 1) or pT3
@@ -296,43 +346,66 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
     for (int Y = n_pt3 > 0 ? d.pls_pt3_begin[p] : 0; !lk && n_pt3 > 0 && Y < d.pls_pt3_begin[p + 1]; ++Y)
       lk = d.keep3[Y];
     d.linked[p] = lk;
-    if (!lk) atomicAdd(d.tc_cnt + 4 * d.pls_event[p] + 3, 1);
+    if (!lk) atomicAdd(d.tc_cnt + kTcClasses * d.pls_event[p] + 3, 1);
   }
-  // ---- last block: tc_begin = exclusive scan of tc_cnt, in chunks of kBlock ----
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    s_last = atomicAdd(&d.ctl->done_rule3, 1) == (int)gridDim.x - 1;
-    s_carry = 0;
-  }
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-  const int m = 4 * d.n_events;  // tc_begin[0 .. m], tc_begin[m] = total
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int c0 = 0; c0 < m; c0 += kBlock) {
-    const int i = c0 + threadIdx.x;
-    const int v = i < m ? __ldcg(d.tc_cnt + i) : 0;
-    const int incl = warp_incl_scan(v);
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    int base = s_carry;
-    for (int w = 0; w < warp; ++w) base += s_warp[w];
-    if (i < m) d.tc_begin[i] = base + incl - v;
-    __syncthreads();
-    if (threadIdx.x == kBlock - 1) s_carry = base + incl;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) {
-    const int total = s_carry;
-    d.tc_begin[m] = total;
-    if (total > d.cap[K_TC]) {
-      atomicOr(&d.ctl->error, E_CAP_TC);
-      d.ctl->total[K_TC] = 0;
-    } else {
-      d.ctl->total[K_TC] = total;
+  if (SCAN) tc_scan_by_last_block(d);
+}
+
+// rule 5 of CUTS.md section 10 (extension): T4 X is removed by a better T4 sharing >= 3 MDs (tasks 0, 1: lists of
+// X.md[0], [1]) or by a surviving pT5 / pT3 / T5 sharing >= 2 MDs (tasks 2..10: lists of X.md[0..2] per kind).
+// Launched (after k_rule3<false>) only when T4s are built; ends with the tc_begin scan.
+__global__ void __launch_bounds__(kBlock) k_rule_t4(Dev d) {
+  load_batch(d);
+  constexpr int kRuleLanes = 16;
+  const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n_md = d.ctl->total[K_MD], n = d.ctl->total[K_T4];
+  const int task = threadIdx.x & (kRuleLanes - 1);
+  const int n_groups = stride / kRuleLanes, g0 = i0 / kRuleLanes;
+  for (int X0 = 0; X0 < n; X0 += n_groups) {
+    const int X = X0 + g0;
+    bool rem = false;
+    int md0 = 0;
+    if (X < n && task < 11) {
+      const float sX = d.t4_score[X];
+      const int4 m = d.t4_md[X];
+      const int mX[4] = {m.x, m.y, m.z, m.w};
+      int mY[5];
+      md0 = m.x;
+      if (task < 2) {
+        for (IdxIt it(d, n_md, 3, mX[task]); it.obj >= 0 && !rem; it.advance()) {
+          const int Y = it.obj;
+          if (Y == X) continue;
+          const int4 y = d.t4_md[Y];
+          mY[0] = y.x; mY[1] = y.y; mY[2] = y.z; mY[3] = y.w;
+          rem = share(mY, 4, mX, 4) >= 3 && better(d, d.t4_score[Y], -1, mY, sX, -1, mX, 4);
+        }
+      } else {
+        const int kind = (task - 2) / 3 == 0 ? 1 : ((task - 2) / 3 == 1 ? 2 : 0);  // pT5, pT3, T5
+        for (IdxIt it(d, n_md, kind, mX[(task - 2) % 3]); it.obj >= 0 && !rem; it.advance()) {
+          const int Z = it.obj;
+          if (kind == 1) {
+            if (!d.keep5[Z]) continue;
+            load_t5_md(d, d.pt5[Z].y, mY);
+            rem = share(mX, 4, mY, 5) >= 2;
+          } else if (kind == 2) {
+            if (!d.keep3[Z]) continue;
+            load_t3_md(d, d.pt3[Z].y, mY);
+            rem = share(mX, 4, mY, 3) >= 2;
+          } else {
+            if (!d.keepT[Z]) continue;
+            load_t5_md(d, Z, mY);
+            rem = share(mX, 4, mY, 5) >= 2;
+          }
+        }
+      }
+    }
+    const bool keep = !group_any<kRuleLanes>(rem);
+    if (X < n && task == 0) {
+      d.keep4[X] = keep;
+      if (keep) atomicAdd(d.tc_cnt + kTcClasses * ev_of_md(d, md0) + 4, 1);
     }
   }
+  tc_scan_by_last_block(d);
 }
 
 // track candidates: (type, pls, t5, t3, hit_idx[12]) per event in class order; event-local indices
@@ -341,9 +414,10 @@ __global__ void __launch_bounds__(kBlock) k_tc_emit(Dev d) {
   const int stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int E1 = d.n_events + 1;
   const int n_pt5 = d.ctl->total[K_PT5], n_pt3 = d.ctl->total[K_PT3], n_t5 = d.ctl->total[K_T5];
+  const int n_t4 = (d.cuts.stage_mask & 64) ? d.ctl->total[K_T4] : 0;
   const int* __restrict__ ev_first = d.ev_first;
-  if (d.tc_begin[4 * d.n_events] > d.cap[K_TC]) return;  // flagged by k_rule3
-  for (int i = i0; i < n_pt5 + n_pt3 + n_t5 + d.n_pls; i += stride) {
+  if (d.tc_begin[kTcClasses * d.n_events] > d.cap[K_TC]) return;  // flagged by the scan of the last rule kernel
+  for (int i = i0; i < n_pt5 + n_pt3 + n_t5 + d.n_pls + n_t4; i += stride) {
     int cls, ev, pls = -1, t5 = -1, t3 = -1, nmd = 0;
     int md[5];
     if (i < n_pt5) {
@@ -359,12 +433,17 @@ __global__ void __launch_bounds__(kBlock) k_tc_emit(Dev d) {
       t5 = i - n_pt5 - n_pt3;
       if (!d.keepT[t5]) continue;
       cls = 2; load_t5_md(d, t5, md); nmd = 5; ev = ev_of_md(d, md[0]);
-    } else {
+    } else if (i < n_pt5 + n_pt3 + n_t5 + d.n_pls) {
       pls = i - n_pt5 - n_pt3 - n_t5;
       if (d.linked[pls]) continue;
       cls = 3; ev = d.pls_event[pls];
+    } else {  // T4 (CUTS.md section 10): t3 = its first T3
+      const int X = i - n_pt5 - n_pt3 - n_t5 - d.n_pls;
+      if (!d.keep4[X]) continue;
+      const int4 m = d.t4_md[X];
+      cls = 4; t3 = d.t4_t3[X].x; md[0] = m.x; md[1] = m.y; md[2] = m.z; md[3] = m.w; nmd = 4; ev = ev_of_md(d, m.x);
     }
-    const int pos = d.tc_begin[4 * ev + cls] + atomicAdd(d.tc_cur + 4 * ev + cls, 1);
+    const int pos = d.tc_begin[kTcClasses * ev + cls] + atomicAdd(d.tc_cur + kTcClasses * ev + cls, 1);
     int* o = d.tc + 16 * (size_t)pos;
     o[0] = cls;
     o[1] = pls >= 0 ? pls - d.pls_ev_off[ev] : -1;

@@ -179,4 +179,43 @@ struct StageT5 {
   }
 };
 
+// ---- extension: T4 (CUTS.md section 10).  owner = T3 (LS1, LS2); candidates = the T3s whose FIRST LS is LS2.
+struct StageT4 {
+  static constexpr int kTicket = T_T4, kKind = K_T4, kErr = E_CAP_T4, kStage = 6;
+  const Dev& d;
+  __device__ explicit StageT4(const Dev& dd) : d(dd) {}
+  __device__ void prologue() const {}
+  __device__ int n_owners() const { return (d.cuts.stage_mask & 64) ? d.ctl->total[K_T3] : 0; }
+  __device__ int* begin() const { return d.t3_t4_begin; }
+  template <bool FILL>
+  __device__ int visit(int t1, int pos, int& ev, unsigned& tests) const {
+    const int l2 = d.t3_ls[t1].y;
+    const int u0 = d.ls_t3_begin[l2], u1 = d.ls_t3_begin[l2 + 1];
+    if (u0 == u1) return 0;
+    const int4 m1 = d.t3_md[t1];
+    if (!FILL) {
+      ev = (d.md_info[m1.x] >> 1) / d.n_mod;
+      tests = (unsigned)(u1 - u0);
+    }
+    const float k1 = d.t3_k[t1];
+    const int cap = d.cap[K_T4];
+    int cnt = 0;
+    for (int t2 = u0; t2 < u1; ++t2) {
+      float score;
+      const unsigned r = t4_test(d.cuts, k1, d.t3_k[t2], score);
+      if (!FILL && (r & NEAR)) count_near(d.ev_cnt, ev, 6);
+      if (r & ACC) {
+        if (FILL && pos < cap) {
+          d.t4_t3[pos] = make_int2(t1, t2);
+          d.t4_md[pos] = make_int4(m1.x, m1.y, m1.z, d.t3_md[t2].z);
+          d.t4_score[pos] = score;
+        }
+        ++pos;
+        ++cnt;
+      }
+    }
+    return cnt;
+  }
+};
+
 }  // namespace lst

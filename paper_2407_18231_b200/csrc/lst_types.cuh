@@ -14,13 +14,15 @@ namespace lst {
 
 struct PtEvent;  // lst_pt.cuh
 
-enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT, T_PP3, T_PP5, T_N };
+enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_T4, K_NKINDS };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT, T_PP3, T_PP5, T_T4, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
-              E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128 };
+              E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128, E_CAP_T4 = 256 };
 
-constexpr int kEvCnt = 12;    // per-event counters: [0, 6) near-threshold candidates, [6, 12) candidates, per stage
+constexpr int kStages = 7;    // MD, LS, T3, T5, pT3, pT5, T4 (CUTS.md section 2)
+constexpr int kEvCnt = 2 * kStages;  // per-event counters: [0, 7) near-threshold candidates, [7, 14) candidates, per stage
+constexpr int kTcClasses = 5;        // pT5, pT3, T5, pLS, T4 (CUTS.md section 10)
 constexpr int kEvSmem = 64;   // events whose candidate counts a block accumulates in shared memory
 
 // Small control block, zeroed (one memset, together with the tile status words) per batch.
@@ -28,7 +30,7 @@ struct Ctl {
   int ticket[T_N];
   int total[K_NKINDS];
   int error;
-  int done_rule3;                    // blocks of k_rule3 that have finished (the last one scans tc_cnt)
+  int done_rule;                     // blocks of the last rule kernel that have finished (the last one scans tc_cnt)
   int scratch_cur[4];                // accepted objects in the scratch lists: [1] LS, [2] pT3, [3] pT5
   int queue_cur;                     // entries of the exact-evaluation queue of the seed linking
   int pad[3];
@@ -99,6 +101,11 @@ struct Dev {
   float* t5_score;
   float4* t5_l;    // last MD, as t3_l
   float2* t5_kio;  // (ki, ko) = k3 of the two T3s
+  // ---- extension: T4 (owner = first T3; CUTS.md section 10) ----
+  int* t3_t4_begin;  // [n_t3 + 1]
+  int2* t4_t3;
+  int4* t4_md;
+  float* t4_score;
   // ---- a5: pT3 / pT5 (owner = pLS) ----
   float4* seed_a;      // [n_pls] x1, y1, vx, vy           (CUTS.md section 7, computed once per seed)
   float4* seed_b;      // [n_pls] lv, kp, tolk, slope
@@ -119,12 +126,12 @@ struct Dev {
   int2* pt5;
   float* pt5_score;
   // ---- a6: duplicate removal + track candidates ----
-  int* idx_head;   // [3 * n_md] objects containing MD m, as linked lists: kind 0 T5, 1 pT5, 2 pT3; 0 = end, else node + 1
-  int* idx_next;   // [5 * cap T5 | 5 * cap pT5 | 3 * cap pT3] node = object * (5 or 3) + position of the MD in it
-  unsigned char *keep5, *keep3, *keepT, *linked;
-  int* tc_cnt;    // [n_events * 4 + 1] survivors per (event, class) (zeroed per batch)
-  int* tc_begin;  // [n_events * 4 + 1]
-  int* tc_cur;    // [n_events * 4] (zeroed per batch)
+  int* idx_head;   // [4 * n_md] objects containing MD m, as linked lists: kind 0 T5, 1 pT5, 2 pT3, 3 T4; 0 = end, else node + 1
+  int* idx_next;   // [5 * cap T5 | 5 * cap pT5 | 3 * cap pT3 | 4 * cap T4] node = object * (5, 3 or 4) + position of the MD in it
+  unsigned char *keep5, *keep3, *keepT, *keep4, *linked;
+  int* tc_cnt;    // [n_events * 5 + 1] survivors per (event, class) (zeroed per batch)
+  int* tc_begin;  // [n_events * 5 + 1]
+  int* tc_cur;    // [n_events * 5] (zeroed per batch)
   int* tc;        // [n_tc][16]
   int* ev_first;  // [K_PT5 + 1][n_events + 1] first object of every event, per kind
   // ---- capacities ----

@@ -52,7 +52,7 @@ def test_default_params_are_the_cuts_md_table(lst):
     p = lst.lst_default_params().as_dict()
     text = open(os.path.join(ROOT, "CUTS.md")).read()
     rows = dict(re.findall(r"^\| `([A-Z0-9_]+)` \| ([0-9.e+-]+) \|", text, flags=re.M))
-    assert len(rows) == 20
+    assert len(rows) == 24   # 20 of sections 3-8 + 4 of the extensions (sections 10, 11)
     for name, val in rows.items():
         assert p[name.lower()] == float(np.float32(float(val))), name
     assert p["stage_mask"] == 0x3F

@@ -133,8 +133,8 @@ def test_benchmark_configuration(lst, oracle_mod):
         summ = lst.lst_ctx_sync(ctx)
         assert summ["n_events"] == 16 and summ["n_hits"] > 16 * 100_000
         tot = np.zeros(7, np.int64)
-        tests = np.zeros(6, np.int64)
-        near = np.zeros(6, np.int64)
+        tests = np.zeros(7, np.int64)
+        near = np.zeros(7, np.int64)
         for i, ev in enumerate(batches[1]):
             want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
             got = lst.lst_ctx_fetch_event(ctx, i)

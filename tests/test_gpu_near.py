@@ -211,7 +211,7 @@ def test_per_event_counters_through_the_abi(lst, oracle_mod):
     ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=4))
     try:
         summ = run_batch(lst, ctx, evs)
-        near, tests = np.zeros(6, np.int64), np.zeros(6, np.int64)
+        near, tests = np.zeros(7, np.int64), np.zeros(7, np.int64)
         for i, ev in enumerate(evs):
             want = oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
             got = lst.lst_ctx_fetch_event(ctx, i)

@@ -74,8 +74,8 @@ def test_c5_batches(lst, oracle_mod, pu, n_ev):
         for rep in range(2):  # the second run reuses the workspace
             summ = run_batch(lst, ctx, evs)
             tot = {k: 0 for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")}
-            near = np.zeros(6, np.int64)
-            tests = np.zeros(6, np.int64)
+            near = np.zeros(7, np.int64)
+            tests = np.zeros(7, np.int64)
             for i, ev in enumerate(evs):
                 got = lst.lst_ctx_fetch_event(ctx, i)
                 want = _oracle(oracle_mod, geom, off, tgt, ev)

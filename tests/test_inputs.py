@@ -101,3 +101,19 @@ def test_strip_like_sensors_quantise_z_and_r():
     rq = (r[far] - ENDCAP_RMIN) / (0.5 * w) - 0.5
     assert far.sum() > 100 and np.allclose(rq, np.round(rq), atol=2e-3)
     assert np.abs(np.hypot(a.x[end], a.y[end]) - np.hypot(b.x[end], b.y[end])).max() < 0.5 * w + 1e-3
+
+
+def test_extension_inputs():
+    """the skip-layer connection map holds the plain one; the committed perceptron weights
+    have the layout of CUTS.md section 11."""
+    from lst_inputs.t5_mlp import T5_MLP, T5_MLP_SCALE, T5_MLP_THR
+
+    assert len(T5_MLP) == 65 and T5_MLP_SCALE == 100.0 and T5_MLP_THR == 1.0 and np.all(np.isfinite(T5_MLP))
+    g, off, tgt = make_config_geometry("C4")
+    g7, off7, tgt7 = make_config_geometry("C7")
+    assert g7.n_modules == g.n_modules and len(tgt7) > 2 * len(tgt)
+    for m in (0, 500, 2000):
+        assert set(tgt[off[m]:off[m + 1]]) <= set(tgt7[off7[m]:off7[m + 1]])
+    src = np.repeat(np.arange(g7.n_modules), np.diff(off7))
+    dl = g7.layer[tgt7] - g7.layer[src]
+    assert set(np.unique(dl)) == {1, 2}        # next layer and the one after it

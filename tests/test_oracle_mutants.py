@@ -90,8 +90,8 @@ MUTANTS = [
     ("T3: flag of B ignored",
      "int e = eA || eB || eC;", "int e = eA || eC;", V.check_t3_thresholds),
     ("T5: second cut compares d1 again",
-     "nr |= near_thr(p, fabsf(d2), tol);\n    if (fabsf(d2) <= tol) {",
-     "nr |= near_thr(p, fabsf(d1), tol);\n    if (fabsf(d1) <= tol) {", V.check_t5_thresholds),
+     "nr |= near_thr(p, fabsf(d2), tol);\n      if (fabsf(d2) <= tol) {",
+     "nr |= near_thr(p, fabsf(d1), tol);\n      if (fabsf(d1) <= tol) {", V.check_t5_thresholds),
     ("T5: score drops d3",
      "vals[2] = (d1 * d1 + d2 * d2) + d3 * d3;", "vals[2] = (d1 * d1 + d2 * d2);", V.check_t5_thresholds),
     ("pT: gate tolerance dropped",
@@ -114,6 +114,29 @@ MUTANTS = [
      "if (!keep5[Z]) continue;\n      const int* mZ", "const int* mZ", V.check_dedup_rule_2b_isolated),
     ("event loop: near counter not accumulated for MDs",
      "ev->near[ORC_ST_MD] += nr;", "ev->near[ORC_ST_MD] += 0 * nr;", V.check_event_near_counts),
+    ("T4: fmaxf(|k1|, |k2|) -> |k1|",
+     "float tol = p->t4_tol0 + p->t4_tol1 * fmaxf(fabsf(k1), fabsf(k2));", "float tol = p->t4_tol0 + p->t4_tol1 * fabsf(k1);",
+     V.check_t4_thresholds),
+    ("T4: relative term dropped",
+     "float tol = p->t4_tol0 + p->t4_tol1 * fmaxf(fabsf(k1), fabsf(k2));", "float tol = p->t4_tol0;", V.check_t4_thresholds),
+    ("T4: second T3 looked up by its SECOND LS",
+     "for (int t = 0; t < n_t3; ++t) t3_of_ls[T3_I(ev, t)[0] + 1]++;", "for (int t = 0; t < n_t3; ++t) t3_of_ls[T3_I(ev, t)[1] + 1]++;",
+     V.check_t4_dedup_and_event),
+    ("rule 5: share threshold 3 -> 2",
+     "if (share(mY, 4, mX, 4) >= 3 && better(md_hits, t4_score[Y], -1, mY, t4_score[X], -1, mX, 4)) keep4[X] = 0;",
+     "if (share(mY, 4, mX, 4) >= 2 && better(md_hits, t4_score[Y], -1, mY, t4_score[X], -1, mX, 4)) keep4[X] = 0;",
+     V.check_t4_dedup_and_event),
+    ("rule 5: removed T5s count too",
+     "if (keepT[Z] && share(mX, 4, t5_md + 5 * Z, 5) >= 2) keep4[X] = 0;", "if (share(mX, 4, t5_md + 5 * Z, 5) >= 2) keep4[X] = 0;",
+     V.check_t4_dedup_and_event),
+    ("rule 5: pT3 clause dropped",
+     "if (keep3[Z] && share(mX, 4, t3_md + 3 * pt3[2 * Z + 1], 3) >= 2) keep4[X] = 0;", "(void)keep3;", V.check_t4_dedup_and_event),
+    ("T5 MLP: rectifier dropped", "h[j] = fmaxf(a, 0.0f);", "h[j] = a;", V.check_t5_mlp),
+    ("T5 MLP: W1 read column-major", "a = a + W1[6 * j + i] * f[i];", "a = a + W1[8 * i + j] * f[i];", V.check_t5_mlp),
+    ("T5 MLP: feature kb and ko swapped",
+     "float f[6] = {fabsf(ki) * S, fabsf(kb) * S, fabsf(ko) * S,", "float f[6] = {fabsf(ki) * S, fabsf(ko) * S, fabsf(kb) * S,",
+     V.check_t5_mlp),
+    ("T5 MLP: output bias dropped", "s = p->t5_mlp[64];", "s = 0.0f;", V.check_t5_mlp),
     ("g: third coefficient", "t = 0.075f + t;", "t = 0.75f + t;", P.test_g_taylor_coefficients),
     ("kappa3: factor 2", "return (2.0f * crs) / ((lpq * lqs) * lps);", "return (1.0f * crs) / ((lpq * lqs) * lps);",
      lambda O: P.test_kappa3_is_textbook_circumradius(O, 100.0, True)),

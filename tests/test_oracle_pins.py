@@ -46,7 +46,7 @@ def test_default_params_match_cuts_md(oracle_mod):
             except ValueError:
                 pass
     p = oracle_mod.default_params().as_dict()
-    assert len(table) == 20
+    assert len(table) == 24   # 20 of sections 3-8 + 4 of the extensions (sections 10, 11)
     for name, val in table.items():
         assert p[name] == float(np.float32(val)), name
 

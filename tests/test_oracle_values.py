@@ -490,9 +490,106 @@ def check_dedup_rule_2b_isolated(O):
     assert k3.tolist() == [True] and kT.tolist() == [False, True]
 
 
+# ------------------------------------------------------------------------------------------------
+# extensions: T4 (CUTS.md section 10) and the learned T5 selection (section 11)
+# ------------------------------------------------------------------------------------------------
+def check_t4_thresholds(O):
+    """tol = T4_TOL0 + T4_TOL1 max(|k1|, |k2|); one cut |k1 - k2| <= tol; score = (k1 - k2)^2."""
+    six = ((-1e-3, True, False), (+1e-3, False, False), (EPS_IN[0], True, True), (EPS_IN[1], False, True),
+           (EPS_OUT[0], True, False), (EPS_OUT[1], False, False))
+    for eps, acc_e, near_e in six:
+        for sgn in (+1.0, -1.0):
+            k = 4e-4 * (1 + eps) / (1 - 0.05 * (1 + eps))       # k2 = 0: |k1| = tol (1 + eps), tol = 4e-4 + 0.05 |k1|
+            acc, near, v = O.t4_test(sgn * k, 0.0)
+            assert (acc, near) == (acc_e, near_e), f"T4 eps={eps}: {(acc, near)}"
+            assert rel(v["tol"], 4e-4 + 0.05 * k) < 2e-6 and rel(v["score"], k * k) < 1e-5
+    # max(|k1|, |k2|) with |k2| > |k1|, both signs: tol = 4e-4 + 0.05 * 0.012 = 1.0e-3 >= |d| = 9.5e-4 (with |k1|: 9.5e-4 < ...)
+    acc, near, v = O.t4_test(0.01105, 0.012)
+    assert acc and rel(v["tol"], 4e-4 + 0.05 * 0.012) < 2e-6 and rel(v["d"], -9.5e-4) < 1e-4
+    assert O.t4_test(-0.01105, -0.012)[0] and O.t4_test(0.012, 0.01105)[0]
+    assert not O.t4_test(0.0110, 0.012)[0]                       # |d| = 1.0e-3 + ... just outside: 1.0e-3 vs tol 1.0e-3
+    assert not O.t4_test(0.001, -0.001)[0]                       # opposite curvature: |d| = 2e-3 > 4.5e-4
+
+
+def check_t5_mlp(O):
+    """Section 11 with weights whose every product and partial sum is exact in binary32:
+    S = 128, ki = 1/128, ko = 1/64, bridge collinear (kb = 0): f = (1, 0, 2, 1, 2, 1).
+    unit 0: b1 = -20, W1 = (1..6): a = -20 + 1 + 0 + 6 + 4 + 10 + 6 = 7 -> h0 = 7
+    unit 1: b1 = 1, W1 = -1: a = 1 - 7 = -6 -> h1 = 0 (rectifier);  units 2..7: 0
+    s = b2 + W2.h = 0.25 + 0.5 * 7 + 100 * 0 = 3.75"""
+    B, C, D = _p4(36.0, 0.0, 0.0), _p4(51.0, 0.0, 0.0), _p4(68.0, 0.0, 0.0)
+    w = np.zeros(65, np.float32)
+    w[0:6] = [1, 2, 3, 4, 5, 6]
+    w[6:12] = -1
+    w[48], w[49] = -20, 1
+    w[56], w[57] = 0.5, 100
+    w[64] = 0.25
+    six = ((-1e-3, False, False), (+1e-3, True, False), (EPS_IN[0], False, True), (EPS_IN[1], True, True),
+           (EPS_OUT[0], False, False), (EPS_OUT[1], True, False))
+    for eps, acc_e, near_e in six:      # accept = s <= thr with thr = 3.75 (1 + eps)
+        p = O.default_params(stage_mask=0x3f | 128, t5_mlp_scale=128.0, t5_mlp_thr=3.75 * (1 + eps), t5_mlp=w)
+        acc, near, v = O.t5_test(1.0 / 128, 1.0 / 64, B, C, D, p)
+        assert float(v["s"]) == 3.75 and (acc, near) == (acc_e, near_e), f"T5 MLP eps={eps}: {(acc, near, v)}"
+        assert rel(v["score"], (1 / 128) ** 2 + (1 / 64) ** 2 + (1 / 128) ** 2) < 1e-6   # score as in section 6
+    # |.| features: signs of the curvatures do not matter
+    p = O.default_params(stage_mask=0x3f | 128, t5_mlp_scale=128.0, t5_mlp_thr=4.0, t5_mlp=w)
+    assert float(O.t5_test(-1.0 / 128, -1.0 / 64, B, C, D, p)[2]["s"]) == 3.75
+    # row-major W1[j][i]: a weight on feature 2 of unit 0 only
+    w2 = np.zeros(65, np.float32)
+    w2[2], w2[56] = 1.0, 1.0
+    p = O.default_params(stage_mask=0x3f | 128, t5_mlp_scale=128.0, t5_mlp_thr=4.0, t5_mlp=w2)
+    assert float(O.t5_test(1.0 / 128, 1.0 / 64, B, C, D, p)[2]["s"]) == 2.0     # = f[2] = |ko| S
+    # without bit 7 the weights are ignored: the candidate fails the pairwise cuts of section 6 (|d2| = 1/64)
+    assert not O.t5_test(1.0 / 128, 1.0 / 64, B, C, D, O.default_params(t5_mlp=w, t5_mlp_thr=100.0))[0]
+
+
+def check_t4_dedup_and_event(O):
+    """Rule 5 (CUTS.md section 10) on hand-made lists, and T4 enumeration / TC class 4 on a real event."""
+    md_hits = np.arange(2 * 40, dtype=np.int32).reshape(40, 2)
+    none2, none_f = np.zeros((0, 2), np.int32), np.zeros(0, np.float32)
+    nk = np.zeros(0, bool)
+    # (a) two T4s sharing 3 MDs: the lower score survives; sharing 2: both survive
+    k4 = O.dedup_t4(md_hits, np.zeros((0, 3)), np.zeros((0, 5)), none2, none2, nk, nk, nk, [[0, 1, 2, 3], [1, 2, 3, 4]], [2.0, 1.0])
+    assert k4.tolist() == [False, True]
+    k4 = O.dedup_t4(md_hits, np.zeros((0, 3)), np.zeros((0, 5)), none2, none2, nk, nk, nk, [[0, 1, 2, 3], [2, 3, 4, 5]], [2.0, 1.0])
+    assert k4.tolist() == [True, True]
+    # (b) removed by a SURVIVING T5 / pT3 / pT5 sharing 2 MDs, not by a removed one
+    t5 = [[0, 1, 10, 11, 12], [20, 21, 22, 23, 24]]
+    k4 = O.dedup_t4(md_hits, np.zeros((0, 3)), t5, none2, none2, nk, nk, np.array([True, False]),
+                    [[0, 1, 30, 31], [20, 21, 32, 33], [0, 34, 35, 36]], [1.0, 1.0, 1.0])
+    assert k4.tolist() == [False, True, True]
+    k4 = O.dedup_t4(md_hits, [[5, 6, 7]], t5, [[3, 0]], [[4, 1]], np.array([True]), np.array([True]), np.array([False, False]),
+                    [[5, 6, 30, 31], [23, 24, 32, 33], [7, 34, 35, 36]], [1.0, 1.0, 1.0])
+    assert k4.tolist() == [False, False, True]
+    # whole event: enumeration by brute force over T3 pairs, structure, class order
+    from lst_inputs import make_config_event, make_config_geometry
+
+    geom, off, tgt = make_config_geometry("C4")
+    ev = make_config_event("C4")
+    r = O.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls, O.default_params(stage_mask=0x7f))
+    want = []
+    for t1 in range(len(r["t3_ls"])):
+        for t2 in np.nonzero(r["t3_ls"][:, 0] == r["t3_ls"][t1, 1])[0]:
+            if O.t4_test(r["t3_k"][t1], r["t3_k"][t2])[0]:
+                want.append((t1, int(t2)))
+    assert sorted(want) == sorted(map(tuple, r["t4_t3"].tolist())) and len(want) > 100
+    assert r["n_tests"][6] >= len(want) and r["n_tests"][6] == sum(
+        int((r["t3_ls"][:, 0] == l).sum()) for l in r["t3_ls"][:, 1])
+    a, b = r["t3_md"][r["t4_t3"][:, 0]], r["t3_md"][r["t4_t3"][:, 1]]
+    assert np.array_equal(a[:, 1:], b[:, :2]) and np.array_equal(r["t4_md"], np.concatenate([a, b[:, 2:]], axis=1))
+    tc = r["tc"]
+    assert np.all(np.diff(tc[:, 0]) >= 0) and (tc[:, 0] == 4).sum() >= 1
+    row = tc[tc[:, 0] == 4][0]
+    t4 = np.nonzero(r["t4_t3"][:, 0] == row[3])[0]
+    assert any(np.array_equal(row[4:12].reshape(4, 2), r["md_hits"][r["t4_md"][k]]) for k in t4) and np.all(row[12:] == -1)
+    # the paper's four classes are untouched by the extension
+    r0 = O.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+    assert np.array_equal(tc[tc[:, 0] < 4], r0["tc"]) and len(r0["t4_md"]) == 0 and r0["n_tests"][6] == 0
+
+
 CHECKS = (check_md_barrel_thresholds, check_md_endcap_thresholds, check_ls_thresholds, check_ls_direction_signs,
           check_t3_thresholds, check_t5_thresholds, check_pt_thresholds, check_event_near_counts,
-          check_dedup_rule_2b_isolated)
+          check_dedup_rule_2b_isolated, check_t4_thresholds, check_t5_mlp, check_t4_dedup_and_event)
 
 
 def test_md_barrel_thresholds(oracle_mod):
@@ -529,3 +626,15 @@ def test_event_near_counts(oracle_mod):
 
 def test_dedup_rule_2b_isolated(oracle_mod):
     check_dedup_rule_2b_isolated(oracle_mod)
+
+
+def test_t4_thresholds(oracle_mod):
+    check_t4_thresholds(oracle_mod)
+
+
+def test_t5_mlp(oracle_mod):
+    check_t5_mlp(oracle_mod)
+
+
+def test_t4_dedup_and_event(oracle_mod):
+    check_t4_dedup_and_event(oracle_mod)

@@ -49,6 +49,11 @@ def canon(res: dict) -> dict:
     tc = np.asarray(res["tc"], dtype=np.int64).reshape(-1, 16)
     out["tc_order_types"] = tc[:, 0].copy()  # class order pT5, pT3, T5, pLS must be non-decreasing
     (out["tc"],) = _sort_rows(np.concatenate([tc[:, 0:2], tc[:, 4:16]], axis=1))
+    # extension (CUTS.md section 10): T4 objects, empty unless stage-mask bit 6 is set
+    t4 = np.asarray(res.get("t4_md", np.zeros((0, 4))), dtype=np.int64).reshape(-1, 4)
+    k, sc = _sort_rows(mdh[t4].reshape(-1, 8) if len(t4) else np.zeros((0, 8), np.int64),
+                       np.asarray(res.get("t4_score", np.zeros(0)), dtype=np.float32))
+    out["t4"], out["t4_score"] = k, sc
     out["near"] = np.asarray(res["near"], dtype=np.int64)
     out["n_tests"] = np.asarray(res["n_tests"], dtype=np.int64)
     return out
@@ -56,10 +61,10 @@ def canon(res: dict) -> dict:
 
 def assert_same(a: dict, b: dict, what: str = ""):
     """Bit-exact equality of two canonical results (index tuples AND float payloads)."""
-    for key in ("md", "md_module", "ls", "t3", "t5", "pt3", "pt5", "tc", "near", "n_tests"):
+    for key in ("md", "md_module", "ls", "t3", "t5", "pt3", "pt5", "t4", "tc", "near", "n_tests"):
         assert a[key].shape == b[key].shape, f"{what}{key}: count {a[key].shape} vs {b[key].shape}"
         assert np.array_equal(a[key], b[key]), f"{what}{key}: tuples differ"
-    for key in ("md_f", "ls_kappa", "t3_k", "t5_score", "pt3_score", "pt5_score"):
+    for key in ("md_f", "ls_kappa", "t3_k", "t5_score", "pt3_score", "pt5_score", "t4_score"):
         fa, fb = np.ascontiguousarray(a[key]), np.ascontiguousarray(b[key])
         na, nb = np.isnan(fa), np.isnan(fb)  # a NaN has no defined bit pattern (x86 and sm_100 produce different ones)
         assert np.array_equal(na, nb), f"{what}{key}: NaN payloads in different places"
