@@ -253,6 +253,7 @@ def run_b200(args):
 
     # device-resident and pinned-host copies of every batch
     dev_in, host_in = [], []
+    u16 = 2 * geom.n_modules <= 65536
     f_hit, f_pls = ("x", "y", "z", "sensor"), ("pt", "x0", "y0", "z0", "x1", "y1", "z1", "q")
     for _, b in batches:
         pin = {k: torch.from_numpy(np.ascontiguousarray(b[k])).pin_memory() for k in f_hit}
@@ -261,11 +262,15 @@ def run_b200(args):
         d_p = {k: v.cuda() for k, v in pin_p.items()}
         hd, keep_d = lst.make_hits(d["x"], d["y"], d["z"], d["sensor"], b["hit_offsets"])
         sd, keep_d = lst.make_pls(d_p, b["pls_offsets"], keep_d)
+        # the host path sends the sensor ids as uint16 when they fit (lst_hits.sensor_u16): 14 bytes per hit over PCIe
+        if u16:
+            pin["sensor"] = torch.from_numpy(np.ascontiguousarray(b["sensor"].astype(np.uint16))).pin_memory()
         hh, keep_h = lst.make_hits(*(pin[k].numpy() for k in f_hit), b["hit_offsets"])
         sh, keep_h = lst.make_pls({k: v.numpy() for k, v in pin_p.items()}, b["pls_offsets"], keep_h)
         dev_in.append((hd, sd, keep_d, d, d_p))
         host_in.append((hh, sh, keep_h, pin, pin_p))
-    in_bytes = [int(b["x"].shape[0]) * 16 + int(b["pls_offsets"][-1]) * 32 + 8 * (E + 1) for _, b in batches]
+    in_bytes = [int(b["x"].shape[0]) * (14 if u16 else 16) + int(b["pls_offsets"][-1]) * 32 + 8 * (E + 1) + 64
+                for _, b in batches]
     torch.cuda.synchronize()
 
     def pipelined(inputs, K, fetch):
@@ -430,6 +435,7 @@ def run_b200(args):
         },
         "e2e": {"value": round(world * args.steps * E / (ms_e2e * 1e-3), 1), "unit": UNIT,
                 "h2d_bytes_per_step": int(np.mean(in_bytes)), "d2h_bytes_per_step": int(d2h / args.steps),
+                "input_format": "x, y, z float32 + sensor %s per hit; 8 x 4 bytes per seed" % ("uint16" if u16 else "int32"),
                 "ms_per_step": round(ms_e2e / args.steps, 5)},
         "gpu_launches": launches,
         "clocks": sampler.summary(),

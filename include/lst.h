@@ -89,11 +89,13 @@ typedef struct lst_hits {
   const float* x;
   const float* y;
   const float* z;
-  const int32_t* sensor;        /* 2*module + {0,1} */
+  const int32_t* sensor;        /* 2*module + {0,1}; with sensor_u16 != 0 the array holds uint16_t instead */
   int32_t n;                    /* hits in the batch */
   const int32_t* event_offsets; /* HOST pointer, n_events+1 entries, [0] = 0, [n_events] = n;
                                    NULL = one event */
   int32_t on_device;            /* 0: x, y, z, sensor are host pointers; 1: device pointers */
+  int32_t sensor_u16;           /* != 0: `sensor` points to uint16_t ids (14 instead of 16 bytes per hit over PCIe);
+                                   needs 2 * n_modules <= 65536, else LST_ERR_ARG */
 } lst_hits;
 
 /* Inner-tracker seeds (pLS) of a batch (reading S6 of DESIGN.md). */

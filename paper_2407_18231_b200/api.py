@@ -42,7 +42,13 @@ def make_hits(x, y, z, sensor, event_offsets=None, keep=None):
     h.x, n, dev = _ptr(x, np.float32, keep)
     h.y, n2, dev2 = _ptr(y, np.float32, keep)
     h.z, n3, dev3 = _ptr(z, np.float32, keep)
-    h.sensor, n4, dev4 = _ptr(sensor, np.int32, keep)
+    u16 = (sensor.dtype == np.uint16) if isinstance(sensor, np.ndarray) else str(getattr(sensor, "dtype", "")) == "torch.uint16"
+    if u16 and _is_torch(sensor):
+        keep.append(sensor)
+        h.sensor, n4, dev4 = C.c_void_p(sensor.data_ptr()), int(sensor.numel()), int(sensor.is_cuda)
+    else:
+        h.sensor, n4, dev4 = _ptr(sensor, np.uint16 if u16 else np.int32, keep)
+    h.sensor_u16 = int(u16)
     if not (n == n2 == n3 == n4) or not (dev == dev2 == dev3 == dev4):
         raise ValueError("hit arrays must have equal length and live on the same side")
     h.n = n

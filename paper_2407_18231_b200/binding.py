@@ -55,7 +55,7 @@ class lst_caps(C.Structure):
 
 class lst_hits(C.Structure):
     _fields_ = [("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p), ("sensor", C.c_void_p),
-                ("n", C.c_int32), ("event_offsets", C.c_void_p), ("on_device", C.c_int32)]
+                ("n", C.c_int32), ("event_offsets", C.c_void_p), ("on_device", C.c_int32), ("sensor_u16", C.c_int32)]
 
 
 class lst_pls(C.Structure):

@@ -107,6 +107,7 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   if (n_events <= 0 || n_events > c.max_events) return n_events > c.max_events ? LST_ERR_CAPACITY : LST_ERR_ARG;
   if (hits->n < 0 || (hits->n > 0 && (!hits->x || !hits->y || !hits->z || !hits->sensor))) return LST_ERR_ARG;
   if (hits->n > c.max_hits) return LST_ERR_CAPACITY;
+  if (hits->sensor_u16 && 2LL * ctx->g->n_mod > 65536) return LST_ERR_ARG;
   const int n_pls = seeds ? seeds->n : 0;
   if (n_pls < 0) return LST_ERR_ARG;
   if (n_pls > c.max_pls) return LST_ERR_CAPACITY;
@@ -141,6 +142,7 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
   bt.n_events = n_events;
   bt.n_hits = hits->n;
   bt.n_pls = n_pls;
+  bt.sensor_u16 = hits->sensor_u16 != 0;
   if (hits->on_device || hits->n == 0) {
     bt.in_x = hits->x;  bt.in_y = hits->y;  bt.in_z = hits->z;  bt.in_sensor = hits->sensor;
   } else {
@@ -148,7 +150,7 @@ extern "C" int lst_ctx_run(lst_ctx* ctx, int32_t n_events, const lst_hits* hits,
     CK(cudaMemcpyAsync(ctx->in_x, hits->x, nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->in_y, hits->y, nb, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->in_z, hits->z, nb, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(ctx->in_sensor, hits->sensor, nb, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->in_sensor, hits->sensor, hits->sensor_u16 ? nb / 2 : nb, cudaMemcpyHostToDevice, st));
     bt.in_x = ctx->in_x;  bt.in_y = ctx->in_y;  bt.in_z = ctx->in_z;  bt.in_sensor = ctx->in_sensor;
   }
   if (n_pls > 0) {

@@ -33,7 +33,8 @@ __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
 #pragma unroll
     for (int u = 0; u < kIngestUnroll; ++u) {
       const int i = i0 + u * stride;
-      s[u] = i < d.n_hits ? __ldg(d.in_sensor + i) : 0;
+      s[u] = i >= d.n_hits ? 0 : (d.sensor_u16 ? (int)__ldg(reinterpret_cast<const unsigned short*>(d.in_sensor) + i)
+                                                 : __ldg(d.in_sensor + i));
     }
 #pragma unroll
     for (int u = 0; u < kIngestUnroll; ++u) {

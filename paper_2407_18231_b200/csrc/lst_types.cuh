@@ -39,7 +39,8 @@ struct Ctl {
 // What changes from batch to batch: sizes and input pointers.  Lives in device memory (copied in front of
 // every launch sequence), so the kernel arguments -- and with them the CUDA graph of a context -- never change.
 struct Batch {
-  int n_events, n_hits, n_pls, pad;
+  int n_events, n_hits, n_pls;
+  int sensor_u16;  // in_sensor holds unsigned short ids (include/lst.h: lst_hits.sensor_u16)
   const float *in_x, *in_y, *in_z;
   const int* in_sensor;
   const float *p_pt, *p_x0, *p_y0, *p_z0, *p_x1, *p_y1, *p_z1;
@@ -54,7 +55,7 @@ struct Dev {
   const int* conn_off;  // [n_mod + 1]
   const int* conn_tgt;
   // ---- batch ----
-  int n_events, n_hits, n_pls;
+  int n_events, n_hits, n_pls, sensor_u16;
   const int* hit_ev_off;  // [n_events + 1] device copy of the event offsets
   const int* pls_ev_off;  // [n_events + 1]
   const float *in_x, *in_y, *in_z;  // input hits (device), caller order
@@ -143,7 +144,7 @@ struct Dev {
 // first statement of every kernel: the batch fields of the by-value argument come from device memory
 __device__ __forceinline__ void load_batch(Dev& d) {
   const Batch* __restrict__ b = d.batch;
-  d.n_events = b->n_events;  d.n_hits = b->n_hits;  d.n_pls = b->n_pls;
+  d.n_events = b->n_events;  d.n_hits = b->n_hits;  d.n_pls = b->n_pls;  d.sensor_u16 = b->sensor_u16;
   d.in_x = b->in_x;  d.in_y = b->in_y;  d.in_z = b->in_z;  d.in_sensor = b->in_sensor;
   d.p_pt = b->p_pt;  d.p_q = b->p_q;
   d.p_x0 = b->p_x0;  d.p_y0 = b->p_y0;  d.p_z0 = b->p_z0;

@@ -63,6 +63,29 @@ def test_device_resident_inputs_match_host_inputs(lst, oracle_mod):
     assert_same(canon(got), canon(_oracle(oracle_mod, geom, off, tgt, ev)), "C4 device inputs: ")
 
 
+def test_uint16_sensor_ids(lst, oracle_mod):
+    """include/lst.h lst_hits.sensor_u16: the same event with 16-bit sensor ids, from host and from device memory."""
+    import torch
+
+    geom, off, tgt = make_config_geometry("C3")
+    ev = make_config_event("C3", seeds=True)
+    want = canon(_oracle(oracle_mod, geom, off, tgt, ev))
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    try:
+        s16 = ev.sensor.astype(np.uint16)
+        assert_same(canon(lst.lst_run_event(g, ev.x, ev.y, ev.z, s16, ev.pls)), want, "uint16 sensors (host): ")
+        dev = [torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z)]
+        pls = {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in ev.pls.items() if k != "truth"}
+        assert_same(canon(lst.lst_run_event(g, *dev, torch.from_numpy(s16).cuda(), pls)), want, "uint16 sensors (device): ")
+        bad = s16.copy()
+        bad[5] = 2 * geom.n_modules
+        with pytest.raises(lst.LstError) as ei:
+            lst.lst_run_event(g, ev.x, ev.y, ev.z, bad, ev.pls)
+        assert ei.value.status == lst.LST_ERR_ARG
+    finally:
+        lst.lst_free(g)
+
+
 @pytest.mark.parametrize("pu,n_ev", [(50, 5), (200, 3)])
 def test_c5_batches(lst, oracle_mod, pu, n_ev):
     """Config 5: several independent events in one launch sequence; every event equals the oracle's."""
