@@ -8,10 +8,14 @@
  * Precision: binary32, fixed operation order, no FMA (north_star fixes the precision; build with
  * -O2 -ffp-contract=off -fno-fast-math).
  *
- * Pins (tests/test_oracle_pins.py): closed-form helix values for every cut quantity, textbook
- * circumradius for kappa3, asin series for g, hand-computed straight/curved single tracks
- * (tests/golden/), brute-force all-pairs enumeration, structural invariants, monotonicity in the
- * cut windows, O(n^2) restatement of the duplicate removal.
+ * Pins (tests/test_oracle_pins.py, test_oracle_values.py, test_oracle_dedup.py): a hand-built candidate
+ * with the expected threshold for every term of every cut (value and accept / reject decision), the
+ * near-threshold rule at t (1 +- 0.5e-5) / t (1 +- 2e-5) and the order of the cuts for every stage,
+ * closed-form helix values, textbook circumradius for kappa3, asin series for g, hand-computed
+ * straight/curved single tracks (tests/golden/), brute-force all-pairs enumeration, structural
+ * invariants, monotonicity in the cut windows, every clause of the duplicate removal.
+ * tests/test_oracle_mutants.py applies 51 one-line mistakes to a copy of lst_oracle.c: each fails a
+ * named pin.  tests/test_oracle_sanitizers.py runs the pins under ASan + UBSan.
  * "parity unpinned" against the paper's own numbers: PAPER.md prints no object counts or
  * intermediate values.
  */
