@@ -229,6 +229,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.tstate[T_T4] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
   d.sens_cnt = b.take<int>(n_sens + 1);
   d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins);
+  d.anc_done = b.take<int>(c.max_events);
   d.pls_pt3_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt5_cnt = b.take<int>((size_t)c.max_pls + 1);
   d.pls_pt3_cur = b.take<int>(c.max_pls);
@@ -269,6 +270,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.t3_md = b.take<int4>(c.max_t3);
   d.t3_k = b.take<float>(c.max_t3);
   d.t3_l = b.take<float4>(c.max_t3);
+  d.t3_q = b.take<float4>(c.max_t3);
   d.t3_t5_begin = b.take<int>((size_t)c.max_t3 + 1);
   d.t5_t3 = b.take<int2>(c.max_t5);
   d.t5_md = b.take<int>(5 * (size_t)c.max_t5);
@@ -283,12 +285,15 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.seed_a = b.take<float4>(c.max_pls);
   d.seed_b = b.take<float4>(c.max_pls);
   d.seed_z1 = b.take<float>(c.max_pls);
+  d.seed_g = b.take<float4>(c.max_pls);
+  d.seed_perm = b.take<int>(c.max_pls);
   d.pls_event = b.take<int>(c.max_pls);
   d.pt_ev = b.take<PtEvent>((size_t)c.max_events + 1);
   d.anc_bin = b.take<int>(c.max_md);
   d.anc_rank = b.take<int>(c.max_md);
   d.anc_a = b.take<float4>(c.max_md);
   d.anc_t = b.take<int4>(c.max_md);
+  d.anc_c = b.take<float4>(5 * ((size_t)c.max_md / 32 + c.max_events + 2));
   d.cap_queue = (int)(2LL * ((long long)c.max_pt3 + c.max_pt5) < 0x7fffffffLL ? 2LL * ((long long)c.max_pt3 + c.max_pt5)
                                                                              : 0x7fffffffLL);
   d.pt_queue = b.take<int2>(d.cap_queue);

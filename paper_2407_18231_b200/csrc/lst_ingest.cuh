@@ -63,6 +63,8 @@ __global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
     d.seed_a[p] = make_float4(s.x1, s.y1, s.vx, s.vy);
     d.seed_b[p] = make_float4(s.lv, s.kp, s.tolk, s.slope);
     d.seed_z1[p] = s.z1;
+    // what k_pt_eval keeps per lane: the coefficients of the gate limit glim = lw (lw c1 + c2), and kp, tolk
+    d.seed_g[p] = make_float4(s.lv * d.cuts.inv_2rmin, s.lv * d.cuts.pt_gate_tol, s.kp, s.tolk);
   }
 }
 

@@ -4,15 +4,19 @@
 // the gate, 0.9 % the curvature match with the seed and 0.06 % are accepted.  Structure:
 //   * anchors: the gate depends only on the seed and the FIRST MD of the candidate, and T3s / T5s are stored
 //     grouped by first MD, so the gate is evaluated once per (seed, anchor) and shared by pT3 and pT5;
-//     anchors are sorted into radius x azimuth bins (lst_stages.cuh, k_anchor_sort);
-//   * k_pt_eval, tile = 32 anchors (one per lane) x 64 seeds of the same event (shared memory, broadcast):
-//     (1a) one seed per lane against the bounding circle of the warp's anchors;
-//     (1b) every lane tests its anchor against the seeds that may match: a necessary condition of the gate
-//          with |A - P1| from rsqrt.approx; only within 1e-4 of the threshold the exact gate decides (and
-//          flags near-threshold);
-//     (2)  gate survivors are expanded into their (seed, T3 / T5) candidates, flattened over the lanes;
-//          kx~ (lst_cuts_pt.cuh) drops those whose curvature match with the seed surely fails;
-//     (3)  the rest of the approximate cascade (stored curvatures, r-z at both ends) on full warps;
+//     anchors are sorted into radius x azimuth bins (lst_stages.cuh, k_anchor_sort), which also writes the
+//     bounding circle of every block of 32 sorted anchors and of its four sub-blocks of 8, and the seeds of
+//     every event in azimuth order (seed_perm);
+//   * k_pt_eval, tile = 32 seeds consecutive in azimuth (one per LANE, their constants in registers) x
+//     kPtBlocks anchor blocks:
+//     (1a) every lane tests its seed against the bounding circle of the block, then of each sub-block;
+//     (1b) the anchors of a surviving sub-block are walked one by one (broadcast from shared memory): a
+//          necessary condition of the gate with |A - P1| from rsqrt.approx; only within 1e-4 of the threshold
+//          the exact gate decides (and flags near-threshold);
+//     (2)  the anchor's T3s and T5s in a warp-uniform loop -- one broadcast load per candidate, no index
+//          decoding: kx~ (lst_cuts_pt.cuh) against the seed's curvature and, behind a sure pass of that cut,
+//          against the candidate's stored curvature(s);
+//     (3)  the rest of the approximate cascade (r-z at both ends) on full warps of survivors;
 //     what cannot be rejected for sure goes to a queue;
 //   * k_pt_exact runs the exact cut list of CUTS.md section 7 on the queue (1.1 x the accepted objects):
 //     accepted pairs go to scratch lists with a count per seed; k_scan2 + k_pt_place group them by seed.
@@ -62,7 +66,8 @@ struct PtCand {
   }
 };
 
-constexpr int kSeedTile = 64;           // seeds staged per tile
+constexpr int kPtBlocks = 2;           // anchor blocks (of 32 sorted anchors) per tile
+constexpr int kSeedSectors = 128;       // azimuth sectors of the seed sort
 constexpr int kAncBlocksPerEvent = 8;   // blocks of k_anchor_sort per event
 
 // per-event table written by k_anchor_sort: anchor range, seed range, first tile
@@ -84,21 +89,36 @@ __device__ __forceinline__ void event_cands(const Dev& d, int ev, int& c0, int& 
   }
 }
 
+// azimuth sector of the point where the straight line through the seed's two pixel hits reaches r ~ 35 cm
+// (diamond angle, as anchor_bin): only the ORDER of the seeds in k_pt_eval depends on it, never a result
+__device__ __forceinline__ int seed_sector(float4 sa) {
+  const float x = sa.x + 7.0f * sa.z, y = sa.y + 7.0f * sa.w;
+  const float a = fabsf(x) + fabsf(y);
+  const float t = a > 0.0f ? y / a : 0.0f;
+  const float ps = x >= 0.0f ? (y >= 0.0f ? t : 4.0f + t) : 2.0f - t;  // [0, 4)
+  int sec = (int)(ps * (kSeedSectors / 4));
+  return sec < 0 ? 0 : (sec > kSeedSectors - 1 ? kSeedSectors - 1 : sec);
+}
+
 // Counting sort of an event's anchors by bin (the counts and arrival ranks come from the T5 kernel's
 // prologue).  grid = n_events * kAncBlocksPerEvent; every block scans the 512 bin counts of its event in
 // shared memory and places its share of the event's MDs; the anchors of event e start at the event's
-// first MD (an event has no more anchors than MDs), so no prefix across events is needed.  Block 0 also
-// writes the per-event table of k_pt_eval (ranges, tile prefix) and the candidate counts of stages 4, 5.
+// first MD (an event has no more anchors than MDs), so no prefix across events is needed.  The last block
+// of an event also sorts the event's seeds by azimuth sector (seed_perm).  Block 0 also writes the
+// per-event table of k_pt_eval (ranges, tile prefix) and the candidate counts of stages 4, 5.
 __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
   load_batch(d);
   __shared__ int s_begin[kAncBins];
   __shared__ int s_warp[kWarps];
+  __shared__ int s_sec[kSeedSectors];
+  __shared__ int s_secw[kSeedSectors / 32];
+  __shared__ int s_last;
   const int E = d.n_events;
   const int e = blockIdx.x / kAncBlocksPerEvent, part = blockIdx.x - e * kAncBlocksPerEvent;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool on = (d.cuts.stage_mask & 16) && d.ctl->total[K_T3] > 0 && d.n_pls > 0;
   const bool on5 = d.ctl->total[K_T5] > 0;
-  if (on) {
+  if (on && e < E) {
     // exclusive scan of the event's 512 bin counts: 2 per thread
     const int c0 = d.anc_bin_cnt[e * kAncBins + 2 * threadIdx.x], c1 = d.anc_bin_cnt[e * kAncBins + 2 * threadIdx.x + 1];
     const int incl = warp_incl_scan(c0 + c1);
@@ -119,6 +139,73 @@ __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
       d.anc_a[pos] = pack_flag(d.md_a[A], d.md_info[A] & 1);
       d.anc_t[pos] = make_int4(t0, t1 - t0, u0, u1 - u0);
     }
+    // ---- the last of the event's blocks to get here: bounding circles (x, y, h) of every block of 32 sorted
+    // anchors and of its four sub-blocks of 8, at anc_c[5 * ((md0 >> 5) + e + block)] (ranges of different
+    // events cannot overlap: an event has no more anchors than MDs) ----
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(d.anc_done + e, 1) == kAncBlocksPerEvent - 1;
+    __syncthreads();
+    if (s_last) {
+      __threadfence();
+      const int n_a = s_begin[kAncBins - 1] + d.anc_bin_cnt[e * kAncBins + kAncBins - 1];
+      const int n_blk = (n_a + 31) / 32;
+      float4* out = d.anc_c + 5 * (size_t)((md0 >> 5) + e);
+      auto circ_of = [](float x0, float x1, float y0, float y1) {
+        return make_float4(0.5f * (x0 + x1), 0.5f * (y0 + y1),
+                           0.5f * sqrtf((x1 - x0) * (x1 - x0) + (y1 - y0) * (y1 - y0)) * 1.001f + 1e-3f, 0.0f);
+      };
+      constexpr int U = 4;  // blocks in flight per warp (independent load + shuffle chains)
+      for (int b0 = warp * U; b0 < n_blk; b0 += kWarps * U) {
+        float x0[U], x1[U], y0[U], y1[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const bool valid = (b0 + u) * 32 + lane < n_a;
+          float4 A = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          if (valid) A = __ldcg(d.anc_a + md0 + (b0 + u) * 32 + lane);
+          x0[u] = valid ? A.x : 3e38f;  x1[u] = valid ? A.x : -3e38f;
+          y0[u] = valid ? A.y : 3e38f;  y1[u] = valid ? A.y : -3e38f;
+        }
+#pragma unroll
+        for (int sh = 1; sh < 32; sh <<= 1) {
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            if (sh == 8 && (lane & 7) == 0 && b0 + u < n_blk)
+              out[5 * (b0 + u) + 1 + (lane >> 3)] = circ_of(x0[u], x1[u], y0[u], y1[u]);
+            x0[u] = fminf(x0[u], __shfl_xor_sync(kFull, x0[u], sh));
+            x1[u] = fmaxf(x1[u], __shfl_xor_sync(kFull, x1[u], sh));
+            y0[u] = fminf(y0[u], __shfl_xor_sync(kFull, y0[u], sh));
+            y1[u] = fmaxf(y1[u], __shfl_xor_sync(kFull, y1[u], sh));
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+          if (lane == 0 && b0 + u < n_blk) out[5 * (b0 + u)] = circ_of(x0[u], x1[u], y0[u], y1[u]);
+      }
+    }
+    if (part == kAncBlocksPerEvent - 1) {
+      // ---- the event's seeds in azimuth order: counting sort over kSeedSectors sectors ----
+      const int s0 = d.pls_ev_off[e], s1 = d.pls_ev_off[e + 1];
+      if (threadIdx.x < kSeedSectors) s_sec[threadIdx.x] = 0;
+      __syncthreads();
+      for (int p = s0 + threadIdx.x; p < s1; p += kBlock) atomicAdd(&s_sec[seed_sector(d.seed_a[p])], 1);
+      __syncthreads();
+      int cs = 0, is = 0;
+      if (threadIdx.x < kSeedSectors) {
+        cs = s_sec[threadIdx.x];
+        is = warp_incl_scan(cs);
+        if (lane == 31) s_secw[warp] = is;
+      }
+      __syncthreads();
+      if (threadIdx.x < kSeedSectors) {
+        int base2 = 0;
+        for (int w = 0; w < warp; ++w) base2 += s_secw[w];
+        s_sec[threadIdx.x] = base2 + is - cs;
+      }
+      __syncthreads();
+      for (int p = s0 + threadIdx.x; p < s1; p += kBlock)
+        d.seed_perm[s0 + atomicAdd(&s_sec[seed_sector(d.seed_a[p])], 1)] = p;
+    }
   }
   if (blockIdx.x != 0) return;
   __syncthreads();
@@ -135,7 +222,8 @@ __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
       pe.a0 = on ? d.mod_md_begin[ev * d.n_mod] : 0;
       pe.a1 = pe.a0 + n_a;
       const int ns = on ? pe.s1 - pe.s0 : 0;
-      pe.tile0 = ((n_a + 31) / 32) * ((ns + kSeedTile - 1) / kSeedTile);  // warp tiles; prefix below
+      const int n_blk = (n_a + 31) / 32;
+      pe.tile0 = ((n_blk + kPtBlocks - 1) / kPtBlocks) * ((ns + 31) / 32);  // warp tiles; prefix below
       d.pt_ev[ev] = pe;
       int c0 = 0, c1 = 0;
       if (on) {  // candidates of CUTS.md section 7: every (seed, T3) and (seed, T5) of the event
@@ -166,19 +254,18 @@ struct PtAccepted {
 };
 
 struct PtWarp {  // per-warp scratch of k_pt_eval (dynamic shared memory: kWarps of these)
-  float4 sa[kSeedTile];  // x1, y1, vx, vy of the tile's seeds
-  float4 sg[kSeedTile];  // gate limit lw (lw c1 + c2), c1 = lv INV_2RMIN, c2 = lv PT_GATE_TOL: upper (c1h, c2h) and lower (c1l, c2l) versions
-  float2 sk[kSeedTile];  // kp, tolk
-  int2 w2[64];           // candidates behind the curvature pre-filter: (T3 / T5 index | T5 flag << 31, seed slot | anchor lane << 16)
-  float4 anc[32];        // the warp's anchors (x, y, z, r | endcap << 31)
-  int4 at[32];           // (first T3, number of T3s, first T5, number of T5s) of each
-  unsigned w1[64];       // gate survivors: seed slot | anchor lane << 16 | gate-near << 31
-  int pref[33];          // exclusive prefix of the candidate counts of w1[0..32)
-  unsigned heads[32];    // head bits of the entries over the first 1024 items
+  float4 anc[32];  // the anchors of the current block (x, y, z, r | endcap << 31)
+  int4 at[32];     // (first T3, number of T3s, first T5, number of T5s) of each
+  int4 w2[64];     // candidates behind the curvature pre-filter: (T3 / T5 index | T5 flag << 31, seed, anchor position in anc_a, 0)
 };
 
-// pT3 and pT5 candidates of the whole batch -> queue of the exact cuts.  Warps take tiles by ticket and
-// never wait for one another.
+// pT3 and pT5 candidates of the whole batch -> queue of the exact cuts.  tile = 32 seeds of one event
+// (consecutive in azimuth order, one per LANE, their constants in registers) x kPtBlocks blocks of 32
+// sorted anchors; warps take tiles by ticket and never wait for one another.  Per block: every lane tests
+// its seed against the bounding circle of the block's anchors; if any lane may match, the block's anchors
+// are walked one by one (anchor data broadcast from shared memory): gate per lane, then the anchor's T3s
+// and T5s in a warp-uniform loop (one broadcast load per candidate, no index decoding) with kx~ against
+// the seed's and the candidate's stored curvatures.
 __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
   load_batch(d);
   extern __shared__ __align__(16) unsigned char s_dyn[];
@@ -188,7 +275,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
   const int n_tiles = d.pt_ev[E].tile0;
   const int cap_q = d.cap_queue;
   const float inv = d.cuts.inv_2rmin, gtol = d.cuts.pt_gate_tol;
-  // the circle test of phase 1a bounds the gate limit at |w| + h, which needs a limit growing with |w|
+  // the circle test bounds the gate limit at |w| + h, which needs a limit growing with |w|
   const bool can_prune = inv >= 0.0f && gtol >= 0.0f;
   // warp-aggregated append to the queue of the exact cuts
   auto push_q = [&](bool go, int p, int cand) {
@@ -199,6 +286,36 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     base = __shfl_sync(kFull, base, __ffs(m) - 1);
     const int pos = base + __popc(m & ((1u << lane) - 1u));
     if (go && pos < cap_q) d.pt_queue[pos] = make_int2(p, cand);
+  };
+  // ---- (3) the rest of the approximate cascade for one entry of w2; what survives goes to the queue ----
+  auto tail = [&](int4 ent, bool active) {
+    bool go = false;
+    if (active) {
+      const int t = ent.x & 0x7fffffff;
+      const bool is5 = ent.x < 0;
+      const float4 s = d.seed_a[ent.y], sb = d.seed_b[ent.y];  // sb = lv, kp, tolk, slope
+      const float4 a = d.anc_a[ent.z];
+      const float4 l = is5 ? d.t5_l[t] : d.t3_l[t];
+      bool ok;
+      const float kx = kx_approx(s.x, s.y, a.x, a.y, l.x, l.y, ok);
+      int c = pt_class_curv(kx, sb.y, sb.z, ok);
+      if (c == PT_PASS) {
+        if (is5) {
+          const float2 kio = d.t5_kio[t];
+          c = pt_class_curv(kx, kio.x, sb.z, ok);
+          if (c == PT_PASS) c = pt_class_curv(kx, kio.y, sb.z, ok);
+        } else {
+          c = pt_class_curv(kx, d.t3_k[t], sb.z, ok);
+        }
+      }
+      if (c == PT_PASS) {
+        const float z1 = d.seed_z1[ent.y];
+        c = pt_class_rz(d.cuts, s.x, s.y, z1, sb.w, kx, a, ok);
+        if (c == PT_PASS) c = pt_class_rz(d.cuts, s.x, s.y, z1, sb.w, kx, l, ok);
+      }
+      go = c != PT_FAIL;  // all cuts surely pass, or one of them cannot be decided here: the exact cuts decide
+    }
+    push_q(go, ent.y, ent.x);
   };
   for (;;) {
     unsigned near3 = 0, near5 = 0;  // candidates failing the gate near its threshold, this tile (one event)
@@ -216,226 +333,158 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     evi = __shfl_sync(kFull, evi, 0);
     if (tile >= n_tiles) break;
     const PtEvent ev = d.pt_ev[evi];
-    const int n_ab = (ev.a1 - ev.a0 + 31) / 32;
+    const int n_blk = (ev.a1 - ev.a0 + 31) / 32;
+    const int n_ch = (n_blk + kPtBlocks - 1) / kPtBlocks;
     const int local = tile - ev.tile0;
-    const int sb = local / n_ab, ab = local - sb * n_ab;
-    const int p0 = ev.s0 + sb * kSeedTile;
-    const int n_seed = min(kSeedTile, ev.s1 - p0);
-    for (int k = lane; k < n_seed; k += 32) {
-      const float4 a = d.seed_a[p0 + k], b = d.seed_b[p0 + k];
-      const float c1 = b.x * inv, c2 = b.x * gtol;
-      w.sa[k] = a;
-      w.sg[k] = make_float4(c1 + 1e-4f * fabsf(c1), c2 + 1e-4f * fabsf(c2), c1 - 1e-4f * fabsf(c1), c2 - 1e-4f * fabsf(c2));
-      w.sk[k] = make_float2(b.y, b.z);
-    }
-    const int anc = ev.a0 + ab * 32 + lane;
-    const bool valid = anc < ev.a1;
-    float4 A = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    int4 at = make_int4(0, 0, 0, 0);
-    if (valid) {
-      A = d.anc_a[anc];
-      at = d.anc_t[anc];
-    }
-    w.anc[lane] = A;
-    w.at[lane] = at;
-    __syncwarp();
-    // ---- (3) the rest of the approximate cascade for one entry of w2; what survives goes to the queue ----
-    auto tail = [&](int2 ent, bool active) {
-      bool go = false;
-      const int t = ent.x & 0x7fffffff, ks = ent.y & 0xffff, src = (ent.y >> 16) & 31;
-      const bool is5 = ent.x < 0;
-      if (active) {
-        const float4 s = w.sa[ks];
-        const float2 kt = w.sk[ks];
-        const float4 a = w.anc[src];
-        const float4 l = is5 ? d.t5_l[t] : d.t3_l[t];
-        bool ok;
-        const float kx = kx_approx(s.x, s.y, a.x, a.y, l.x, l.y, ok);
-        int c = pt_class_curv(kx, kt.x, kt.y, ok);
-        if (c == PT_PASS) {
-          if (is5) {
-            const float2 kio = d.t5_kio[t];
-            c = pt_class_curv(kx, kio.x, kt.y, ok);
-            if (c == PT_PASS) c = pt_class_curv(kx, kio.y, kt.y, ok);
-          } else {
-            c = pt_class_curv(kx, d.t3_k[t], kt.y, ok);
-          }
-        }
-        if (c == PT_PASS) {
-          const float z1 = d.seed_z1[p0 + ks], slope = d.seed_b[p0 + ks].w;
-          c = pt_class_rz(d.cuts, s.x, s.y, z1, slope, kx, a, ok);
-          if (c == PT_PASS) c = pt_class_rz(d.cuts, s.x, s.y, z1, slope, kx, l, ok);
-        }
-        go = c != PT_FAIL;  // all cuts surely pass, or one of them cannot be decided here: the exact cuts decide
-      }
-      push_q(go, p0 + ks, ent.x);
-    };
+    const int sg = local / n_ch, ch = local - sg * n_ch;
+    const int cbase = (ev.a0 >> 5) + evi;  // first bounding circle of the event's anchor blocks (k_anchor_sort)
+    // ---- this lane's seed (CUTS.md section 7: the per-seed quantities) ----
+    const int si = ev.s0 + sg * 32 + lane;
+    const bool has_seed = si < ev.s1;
+    const int p = d.seed_perm[has_seed ? si : ev.s1 - 1];
+    const float4 sa = d.seed_a[p], sgc = d.seed_g[p];
+    const float x1 = sa.x, y1 = sa.y, vx = sa.z, vy = sa.w;
+    // gate limit glim = lw (lw c1 + c2), c1 = lv INV_2RMIN, c2 = lv PT_GATE_TOL (both >= 0 when can_prune);
+    // loaded, not computed here, so that they stay in registers
+    const float c1 = sgc.x, c2 = sgc.y, kp = sgc.z, tolk = sgc.w;
+    const float lv2 = vx * vx + vy * vy;
+    const float lvh = lv2 * rsqrt_approx(lv2) * 1.001f;
+    const bool v_in_range = lv2 >= 1e-30f && lv2 <= 1e30f;
+    const float tband = 1.2e-5f * fabsf(tolk);  // pt_class_curv's band = tband + 4e-6 |kx~|
     int n2 = 0;
     // pushes up to one entry per lane onto w2; runs the cascade whenever 32 are waiting
-    auto push2 = [&](bool go, int cand, int tag) {
+    auto push2 = [&](bool go, int cand, int anc_pos) {
       const unsigned m = __ballot_sync(kFull, go);
       if (m == 0u) return;
-      if (go) w.w2[n2 + __popc(m & ((1u << lane) - 1u))] = make_int2(cand, tag);
+      if (go) w.w2[n2 + __popc(m & ((1u << lane) - 1u))] = make_int4(cand, p, anc_pos, 0);
       n2 += __popc(m);
       if (n2 >= 32) {
         __syncwarp();
         tail(w.w2[lane], true);
-        const int2 rest = (32 + lane < n2) ? w.w2[32 + lane] : make_int2(0, 0);
+        const int4 rest = (32 + lane < n2) ? w.w2[32 + lane] : make_int4(0, 0, 0, 0);
         __syncwarp();
         w.w2[lane] = rest;
         n2 -= 32;
         __syncwarp();
       }
     };
-    // ---- (2) expansion of up to 32 gate survivors into their (seed, T3) / (seed, T5) candidates, flattened
-    // over the lanes; kx~ against the seed's curvature decides which go on ----
-    auto expand = [&](int n_ent) {
-      int n_c = 0;
-      if (lane < n_ent) {
-        const int4 a = w.at[(w.w1[lane] >> 16) & 31];
-        n_c = a.y + a.w;
-      }
-      const int incl = warp_incl_scan(n_c);
-      const int excl = incl - n_c;
-      w.pref[lane] = excl;
-      const int T = __shfl_sync(kFull, incl, 31);
-      // item -> entry in O(1): one head bit per entry at the position of its first item; the entry of item
-      // `it` = number of head bits at or before it, minus one (bisection beyond 1024 items)
-      w.heads[lane] = 0u;
-      __syncwarp();
-      if (n_c > 0 && excl < 1024) atomicOr(&w.heads[excl >> 5], 1u << (excl & 31));
-      __syncwarp();
-      int heads_before = 0;
-      for (int i0 = 0; i0 < T; i0 += 32) {
-        const int it = i0 + lane;
-        bool go = false, direct = false;
-        int cand = 0, tag = 0;
-        const unsigned hw = i0 < 1024 ? w.heads[i0 >> 5] : 0u;
-        if (it < T) {
-          int lo;
-          if (i0 < 1024) {
-            lo = heads_before + __popc(hw & (0xffffffffu >> (31 - lane))) - 1;
-          } else {
-            lo = 0;
-            int hi = 32;  // largest e with pref[e] <= it
-#pragma unroll
-            for (int sft = 0; sft < 5; ++sft) {
-              const int mid = (lo + hi) >> 1;
-              if (w.pref[mid] <= it) lo = mid; else hi = mid;
-            }
-          }
-          const unsigned ent = w.w1[lo];
-          const int src = (ent >> 16) & 31, ks = ent & 0xffff, c = it - w.pref[lo];
-          const int4 a = w.at[src];
-          const bool is5 = c >= a.y;
-          const int t = is5 ? a.z + (c - a.y) : a.x + c;
-          cand = t | (is5 ? 0x80000000 : 0);
-          tag = ks | (src << 16);
-          if (ent >> 31) {
-            direct = true;  // the gate was near its threshold: every candidate of the pair is flagged by the exact cuts
-          } else {
-            const float4 s = w.sa[ks];
-            const float2 kt = w.sk[ks];
-            const float4 an = w.anc[src];
-            const float2 l = *reinterpret_cast<const float2*>(is5 ? d.t5_l + t : d.t3_l + t);
-            bool ok;
-            const float kx = kx_approx(s.x, s.y, an.x, an.y, l.x, l.y, ok);
-            go = pt_class_curv(kx, kt.x, kt.y, ok) != PT_FAIL;
-          }
-        }
-        heads_before += __popc(hw);
-        push_q(direct, p0 + (tag & 0xffff), cand);
-        push2(go, cand, tag);
-      }
-      __syncwarp();
-    };
-    int n1 = 0;  // gate survivors waiting in w.w1
-    // ---- bounding circle of the warp's anchors (sorted by radius class and azimuth: a few cm) ----
-    float bx0 = valid ? A.x : 3e38f, bx1 = valid ? A.x : -3e38f, by0 = valid ? A.y : 3e38f, by1 = valid ? A.y : -3e38f;
-#pragma unroll
-    for (int sh = 16; sh > 0; sh >>= 1) {
-      bx0 = fminf(bx0, __shfl_xor_sync(kFull, bx0, sh));
-      bx1 = fmaxf(bx1, __shfl_xor_sync(kFull, bx1, sh));
-      by0 = fminf(by0, __shfl_xor_sync(kFull, by0, sh));
-      by1 = fmaxf(by1, __shfl_xor_sync(kFull, by1, sh));
-    }
-    const bool warp_has = bx0 <= bx1;
-    const float bcx = 0.5f * (bx0 + bx1), bcy = 0.5f * (by0 + by1);
-    const float bh = 0.5f * sqrtf((bx1 - bx0) * (bx1 - bx0) + (by1 - by0) * (by1 - by0)) * 1.001f + 1e-3f;
-    // ---- (1) 32 seeds at a time ----
-    for (int kb = 0; kb < n_seed && warp_has; kb += 32) {
-      // (1a) one seed per lane against the circle: can its gate accept ANY point within bh of the centre?
-      //      gdot(A) <= v.wc + lv bh, gcrs(A) >= |v x wc| - lv bh, glim(A) <= glim at |wc| + bh (c1h, c2h >= 0
-      //      here); the 1e-4 inflation of c1h, c2h and the 1.001 factors cover the rounding of both sides.
-      //      Out of range: tested by every lane.
-      bool maybe = false;
-      if (kb + lane < n_seed) {
-        const float4 s = w.sa[kb + lane];
-        const float4 g = w.sg[kb + lane];
-        const float wx = bcx - s.x, wy = bcy - s.y;
+    const int b_end = min(n_blk, (ch + 1) * kPtBlocks);
+    for (int b = ch * kPtBlocks; b < b_end; ++b) {
+      const int anc0 = ev.a0 + b * 32;
+      const int nb = min(32, ev.a1 - anc0);
+      // ---- (1a) lanes as seeds: can this seed's gate accept ANY point within h of the centre (cx, cy)?
+      //      gdot(A) <= v.wc + lv h, gcrs(A) >= |v x wc| - lv h, glim(A) <= glim at |wc| + h (c1, c2 >= 0
+      //      here); the 1e-4 inflation of the limit and the 1.001 factors cover the rounding of both sides.
+      //      Out of range: every anchor is tested.  First the bounding circle of the block (k_anchor_sort),
+      //      then those of its four sub-blocks of 8 consecutive anchors. ----
+      auto circle = [&](float4 c) {
+        const float wx = c.x - x1, wy = c.y - y1;
         const float lw2 = wx * wx + wy * wy;
-        const float Lw = (lw2 * rsqrt_approx(lw2) + bh) * 1.001f;
-        const float lv2 = s.z * s.z + s.w * s.w;
-        const float lvh = lv2 * rsqrt_approx(lv2) * 1.001f;
-        const float slack = lvh * (bh * 1.001f + 1e-4f);
-        const float dotc = s.z * wx + s.w * wy;
-        const float crsc = fabsf(s.z * wy - s.w * wx);
-        const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f && lv2 >= 1e-30f && lv2 <= 1e30f;
-        maybe = !can_prune || !in_range || (dotc + slack > 0.0f && crsc - slack <= Lw * (Lw * g.x + g.y));
+        const float Lw = (lw2 * rsqrt_approx(lw2) + c.z) * 1.001f;
+        const float slack = lvh * (c.z * 1.001f + 1e-4f);
+        const float dotc = vx * wx + vy * wy;
+        const float crsc = fabsf(vx * wy - vy * wx);
+        const bool in_range = lw2 >= 1e-30f && lw2 <= 1e30f && v_in_range;
+        return !can_prune || !in_range || (dotc + slack > 0.0f && crsc - slack <= (Lw * (Lw * c1 + c2)) * 1.0001f);
+      };
+      const float4* __restrict__ circ = d.anc_c + 5 * (size_t)(cbase + b);
+      const bool maybe_b = has_seed && circle(__ldg(circ));
+      if (!__any_sync(kFull, maybe_b)) continue;
+      __syncwarp();
+      if (lane < nb) {  // lanes as anchors: the block goes to shared memory
+        w.anc[lane] = d.anc_a[anc0 + lane];
+        w.at[lane] = d.anc_t[anc0 + lane];
       }
-      unsigned word = __ballot_sync(kFull, maybe);
-      // (1b) the seeds that may match: every lane tests its own anchor
-      while (word) {
-        const int k = kb + __ffs(word) - 1;
-        word &= word - 1;
-        bool pass = false;
-        unsigned ent = 0u;
-        if (valid) {
-          const float4 s = w.sa[k];
-          const float4 g = w.sg[k];
-          const float wx = A.x - s.x, wy = A.y - s.y;
-          const float gdot = s.z * wx + s.w * wy;          // exactly the spec's gdot and gcrs (no FMA)
-          const float gcrs = fabsf(s.z * wy - s.w * wx);
+      __syncwarp();
+      // ---- (1b) the block's anchors one by one: gate of CUTS.md section 7 for this lane's seed ----
+      for (int j0 = 0; j0 < nb; j0 += 8) {
+        // a sub-block is skipped if no seed of the warp can match any of its anchors
+        const bool maybe = maybe_b && circle(__ldg(circ + 1 + (j0 >> 3)));
+        if (!__any_sync(kFull, maybe)) continue;
+        const int j1 = min(nb, j0 + 8);
+        for (int j = j0; j < j1; ++j) {
+          const float4 Aj = w.anc[j];
+          const int4 tj = w.at[j];
+          const float wx = Aj.x - x1, wy = Aj.y - y1;
+          const float gdot = vx * wx + vy * wy;          // exactly the spec's gdot and gcrs (no FMA)
+          const float gcrs = fabsf(vx * wy - vy * wx);
           const float lw2 = fmaf(wx, wx, wy * wy);
           const float lw = lw2 * rsqrt_approx(lw2);
           // three outcomes: surely rejected (dropped), surely accepted and not near-threshold (the exact gate
           // is skipped), uncertain = within 1e-4 of the threshold or out of the approximation's range (NaN
           // limits compare false both ways): the exact gate decides
-          pass = gdot > 0.0f && !(gcrs > lw * fmaf(lw, g.x, g.y));
-          if (pass && !(gcrs <= lw * fmaf(lw, g.z, g.w) && lw2 >= 1e-30f && lw2 <= 1e30f)) {
-            Seed sd;
-            sd.x1 = s.x;  sd.y1 = s.y;  sd.vx = s.z;  sd.vy = s.w;  sd.lv = d.seed_b[p0 + k].x;
-            const unsigned r = pt_gate(d.cuts, sd, A.x, A.y);
-            pass = (r & ACC) != 0;
-            if (!pass && (r & NEAR)) {  // every candidate of the anchor fails the gate near its threshold
-              near3 += (unsigned)at.y;
-              near5 += (unsigned)at.w;
+          const float G = lw * fmaf(lw, c1, c2);  // >= 0 when can_prune; within 1e-6 of the spec's glim
+          bool pass = maybe && gdot > 0.0f && !(can_prune && gcrs > G * 1.0001f);
+          const bool sure = can_prune && gcrs <= G * 0.9999f && lw2 >= 1e-30f && lw2 <= 1e30f;
+          if (!__any_sync(kFull, pass)) continue;
+          bool gnear = false;
+          if (__any_sync(kFull, pass && !sure)) {
+            if (pass && !sure) {
+              Seed sd;
+              sd.x1 = x1;  sd.y1 = y1;  sd.vx = vx;  sd.vy = vy;  sd.lv = d.seed_b[p].x;
+              const unsigned r = pt_gate(d.cuts, sd, Aj.x, Aj.y);
+              pass = (r & ACC) != 0;
+              gnear = (r & NEAR) != 0;
+              if (!pass && gnear) {  // every candidate of the anchor fails the gate near its threshold
+                near3 += (unsigned)tj.y;
+                near5 += (unsigned)tj.w;
+              }
             }
-            if (r & NEAR) ent = 0x80000000u;
+            // the gate passed near its threshold: every candidate of the pair is flagged by the exact cuts
+            unsigned dm = __ballot_sync(kFull, pass && gnear);
+            while (dm) {
+              const int src = __ffs(dm) - 1;
+              dm &= dm - 1;
+              const int pp = __shfl_sync(kFull, p, src);
+              for (int c0 = 0; c0 < tj.y + tj.w; c0 += 32) {
+                const int c = c0 + lane;
+                const bool in = c < tj.y + tj.w;
+                push_q(in, pp, c < tj.y ? tj.x + c : (tj.z + (c - tj.y)) | 0x80000000);
+              }
+            }
           }
-          ent |= (unsigned)k | ((unsigned)lane << 16);
-        }
-        // gate survivors onto the warp's list, in (seed, lane) order; a full warp of them is expanded at once
-        const unsigned m = __ballot_sync(kFull, pass);
-        if (m == 0u) continue;
-        if (pass) w.w1[n1 + __popc(m & ((1u << lane) - 1u))] = ent;
-        n1 += __popc(m);
-        if (n1 >= 32) {
-          __syncwarp();
-          expand(32);
-          const unsigned rest = (32 + lane < n1) ? w.w1[32 + lane] : 0u;
-          __syncwarp();
-          w.w1[lane] = rest;
-          n1 -= 32;
-          __syncwarp();
+          const bool active = pass && !gnear;
+          // ---- (2) the anchor's T3s, then its T5s: kx~ (lst_cuts_pt.cuh) with a = A - P1 and |a|^2 from the
+          // gate, one broadcast load per candidate.  A candidate is dropped if its curvature match with the seed
+          // surely fails, or -- behind a sure pass of that cut -- the match with its own stored curvature(s)
+          // surely fails (pt_class_curv's bands, written out as predicates); NaNs drop nothing. ----
+          const float4* __restrict__ q3 = d.t3_q + tj.x;
+          for (int c = 0; c < tj.y; ++c, ++q3) {
+            const float4 q = __ldg(q3);  // last MD x, y; k3; |AL|^2
+            const float cx = q.x - x1, cy = q.y - y1;
+            const float crs = wx * cy - wy * cx;  // the spec's crs (no FMA contraction in this translation unit)
+            const float prod = (lw2 * q.w) * fmaf(cx, cx, cy * cy);
+            const float kx = (crs + crs) * rsqrt_approx(prod);
+            const float band = fmaf(fabsf(kx), 4e-6f, tband);
+            const float hi = tolk + band, lo = tolk - band;
+            const float dp = fabsf(kx - kp), dt = fabsf(kx - q.z);
+            const bool ok = prod >= 1e-30f && prod <= 1e30f;
+            const bool drop = ok && (dp > hi || (dp < lo && dt > hi));
+            push2(active && !drop, tj.x + c, anc0 + j);
+          }
+          const float4* __restrict__ l5 = d.t5_l + tj.z;
+          const float2* __restrict__ k5 = d.t5_kio + tj.z;
+          for (int c = 0; c < tj.w; ++c, ++l5, ++k5) {
+            const float2 l = __ldg(reinterpret_cast<const float2*>(l5));
+            const float2 kio = __ldg(k5);
+            const float bx = l.x - Aj.x, by = l.y - Aj.y;
+            const float cx = l.x - x1, cy = l.y - y1;
+            const float crs = wx * cy - wy * cx;
+            const float prod = (lw2 * fmaf(bx, bx, by * by)) * fmaf(cx, cx, cy * cy);
+            const float kx = (crs + crs) * rsqrt_approx(prod);
+            const float band = fmaf(fabsf(kx), 4e-6f, tband);
+            const float hi = tolk + band, lo = tolk - band;
+            const float dp = fabsf(kx - kp), di = fabsf(kx - kio.x), dq = fabsf(kx - kio.y);
+            const bool ok = prod >= 1e-30f && prod <= 1e30f;
+            const bool drop = ok && (dp > hi || (dp < lo && (di > hi || (di < lo && dq > hi))));
+            push2(active && !drop, (tj.z + c) | 0x80000000, anc0 + j);
+          }
         }
       }
     }
-    __syncwarp();
-    if (n1 > 0) expand(n1);
     if (n2 > 0) {
       __syncwarp();
-      tail(lane < n2 ? w.w2[lane] : make_int2(0, 0), lane < n2);
+      tail(lane < n2 ? w.w2[lane] : make_int4(0, 0, 0, 0), lane < n2);
     }
     if (__any_sync(kFull, (near3 | near5) != 0u)) {
       const int s3 = warp_sum((int)near3), s5 = warp_sum((int)near5);

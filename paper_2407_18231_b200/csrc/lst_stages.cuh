@@ -110,6 +110,7 @@ struct StageT3 {
           d.t3_md[pos] = make_int4(ab.x, ab.y, C, eAB | (eC << 2));
           d.t3_k[pos] = k3;
           d.t3_l[pos] = pack_flag(c, eC);
+          d.t3_q[pos] = make_float4(c.x, c.y, k3, fmaf(c.x - a.x, c.x - a.x, (c.y - a.y) * (c.y - a.y)));
         }
         ++pos;
         ++cnt;

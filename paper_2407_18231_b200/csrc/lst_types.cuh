@@ -95,6 +95,7 @@ struct Dev {
   int4* t3_md;  // (A, B, C, endcap flags bit0 A, bit1 B, bit2 C)
   float* t3_k;
   float4* t3_l;  // last MD (x, y, z, r | endcap << 31): the operand of the seed linking's pre-filters
+  float4* t3_q;  // (x, y of the last MD, k3, |first MD - last MD|^2 in the transverse plane): one load per candidate in k_pt_eval
   // ---- a4: T5 (owner = first T3) ----
   int* t3_t5_begin;  // [n_t3 + 1]
   int2* t5_t3;
@@ -111,11 +112,15 @@ struct Dev {
   float4* seed_a;      // [n_pls] x1, y1, vx, vy           (CUTS.md section 7, computed once per seed)
   float4* seed_b;      // [n_pls] lv, kp, tolk, slope
   float* seed_z1;      // [n_pls]
+  float4* seed_g;      // [n_pls] lv INV_2RMIN, lv PT_GATE_TOL, kp, tolk: the per-lane constants of k_pt_eval
+  int* seed_perm;      // [n_pls] the seeds of every event in azimuth order (k_anchor_sort)
   PtEvent* pt_ev;      // [n_events + 1] anchor / seed ranges and first tile of every event
   int *anc_bin, *anc_rank;  // [n_md] bin (radial class * 64 + sector, -1 = no anchor) and arrival rank in the event's bin
   int* anc_bin_cnt;    // [n_events * 512] anchors per (event, bin) (zeroed per batch)
   float4* anc_a;       // [n_md] anchor (x, y, z, r | endcap << 31), the anchors of event e from mod_md_begin[e * n_mod] on
   int4* anc_t;         // [n_md] (first T3, number of T3s, first T5, number of T5s) starting at the anchor
+  float4* anc_c;       // [5 * (n_md / 32 + n_events + 1)] bounding circle (x, y, h) of every block of 32 sorted anchors, then of its 4 sub-blocks of 8
+  int* anc_done;       // [n_events] blocks of k_anchor_sort that have placed their share of the event (zeroed per batch)
   int2* pt_queue;      // candidates for the exact cuts: (seed, T3 / T5 index | T5 flag << 31)
   int *pls_pt3_cnt, *pls_pt5_cnt;  // [n_pls + 1] accepted per seed (zeroed per batch)
   int *pls_pt3_cur, *pls_pt5_cur;  // [n_pls] next free slot of a seed's range (zeroed per batch)
