@@ -53,6 +53,9 @@ def parse_args():
                          "metrics (PAPER.md:54-58, Figs. 3-4 in form) as JSON")
     ap.add_argument("--events", type=int, default=16, help="events per batch (= per step)")
     ap.add_argument("--streams", type=int, default=8, help="contexts / CUDA streams in flight")
+    ap.add_argument("--blocks-per-sm", type=int, default=2,
+                    help="lst_ctx_set_blocks_per_sm of every context: resident blocks per SM one kernel may take "
+                         "(8 = every kernel fills the GPU; 1-2 let kernels of different batches share the SMs)")
     ap.add_argument("--batches", type=int, default=6, help="distinct input batches rotated through")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-kernels-only", action="store_true",
@@ -248,6 +251,8 @@ def run_b200(args):
     caps = lst.lst_default_caps(max_events=E)
     streams = [torch.cuda.Stream() for _ in range(S)]
     ctxs = [lst.lst_ctx_create(g, caps, st.cuda_stream) for st in streams]
+    for c in ctxs:
+        lst.lst_ctx_set_blocks_per_sm(c, args.blocks_per_sm)
     sampler = ClockSampler(local)
     sampler.start()
 
@@ -336,65 +341,87 @@ def run_b200(args):
     alu_peak_tflops = 148 * 128 * sm_max_mhz * 1e6 / 1e12  # FP32 lanes x clock, no FMA (CUTS.md section 0)
     flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device="cuda")
     reps = 3 if args.profile_kernels_only else 12
-    lst.lst_ctx_set_timing(ctxs[0], True)
-    per_kernel = {}
-    order = []
-    ksum = None
+
+    def per_kernel_pass(blocks_per_sm):
+        """Single-stream loop with CUDA events between the kernels (no graph), L2 flushed before every batch."""
+        lst.lst_ctx_set_blocks_per_sm(ctxs[0], blocks_per_sm)
+        lst.lst_ctx_set_timing(ctxs[0], True)
+        per_kernel = {}
+        order = []
+        ksum = None
+        for r in range(reps + 2):
+            b = r % NB
+            with torch.cuda.stream(streams[0]):
+                if not os.environ.get("LST_BENCH_NO_FLUSH"):  # diagnostic only: warm-L2 kernel times
+                    flush.zero_()
+            lst.lst_ctx_run(ctxs[0], E, dev_in[b][0], dev_in[b][1])
+            s_b = lst.lst_ctx_sync(ctxs[0])
+            if r < 2:
+                continue  # warm-up
+            for name, t in lst.lst_ctx_kernel_times(ctxs[0]):
+                if name not in per_kernel:
+                    per_kernel[name] = []
+                    order.append(name)
+                w = algorithmic_work(name, s_b, n_sens)
+                per_kernel[name].append((t, w[0], w[1]))
+            ksum = s_b
+        lst.lst_ctx_set_timing(ctxs[0], False)
+        kernels = []
+        tot_ms = sum(float(np.mean([v[0] for v in per_kernel[n]])) for n in order)
+        for n in order:
+            t = float(np.mean([v[0] for v in per_kernel[n]]))
+            by = float(np.mean([v[1] for v in per_kernel[n]]))
+            fl = float(np.mean([v[2] for v in per_kernel[n]]))
+            gbs = by / (t * 1e-3) / 1e9 if t > 0 else 0.0
+            tf = fl / (t * 1e-3) / 1e12 if t > 0 else 0.0
+            kernels.append({"name": n, "ms": round(t, 5), "share": round(t / tot_ms, 4), "alg_bytes": int(by),
+                            "gbs": round(gbs, 1), "hbm_frac": round(gbs / hbm_gbs, 4), "alg_flops": int(fl),
+                            "tflops": round(tf, 3), "alu_frac": round(tf / alu_peak_tflops, 4)})
+        return kernels, ksum
+
     sampler.active.set()
-    for r in range(reps + 2):
-        b = r % NB
-        with torch.cuda.stream(streams[0]):
-            if not os.environ.get("LST_BENCH_NO_FLUSH"):  # diagnostic only: warm-L2 kernel times
-                flush.zero_()
-        lst.lst_ctx_run(ctxs[0], E, dev_in[b][0], dev_in[b][1])
-        s_b = lst.lst_ctx_sync(ctxs[0])
-        if r < 2:
-            continue  # warm-up
-        for name, t in lst.lst_ctx_kernel_times(ctxs[0]):
-            if name not in per_kernel:
-                per_kernel[name] = []
-                order.append(name)
-            w = algorithmic_work(name, s_b, n_sens)
-            per_kernel[name].append((t, w[0], w[1]))
-        ksum = s_b
+    kernels, ksum = per_kernel_pass(args.blocks_per_sm)  # the launch configuration of the timed region
+    kernels_alone = None
+    if not args.profile_kernels_only and args.blocks_per_sm not in (0, 8):
+        kernels_alone, _ = per_kernel_pass(8)            # every kernel filling the GPU on its own
+        lst.lst_ctx_set_blocks_per_sm(ctxs[0], args.blocks_per_sm)
     sampler.active.clear()
-    lst.lst_ctx_set_timing(ctxs[0], False)
-    kernels = []
-    tot_ms = sum(float(np.mean([v[0] for v in per_kernel[n]])) for n in order)
-    for n in order:
-        t = float(np.mean([v[0] for v in per_kernel[n]]))
-        by = float(np.mean([v[1] for v in per_kernel[n]]))
-        fl = float(np.mean([v[2] for v in per_kernel[n]]))
-        gbs = by / (t * 1e-3) / 1e9 if t > 0 else 0.0
-        tf = fl / (t * 1e-3) / 1e12 if t > 0 else 0.0
-        kernels.append({"name": n, "ms": round(t, 5), "share": round(t / tot_ms, 4), "alg_bytes": int(by),
-                        "gbs": round(gbs, 1), "hbm_frac": round(gbs / hbm_gbs, 4), "alg_flops": int(fl),
-                        "tflops": round(tf, 3), "alu_frac": round(tf / alu_peak_tflops, 4)})
-    top = max(kernels, key=lambda k: k["ms"])
-    if top["alu_frac"] >= top["hbm_frac"]:
-        roof = {"bound": "alu", "kernel": top["name"], "achieved": top["tflops"], "peak": round(alu_peak_tflops, 2),
-                "unit": "TFLOP/s", "frac": top["alu_frac"], "traffic": None,
-                "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, 1 flop/lane/clk (no FMA)" % sm_max_mhz}
-    else:
-        roof = {"bound": "hbm", "kernel": top["name"], "achieved": top["gbs"], "peak": hbm_gbs, "unit": "GB/s",
-                "frac": top["hbm_frac"], "traffic": None, "peak_source": peak_src + " copy bandwidth"}
     # DRAM traffic and executed warp instructions of the dominant kernel cannot be measured without a profiler:
     # they come from the committed ncu --set full capture (profiles/traffic.json), and only when that capture was
     # taken on this workload; the field says so
-    traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
-    roof["traffic_source"] = None
-    if os.path.exists(traffic_path):
-        with open(traffic_path) as f:
-            cap = json.load(f)
-        if cap.get("workload") == args.workload and cap.get("pu") == args.pu and cap.get("events") == E \
-                and top["name"] in cap.get("kernels", {}):
-            k = cap["kernels"][top["name"]]
-            roof["traffic"] = k.get("dram_bytes")
-            roof["traffic_source"] = "ncu capture %s (stored, not measured in this run)" % cap.get("capture", "?")
-            if k.get("warp_inst"):  # issue-rate roofline: 148 SMs x 4 schedulers x clock
-                issue_peak = 148 * 4 * sm_max_mhz * 1e6
-                roof["issue_frac"] = round(k["warp_inst"] / (top["ms"] * 1e-3) / issue_peak, 4)
-                roof["warp_inst"] = k["warp_inst"]
+    def make_roof(kernels):
+        top = max(kernels, key=lambda k: k["ms"])
+        if top["alu_frac"] >= top["hbm_frac"]:
+            roof = {"bound": "alu", "kernel": top["name"], "achieved": top["tflops"], "peak": round(alu_peak_tflops, 2),
+                    "unit": "TFLOP/s", "frac": top["alu_frac"], "traffic": None,
+                    "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, 1 flop/lane/clk (no FMA)" % sm_max_mhz}
+        else:
+            roof = {"bound": "hbm", "kernel": top["name"], "achieved": top["gbs"], "peak": hbm_gbs, "unit": "GB/s",
+                    "frac": top["hbm_frac"], "traffic": None, "peak_source": peak_src + " copy bandwidth"}
+        roof["ms"] = top["ms"]
+        traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
+        roof["traffic_source"] = None
+        if os.path.exists(traffic_path):
+            with open(traffic_path) as f:
+                cap = json.load(f)
+            if cap.get("workload") == args.workload and cap.get("pu") == args.pu and cap.get("events") == E \
+                    and top["name"] in cap.get("kernels", {}):
+                k = cap["kernels"][top["name"]]
+                roof["traffic"] = k.get("dram_bytes")
+                roof["traffic_source"] = "ncu capture %s (stored, not measured in this run)" % cap.get("capture", "?")
+                if k.get("warp_inst"):  # issue-rate roofline: 148 SMs x 4 schedulers x clock (SURVEY.md 8(d))
+                    issue_peak = 148 * 4 * sm_max_mhz * 1e6
+                    roof["issue_frac"] = round(k["warp_inst"] / (top["ms"] * 1e-3) / issue_peak, 4)
+                    roof["warp_inst"] = k["warp_inst"]
+        return roof
+
+    roof = make_roof(kernels)
+    roof["launch"] = "%d blocks per SM per kernel (the timed region's configuration), kernel alone on one stream" % (
+        args.blocks_per_sm or 8)
+    roof_alone = None
+    if kernels_alone:
+        roof_alone = make_roof(kernels_alone)
+        roof_alone["launch"] = "8 blocks per SM per kernel (every kernel fills the GPU), kernel alone on one stream"
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -421,6 +448,7 @@ def run_b200(args):
             "workload": workload_string(args),
             "events_per_step": E, "hits_per_event": int(np.mean(n_hits) / E), "pls_per_event": ksum["n_pls"] // E,
             "modules": int(geom.n_modules), "parallelism": "replicas x%d, no collective" % world,
+            "streams": S, "blocks_per_sm": args.blocks_per_sm,
             "l2": "inputs rotate over %d distinct batches + %d context workspaces (> 126 MB L2); per-kernel "
                   "times taken with an L2 flush (252 MB write) before every batch" % (NB, S),
             "objects_per_step": {k: ksum["n_" + k] for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
@@ -441,6 +469,8 @@ def run_b200(args):
         "clocks": sampler.summary(),
         "roofline": roof,
         "kernels": kernels,
+        "roofline_full_grid": roof_alone,
+        "kernels_full_grid": kernels_alone,
         "objects_per_s": {k: round(ksum["n_" + k] / (ms / args.steps * 1e-3), 1)
                           for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
         "cpu_baseline": cpu,

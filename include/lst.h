@@ -196,6 +196,15 @@ int lst_ctx_fetch_event(lst_ctx* ctx, int32_t event, lst_event_out** out);
  * batch holds more than cap_tc candidates. */
 int lst_ctx_fetch_tc(lst_ctx* ctx, int32_t* tc, int32_t cap_tc, int32_t* tc_event_offsets);
 
+/* How much of the GPU one kernel of this context may occupy: `blocks` = resident 256-thread blocks per SM
+ * (1..8; 0 = the default, 8: every kernel fills the GPU, best for a context that runs alone, e.g.
+ * lst_run_event).  Every kernel of the chain is a persistent ticket / grid-stride loop, so the grid size
+ * changes no result, only who shares the SMs: with several contexts in flight on different streams
+ * (PAPER.md:79 ran 2 streams; BASELINE.json configs[4] "pipelined over CUDA streams") kernels of different
+ * batches co-reside and hide each other's latency when each takes 1-2 blocks per SM.  May be called
+ * between batches (the captured launch sequence is rebuilt).  Returns LST_ERR_ARG for blocks outside 0..8. */
+int lst_ctx_set_blocks_per_sm(lst_ctx* ctx, int32_t blocks);
+
 /* Per-kernel device times of the last batch, measured with CUDA events on the context's stream.
  * enable != 0 switches the recording on for the following lst_ctx_run calls. */
 int lst_ctx_set_timing(lst_ctx* ctx, int32_t enable);

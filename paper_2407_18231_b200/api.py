@@ -165,6 +165,11 @@ def lst_ctx_fetch_tc(ctx, tc_buf: np.ndarray, n_events: int):
     return tc_buf[: off[-1]], off
 
 
+def lst_ctx_set_blocks_per_sm(ctx, blocks: int) -> None:
+    """Resident blocks per SM a kernel of this context may take (include/lst.h); 0 = default (fill the GPU)."""
+    _check(_lib().lst_ctx_set_blocks_per_sm(ctx, int(blocks)), "lst_ctx_set_blocks_per_sm")
+
+
 def lst_ctx_set_timing(ctx, enable: bool) -> None:
     _check(_lib().lst_ctx_set_timing(ctx, int(bool(enable))), "lst_ctx_set_timing")
 

@@ -70,7 +70,8 @@ struct lst_ctx {
   std::vector<int> last_hit_off, last_pls_off;
   int last_n_events;
   bool synced;
-  int grid_md, grid_ls, grid_pt;  // resident blocks of the three heavy kernels (occupancy x SMs)
+  int occ_md, occ_ls, occ_pt;  // resident blocks per SM of the three heavy kernels (occupancy)
+  int blocks_per_sm;           // lst_ctx_set_blocks_per_sm (default 8 = fill the GPU)
   // timing
   bool timing;
   cudaEvent_t ev[kMaxKernels + 1];
@@ -227,6 +228,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.tstate[T_PP3] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_T4] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
+  d.tstate[T_LSE] = nullptr;  // ticket only
   d.sens_cnt = b.take<int>(n_sens + 1);
   d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins);
   d.anc_done = b.take<int>(c.max_events);
@@ -237,6 +239,8 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.tc_cnt = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
   d.tc_cur = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
   d.linked = b.take<unsigned char>(c.max_pls);
+  d.ls_cnt = b.take<int>(c.max_md);
+  d.ls_cur = b.take<int>(c.max_md);
   b.off = (b.off + 255) & ~size_t(255);
   if (zero_bytes) *zero_bytes = b.off;
   // --- a0 ---
@@ -261,8 +265,6 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.md_a = b.take<float4>(c.max_md);
   d.md_u = b.take<float2>(c.max_md);
   d.md_ls_begin = b.take<int>((size_t)c.max_md + 1);
-  d.ls_cnt = b.take<int>(c.max_md);
-  d.ls_sbase = b.take<int>(c.max_md);
   d.ls_md = b.take<int2>(c.max_ls);
   d.ls_kappa = b.take<float>(c.max_ls);
   d.ls_t3_begin = b.take<int>((size_t)c.max_ls + 1);
@@ -437,9 +439,10 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
     ctx_destroy(ctx);
     return LST_ERR_CUDA;
   }
-  ctx->grid_md = g->n_sm * occ_md;
-  ctx->grid_ls = g->n_sm * occ_ls;
-  ctx->grid_pt = g->n_sm * occ_pt;
+  ctx->occ_md = occ_md;
+  ctx->occ_ls = occ_ls;
+  ctx->occ_pt = occ_pt;
+  ctx->blocks_per_sm = 8;
   *out = ctx;
   return LST_OK;
 }

@@ -34,8 +34,14 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   const lst_geometry* g = ctx->g;
   const Dev& d = ctx->dev;
   const int mask = g->cuts.stage_mask;
-  const int gp = g->n_sm * 4;  // persistent ticket / grid-stride kernels
-  const int gw = g->n_sm * 8;
+  // resident blocks per SM a kernel of this context may take (lst_ctx_set_blocks_per_sm): the streaming
+  // kernels take all of them, the ticket kernels half, the three heavy kernels what their occupancy allows
+  const int bps = ctx->blocks_per_sm;
+  const int gw = g->n_sm * bps;
+  const int gp = g->n_sm * (bps > 1 ? bps / 2 : 1);
+  const int g_md = g->n_sm * (ctx->occ_md < bps ? ctx->occ_md : bps);
+  const int g_ls = g->n_sm * (ctx->occ_ls < bps ? ctx->occ_ls : bps);
+  const int g_pt = g->n_sm * (ctx->occ_pt < bps ? ctx->occ_pt : bps);
   CK(cudaMemsetAsync(ctx->zero_region, 0, ctx->zero_bytes, st));
   L.mark("hist");
   k_hist<<<gw, kBlock, 0, st>>>(d);
@@ -45,11 +51,11 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   L.mark("scatter");
   k_scatter<<<gw, kBlock, 0, st>>>(d);
   L.mark("md");
-  k_md_eval<<<ctx->grid_md, kBlock, 0, st>>>(d);
+  k_md_eval<<<g_md, kBlock, 0, st>>>(d);
   L.mark("md_place");
   k_md_place<<<gw, kBlock, 0, st>>>(d);
   L.mark("ls");
-  k_ls_eval<<<ctx->grid_ls, kBlock, 0, st>>>(d);
+  k_ls_eval<<<g_ls, kBlock, 0, st>>>(d);
   L.mark("ls_place");
   k_ls_place<<<gp, kBlock, 0, st>>>(d);
   L.mark("t3");
@@ -63,7 +69,7 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   L.mark("anchor_sort");
   k_anchor_sort<<<ctx->caps.max_events * kAncBlocksPerEvent, kBlock, 0, st>>>(d);
   L.mark("pt");
-  k_pt_eval<<<ctx->grid_pt, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
+  k_pt_eval<<<g_pt, kBlock, sizeof(PtWarp) * kWarps, st>>>(d);
   L.mark("pt_exact");
   k_pt_exact<<<gp, kBlock, 0, st>>>(d);
   L.mark("pt_scan");
@@ -242,6 +248,17 @@ extern "C" int lst_ctx_sync(lst_ctx* ctx, lst_batch_summary* s) {
   }
   if (h.error & E_BAD_SENSOR) return LST_ERR_ARG;
   if (h.error) return LST_ERR_CAPACITY;
+  return LST_OK;
+}
+
+extern "C" int lst_ctx_set_blocks_per_sm(lst_ctx* ctx, int32_t blocks) {
+  if (!ctx || ctx->magic != MAGIC_CTX || blocks < 0 || blocks > 8) return LST_ERR_ARG;
+  const int b = blocks == 0 ? 8 : blocks;
+  if (b != ctx->blocks_per_sm && ctx->graph) {  // the captured launch sequence holds the old grids
+    cudaGraphExecDestroy(ctx->graph);
+    ctx->graph = nullptr;
+  }
+  ctx->blocks_per_sm = b;
   return LST_OK;
 }
 

@@ -2,18 +2,18 @@
 //
 // Candidates of an inner MD A: the MDs of every module in conn[module(A)] (the CSR row of the
 // precomputed connection map).  A PU200 batch holds 2.1e5 MDs, rows of 7.7 targets on average and
-// 1.4 MDs per target: 5e6 candidate pairs in 1.6e6 tiny (MD, target) lists.  Flattening the pairs of
-// the whole batch (an earlier engine, profiles/r01_v2_even_split.md) costs more in decoding (pair -> module -> MD -> row edge -> B: ~290 thread
-// instructions per pair, ncu) than the cuts themselves (~40), because a 32-pair step crosses a
-// module boundary almost every time.  Here the unit is the list:
-//   * a warp takes 8 consecutive inner MDs and builds, once, the table of their (MD, target) lists
-//     in shared memory (first candidate, length prefix): the CSR walk is done once per list;
-//   * the ~180 candidate pairs of the 8 MDs are then taken 32 at a time (pair -> list through a
-//     bit mask of list starts, inner-MD operands from shared memory), so lanes stay busy
-//     whatever the list lengths; accepted (B, kappa) pairs are compacted in pair order with one
-//     ballot per step and copied to a scratch list with one atomic per warp pass (a pass with more
-//     than kLsStage LSs evaluates its pairs again and writes directly);
-//   * k_ls_place scans the per-MD counts into md_ls_begin (fused, look-back) and copies each MD's LSs to their slot.
+// 1.4 MDs per target: 5e6 candidate pairs.  All inner MDs of a module share the same candidates, so the
+// unit of work is the MODULE (the "thread group per module" of north_star, here a warp):
+//   * a warp takes kLsModules modules by ticket and handles the non-empty ones one by one;
+//   * the module's row is walked ONCE: lanes = targets, their MD ranges are concatenated (prefix sum) and
+//     taken 32 at a time, one candidate B per lane, its operands loaded into registers;
+//   * the module's inner MDs are then a warp-uniform loop (A broadcast, no pair decoding): the first cut
+//     of the approximate list (ls_class: curvature) runs here and drops 73 % of the pairs;
+//   * survivors queue up (across modules) and take the rest of ls_class, then the exact cuts of CUTS.md
+//     section 4, on full warps; accepted (A, B, kappa) go to a scratch list with one atomic per 32 LSs and
+//     a count per inner MD;
+//   * k_ls_place scans the per-MD counts into md_ls_begin (tiles by ticket + look-back), waits until every
+//     tile is done, and moves the LSs to their slot (one cursor per inner MD).
 // LSs therefore sit grouped by inner MD (what T3 building looks up); the order inside an MD's range
 // is free (reading S9).
 #pragma once
@@ -21,29 +21,21 @@
 
 namespace lst {
 
-constexpr int kLsOwners = 8;    // inner MDs per warp
-constexpr int kLsRanges = 256;  // (MD, target) lists per warp pass; also the longest row supported
-constexpr int kLsStage = 96;    // staged LSs per warp pass
-constexpr int kLsHeadWords = 64;
+constexpr int kLsRanges = 256;  // longest connection-map row accepted by lst_load_geometry
+constexpr int kLsModules = 4;   // modules per ticket (the non-empty ones are handled one after the other)
+constexpr int kLsStride = 1187; // module-index distance between the modules of a ticket
 
 struct LsAccepted {
-  int B;
+  int A, B;
   float kappa;
 };
 
-struct LsWarp {  // per-warp scratch in shared memory
-  float4 a[kLsOwners];
-  float2 u[kLsOwners];
-  int e[kLsOwners];
-  int cnt[kLsOwners];
-  int dex[kLsOwners + 1];  // exclusive prefix of the row lengths
-  int k0[kLsOwners];
-  int gb[kLsOwners];       // event * n_mod
-  int pref[kLsRanges + 1];  // exclusive prefix of the list lengths
-  int b0[kLsRanges];        // first MD of the list | endcap(target) << 27 | owner slot << 28
-  unsigned heads[kLsHeadWords];  // bit p set = a list starts at pair p (pairs below 32 * kLsHeadWords)
-  int2 cq[64];                   // pairs the pre-filter could not reject: (B, owner slot | endcap(B) << 8), in pair order
-  LsAccepted stage[kLsStage];
+struct LsWarp {    // per-warp scratch in shared memory
+  int pref[33];    // exclusive prefix of the MD counts of the round's 32 targets
+  int b0[32];      // first MD of each target | endcap(target) << 30
+  int2 q1[64];     // pairs behind the curvature cut: (A, B | endcap(B) << 30)
+  int2 q2[64];     // pairs the approximate list could not reject
+  LsAccepted acc[64];
 };
 
 __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
@@ -51,180 +43,173 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
   __shared__ LsWarp s_w[kWarps];
   __shared__ unsigned s_tests[2 * kEvSmem];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned below = (1u << lane) - 1u;
   LsWarp& w = s_w[warp];
   EvTests tbl;
   tbl.init(s_tests, d.ev_cnt, 1, d.n_events);
   const bool on = (d.cuts.stage_mask & 2) != 0;
-  const int n_md = d.ctl->total[K_MD];
+  const int n_gm = on && d.ctl->total[K_MD] > 0 ? d.n_events * d.n_mod : 0;
   const int cap = d.cap[K_LS];
   LsAccepted* scratch = reinterpret_cast<LsAccepted*>(d.ev_scratch);
-  for (int A0 = (blockIdx.x * kWarps + warp) * kLsOwners; A0 < n_md; A0 += gridDim.x * kWarps * kLsOwners) {
-    // ---- lanes 0..7: one inner MD each ----
-    const int A = A0 + lane;
-    int k0 = 0, deg = 0, gm_base = 0;
-    if (lane < kLsOwners && A < n_md && on) {
-      const int info = d.md_info[A];
-      const int gm = info >> 1;
-      const int ev = gm / d.n_mod;
-      w.a[lane] = d.md_a[A];
-      w.u[lane] = d.md_u[A];
-      w.e[lane] = info & 1;
-      k0 = __ldg(d.conn_off + (gm - ev * d.n_mod));
-      deg = __ldg(d.conn_off + (gm - ev * d.n_mod) + 1) - k0;
-      gm_base = ev * d.n_mod;
+  int n1 = 0, n2 = 0, n3 = 0;  // entries waiting in q1, q2, acc
+  // ---- accepted LSs -> scratch list (one atomic per flush) and the count of their inner MD ----
+  auto flush = [&](int n_now) {
+    int base = 0;
+    if (lane == 0) base = atomicAdd(&d.ctl->scratch_cur[1], n_now);
+    base = __shfl_sync(kFull, base, 0);
+    if (lane < n_now) {
+      const LsAccepted a = w.acc[lane];
+      if (base + lane < cap) scratch[base + lane] = a;
+      atomicAdd(d.ls_cnt + a.A, 1);
     }
-    const int dincl = warp_incl_scan(deg);  // rows of the 8 MDs, concatenated
-    if (lane < kLsOwners) {
-      w.dex[lane] = dincl - deg;
-      w.k0[lane] = k0;
-      w.gb[lane] = gm_base;
+  };
+  // ---- the exact cuts of CUTS.md section 4 on up to 32 queued pairs ----
+  auto exact = [&](int n_now) {
+    unsigned res = 0;
+    LsAccepted a{0, 0, 0.0f};
+    if (lane < n_now) {
+      const int2 q = w.q2[lane];
+      a.A = q.x;
+      a.B = q.y & 0x3fffffff;
+      const int infoA = d.md_info[a.A];
+      res = ls_test(d.cuts, d.md_a[a.A], d.md_u[a.A], infoA & 1, d.md_a[a.B], d.md_u[a.B], (q.y >> 30) & 1, a.kappa);
+      if (res & NEAR) count_near(d.ev_cnt, (infoA >> 1) / d.n_mod, 1);
     }
-    if (lane == kLsOwners - 1) w.dex[kLsOwners] = dincl;
+    const unsigned m = __ballot_sync(kFull, res & ACC);
+    if (m == 0u) return;
+    if (res & ACC) w.acc[n3 + __popc(m & below)] = a;
+    n3 += __popc(m);
     __syncwarp();
-    int first = 0;                          // MDs [first, first + take) are handled per pass
-    while (first < kLsOwners) {
-      const int d_first = w.dex[first];
-      // as many MDs as fit the range table (a single row always fits: lst_load_geometry checks)
-      const unsigned fit = __ballot_sync(kFull, lane >= first && lane < kLsOwners && dincl - d_first <= kLsRanges);
-      const int take = __popc(fit >> first & ~((fit >> first) + 1u)) ;  // length of the run of ones starting at `first`
-      const int last = first + take;  // exclusive
-      const int R = w.dex[last] - d_first;
-      const bool one_event = w.gb[first] == w.gb[last - 1];  // the MDs of the pass belong to one event (nearly always)
-      if (lane < kLsOwners) w.cnt[lane] = 0;
-      // ---- table of the non-empty lists (owner, target e) in row order, and their head bits ----
-      for (int k = lane; k < kLsHeadWords; k += 32) w.heads[k] = 0u;
+    if (n3 >= 32) {
+      flush(32);
+      const LsAccepted rest = (32 + lane < n3) ? w.acc[32 + lane] : a;
       __syncwarp();
-      int carry = 0, Rn = 0;
-      for (int r0 = 0; r0 < R; r0 += 32) {
-        const int r = r0 + lane;
+      w.acc[lane] = rest;
+      n3 -= 32;
+      __syncwarp();
+    }
+  };
+  // ---- the approximate cut list (ls_class) on up to 32 pairs behind the curvature cut ----
+  auto second = [&](int n_now) {
+    bool go = false;
+    int2 q = make_int2(0, 0);
+    if (lane < n_now) {
+      q = w.q1[lane];
+      const int B = q.y & 0x3fffffff;
+      go = ls_class(d.cuts, d.md_a[q.x], d.md_u[q.x], d.md_info[q.x] & 1, d.md_a[B], d.md_u[B], (q.y >> 30) & 1) != PT_FAIL;
+    }
+    const unsigned m = __ballot_sync(kFull, go);
+    if (m == 0u) return;
+    if (go) w.q2[n2 + __popc(m & below)] = q;
+    n2 += __popc(m);
+    __syncwarp();
+    if (n2 >= 32) {
+      exact(32);
+      const int2 rest = (32 + lane < n2) ? w.q2[32 + lane] : q;
+      __syncwarp();
+      w.q2[lane] = rest;
+      n2 -= 32;
+      __syncwarp();
+    }
+  };
+  const int n_tickets = (n_gm + kLsModules - 1) / kLsModules;
+  for (;;) {
+    int ticket = 0;
+    if (lane == 0) ticket = atomicAdd(d.ctl->ticket + T_LSE, 1);
+    ticket = __shfl_sync(kFull, ticket, 0);
+    if (ticket >= n_tickets) break;
+    // ---- kLsModules modules, one per lane, from different parts of the module table (neighbouring modules,
+    // and the same module in different events, are equally busy: a ticket gets a mix); the non-empty ones
+    // are handled one by one ----
+    const int gm_l = lane * n_tickets + (int)(((long long)ticket + (long long)lane * kLsStride) % n_tickets);
+    int A0_l = 0, A1_l = 0;
+    if (lane < kLsModules && gm_l < n_gm) {
+      A0_l = d.mod_md_begin[gm_l];
+      A1_l = d.mod_md_begin[gm_l + 1];
+    }
+    unsigned todo = __ballot_sync(kFull, A1_l > A0_l);
+    while (todo) {
+      const int src = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const int gm = __shfl_sync(kFull, gm_l, src);
+      const int A0 = __shfl_sync(kFull, A0_l, src), A1 = __shfl_sync(kFull, A1_l, src);
+      const int ev = gm / d.n_mod, gb = ev * d.n_mod, mod = gm - gb;
+      const int k0 = __ldg(d.conn_off + mod), deg = __ldg(d.conn_off + mod + 1) - k0;
+      for (int r0 = 0; r0 < deg; r0 += 32) {
+        // ---- the row, 32 targets at a time: lanes = targets, their MD ranges concatenated ----
         int n_t = 0, ent = 0;
-        if (r < R) {
-          int o = first;  // owner slot of list r: last o with (dex[o] - d_first) <= r
-          for (int k = first + 1; k < last; ++k)
-            if (w.dex[k] - d_first <= r) o = k;
-          const int e = r - (w.dex[o] - d_first);
-          const int m2 = __ldg(d.conn_tgt + w.k0[o] + e);
-          const int gb = w.gb[o];
+        if (r0 + lane < deg) {
+          const int m2 = __ldg(d.conn_tgt + k0 + r0 + lane);
           const int B0 = d.mod_md_begin[gb + m2];
           n_t = d.mod_md_begin[gb + m2 + 1] - B0;
-          ent = B0 | ((__ldg(d.subdet + m2) != 0) << 27) | (o << 28);
-          if (!one_event) tbl.add(gb / d.n_mod, (unsigned)n_t);
+          ent = B0 | ((__ldg(d.subdet + m2) != 0) << 30);
         }
         const int incl = warp_incl_scan(n_t);
-        const unsigned nz = __ballot_sync(kFull, n_t > 0);
-        if (n_t > 0) {
-          const int idx = Rn + __popc(nz & ((1u << lane) - 1u));
-          const int start = carry + incl - n_t;
-          w.pref[idx] = start;
-          w.b0[idx] = ent;
-          if (start < 32 * kLsHeadWords) atomicOr(&w.heads[start >> 5], 1u << (start & 31));
-        }
-        Rn += __popc(nz);
-        carry += __shfl_sync(kFull, incl, 31);
-      }
-      const int P = carry;
-      if (lane == 0) w.pref[Rn] = P;
-      __syncwarp();
-      if (one_event && lane == 0) tbl.add(w.gb[first] / d.n_mod, (unsigned)P);
-      // ---- pairs of the pass, 32 at a time: the approximate cut list (ls_class) drops 95 % of them; the rest
-      // queue up in pair order and take the exact cuts of CUTS.md section 4 on full warps.  Pass 1 runs only
-      // if the stage overflowed: it evaluates the pairs again and writes straight to the scratch list. ----
-      int base = 0, run = 0;
-      for (int pass = 0; pass < 2; ++pass) {
-        run = 0;
-        int heads_before = 0, n_c = 0;
-        auto exact = [&](int n_now) {  // lanes below n_now take one queued pair each
-          unsigned res = 0;
-          LsAccepted acc;
-          int o = 0;
-          if (lane < n_now) {
-            const int2 q = w.cq[lane];
-            o = q.y & 0xff;
-            acc.B = q.x;
-            res = ls_test(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[acc.B], d.md_u[acc.B], (q.y >> 8) & 1, acc.kappa);
-          }
-          if (pass == 0 && (res & NEAR)) count_near(d.ev_cnt, w.gb[o] / d.n_mod, 1);
-          const unsigned m = __ballot_sync(kFull, res & ACC);
-          if (res & ACC) {
-            const int pos = run + __popc(m & ((1u << lane) - 1u));
-            if (pass == 0) {
-              if (pos < kLsStage) w.stage[pos] = acc;
-              atomicAdd(&w.cnt[o], 1);
-            } else if (base + pos < cap) {
-              scratch[base + pos] = acc;
-            }
-          }
-          run += __popc(m);
-        };
-        for (int p0 = 0; p0 < P; p0 += 32) {
-          const int p = p0 + lane;
-          bool go = false;
-          int2 q = make_int2(0, 0);
-          const unsigned hw = p0 < 32 * kLsHeadWords ? w.heads[p0 >> 5] : 0u;
-          if (p < P) {
-            int lo;  // list of pair p: the last list starting at or before p
-            if (p0 < 32 * kLsHeadWords) {
-              lo = heads_before + __popc(hw & (0xffffffffu >> (31 - lane))) - 1;
-            } else {
-              lo = 0;
-              int hi = Rn;
-              while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                if (w.pref[mid] <= p) lo = mid; else hi = mid;
-              }
-            }
-            const int ent = w.b0[lo];
-            const int o = (unsigned)ent >> 28, eB = (ent >> 27) & 1;
-            q.x = (ent & 0x7ffffff) + (p - w.pref[lo]);
-            q.y = o | (eB << 8);
-            go = ls_class(d.cuts, w.a[o], w.u[o], w.e[o] != 0, d.md_a[q.x], d.md_u[q.x], eB != 0) != PT_FAIL;
-          }
-          heads_before += __popc(hw);
-          const unsigned m = __ballot_sync(kFull, go);
-          if (m == 0u) continue;
-          if (go) w.cq[n_c + __popc(m & ((1u << lane) - 1u))] = q;
-          n_c += __popc(m);
-          if (n_c >= 32) {
-            __syncwarp();
-            exact(32);
-            const int2 rest = (32 + lane < n_c) ? w.cq[32 + lane] : make_int2(0, 0);
-            __syncwarp();
-            w.cq[lane] = rest;
-            n_c -= 32;
-            __syncwarp();
-          }
-        }
-        if (n_c > 0) {
-          __syncwarp();
-          exact(n_c);
-        }
-        if (pass == 1) break;
-        // ---- one atomic for the pass; per-MD count and scratch position ----
-        if (lane == 0 && run > 0) base = atomicAdd(&d.ctl->scratch_cur[1], run);
-        base = __shfl_sync(kFull, base, 0);
+        const int NB = __shfl_sync(kFull, incl, 31);
+        if (NB == 0) continue;
         __syncwarp();
-        const int c = (lane >= first && lane < last) ? w.cnt[lane] : 0;
-        const int cincl = warp_incl_scan(c);
-        if (lane >= first && lane < last && A < n_md) {
-          d.ls_cnt[A] = c;
-          d.ls_sbase[A] = base + cincl - c;
+        w.pref[lane] = incl - n_t;
+        w.b0[lane] = ent;
+        if (lane == 31) w.pref[32] = NB;
+        __syncwarp();
+        if (lane == 0) {  // candidates of CUTS.md section 4: (MDs of the module) x (MDs of its targets)
+          const unsigned long long t64 = (unsigned long long)(A1 - A0) * (unsigned long long)NB;
+          if (t64 < (1ull << 32)) tbl.add(ev, (unsigned)t64);
+          else atomicAdd(d.ev_cnt + (size_t)ev * kEvCnt + kStages + 1, t64);
         }
-        if (run <= kLsStage) {
-          for (int k = lane; k < run; k += 32)
-            if (base + k < cap) scratch[base + k] = w.stage[k];
-          break;
+        for (int c0 = 0; c0 < NB; c0 += 32) {
+          // ---- one candidate B per lane: target = the last list starting at or before c0 + lane ----
+          const int i = c0 + lane;
+          const bool has = i < NB;
+          int lo = 0;
+#pragma unroll
+          for (int step = 16; step > 0; step >>= 1)
+            if (w.pref[lo + step] <= i) lo += step;
+          const int e = w.b0[lo];
+          const int B = has ? (e & 0x3fffffff) + (i - w.pref[lo]) : A0;
+          const int tagB = B | (e & 0x40000000);
+          const float4 b = d.md_a[B];
+          // ---- the module's inner MDs, warp-uniform: first cut of ls_class (|kappa| R_MIN <= LS_KAPPA_MAX), same
+          // arithmetic and band; a pair is dropped only if that cut surely fails ----
+          for (int A = A0; A < A1; ++A) {
+            const float4 a = __ldg(d.md_a + A);
+            const float ex = b.x - a.x, ey = b.y - a.y;
+            const float c2 = fmaf(ex, ex, ey * ey);
+            const float crs = a.x * b.y - a.y * b.x;
+            const float rr = a.w * b.w;
+            const float den2 = (rr * rr) * c2;
+            const bool ok = den2 >= 1e-30f && den2 <= 1e30f && c2 >= 1e-30f && c2 <= 1e30f && rr >= 0.0f;
+            const float kv = fabsf((2.0f * crs) * rsqrt_approx(den2)) * d.cuts.r_min;
+            const bool go = has && classify(kv, d.cuts.ls_kappa_max, 2e-5f * fabsf(d.cuts.ls_kappa_max) + 3e-6f * kv, ok) != PT_FAIL;
+            const unsigned m = __ballot_sync(kFull, go);
+            if (m == 0u) continue;
+            if (go) w.q1[n1 + __popc(m & below)] = make_int2(A, tagB);
+            n1 += __popc(m);
+            __syncwarp();
+            if (n1 >= 32) {
+              second(32);
+              const int2 rest = (32 + lane < n1) ? w.q1[32 + lane] : make_int2(0, 0);
+              __syncwarp();
+              w.q1[lane] = rest;
+              n1 -= 32;
+              __syncwarp();
+            }
+          }
         }
       }
-      __syncwarp();  // the tables are reused by the next pass
-      first = last;
     }
   }
+  // ---- drain the queues ----
+  if (n1 > 0) second(n1);
+  if (n2 > 0) exact(n2);
+  if (n3 > 0) flush(n3);
   tbl.flush();
 }
 
-// Placement with the exclusive scan of ls_cnt fused in (tiles of kBlock inner MDs by ticket, block scan +
-// look-back): every MD's LSs go from the scratch list to their final slot, md_ls_begin is written on the
-// way.  Rides along: the four list heads of every MD of the duplicate-removal index are cleared.
+// Placement.  Phase 1: exclusive scan of ls_cnt into md_ls_begin (tiles of kBlock inner MDs by ticket, block
+// scan + look-back); rides along: the four list heads of every MD of the duplicate-removal index are
+// cleared.  Phase 2, once every tile is done (all tiles are taken by running blocks before any block gets
+// here, so the wait cannot deadlock): every LS of the scratch list goes to the next free slot of its inner MD.
 __global__ void __launch_bounds__(kBlock) k_ls_place(Dev d) {
   load_batch(d);
   __shared__ int s_tile;
@@ -250,12 +235,6 @@ __global__ void __launch_bounds__(kBlock) k_ls_place(Dev d) {
       d.idx_head[n_md + A] = 0;
       d.idx_head[2 * n_md + A] = 0;
       d.idx_head[3 * n_md + A] = 0;
-      const int src = d.ls_sbase[A];
-      for (int k = 0; k < n; ++k) {
-        const LsAccepted s = scratch[src + k];
-        d.ls_md[dst + k] = make_int2(A, s.B);
-        d.ls_kappa[dst + k] = s.kappa;
-      }
     }
     if (tile == n_tiles - 1 && threadIdx.x == 0) {
       d.md_ls_begin[n_md] = tb + tt;
@@ -266,6 +245,21 @@ __global__ void __launch_bounds__(kBlock) k_ls_place(Dev d) {
         d.ctl->total[K_LS] = total;
       }
     }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) atomicAdd(&d.ctl->ls_tiles_done, 1);
+  }
+  if (!fits) return;
+  if (threadIdx.x == 0) {
+    while (atomicAdd(&d.ctl->ls_tiles_done, 0) < n_tiles) __nanosleep(64);
+    __threadfence();
+  }
+  __syncthreads();
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+    const LsAccepted s = scratch[i];
+    const int pos = __ldcg(d.md_ls_begin + s.A) + atomicAdd(d.ls_cur + s.A, 1);
+    d.ls_md[pos] = make_int2(s.A, s.B);
+    d.ls_kappa[pos] = s.kappa;
   }
 }
 

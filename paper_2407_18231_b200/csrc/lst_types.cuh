@@ -15,7 +15,7 @@ namespace lst {
 struct PtEvent;  // lst_pt.cuh
 
 enum Kind { K_MD = 0, K_LS, K_T3, K_T5, K_PT3, K_PT5, K_TC, K_T4, K_NKINDS };
-enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT, T_PP3, T_PP5, T_T4, T_N };
+enum Tkt { T_SENS = 0, T_MD, T_LS, T_T3, T_T5, T_PT, T_PP3, T_PP5, T_T4, T_LSE, T_N };
 
 enum ErrBit { E_BAD_SENSOR = 1, E_CAP_MD = 2, E_CAP_LS = 4, E_CAP_T3 = 8, E_CAP_T5 = 16,
               E_CAP_PT3 = 32, E_CAP_PT5 = 64, E_CAP_TC = 128, E_CAP_T4 = 256 };
@@ -33,7 +33,8 @@ struct Ctl {
   int done_rule;                     // blocks of the last rule kernel that have finished (the last one scans tc_cnt)
   int scratch_cur[4];                // accepted objects in the scratch lists: [1] LS, [2] pT3, [3] pT5
   int queue_cur;                     // entries of the exact-evaluation queue of the seed linking
-  int pad[3];
+  int ls_tiles_done;                 // scan tiles of k_ls_place that are finished
+  int pad[1];
 };
 
 // What changes from batch to batch: sizes and input pointers.  Lives in device memory (copied in front of
@@ -86,7 +87,7 @@ struct Dev {
   float2* md_u;       // unit direction (barrel), 0 (endcap)
   // ---- a2: LS (owner = inner MD) ----
   int* md_ls_begin;  // [n_md + 1]
-  int *ls_cnt, *ls_sbase;  // [n_md] LSs of an inner MD and their position in the scratch list
+  int *ls_cnt, *ls_cur;  // [n_md] LSs of an inner MD, and the next free slot of its range (both zeroed per batch)
   int2* ls_md;       // (md_in, md_out) batch-global MD indices
   float* ls_kappa;
   // ---- a3: T3 (owner = first LS) ----

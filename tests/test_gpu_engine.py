@@ -181,6 +181,30 @@ def test_randomised_batches(lst, oracle_mod):
         lst.lst_free(g)
 
 
+def test_blocks_per_sm_changes_no_result(lst, oracle_mod):
+    """lst_ctx_set_blocks_per_sm (include/lst.h): every kernel is a ticket / grid-stride loop, so the grid size
+    changes who shares the SMs, never a result.  One context, grids of 1, 2, 3 and 8 blocks per SM in turn
+    (the captured launch sequence is rebuilt each time); out-of-range values are argument errors."""
+    geom, off, tgt = make_config_geometry("C4")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=3))
+    try:
+        evs = [make_config_event("C4"), make_config_event("C2"), make_config_event("C4")]
+        want = [canon(oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)) for ev in evs]
+        for blocks in (1, 2, 3, 8, 0, 1):
+            lst.lst_ctx_set_blocks_per_sm(ctx, blocks)
+            for rep in range(2):  # the second run replays the captured graph
+                run_batch(lst, ctx, evs)
+                for i in range(len(evs)):
+                    assert_same(canon(lst.lst_ctx_fetch_event(ctx, i)), want[i], f"{blocks} blocks per SM, event {i}: ")
+        for bad in (-1, 9):
+            with pytest.raises(lst.LstError):
+                lst.lst_ctx_set_blocks_per_sm(ctx, bad)
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
 def test_many_small_events_in_one_batch(lst, oracle_mod):
     """40 events per launch sequence (more events than any table is sized for by default)."""
     geom, off, tgt = make_config_geometry("C4")
