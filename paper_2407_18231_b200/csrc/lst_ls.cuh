@@ -22,7 +22,7 @@
 namespace lst {
 
 constexpr int kLsRanges = 256;  // longest connection-map row accepted by lst_load_geometry
-constexpr int kLsModules = 4;   // modules per ticket (the non-empty ones are handled one after the other)
+constexpr int kLsModules = 4;   // modules per ticket (the non-empty ones are handled one after the other); fewer in small batches
 constexpr int kLsStride = 1187; // module-index distance between the modules of a ticket
 
 struct LsAccepted {
@@ -112,7 +112,9 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
       __syncwarp();
     }
   };
-  const int n_tickets = (n_gm + kLsModules - 1) / kLsModules;
+  // modules per ticket: kLsModules, fewer when that leaves less than two tickets per warp (a small batch)
+  const int mpt = max(1, min(kLsModules, n_gm / (2 * (int)gridDim.x * kWarps)));
+  const int n_tickets = (n_gm + mpt - 1) / mpt;
   for (;;) {
     int ticket = 0;
     if (lane == 0) ticket = atomicAdd(d.ctl->ticket + T_LSE, 1);
@@ -123,7 +125,7 @@ __global__ void __launch_bounds__(kBlock) k_ls_eval(Dev d) {
     // are handled one by one ----
     const int gm_l = lane * n_tickets + (int)(((long long)ticket + (long long)lane * kLsStride) % n_tickets);
     int A0_l = 0, A1_l = 0;
-    if (lane < kLsModules && gm_l < n_gm) {
+    if (lane < mpt && gm_l < n_gm) {
       A0_l = d.mod_md_begin[gm_l];
       A1_l = d.mod_md_begin[gm_l + 1];
     }

@@ -66,7 +66,8 @@ struct PtCand {
   }
 };
 
-constexpr int kPtBlocks = 2;           // anchor blocks (of 32 sorted anchors) per tile
+constexpr int kPtBlocks = 2;           // anchor blocks (of 32 sorted anchors) per tile; 1 when that leaves fewer than kPtMinTiles tiles
+constexpr int kPtMinTiles = 12288;     // about two tiles per resident warp of k_pt_eval
 constexpr int kSeedSectors = 128;       // azimuth sectors of the seed sort
 constexpr int kAncBlocksPerEvent = 8;   // blocks of k_anchor_sort per event
 
@@ -222,8 +223,7 @@ __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
       pe.a0 = on ? d.mod_md_begin[ev * d.n_mod] : 0;
       pe.a1 = pe.a0 + n_a;
       const int ns = on ? pe.s1 - pe.s0 : 0;
-      const int n_blk = (n_a + 31) / 32;
-      pe.tile0 = ((n_blk + kPtBlocks - 1) / kPtBlocks) * ((ns + 31) / 32);  // warp tiles; prefix below
+      pe.tile0 = 0;  // first tile: prefix below
       d.pt_ev[ev] = pe;
       int c0 = 0, c1 = 0;
       if (on) {  // candidates of CUTS.md section 7: every (seed, T3) and (seed, T5) of the event
@@ -237,14 +237,23 @@ __global__ void __launch_bounds__(kBlock) k_anchor_sort(Dev d) {
     }
   }
   __syncthreads();
-  if (threadIdx.x == 0) {  // exclusive prefix of the tile counts (n_events is small)
+  if (threadIdx.x == 0) {  // blocks per tile, and the exclusive prefix of the tile counts (n_events is small)
+    auto tiles_of = [&](int ev, int K) {
+      const PtEvent pe = d.pt_ev[ev];
+      const int n_blk = (pe.a1 - pe.a0 + 31) / 32, ns = on ? pe.s1 - pe.s0 : 0;
+      return ((n_blk + K - 1) / K) * ((ns + 31) / 32);
+    };
+    long long t2 = 0;
+    for (int ev = 0; ev < E; ++ev) t2 += tiles_of(ev, kPtBlocks);
+    const int K = t2 >= kPtMinTiles ? kPtBlocks : 1;  // a small batch: shorter tiles, more warps busy
     int a = 0;
     for (int ev = 0; ev < E; ++ev) {
-      const int ta = d.pt_ev[ev].tile0;
+      const int ta = tiles_of(ev, K);
       d.pt_ev[ev].tile0 = a;
       a += ta;
     }
     d.pt_ev[E].tile0 = a;
+    d.pt_ev[E].a0 = K;
   }
 }
 
@@ -273,6 +282,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
   PtWarp& w = reinterpret_cast<PtWarp*>(s_dyn)[warp];
   const int E = d.n_events;
   const int n_tiles = d.pt_ev[E].tile0;
+  const int K = d.pt_ev[E].a0;  // anchor blocks per tile (k_anchor_sort)
   const int cap_q = d.cap_queue;
   const float inv = d.cuts.inv_2rmin, gtol = d.cuts.pt_gate_tol;
   // the circle test bounds the gate limit at |w| + h, which needs a limit growing with |w|
@@ -334,7 +344,7 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
     if (tile >= n_tiles) break;
     const PtEvent ev = d.pt_ev[evi];
     const int n_blk = (ev.a1 - ev.a0 + 31) / 32;
-    const int n_ch = (n_blk + kPtBlocks - 1) / kPtBlocks;
+    const int n_ch = (n_blk + K - 1) / K;
     const int local = tile - ev.tile0;
     const int sg = local / n_ch, ch = local - sg * n_ch;
     const int cbase = (ev.a0 >> 5) + evi;  // first bounding circle of the event's anchor blocks (k_anchor_sort)
@@ -368,8 +378,8 @@ __global__ void __launch_bounds__(kBlock) k_pt_eval(Dev d) {
         __syncwarp();
       }
     };
-    const int b_end = min(n_blk, (ch + 1) * kPtBlocks);
-    for (int b = ch * kPtBlocks; b < b_end; ++b) {
+    const int b_end = min(n_blk, (ch + 1) * K);
+    for (int b = ch * K; b < b_end; ++b) {
       const int anc0 = ev.a0 + b * 32;
       const int nb = min(32, ev.a1 - anc0);
       // ---- (1a) lanes as seeds: can this seed's gate accept ANY point within h of the centre (cx, cy)?
