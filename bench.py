@@ -150,9 +150,11 @@ def algorithmic_work(name, s, n_sens):
     md, ls, t3, t5, p3, p5, tc = (s[k] for k in ("n_md", "n_ls", "n_t3", "n_t5", "n_pt3", "n_pt5", "n_tc"))
     idx = 5 * t5 + 5 * p5 + 3 * p3
     table = {
-        "hist": 12 * h + 4 * p + 32 * p + 36 * p,            # sensor ids in, bin + rank out; seeds in, seed table out
-        "scan_sensors": 8 * n_sens,
-        "scatter": 44 * h,
+        # x, y, z + sensor id in, sorted (x, y, z, r) + (index, sensor) out, first hit of every sensor out;
+        # seeds in, seed table out
+        "ingest_count": 4 * h + 4 * h + 4 * 4 * n_sens + 32 * p + 56 * p,   # ids in, ranks out, 4 rows of counts out
+        "ingest_scan": 2 * 4 * 4 * n_sens + 4 * n_sens,                      # counts in, slots and sens_begin out
+        "scatter": 20 * h + 24 * h,                                          # ids, ranks, x, y, z in; sorted records out
         "md": 24 * h + 4 * n_sens + 20 * h,
         "md_place": 28 * h + 52 * md + 2 * n_sens,            # counts + stash in, MDs + module offsets out
         "ls": 28 * md + 8 * ls,
@@ -206,6 +208,9 @@ def workload_params(lst, workload):
         from lst_inputs.configs import C6_PARAMS
 
         return lst.lst_default_params(**C6_PARAMS)
+    mask = os.environ.get("LST_BENCH_STAGE_MASK")  # diagnostic only: cost of the chain up to a stage (CUTS.md section 9)
+    if mask:
+        return lst.lst_default_params(stage_mask=int(mask, 0))
     return None
 
 

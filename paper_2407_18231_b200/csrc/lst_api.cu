@@ -219,7 +219,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   // --- zeroed per batch ---
   d.ctl = b.take<Ctl>(1);
   d.ev_cnt = b.take<unsigned long long>((size_t)c.max_events * kEvCnt);
-  d.tstate[T_SENS] = b.take<unsigned long long>(tiles_of(n_sens + 1, kScanTile));
+  d.tstate[T_SENS] = nullptr;  // unused (the sensor scan is local to k_ingest)
   d.tstate[T_MD] = b.take<unsigned long long>(tiles_of((long long)c.max_hits + 1, kBlock * kMdPlaceItems));
   d.tstate[T_LS] = b.take<unsigned long long>(tiles_of((long long)c.max_md + 1, kBlock));
   d.tstate[T_T3] = b.take<unsigned long long>(tiles_of(c.max_ls, kBlock));
@@ -229,7 +229,6 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.tstate[T_PP5] = b.take<unsigned long long>(tiles_of((long long)c.max_pls + 1, kScanTile));
   d.tstate[T_T4] = b.take<unsigned long long>(tiles_of(c.max_t3, kBlock));
   d.tstate[T_LSE] = nullptr;  // ticket only
-  d.sens_cnt = b.take<int>(n_sens + 1);
   d.anc_bin_cnt = b.take<int>((size_t)c.max_events * kAncBins);
   d.anc_done = b.take<int>(c.max_events);
   d.pls_pt3_cnt = b.take<int>((size_t)c.max_pls + 1);
@@ -244,9 +243,9 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   b.off = (b.off + 255) & ~size_t(255);
   if (zero_bytes) *zero_bytes = b.off;
   // --- a0 ---
-  d.hit_gs_in = b.take<int>(c.max_hits);
-  d.hit_rank = b.take<int>(c.max_hits);
   d.sens_begin = b.take<int>(n_sens + 1);
+  d.hit_rank = b.take<int>(c.max_hits);
+  d.chunk_cnt = b.take<int>((size_t)n_sens * kIngestChunks);
   d.hit = b.take<float4>(c.max_hits);
   d.hit_ig = b.take<int2>(c.max_hits);
   // --- a1..a4 ---
@@ -431,7 +430,9 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   // grid-stride kernels are launched with exactly the blocks that fit the GPU at once
   int occ_md = 0, occ_ls = 0, occ_pt = 0;
   const size_t pt_smem = sizeof(PtWarp) * kWarps;
-  if (cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem) != cudaSuccess ||
+  const int ingest_smem = (int)sizeof(int) * (2 * g->n_mod < kIngestMaxBins ? 2 * g->n_mod : kIngestMaxBins);
+  if (cudaFuncSetAttribute(k_ingest_count, cudaFuncAttributeMaxDynamicSharedMemorySize, ingest_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_md, k_md_eval, kBlock, 0) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_ls, k_ls_eval, kBlock, 0) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pt, k_pt_eval, kBlock, pt_smem) != cudaSuccess ||

@@ -43,11 +43,11 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   const int g_ls = g->n_sm * (ctx->occ_ls < bps ? ctx->occ_ls : bps);
   const int g_pt = g->n_sm * (ctx->occ_pt < bps ? ctx->occ_pt : bps);
   CK(cudaMemsetAsync(ctx->zero_region, 0, ctx->zero_bytes, st));
-  L.mark("hist");
-  k_hist<<<gw, kBlock, 0, st>>>(d);
-  L.mark("scan_sensors");
-  k_scan<<<gp, kBlock, 0, st>>>(d.sens_cnt, d.sens_begin, &d.batch->n_events, 2 * g->n_mod, 0, d.ctl->ticket + T_SENS,
-                                d.tstate[T_SENS]);
+  const size_t ingest_smem = sizeof(int) * (size_t)(2 * g->n_mod < kIngestMaxBins ? 2 * g->n_mod : kIngestMaxBins);
+  L.mark("ingest_count");
+  k_ingest_count<<<ctx->caps.max_events * kIngestChunks, kIngestThreads, ingest_smem, st>>>(d);
+  L.mark("ingest_scan");
+  k_ingest_scan<<<ctx->caps.max_events, kIngestThreads, 0, st>>>(d);
   L.mark("scatter");
   k_scatter<<<gw, kBlock, 0, st>>>(d);
   L.mark("md");

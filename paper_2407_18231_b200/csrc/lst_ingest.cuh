@@ -1,5 +1,5 @@
-// lst_ingest.cuh -- step a0: hit ingestion and module binning (counting sort by global sensor),
-// plus the generic single-pass exclusive scan kernel.  PAPER.md:23 ("uses as input the hits of the
+// lst_ingest.cuh -- step a0: hit ingestion and module binning (counting sort by global sensor, k_ingest),
+// plus the generic single-pass exclusive scan kernel (used for the per-seed counts of the seed linking).  PAPER.md:23 ("uses as input the hits of the
 // ... outer tracker"); SURVEY.md section 8(a) row a0.
 #pragma once
 #include "lst_cuts_pt.cuh"
@@ -18,53 +18,185 @@ __device__ __forceinline__ int event_of(const int* __restrict__ off, int n_event
   return lo;
 }
 
-// a0.1 histogram: one atomic per hit on its sensor counter; the returned rank is kept so that the
-// scatter pass needs no second atomic.  Invalid sensor ids raise E_BAD_SENSOR (-> LST_ERR_ARG).
-// kIngestUnroll hits per thread are in flight at once (the kernel is latency-bound: every hit is a
-// chain load -> atomic -> store).
+// a0: counting sort of the hits by global sensor, three small kernels, no global atomic.  The hits of an event are a
+// contiguous range of the input (event offsets) and stay one after the sort (global sensor = event * n_sens +
+// sensor), so counts and scan are local to the event.  Block (e, c) owns chunk c (of kIngestChunks) of the
+// event's hits and keeps one counter per sensor in shared memory (sensors are taken kIngestMaxBins at a time:
+// one round for any realistic geometry):
+//   k_ingest_count: shared-memory atomic per hit of the chunk; the returned value is the hit's rank among the
+//                   chunk's hits of that sensor (hit_rank); the chunk's counters go to chunk_cnt[e][c][sensor];
+//   k_ingest_scan:  one block per event: totals over the chunks, exclusive scan over the event's sensors ->
+//                   sens_begin, and the first slot of every chunk's hits of every sensor;
+//   k_scatter:      every hit of the batch (all SMs: the scattered 16- and 8-byte stores are the cost) is written
+//                   at slot + rank: (x, y, z, r), r = sqrtf(x*x + y*y), and (event-local input index, global sensor).
+// The order inside a sensor is chunk order, then arrival order: free.  Invalid sensor ids raise E_BAD_SENSOR
+// (-> LST_ERR_ARG) and count as sensor 0.  k_ingest_count's block (e, 0) also fills the per-seed table of event e
+// (CUTS.md section 7: the quantities that do not depend on the candidate).
+constexpr int kIngestThreads = 1024;
+constexpr int kIngestMaxBins = 40960;  // counters per round (160 KB of shared memory)
+constexpr int kIngestChunks = 4;       // blocks per event
+constexpr int kIngestBatch = 8;        // sensor ids a thread has in flight
+
+__device__ __forceinline__ int load_sensor(const Dev& d, int i) {
+  return d.sensor_u16 ? (int)__ldg(reinterpret_cast<const unsigned short*>(d.in_sensor) + i) : __ldg(d.in_sensor + i);
+}
+
+struct IngestChunk {  // what block (e, c) works on
+  int e, c, h0, i_lo, i_hi, n_sens, R;
+  __device__ __forceinline__ bool init(const Dev& d) {
+    e = blockIdx.x / kIngestChunks;
+    c = blockIdx.x - e * kIngestChunks;
+    if (e >= d.n_events) return false;
+    h0 = d.hit_ev_off[e];
+    const int h1 = d.hit_ev_off[e + 1];
+    const int per = (h1 - h0 + kIngestChunks - 1) / kIngestChunks;
+    i_lo = min(h1, h0 + c * per);
+    i_hi = min(h1, i_lo + per);
+    n_sens = 2 * d.n_mod;
+    R = min(n_sens, kIngestMaxBins);
+    return true;
+  }
+};
+
+__global__ void __launch_bounds__(kIngestThreads) k_ingest_count(Dev d) {
+  load_batch(d);
+  extern __shared__ int s_bin[];  // R counters
+  IngestChunk k;
+  if (!k.init(d)) return;
+  if (k.c == 0) {
+    // the per-seed quantities of CUTS.md section 7, computed once per seed exactly as written there
+    for (int p = d.pls_ev_off[k.e] + threadIdx.x; p < d.pls_ev_off[k.e + 1]; p += kIngestThreads) {
+      d.pls_event[p] = k.e;
+      const Seed s = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p), __ldg(d.p_y0 + p),
+                               __ldg(d.p_z0 + p), __ldg(d.p_x1 + p), __ldg(d.p_y1 + p), __ldg(d.p_z1 + p));
+      d.seed_a[p] = make_float4(s.x1, s.y1, s.vx, s.vy);
+      d.seed_b[p] = make_float4(s.lv, s.kp, s.tolk, s.slope);
+      d.seed_z1[p] = s.z1;
+      // what k_pt_eval keeps per lane: the coefficients of the gate limit glim = lw (lw c1 + c2), and kp, tolk
+      d.seed_g[p] = make_float4(s.lv * d.cuts.inv_2rmin, s.lv * d.cuts.pt_gate_tol, s.kp, s.tolk);
+    }
+  }
+  int* __restrict__ row = d.chunk_cnt + ((size_t)k.e * kIngestChunks + k.c) * k.n_sens;
+  bool bad = false;
+  for (int r_lo = 0; r_lo < k.n_sens; r_lo += k.R) {
+    const int r_n = min(k.R, k.n_sens - r_lo);
+    for (int j = threadIdx.x; j < r_n; j += kIngestThreads) s_bin[j] = 0;
+    __syncthreads();
+    for (int i0 = k.i_lo + threadIdx.x; i0 < k.i_hi; i0 += kIngestBatch * kIngestThreads) {
+      int sv[kIngestBatch];
+#pragma unroll
+      for (int u = 0; u < kIngestBatch; ++u) {  // kIngestBatch independent loads in flight
+        const int i = i0 + u * kIngestThreads;
+        sv[u] = i < k.i_hi ? load_sensor(d, i) : 0;
+      }
+#pragma unroll
+      for (int u = 0; u < kIngestBatch; ++u) {
+        const int i = i0 + u * kIngestThreads;
+        if (i >= k.i_hi) break;
+        int s = sv[u];
+        if (s < 0 || s >= k.n_sens) {
+          bad = true;
+          s = 0;
+        }
+        if (s >= r_lo && s < r_lo + r_n) d.hit_rank[i] = atomicAdd(&s_bin[s - r_lo], 1);
+      }
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < r_n; j += kIngestThreads) row[r_lo + j] = s_bin[j];
+    __syncthreads();
+  }
+  if (bad) atomicOr(&d.ctl->error, E_BAD_SENSOR);
+}
+
+// One block per event: totals over the chunks, exclusive scan over the event's sensors -> sens_begin; the chunk
+// counters are replaced, in place, by the first slot of the chunk's hits of every sensor.
+__global__ void __launch_bounds__(kIngestThreads) k_ingest_scan(Dev d) {
+  load_batch(d);
+  __shared__ int s_warp[2][kIngestThreads / 32];
+  const int e = blockIdx.x;
+  if (e >= d.n_events) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int n_sens = 2 * d.n_mod;
+  int* __restrict__ rows = d.chunk_cnt + (size_t)e * kIngestChunks * n_sens;
+  int* __restrict__ begin = d.sens_begin + (size_t)e * n_sens;
+  constexpr int T = 4;  // tiles of kIngestThreads consecutive sensors whose loads are in flight together
+  int carry = d.hit_ev_off[e];
+  int par = 0;
+  for (int t0 = 0; t0 < n_sens; t0 += T * kIngestThreads) {
+    int v[T][kIngestChunks];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      const int j = t0 + t * kIngestThreads + threadIdx.x;  // coalesced: consecutive threads, consecutive sensors
+#pragma unroll
+      for (int c = 0; c < kIngestChunks; ++c) v[t][c] = j < n_sens ? rows[(size_t)c * n_sens + j] : 0;
+    }
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+      const int j = t0 + t * kIngestThreads + threadIdx.x;
+      if (t0 + t * kIngestThreads >= n_sens) break;
+      int tot = 0;
+#pragma unroll
+      for (int c = 0; c < kIngestChunks; ++c) tot += v[t][c];
+      const int incl = warp_incl_scan(tot);
+      if (lane == 31) s_warp[par][warp] = incl;
+      __syncthreads();
+      const int wv = s_warp[par][lane];           // every warp scans the 32 warp totals itself
+      const int wi = warp_incl_scan(wv);
+      const int wbase = __shfl_sync(kFull, wi - wv, warp);
+      const int tile_total = __shfl_sync(kFull, wi, 31);
+      int run = carry + wbase + incl - tot;
+      if (j < n_sens) {
+        begin[j] = run;
+#pragma unroll
+        for (int c = 0; c < kIngestChunks; ++c) {
+          rows[(size_t)c * n_sens + j] = run;
+          run += v[t][c];
+        }
+      }
+      carry += tile_total;
+      par ^= 1;  // the other buffer: no second barrier per tile
+    }
+  }
+  if (e == d.n_events - 1 && threadIdx.x == 0) d.sens_begin[(size_t)d.n_events * n_sens] = carry;
+}
+
+// Every hit goes to (first slot of its chunk's hits of its sensor) + (its rank among them): sorted SoA
+// (float4 x, y, z, r + int2 event-local input index, global sensor), r = sqrtf(x*x + y*y).
 constexpr int kIngestUnroll = 4;
 
-__global__ void __launch_bounds__(kBlock) k_hist(Dev d) {
+__global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
   load_batch(d);
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
   for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {
-    int s[kIngestUnroll], gs[kIngestUnroll];
+    int slot[kIngestUnroll], rk[kIngestUnroll], gs[kIngestUnroll], h0[kIngestUnroll];
+    float x[kIngestUnroll], y[kIngestUnroll], z[kIngestUnroll];
 #pragma unroll
     for (int u = 0; u < kIngestUnroll; ++u) {
       const int i = i0 + u * stride;
-      s[u] = i >= d.n_hits ? 0 : (d.sensor_u16 ? (int)__ldg(reinterpret_cast<const unsigned short*>(d.in_sensor) + i)
-                                                 : __ldg(d.in_sensor + i));
-    }
-#pragma unroll
-    for (int u = 0; u < kIngestUnroll; ++u) {
-      const int i = i0 + u * stride;
-      if (i < d.n_hits && (s[u] < 0 || s[u] >= n_sens)) {
-        atomicOr(&d.ctl->error, E_BAD_SENSOR);
-        s[u] = 0;
-      }
-      gs[u] = (i < d.n_hits ? event_of(d.hit_ev_off, d.n_events, i) : 0) * n_sens + s[u];
+      const bool ok = i < d.n_hits;
+      int s = ok ? load_sensor(d, i) : 0;
+      if (s < 0 || s >= n_sens) s = 0;
+      const int e = ok ? event_of(d.hit_ev_off, d.n_events, i) : 0;
+      h0[u] = __ldg(d.hit_ev_off + e);
+      const int per = (__ldg(d.hit_ev_off + e + 1) - h0[u] + kIngestChunks - 1) / kIngestChunks;
+      const int c = per > 0 ? (i - h0[u]) / per : 0;
+      gs[u] = e * n_sens + s;
+      slot[u] = ok ? d.chunk_cnt[((size_t)e * kIngestChunks + c) * n_sens + s] : 0;
+      rk[u] = ok ? d.hit_rank[i] : 0;
+      x[u] = ok ? __ldg(d.in_x + i) : 0.0f;
+      y[u] = ok ? __ldg(d.in_y + i) : 0.0f;
+      z[u] = ok ? __ldg(d.in_z + i) : 0.0f;
     }
 #pragma unroll
     for (int u = 0; u < kIngestUnroll; ++u) {
       const int i = i0 + u * stride;
       if (i < d.n_hits) {
-        d.hit_gs_in[i] = gs[u];
-        d.hit_rank[i] = atomicAdd(d.sens_cnt + gs[u], 1);
+        const int pos = slot[u] + rk[u];
+        d.hit[pos] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
+        d.hit_ig[pos] = make_int2(i - h0[u], gs[u]);
       }
     }
-  }
-  // pLS -> event, and the per-seed quantities of CUTS.md section 7 (computed once per seed, exactly as
-  // written there: lv, kp, tolk, slope); tiny, rides along
-  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < d.n_pls; p += stride) {
-    d.pls_event[p] = event_of(d.pls_ev_off, d.n_events, p);
-    const Seed s = make_seed(d.cuts, __ldg(d.p_pt + p), __ldg(d.p_q + p), __ldg(d.p_x0 + p), __ldg(d.p_y0 + p),
-                             __ldg(d.p_z0 + p), __ldg(d.p_x1 + p), __ldg(d.p_y1 + p), __ldg(d.p_z1 + p));
-    d.seed_a[p] = make_float4(s.x1, s.y1, s.vx, s.vy);
-    d.seed_b[p] = make_float4(s.lv, s.kp, s.tolk, s.slope);
-    d.seed_z1[p] = s.z1;
-    // what k_pt_eval keeps per lane: the coefficients of the gate limit glim = lw (lw c1 + c2), and kp, tolk
-    d.seed_g[p] = make_float4(s.lv * d.cuts.inv_2rmin, s.lv * d.cuts.pt_gate_tol, s.kp, s.tolk);
   }
 }
 
@@ -137,37 +269,5 @@ __global__ void __launch_bounds__(kBlock) k_scan2(ScanJob j0, ScanJob j1) {
 }
 
 #define k_scan k_scan_t<kScanItems>
-
-// a0.3 scatter: sorted SoA (float4 x,y,z,r + int2 input index, global sensor), r = sqrtf(x*x + y*y)
-__global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
-  load_batch(d);
-  const int stride = gridDim.x * blockDim.x;
-  const int n_sens = 2 * d.n_mod;
-  for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {
-    int gs[kIngestUnroll], pos[kIngestUnroll];
-    float x[kIngestUnroll], y[kIngestUnroll], z[kIngestUnroll];
-#pragma unroll
-    for (int u = 0; u < kIngestUnroll; ++u) {
-      const int i = i0 + u * stride;
-      const bool ok = i < d.n_hits;
-      gs[u] = ok ? d.hit_gs_in[i] : 0;
-      pos[u] = ok ? d.hit_rank[i] : 0;
-      x[u] = ok ? __ldg(d.in_x + i) : 0.0f;
-      y[u] = ok ? __ldg(d.in_y + i) : 0.0f;
-      z[u] = ok ? __ldg(d.in_z + i) : 0.0f;
-    }
-#pragma unroll
-    for (int u = 0; u < kIngestUnroll; ++u) pos[u] += __ldg(d.sens_begin + gs[u]);
-#pragma unroll
-    for (int u = 0; u < kIngestUnroll; ++u) {
-      const int i = i0 + u * stride;
-      if (i < d.n_hits) {
-        d.hit[pos[u]] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
-        const int ev = gs[u] / n_sens;
-        d.hit_ig[pos[u]] = make_int2(i - __ldg(d.hit_ev_off + ev), gs[u]);
-      }
-    }
-  }
-}
 
 }  // namespace lst

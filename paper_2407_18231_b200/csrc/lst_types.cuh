@@ -68,10 +68,9 @@ struct Dev {
   unsigned long long* ev_cnt;       // [n_events][kEvCnt]: near[6] then n_tests[6] of every event (zeroed per batch)
   unsigned long long* tstate[T_N];  // look-back status words per scanning kernel
   // ---- a0: hits binned by global sensor ----
-  int* hit_gs_in;    // [n_hits] global sensor of input hit i
-  int* hit_rank;     // [n_hits] arrival rank inside its sensor bin
-  int* sens_cnt;     // [n_events * 2 * n_mod + 1]
-  int* sens_begin;   // [n_events * 2 * n_mod + 1] exclusive scan of sens_cnt
+  int* hit_rank;     // [n_hits] rank of input hit i among the hits of its (chunk, sensor) (k_ingest_count)
+  int* chunk_cnt;    // [n_events][kIngestChunks][2 * n_mod] hits per (chunk of the event's hits, sensor)
+  int* sens_begin;   // [n_events * 2 * n_mod + 1] first sorted hit of every global sensor
   float4* hit;       // [n_hits] sorted (x, y, z, r)
   int2* hit_ig;      // [n_hits] (event-local input index, global sensor) of the sorted hit
   // ---- scratch lists of accepted objects in arrival order (LS, then pT3; pT5) ----
