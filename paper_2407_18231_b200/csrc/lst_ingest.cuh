@@ -164,6 +164,12 @@ __global__ void __launch_bounds__(kIngestThreads) k_ingest_scan(Dev d) {
 // (float4 x, y, z, r + int2 event-local input index, global sensor), r = sqrtf(x*x + y*y).
 constexpr int kIngestUnroll = 4;
 
+// sorted hit `i`: one 32-byte record = one sector, (x, y, z, r) then (event-local input index, global sensor, -, -)
+__device__ __forceinline__ float4 hit_xyzr(const Dev& d, int i) { return d.hit[2 * (size_t)i]; }
+__device__ __forceinline__ int2 hit_ig(const Dev& d, int i) {
+  return *reinterpret_cast<const int2*>(d.hit + 2 * (size_t)i + 1);
+}
+
 __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
   load_batch(d);
   const int stride = gridDim.x * blockDim.x;
@@ -193,8 +199,8 @@ __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
       const int i = i0 + u * stride;
       if (i < d.n_hits) {
         const int pos = slot[u] + rk[u];
-        d.hit[pos] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
-        d.hit_ig[pos] = make_int2(i - h0[u], gs[u]);
+        d.hit[2 * (size_t)pos] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
+        d.hit[2 * (size_t)pos + 1] = make_float4(__int_as_float(i - h0[u]), __int_as_float(gs[u]), 0.0f, 0.0f);
       }
     }
   }

@@ -52,20 +52,20 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
     float4 hb = make_float4(0.f, 0.f, 0.f, 0.f);
     if (lane < n_now) {
       i = s_own[warp][lane];
-      const int gs = d.hit_ig[i].y;
+      const int gs = hit_ig(d, i).y;
       const int gm = gs >> 1;
       ev = gm / d.n_mod;
       a = __ldg(d.sens_begin + gs - 1);
       a1 = __ldg(d.sens_begin + gs);
       endcap = __ldg(d.subdet + (gm - ev * d.n_mod)) != 0;
-      hb = d.hit[i];
+      hb = hit_xyzr(d, i);
     }
     int cnt = 0, near = 0;
     int stash[kMdStash];
 #pragma unroll
     for (int k = 0; k < kMdStash; ++k) stash[k] = 0;
     for (; a < a1; ++a) {
-      const float4 ha = d.hit[a];
+      const float4 ha = hit_xyzr(d, a);
       int cl = md_class(d.cuts, endcap, ha, hb);  // sqrt- and division-free; the exact cuts only where it cannot decide
       if (cl == PT_UNSURE) {
         float ux, uy;
@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
   for (int w0 = (blockIdx.x * kWarps + warp) * 64; w0 < d.n_hits; w0 += gridDim.x * kWarps * 64) {
     // ---- the upper-sensor hits of the window join the queue, in order ----
     const int i0 = w0 + lane, i1 = w0 + 32 + lane;
-    const int gs0 = i0 < n ? d.hit_ig[i0].y : 0, gs1 = i1 < n ? d.hit_ig[i1].y : 0;
+    const int gs0 = i0 < n ? hit_ig(d, i0).y : 0, gs1 = i1 < n ? hit_ig(d, i1).y : 0;
     const unsigned m0 = __ballot_sync(kFull, gs0 & 1), m1 = __ballot_sync(kFull, gs1 & 1);
     const int n0 = __popc(m0);
     if (gs0 & 1) s_own[warp][n_q + __popc(m0 & ((1u << lane) - 1u))] = i0;
@@ -166,21 +166,21 @@ __global__ void __launch_bounds__(kBlock) k_md_place(Dev d) {
     }
     int tb, tt;
     int pos = tile_alloc(sum, d.tstate[T_MD], tile, s_scan, tb, tt);
-    int gm_prev = (i0 > 0 && i0 <= n) ? (d.hit_ig[i0 - 1].y >> 1) : -1;
+    int gm_prev = (i0 > 0 && i0 <= n) ? (hit_ig(d, i0 - 1).y >> 1) : -1;
 #pragma unroll
     for (int k = 0; k < kMdPlaceItems; ++k) {
       const int i = i0 + k;
       if (i >= n) break;
-      const int2 ib = d.hit_ig[i];
+      const int2 ib = hit_ig(d, i);
       const int gs = ib.y, gm = gs >> 1;
       if (gm != gm_prev) fill(gm_prev + 1, gm + 1, pos);  // the modules that begin at hit i
       gm_prev = gm;
       if (cnt[k] == 0) continue;
       const int endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
-      const float4 hb = d.hit[i];
+      const float4 hb = hit_xyzr(d, i);
       auto emit = [&](int a) {  // unit direction exactly as in md_test (CUTS.md section 3)
         if (pos < cap) {
-          const float4 ha = d.hit[a];
+          const float4 ha = hit_xyzr(d, a);
           float ux = 0.0f, uy = 0.0f;
           if (!endcap) {
             const float dx = hb.x - ha.x, dy = hb.y - ha.y;
@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(kBlock) k_md_place(Dev d) {
             ux = dx / dd;
             uy = dy / dd;
           }
-          d.md_hit[pos] = make_int2(d.hit_ig[a].x, ib.x);
+          d.md_hit[pos] = make_int2(hit_ig(d, a).x, ib.x);
           d.md_info[pos] = (gs - 1) | endcap;
           d.md_a[pos] = ha;
           d.md_u[pos] = make_float2(ux, uy);
@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(kBlock) k_md_place(Dev d) {
         const int a1 = __ldg(d.sens_begin + gs);
         for (int a = __ldg(d.sens_begin + gs - 1); a < a1; ++a) {
           float ux, uy;
-          if (md_test(d.cuts, endcap, d.hit[a], hb, ux, uy) & ACC) emit(a);
+          if (md_test(d.cuts, endcap, hit_xyzr(d, a), hb, ux, uy) & ACC) emit(a);
         }
       }
     }
