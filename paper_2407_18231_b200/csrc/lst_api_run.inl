@@ -49,7 +49,7 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   L.mark("ingest_scan");
   k_ingest_scan<<<ctx->caps.max_events, kIngestThreads, 0, st>>>(d);
   L.mark("scatter");
-  k_scatter<<<gw, kBlock, 0, st>>>(d);
+  k_scatter<<<dim3(gw / ctx->caps.max_events > 0 ? gw / ctx->caps.max_events : 1, ctx->caps.max_events), kBlock, 0, st>>>(d);
   L.mark("md");
   k_md_eval<<<g_md, kBlock, 0, st>>>(d);
   L.mark("md_place");

@@ -8,16 +8,6 @@
 
 namespace lst {
 
-// event of a batch-global index, from the (<= a few dozen entries) offsets array
-__device__ __forceinline__ int event_of(const int* __restrict__ off, int n_events, int i) {
-  int lo = 0, hi = n_events;  // invariant: off[lo] <= i < off[hi]
-  while (hi - lo > 1) {
-    int mid = (lo + hi) >> 1;
-    if (__ldg(off + mid) <= i) lo = mid; else hi = mid;
-  }
-  return lo;
-}
-
 // a0: counting sort of the hits by global sensor, three small kernels, no global atomic.  The hits of an event are a
 // contiguous range of the input (event offsets) and stay one after the sort (global sensor = event * n_sens +
 // sensor), so counts and scan are local to the event.  Block (e, c) owns chunk c (of kIngestChunks) of the
@@ -170,25 +160,31 @@ __device__ __forceinline__ int2 hit_ig(const Dev& d, int i) {
   return *reinterpret_cast<const int2*>(d.hit + 2 * (size_t)i + 1);
 }
 
-__global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
+__global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {  // grid (blocks per event, max_events)
   load_batch(d);
+  const int e = blockIdx.y;
+  if (e >= d.n_events) return;
   const int stride = gridDim.x * blockDim.x;
   const int n_sens = 2 * d.n_mod;
-  for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < d.n_hits; i0 += kIngestUnroll * stride) {
-    int slot[kIngestUnroll], rk[kIngestUnroll], gs[kIngestUnroll], h0[kIngestUnroll];
+  const int h0 = d.hit_ev_off[e], h1 = d.hit_ev_off[e + 1];
+  const int per = (h1 - h0 + kIngestChunks - 1) / kIngestChunks;  // as IngestChunk::init
+  const int* __restrict__ slots = d.chunk_cnt + (size_t)e * kIngestChunks * n_sens;
+  const int gs0 = e * n_sens;
+  for (int i0 = h0 + blockIdx.x * blockDim.x + threadIdx.x; i0 < h1; i0 += kIngestUnroll * stride) {
+    int slot[kIngestUnroll], rk[kIngestUnroll], sv[kIngestUnroll];
     float x[kIngestUnroll], y[kIngestUnroll], z[kIngestUnroll];
 #pragma unroll
     for (int u = 0; u < kIngestUnroll; ++u) {
       const int i = i0 + u * stride;
-      const bool ok = i < d.n_hits;
+      const bool ok = i < h1;
       int s = ok ? load_sensor(d, i) : 0;
       if (s < 0 || s >= n_sens) s = 0;
-      const int e = ok ? event_of(d.hit_ev_off, d.n_events, i) : 0;
-      h0[u] = __ldg(d.hit_ev_off + e);
-      const int per = (__ldg(d.hit_ev_off + e + 1) - h0[u] + kIngestChunks - 1) / kIngestChunks;
-      const int c = per > 0 ? (i - h0[u]) / per : 0;
-      gs[u] = e * n_sens + s;
-      slot[u] = ok ? d.chunk_cnt[((size_t)e * kIngestChunks + c) * n_sens + s] : 0;
+      const int k = i - h0;
+      int c = 0;  // chunk of hit i: k / per
+#pragma unroll
+      for (int cc = 1; cc < kIngestChunks; ++cc) c += k >= cc * per;
+      sv[u] = s;
+      slot[u] = ok ? slots[(size_t)c * n_sens + s] : 0;
       rk[u] = ok ? d.hit_rank[i] : 0;
       x[u] = ok ? __ldg(d.in_x + i) : 0.0f;
       y[u] = ok ? __ldg(d.in_y + i) : 0.0f;
@@ -197,10 +193,10 @@ __global__ void __launch_bounds__(kBlock) k_scatter(Dev d) {
 #pragma unroll
     for (int u = 0; u < kIngestUnroll; ++u) {
       const int i = i0 + u * stride;
-      if (i < d.n_hits) {
+      if (i < h1) {
         const int pos = slot[u] + rk[u];
         d.hit[2 * (size_t)pos] = make_float4(x[u], y[u], z[u], sqrtf(x[u] * x[u] + y[u] * y[u]));
-        d.hit[2 * (size_t)pos + 1] = make_float4(__int_as_float(i - h0[u]), __int_as_float(gs[u]), 0.0f, 0.0f);
+        d.hit[2 * (size_t)pos + 1] = make_float4(__int_as_float(i - h0), __int_as_float(gs0 + sv[u]), 0.0f, 0.0f);
       }
     }
   }
