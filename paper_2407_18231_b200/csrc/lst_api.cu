@@ -246,6 +246,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.sens_begin = b.take<int>(n_sens + 1);
   d.hit_rank = b.take<int>(c.max_hits);
   d.chunk_cnt = b.take<int>((size_t)n_sens * kIngestChunks);
+  d.chunk_part = b.take<int>((size_t)c.max_events * kIngestChunks * kIngestScanParts);
   d.hit = b.take<float4>(2 * (size_t)c.max_hits);
   // --- a1..a4 ---
   {

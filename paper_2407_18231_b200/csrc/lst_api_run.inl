@@ -47,7 +47,7 @@ int enqueue(lst_ctx* ctx, cudaStream_t st, Launcher* Lp) {
   L.mark("ingest_count");
   k_ingest_count<<<ctx->caps.max_events * kIngestChunks, kIngestThreads, ingest_smem, st>>>(d);
   L.mark("ingest_scan");
-  k_ingest_scan<<<ctx->caps.max_events, kIngestThreads, 0, st>>>(d);
+  k_ingest_scan<<<ctx->caps.max_events * kIngestScanParts, kIngestThreads, 0, st>>>(d);
   L.mark("scatter");
   k_scatter<<<dim3(gw / ctx->caps.max_events > 0 ? gw / ctx->caps.max_events : 1, ctx->caps.max_events), kBlock, 0, st>>>(d);
   L.mark("md");

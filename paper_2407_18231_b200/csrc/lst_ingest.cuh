@@ -26,6 +26,7 @@ constexpr int kIngestThreads = 1024;
 constexpr int kIngestMaxBins = 40960;  // counters per round (160 KB of shared memory)
 constexpr int kIngestChunks = 4;       // blocks per event
 constexpr int kIngestBatch = 8;        // sensor ids a thread has in flight
+constexpr int kIngestScanParts = 4;    // blocks per event of k_ingest_scan
 
 __device__ __forceinline__ int load_sensor(const Dev& d, int i) {
   return d.sensor_u16 ? (int)__ldg(reinterpret_cast<const unsigned short*>(d.in_sensor) + i) : __ldg(d.in_sensor + i);
@@ -67,6 +68,12 @@ __global__ void __launch_bounds__(kIngestThreads) k_ingest_count(Dev d) {
     }
   }
   int* __restrict__ row = d.chunk_cnt + ((size_t)k.e * kIngestChunks + k.c) * k.n_sens;
+  __shared__ int s_part[kIngestScanParts];
+  if (threadIdx.x < kIngestScanParts) s_part[threadIdx.x] = 0;
+  const int plen = (k.n_sens + kIngestScanParts - 1) / kIngestScanParts;  // sensors per block of k_ingest_scan
+  int part_sum[kIngestScanParts];
+#pragma unroll
+  for (int q = 0; q < kIngestScanParts; ++q) part_sum[q] = 0;
   bool bad = false;
   for (int r_lo = 0; r_lo < k.n_sens; r_lo += k.R) {
     const int r_n = min(k.R, k.n_sens - r_lo);
@@ -92,33 +99,52 @@ __global__ void __launch_bounds__(kIngestThreads) k_ingest_count(Dev d) {
       }
     }
     __syncthreads();
-    for (int j = threadIdx.x; j < r_n; j += kIngestThreads) row[r_lo + j] = s_bin[j];
+    for (int j = threadIdx.x; j < r_n; j += kIngestThreads) {
+      const int v = s_bin[j];
+      row[r_lo + j] = v;
+#pragma unroll
+      for (int q = 0; q < kIngestScanParts; ++q) part_sum[q] += (r_lo + j) / plen == q ? v : 0;
+    }
     __syncthreads();
   }
+  // the chunk's hits per part of the sensor range: where the blocks of k_ingest_scan start
+#pragma unroll
+  for (int q = 0; q < kIngestScanParts; ++q) {
+    const int v = warp_sum(part_sum[q]);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(&s_part[q], v);
+  }
+  __syncthreads();
+  if (threadIdx.x < kIngestScanParts)
+    d.chunk_part[((size_t)k.e * kIngestChunks + k.c) * kIngestScanParts + threadIdx.x] = s_part[threadIdx.x];
   if (bad) atomicOr(&d.ctl->error, E_BAD_SENSOR);
 }
 
-// One block per event: totals over the chunks, exclusive scan over the event's sensors -> sens_begin; the chunk
-// counters are replaced, in place, by the first slot of the chunk's hits of every sensor.
+// kIngestScanParts blocks per event, each a part of the sensor range: totals over the chunks, exclusive scan over
+// the sensors -> sens_begin; the chunk counters are replaced, in place, by the first slot of the chunk's hits of
+// every sensor.
 __global__ void __launch_bounds__(kIngestThreads) k_ingest_scan(Dev d) {
   load_batch(d);
   __shared__ int s_warp[2][kIngestThreads / 32];
-  const int e = blockIdx.x;
+  const int e = blockIdx.x / kIngestScanParts, part = blockIdx.x - e * kIngestScanParts;
   if (e >= d.n_events) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int n_sens = 2 * d.n_mod;
-  int* __restrict__ rows = d.chunk_cnt + (size_t)e * kIngestChunks * n_sens;
-  int* __restrict__ begin = d.sens_begin + (size_t)e * n_sens;
+  const int n_all = 2 * d.n_mod;
+  const int plen = (n_all + kIngestScanParts - 1) / kIngestScanParts;
+  const int n_sens = min(n_all, (part + 1) * plen);  // this block: sensors [part * plen, n_sens)
+  int* __restrict__ rows = d.chunk_cnt + (size_t)e * kIngestChunks * n_all;
+  int* __restrict__ begin = d.sens_begin + (size_t)e * n_all;
   constexpr int T = 4;  // tiles of kIngestThreads consecutive sensors whose loads are in flight together
-  int carry = d.hit_ev_off[e];
+  int carry = d.hit_ev_off[e];  // + the event's hits on the sensors of the lower parts (k_ingest_count)
+  for (int c = 0; c < kIngestChunks; ++c)
+    for (int q = 0; q < part; ++q) carry += d.chunk_part[((size_t)e * kIngestChunks + c) * kIngestScanParts + q];
   int par = 0;
-  for (int t0 = 0; t0 < n_sens; t0 += T * kIngestThreads) {
+  for (int t0 = part * plen; t0 < n_sens; t0 += T * kIngestThreads) {
     int v[T][kIngestChunks];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
       const int j = t0 + t * kIngestThreads + threadIdx.x;  // coalesced: consecutive threads, consecutive sensors
 #pragma unroll
-      for (int c = 0; c < kIngestChunks; ++c) v[t][c] = j < n_sens ? rows[(size_t)c * n_sens + j] : 0;
+      for (int c = 0; c < kIngestChunks; ++c) v[t][c] = j < n_sens ? rows[(size_t)c * n_all + j] : 0;
     }
 #pragma unroll
     for (int t = 0; t < T; ++t) {
@@ -139,7 +165,7 @@ __global__ void __launch_bounds__(kIngestThreads) k_ingest_scan(Dev d) {
         begin[j] = run;
 #pragma unroll
         for (int c = 0; c < kIngestChunks; ++c) {
-          rows[(size_t)c * n_sens + j] = run;
+          rows[(size_t)c * n_all + j] = run;
           run += v[t][c];
         }
       }
@@ -147,7 +173,7 @@ __global__ void __launch_bounds__(kIngestThreads) k_ingest_scan(Dev d) {
       par ^= 1;  // the other buffer: no second barrier per tile
     }
   }
-  if (e == d.n_events - 1 && threadIdx.x == 0) d.sens_begin[(size_t)d.n_events * n_sens] = carry;
+  if (e == d.n_events - 1 && part == kIngestScanParts - 1 && threadIdx.x == 0) d.sens_begin[(size_t)d.n_events * n_all] = carry;
 }
 
 // Every hit goes to (first slot of its chunk's hits of its sensor) + (its rank among them): sorted SoA

@@ -70,6 +70,7 @@ struct Dev {
   // ---- a0: hits binned by global sensor ----
   int* hit_rank;     // [n_hits] rank of input hit i among the hits of its (chunk, sensor) (k_ingest_count)
   int* chunk_cnt;    // [n_events][kIngestChunks][2 * n_mod] hits per (chunk of the event's hits, sensor)
+  int* chunk_part;   // [n_events][kIngestChunks][kIngestScanParts] hits of a chunk per part of the sensor range
   int* sens_begin;   // [n_events * 2 * n_mod + 1] first sorted hit of every global sensor
   float4* hit;       // [2 * n_hits] sorted hits, 32 bytes each: (x, y, z, r), (event-local input index, global sensor, -, -)
   // ---- scratch lists of accepted objects in arrival order (LS, then pT3; pT5) ----
