@@ -256,7 +256,7 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
     d.ev_scratch = b.take<char>(sz);
     d.ev_scratch2 = b.take<char>(sizeof(PtAccepted) * (size_t)c.max_pt5);
   }
-  d.md_cnt = b.take<int>(c.max_hits);
+  d.md_cnt = b.take<int2>(c.max_hits);
   d.md_stash = b.take<int>(4 * (size_t)c.max_hits);
   d.mod_md_begin = b.take<int>(n_sens / 2 + 1);
   d.md_hit = b.take<int2>(c.max_md);

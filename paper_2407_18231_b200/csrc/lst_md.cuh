@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
     }
     if (near) atomicAdd(d.ev_cnt + (size_t)ev * kEvCnt + 0, (unsigned long long)near);
     if (i >= 0) {
-      d.md_cnt[i] = cnt;
+      d.md_cnt[i].x = cnt;
       reinterpret_cast<int4*>(d.md_stash)[i] = make_int4(stash[0], stash[1], stash[2], stash[3]);
     }
   };
@@ -95,8 +95,10 @@ __global__ void __launch_bounds__(kBlock) k_md_eval(Dev d) {
     const int n0 = __popc(m0);
     if (gs0 & 1) s_own[warp][n_q + __popc(m0 & ((1u << lane) - 1u))] = i0;
     if (gs1 & 1) s_own[warp][n_q + n0 + __popc(m1 & ((1u << lane) - 1u))] = i1;
-    if (i0 < d.n_hits && !(gs0 & 1)) d.md_cnt[i0] = 0;  // lower-sensor hits own no MD
-    if (i1 < d.n_hits && !(gs1 & 1)) d.md_cnt[i1] = 0;
+    // (MDs owned, global sensor) of every hit, for k_md_place: lower-sensor hits own no MD, the count of an
+    // upper-sensor hit follows from its round
+    if (i0 < d.n_hits) d.md_cnt[i0] = make_int2(0, gs0);
+    if (i1 < d.n_hits) d.md_cnt[i1] = make_int2(0, gs1);
     n_q += n0 + __popc(m1);
     __syncwarp();
     while (n_q >= 32) {  // full rounds only; the remainder waits for the next window
@@ -158,24 +160,26 @@ __global__ void __launch_bounds__(kBlock) k_md_place(Dev d) {
     const int tile = s_tile;
     if (tile >= n_tiles) break;
     const int i0 = tile * kTile + threadIdx.x * kMdPlaceItems;
-    int cnt[kMdPlaceItems], sum = 0;
+    int cnt[kMdPlaceItems], gsv[kMdPlaceItems], sum = 0;
 #pragma unroll
     for (int k = 0; k < kMdPlaceItems; ++k) {
-      cnt[k] = (i0 + k < n) ? d.md_cnt[i0 + k] : 0;
+      const int2 cg = (i0 + k < n) ? d.md_cnt[i0 + k] : make_int2(0, 0);
+      cnt[k] = cg.x;
+      gsv[k] = cg.y;
       sum += cnt[k];
     }
     int tb, tt;
     int pos = tile_alloc(sum, d.tstate[T_MD], tile, s_scan, tb, tt);
-    int gm_prev = (i0 > 0 && i0 <= n) ? (hit_ig(d, i0 - 1).y >> 1) : -1;
+    int gm_prev = (i0 > 0 && i0 <= n) ? (d.md_cnt[i0 - 1].y >> 1) : -1;
 #pragma unroll
     for (int k = 0; k < kMdPlaceItems; ++k) {
       const int i = i0 + k;
       if (i >= n) break;
-      const int2 ib = hit_ig(d, i);
-      const int gs = ib.y, gm = gs >> 1;
+      const int gs = gsv[k], gm = gs >> 1;
       if (gm != gm_prev) fill(gm_prev + 1, gm + 1, pos);  // the modules that begin at hit i
       gm_prev = gm;
       if (cnt[k] == 0) continue;
+      const int2 ib = hit_ig(d, i);
       const int endcap = __ldg(d.subdet + (gm - (gm / d.n_mod) * d.n_mod)) != 0;
       const float4 hb = hit_xyzr(d, i);
       auto emit = [&](int a) {  // unit direction exactly as in md_test (CUTS.md section 3)

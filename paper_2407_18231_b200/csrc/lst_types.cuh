@@ -77,7 +77,7 @@ struct Dev {
   void* ev_scratch;
   void* ev_scratch2;
   // ---- a1: MD (grouped by global module) ----
-  int* md_cnt;        // [n_hits] MDs owned by a sorted hit (upper-sensor hits only)
+  int2* md_cnt;       // [n_hits] (MDs owned by a sorted hit: upper-sensor hits only, its global sensor)
   int* md_stash;      // [n_hits][4] sorted positions of the first accepted lower hits
   int* mod_md_begin;  // [n_events * n_mod + 1] first MD of a global module
   int2* md_hit;       // (h_lo, h_hi) event-local input indices
