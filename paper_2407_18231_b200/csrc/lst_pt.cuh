@@ -66,7 +66,7 @@ struct PtCand {
   }
 };
 
-constexpr int kPtBlocks = 4;           // anchor blocks (of 32 sorted anchors) per tile; 1 when that leaves fewer than kPtMinTiles tiles
+constexpr int kPtBlocks = 2;           // anchor blocks (of 32 sorted anchors) per tile; 1 when that leaves fewer than kPtMinTiles tiles
 constexpr int kPtMinTiles = 12288;     // about two tiles per resident warp of k_pt_eval
 constexpr int kSeedSectors = 128;       // azimuth sectors of the seed sort
 constexpr int kAncBlocksPerEvent = 8;   // blocks of k_anchor_sort per event

@@ -106,6 +106,35 @@ def test_hits_on_one_sensor_only(lst, oracle_mod):
     assert_same(canon(got), canon(want), "lower sensors only: ")
 
 
+def test_many_sensors_span_several_ingest_rounds(lst, oracle_mod):
+    """A module table of 8 copies of C4's (45,696 sensors): the ingest kernels keep at most 40,960 sensor counters
+    in shared memory and take the sensors in rounds.  Event 0 sits in the first copy, event 1 in the last, event
+    2 is spread over all of them (module copy = hit index mod 8: no hit pair survives, which is a result too)."""
+    import dataclasses
+
+    geom, off, tgt = make_config_geometry("C4")
+    n_mod, copies = geom.n_modules, 8
+    table = np.tile(geom.module_table(), (copies, 1))
+    subdet = np.tile(geom.subdet, copies)
+    deg = np.diff(off)
+    off_big = np.concatenate([[0], np.cumsum(np.tile(deg, copies))]).astype(np.int32)
+    tgt_big = np.concatenate([tgt + k * n_mod for k in range(copies)]).astype(np.int32)
+    ev = make_config_event("C4")
+    shifts = [np.zeros(ev.n_hits, np.int32), np.full(ev.n_hits, (copies - 1) * 2 * n_mod, np.int32),
+              (np.arange(ev.n_hits, dtype=np.int32) % copies) * 2 * n_mod]
+    evs = [dataclasses.replace(ev, sensor=(ev.sensor + sh).astype(np.int32)) for sh in shifts]
+    g = lst.lst_load_geometry(table, off_big, tgt_big)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=3))
+    try:
+        run_batch(lst, ctx, evs)
+        for i, e in enumerate(evs):
+            want = oracle_mod.run_event(subdet, off_big, tgt_big, e.x, e.y, e.z, e.sensor, e.pls)
+            assert_same(canon(lst.lst_ctx_fetch_event(ctx, i)), canon(want), f"8 x C4 modules, event {i}: ")
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
 def test_benchmark_configuration(lst, oracle_mod):
     """BASELINE.json config 5 as bench.py times it: 16 PU200 events (seeds on) in one launch sequence
     on a non-default stream, default capacities, device-resident inputs, two batches back to back on
