@@ -12,7 +12,11 @@ T5, pT3, pT5, duplicate removal, track-candidate selection) = SURVEY.md section 
   value  : events/s with the batch inputs already resident in HBM (device pointers through the ABI)
   e2e    : events/s through the same C-ABI calls with HOST (pinned) buffers: H2D of the hits and
            seeds and D2H of the track candidates inside the timed region
-  roofline / kernels : per-kernel CUDA-event times (lst_ctx_kernel_times) of L2-flushed batches
+  kernels / kernels_full_grid : per-kernel CUDA-event times (lst_ctx_kernel_times) of L2-flushed batches on one
+           stream, in the configuration of the timed region (--blocks-per-sm, default 2: kernels of different
+           batches share the SMs) and with every kernel filling the GPU (8 blocks per SM)
+  roofline : the dominant kernel alone on the GPU (full grid); roofline_timed_config: the same in the timed
+           region's configuration
   cpu_baseline : the oracle (oracle/) on the host cores over a bounded sample of the same events
 
 Multi-GPU (N > 1): replicas only -- every rank runs its own batches (different seeds), no
@@ -394,7 +398,7 @@ def run_b200(args):
     # DRAM traffic and executed warp instructions of the dominant kernel cannot be measured without a profiler:
     # they come from the committed ncu --set full capture (profiles/traffic.json), and only when that capture was
     # taken on this workload; the field says so
-    def make_roof(kernels):
+    def make_roof(kernels, cap_key="kernels"):
         top = max(kernels, key=lambda k: k["ms"])
         if top["alu_frac"] >= top["hbm_frac"]:
             roof = {"bound": "alu", "kernel": top["name"], "achieved": top["tflops"], "peak": round(alu_peak_tflops, 2),
@@ -410,8 +414,8 @@ def run_b200(args):
             with open(traffic_path) as f:
                 cap = json.load(f)
             if cap.get("workload") == args.workload and cap.get("pu") == args.pu and cap.get("events") == E \
-                    and top["name"] in cap.get("kernels", {}):
-                k = cap["kernels"][top["name"]]
+                    and top["name"] in cap.get(cap_key, {}):
+                k = cap[cap_key][top["name"]]
                 roof["traffic"] = k.get("dram_bytes")
                 roof["traffic_source"] = "ncu capture %s (stored, not measured in this run)" % cap.get("capture", "?")
                 if k.get("warp_inst"):  # issue-rate roofline: 148 SMs x 4 schedulers x clock
@@ -420,13 +424,20 @@ def run_b200(args):
                     roof["warp_inst"] = k["warp_inst"]
         return roof
 
-    roof = make_roof(kernels)
-    roof["launch"] = "%d blocks per SM per kernel (the timed region's configuration), kernel alone on one stream" % (
-        args.blocks_per_sm or 8)
-    roof_alone = None
+    # `roofline`: the dominant kernel ALONE ON THE GPU with its full grid (8 blocks per SM) -- what the kernel achieves
+    # of the peak.  With --blocks-per-sm 1..4 (the timed region) a kernel takes only that share of every SM by design
+    # and leaves the rest to the kernels of other batches, so its duration alone in that configuration
+    # (`roofline_timed_config`) measures the share it was given, not its efficiency.
+    cfg = "%d blocks per SM per kernel, kernel alone on one stream, L2 flushed"
     if kernels_alone:
-        roof_alone = make_roof(kernels_alone)
-        roof_alone["launch"] = "8 blocks per SM per kernel (every kernel fills the GPU), kernel alone on one stream"
+        roof = make_roof(kernels_alone, "kernels_full_grid")
+        roof["launch"] = cfg % 8
+        roof_cfg = make_roof(kernels, "kernels")
+        roof_cfg["launch"] = cfg % args.blocks_per_sm + " (the configuration of the timed region)"
+    else:
+        roof = make_roof(kernels, "kernels" if args.blocks_per_sm not in (0, 8) else "kernels_full_grid")
+        roof["launch"] = cfg % (args.blocks_per_sm or 8)
+        roof_cfg = None
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -474,7 +485,7 @@ def run_b200(args):
         "clocks": sampler.summary(),
         "roofline": roof,
         "kernels": kernels,
-        "roofline_full_grid": roof_alone,
+        "roofline_timed_config": roof_cfg,
         "kernels_full_grid": kernels_alone,
         "objects_per_s": {k: round(ksum["n_" + k] / (ms / args.steps * 1e-3), 1)
                           for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
