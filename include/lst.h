@@ -70,7 +70,8 @@ typedef struct lst_params {
 void lst_default_params(lst_params* p);
 
 /* Capacities of one context (object counts summed over the events of a batch).  max_md may not exceed
- * LST_MAX_MD (the Line-Segment stage packs an MD index into 27 bits): lst_ctx_create returns LST_ERR_ARG. */
+ * LST_MAX_MD (the Line-Segment stage packs an MD index and two flags into one 32-bit word): lst_ctx_create
+ * returns LST_ERR_ARG. */
 #define LST_MAX_MD (1 << 27)
 typedef struct lst_caps {
   int32_t max_events;
