@@ -430,7 +430,8 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   // grid-stride kernels are launched with exactly the blocks that fit the GPU at once
   int occ_md = 0, occ_ls = 0, occ_pt = 0;
   const size_t pt_smem = sizeof(PtWarp) * kWarps;
-  const int ingest_smem = (int)sizeof(int) * (2 * g->n_mod < kIngestMaxBins ? 2 * g->n_mod : kIngestMaxBins);
+  // the limit is a property of the function, shared by every geometry and context of the process: the largest a launch can ask for
+  const int ingest_smem = (int)sizeof(int) * kIngestMaxBins;
   if (cudaFuncSetAttribute(k_ingest_count, cudaFuncAttributeMaxDynamicSharedMemorySize, ingest_smem) != cudaSuccess ||
       cudaFuncSetAttribute(k_pt_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pt_smem) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_md, k_md_eval, kBlock, 0) != cudaSuccess ||

@@ -125,12 +125,21 @@ def test_many_sensors_span_several_ingest_rounds(lst, oracle_mod):
     evs = [dataclasses.replace(ev, sensor=(ev.sensor + sh).astype(np.int32)) for sh in shifts]
     g = lst.lst_load_geometry(table, off_big, tgt_big)
     ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=3))
+    # a second, small geometry created afterwards and alive at the same time: per-function launch limits
+    # (shared memory of the ingest) must not depend on which context was created last
+    g_small = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx_small = lst.lst_ctx_create(g_small, lst.lst_default_caps(max_events=1))
     try:
+        run_batch(lst, ctx_small, [ev])
+        want_small = canon(oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls))
+        assert_same(canon(lst.lst_ctx_fetch_event(ctx_small, 0)), want_small, "C4 next to 8 x C4: ")
         run_batch(lst, ctx, evs)
         for i, e in enumerate(evs):
             want = oracle_mod.run_event(subdet, off_big, tgt_big, e.x, e.y, e.z, e.sensor, e.pls)
             assert_same(canon(lst.lst_ctx_fetch_event(ctx, i)), canon(want), f"8 x C4 modules, event {i}: ")
     finally:
+        lst.lst_free(ctx_small)
+        lst.lst_free(g_small)
         lst.lst_free(ctx)
         lst.lst_free(g)
 
