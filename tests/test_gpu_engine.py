@@ -243,6 +243,48 @@ def test_blocks_per_sm_changes_no_result(lst, oracle_mod):
         lst.lst_free(g)
 
 
+def test_contexts_in_flight_share_the_sms(lst, oracle_mod):
+    """The configuration of the bench's timed region: several contexts on streams of their own, every kernel at 2
+    (then 1) blocks per SM, all batches launched before any is awaited, three rounds back to back -- kernels of
+    different batches co-reside on the SMs (and k_ls_place's wait for its scan tiles runs next to other kernels).
+    Every event of every batch of every round equals the oracle's."""
+    import torch
+
+    geom, off, tgt = make_config_geometry("C5")
+    n_ctx, n_ev = 6, 3
+    batches = [[make_config_event("C5", pu=50, index=100 + n_ev * c + i, seeds=True) for i in range(n_ev)] for c in range(n_ctx)]
+    want = [[canon(oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)) for ev in b] for b in batches]
+    from lst_inputs.events import concat_events
+
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    streams = [torch.cuda.Stream() for _ in range(n_ctx)]
+    ctxs = [lst.lst_ctx_create(g, lst.lst_default_caps(max_events=n_ev), st.cuda_stream) for st in streams]
+    try:
+        inputs = []
+        for b in batches:
+            cb = concat_events(b)
+            h, keep = lst.make_hits(cb["x"], cb["y"], cb["z"], cb["sensor"], cb["hit_offsets"])
+            s, keep = lst.make_pls(cb["pls"], cb["pls_offsets"], keep)
+            inputs.append((h, s, keep))
+        for blocks in (2, 1):
+            for c in ctxs:
+                lst.lst_ctx_set_blocks_per_sm(c, blocks)
+            for rnd in range(3):
+                for c in range(n_ctx):  # context c runs batch (c + rnd) mod n_ctx: every workspace sees every batch
+                    b = (c + rnd) % n_ctx
+                    lst.lst_ctx_run(ctxs[c], n_ev, inputs[b][0], inputs[b][1])
+                for c in range(n_ctx):
+                    b = (c + rnd) % n_ctx
+                    lst.lst_ctx_sync(ctxs[c])
+                    for i in range(n_ev):
+                        assert_same(canon(lst.lst_ctx_fetch_event(ctxs[c], i)), want[b][i],
+                                    f"{blocks} blocks per SM, round {rnd}, context {c}, event {i}: ")
+    finally:
+        for c in ctxs:
+            lst.lst_free(c)
+        lst.lst_free(g)
+
+
 def test_many_small_events_in_one_batch(lst, oracle_mod):
     """40 events per launch sequence (more events than any table is sized for by default)."""
     geom, off, tgt = make_config_geometry("C4")
