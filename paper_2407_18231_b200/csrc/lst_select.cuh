@@ -210,13 +210,15 @@ __global__ void __launch_bounds__(kBlock) k_rule2(Dev d) {
     const int X = X0 + g0;
     bool rem = false;
     int2 x = make_int2(0, 0);
-    if (X < n && task < 5) {
+    if (X < n) {
       x = d.pt3[X];
+      rem = d.linked[x.x] & 1;  // rule 2b: seed already in a surviving pT5 (about half of the pT3s: the whole group skips its lists)
+    }
+    if (X < n && task < 5 && !rem) {
       const float sX = d.pt3_score[X];
       int mX[3], mY[5];
       load_t3_md(d, x.y, mX);
       if (task == 0) {
-        rem = d.linked[x.x] & 1;  // rule 2b: seed already in a surviving pT5
         for (int Y = d.pls_pt3_begin[x.x]; Y < d.pls_pt3_begin[x.x + 1] && !rem; ++Y) {
           if (Y == X) continue;
           load_t3_md(d, d.pt3[Y].y, mY);
