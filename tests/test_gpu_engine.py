@@ -285,6 +285,33 @@ def test_contexts_in_flight_share_the_sms(lst, oracle_mod):
         lst.lst_free(g)
 
 
+def test_more_pu200_batches_at_small_grids(lst, oracle_mod):
+    """Two more batches of 16 PU200 events (event numbers 48-63 and 80-95) on one context at 2 and 1 blocks per SM,
+    each run twice (the second replays the graph on a used workspace): every event equals the oracle's.  These
+    are the batches on which a dropped variant of k_rule3 failed (profiles/r02_iterations.md, section 6)."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    geom, off, tgt = make_config_geometry("C5")
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt)
+    ctx = lst.lst_ctx_create(g, lst.lst_default_caps(max_events=16))
+    try:
+        for first in (48, 80):
+            evs = [make_config_event("C5", pu=200, index=first + i, seeds=True) for i in range(16)]
+            with ThreadPoolExecutor(16) as ex:  # ctypes releases the GIL: one oracle call per core
+                want = list(ex.map(lambda ev: canon(oracle_mod.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z,
+                                                                         ev.sensor, ev.pls)), evs))
+            for blocks in (2, 1):
+                lst.lst_ctx_set_blocks_per_sm(ctx, blocks)
+                for rep in range(2):
+                    run_batch(lst, ctx, evs)
+                    for i in range(16):
+                        assert_same(canon(lst.lst_ctx_fetch_event(ctx, i)), want[i],
+                                    f"events {first}+, {blocks} blocks per SM, rep {rep}, event {i}: ")
+    finally:
+        lst.lst_free(ctx)
+        lst.lst_free(g)
+
+
 def test_many_small_events_in_one_batch(lst, oracle_mod):
     """40 events per launch sequence (more events than any table is sized for by default)."""
     geom, off, tgt = make_config_geometry("C4")
