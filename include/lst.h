@@ -35,7 +35,8 @@ typedef enum lst_status {
   LST_ERR_ARG = -1,      /* NULL / negative size / sensor id or event offsets out of range */
   LST_ERR_CUDA = -2,     /* CUDA runtime error (no device, out of memory, launch failure) */
   LST_ERR_CAPACITY = -3, /* an object array of the context is too small for this batch */
-  LST_ERR_GEOMETRY = -4  /* malformed module table or connection map */
+  LST_ERR_GEOMETRY = -4, /* malformed module table or connection map */
+  LST_ERR_LIMIT = -5     /* size beyond the fixed maximum of an entry point that cannot allocate */
 } lst_status;
 
 /* Static string for a status code. */
@@ -221,6 +222,38 @@ int lst_ctx_launch_count(lst_ctx* ctx);
  * those the approximate pre-filters could not decide.  Returns the value (>= 0) or a negative lst_status. */
 enum { LST_STAT_PT_QUEUE = 0, LST_STAT_WORKSPACE_MB = 1 };
 int64_t lst_ctx_stat(lst_ctx* ctx, int32_t which);
+
+/* ---- slot offsets from per-owner counts, stand-alone ------------------------------------------- */
+
+/* Every stage of the chain is "owner -> a variable number of accepted objects" (an MD owns its
+ * Line Segments, a seed its pT3s / pT5s); an owner's objects are stored from slot
+ *     offsets[i] = counts[0] + ... + counts[i-1],   i = 0 .. n,     offsets[n] = number of objects.
+ * The chain computes this with a one-launch tile scan (tiles publish their totals in status words and look back
+ * over their predecessors'), which needs scratch memory beyond input and output: one ticket and one 64-bit
+ * status word per tile of 1024 counts.  The two calls below run that scan on caller-owned arrays.
+ *   counts:  DEVICE, n int32 (not read for n == 0), 16-byte aligned, each >= 0, total < 2^31.
+ *   offsets: DEVICE, n + 1 int32, caller-owned, must not overlap counts.
+ *   cuda_stream: a cudaStream_t as void* (NULL = the legacy default stream).
+ * Errors: LST_ERR_ARG (n < 0, NULL or misaligned pointer), LST_ERR_CUDA.
+ *
+ * lst_scan_counts takes its scratch from cudaMalloc, waits for the result and frees the scratch again. */
+int lst_scan_counts(const int32_t* counts, int32_t n, int32_t* offsets, void* cuda_stream);
+
+/* The same scan for callers that must not allocate device memory: a trigger or reconstruction framework that
+ * owns all device memory and forbids cudaMalloc / cudaFree inside its event loop (both synchronise the whole
+ * device and stall every other stream on it), or any code running where the CUDA runtime refuses allocations.
+ * This call makes no cudaMalloc, cudaFree or other allocating call.  Its scratch is a fixed array inside the
+ * library image (about 128 KB; every GPU the library is loaded on keeps it until the process exits), which
+ * bounds the size: n > LST_SCAN_STATIC_MAX_N returns LST_ERR_LIMIT and touches nothing.
+ *   - Asynchronous: enqueues one memset and one kernel on cuda_stream and returns; offsets are valid once the
+ *     stream has reached that point.
+ *   - The first call on each device looks up the array's device address (that device must be current, as for
+ *     every call); make that first call before starting any stream capture on the device.
+ *   - All calls on a device share the one array, which still holds what the previous call left: each call
+ *     clears the part it uses, in stream order.  Two calls that can overlap on the GPU (different streams, no
+ *     dependency between them) race on it and give wrong offsets; order them, or use lst_scan_counts. */
+#define LST_SCAN_STATIC_MAX_N (1 << 24)
+int lst_scan_counts_static(const int32_t* counts, int32_t n, int32_t* offsets, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -195,3 +195,35 @@ def lst_ctx_stat(ctx, which: int) -> int:
     if v < 0:
         raise LstError(v, "lst_ctx_stat")
     return v
+
+
+def _scan_args(counts, offsets, where):
+    """Device pointers of two CUDA int32 torch tensors (counts [n], offsets [n + 1]); nothing is copied or allocated."""
+    import torch
+
+    for t in (counts, offsets):
+        if not (_is_torch(t) and t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.dim() == 1):
+            raise ValueError(f"{where}: counts and offsets must be contiguous 1-d CUDA int32 tensors")
+    n = int(counts.numel())
+    if int(offsets.numel()) != n + 1:
+        raise ValueError(f"{where}: offsets must hold len(counts) + 1 entries")
+    return C.c_void_p(counts.data_ptr() if n else None), n, C.c_void_p(offsets.data_ptr())
+
+
+def lst_scan_counts(counts, offsets, cuda_stream: int | None = None) -> None:
+    """offsets[i] = counts[0] + ... + counts[i-1] with the chain's scan kernel; scratch from cudaMalloc, returns
+    when the result is there (include/lst.h)."""
+    c, n, o = _scan_args(counts, offsets, "lst_scan_counts")
+    _check(_lib().lst_scan_counts(c, n, o, C.c_void_p(cuda_stream) if cuda_stream else None), "lst_scan_counts")
+
+
+def lst_scan_counts_static(counts, offsets, cuda_stream: int | None = None) -> None:
+    """The same scan for callers that may not allocate device memory (a framework that owns the device memory and
+    bans cudaMalloc / cudaFree from its event loop because they stall every stream of the device): the scratch is a
+    fixed array inside the library, so len(counts) is limited to LST_SCAN_STATIC_MAX_N (LstError with
+    LST_ERR_LIMIT beyond it).  Asynchronous on `cuda_stream`; both tensors are the caller's and nothing is
+    allocated here either.  Calls that could overlap on the GPU share the array and race: keep them ordered.
+    Make the first call on a device outside any stream capture (it looks up the array's address)."""
+    c, n, o = _scan_args(counts, offsets, "lst_scan_counts_static")
+    _check(_lib().lst_scan_counts_static(c, n, o, C.c_void_p(cuda_stream) if cuda_stream else None),
+           "lst_scan_counts_static")

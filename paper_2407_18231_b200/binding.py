@@ -13,7 +13,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liblst_b200.so")
 
-LST_OK, LST_ERR_ARG, LST_ERR_CUDA, LST_ERR_CAPACITY, LST_ERR_GEOMETRY = 0, -1, -2, -3, -4
+LST_OK, LST_ERR_ARG, LST_ERR_CUDA, LST_ERR_CAPACITY, LST_ERR_GEOMETRY, LST_ERR_LIMIT = 0, -1, -2, -3, -4, -5
+LST_SCAN_STATIC_MAX_N = 1 << 24  # include/lst.h
 N_STAGES = 7
 STAGES = ("md", "ls", "t3", "t5", "pt3", "pt5", "t4")
 _EXT_FIELDS = ("t4_tol0", "t4_tol1", "t5_mlp_scale", "t5_mlp_thr")
@@ -91,6 +92,7 @@ ABI_SYMBOLS = (
     "lst_strerror", "lst_default_params", "lst_default_caps", "lst_workspace_bytes", "lst_load_geometry",
     "lst_run_event", "lst_free", "lst_ctx_create", "lst_ctx_run", "lst_ctx_sync", "lst_ctx_fetch_event",
     "lst_ctx_fetch_tc", "lst_ctx_set_blocks_per_sm", "lst_ctx_set_timing", "lst_ctx_kernel_times", "lst_ctx_launch_count", "lst_ctx_stat",
+    "lst_scan_counts", "lst_scan_counts_static",
 )
 
 _LIB = None
@@ -133,6 +135,8 @@ def _lib():
     L.lst_ctx_launch_count.argtypes = [vp]
     L.lst_ctx_stat.argtypes = [vp, C.c_int32]
     L.lst_ctx_stat.restype = C.c_int64
+    L.lst_scan_counts.argtypes = [vp, C.c_int32, vp, vp]
+    L.lst_scan_counts_static.argtypes = [vp, C.c_int32, vp, vp]
     _LIB = L
     return L
 

@@ -86,6 +86,7 @@ extern "C" const char* lst_strerror(int s) {
     case LST_ERR_CUDA: return "CUDA runtime error (no device, out of memory or launch failure)";
     case LST_ERR_CAPACITY: return "object array capacity of the context exceeded (nothing was truncated)";
     case LST_ERR_GEOMETRY: return "malformed module table or connection map";
+    case LST_ERR_LIMIT: return "size beyond the fixed maximum of a non-allocating entry point (LST_SCAN_STATIC_MAX_N)";
     default: return "unknown status";
   }
 }
@@ -451,3 +452,4 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
 
 #include "lst_api_run.inl"
 #include "lst_api_fetch.inl"
+#include "lst_api_static.inl"

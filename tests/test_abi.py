@@ -92,6 +92,23 @@ def test_argument_errors_are_reported_before_any_cuda_call(lst):
     lst.lst_free(None)  # NULL is a no-op
 
 
+def test_scan_entry_points_check_their_arguments_first(lst):
+    """n < 0, NULL / misaligned pointers and n beyond the fixed limit are turned down before any CUDA call."""
+    from paper_2407_18231_b200 import binding
+
+    lib = binding._lib()
+    buf = C.c_void_p(4096)  # never dereferenced
+    for f in (lib.lst_scan_counts, lib.lst_scan_counts_static):
+        assert f(buf, -1, buf, None) == lst.LST_ERR_ARG
+        assert f(buf, 8, None, None) == lst.LST_ERR_ARG
+        assert f(None, 8, buf, None) == lst.LST_ERR_ARG
+        assert f(C.c_void_p(4100), 8, buf, None) == lst.LST_ERR_ARG  # counts must be 16-byte aligned
+    assert lib.lst_scan_counts_static(buf, lst.LST_SCAN_STATIC_MAX_N + 1, buf, None) == lst.LST_ERR_LIMIT
+    assert "LST_SCAN_STATIC_MAX_N" in lib.lst_strerror(lst.LST_ERR_LIMIT).decode()
+    hdr = open(os.path.join(ROOT, "include", "lst.h")).read()
+    assert re.search(r"#define LST_SCAN_STATIC_MAX_N \(1 << 24\)", hdr) and lst.LST_SCAN_STATIC_MAX_N == 1 << 24
+
+
 def test_no_gpu_means_an_error_not_a_fallback(lst):
     import torch
 
