@@ -182,7 +182,7 @@ def test_benchmark_configuration(lst, oracle_mod):
             near += want["near"]
         assert [summ["n_" + k] for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")] == tot.tolist()
         assert summ["n_tests"] == tests.tolist() and summ["near"] == near.tolist()
-        assert np.all(near <= 1e-4 * tests), "near-threshold candidates above 0.01% of the candidates (DESIGN.md N2)"
+        assert np.all(near <= 1e-4 * tests), "near-threshold candidates above 0.01 % of the stage's candidates (CUTS.md section 0, DESIGN.md N2)"
     finally:
         lst.lst_free(ctx)
         lst.lst_free(g)

@@ -44,8 +44,10 @@ def test_single_event_configs(lst, oracle_mod, cfg, mask):
     assert len(want["t5_md"]) > 0
     assert_same(canon(got), canon(want), f"{cfg}: ")
     tests = want["n_tests"].astype(float)
-    # DESIGN.md reading N2: the 0.01 % bar is checked against the candidates of the stage
-    assert np.all(want["near"] <= np.maximum(1e-4 * tests, 0)), "near-threshold candidates above 0.01% of the candidates"
+    # the bar as CUTS.md section 0 states it (reading N2): against the candidates of the stage; the
+    # objects-denominated bar of north_star is missed by LS, T5, pT3, pT5 on PU200 and not asserted
+    assert np.all(want["near"] <= 1e-4 * tests), \
+        "near-threshold candidates above 0.01 % of the stage's candidates (CUTS.md section 0, DESIGN.md N2)"
 
 
 def test_device_resident_inputs_match_host_inputs(lst, oracle_mod):

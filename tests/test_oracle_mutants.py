@@ -137,6 +137,24 @@ MUTANTS = [
      "float f[6] = {fabsf(ki) * S, fabsf(kb) * S, fabsf(ko) * S,", "float f[6] = {fabsf(ki) * S, fabsf(ko) * S, fabsf(kb) * S,",
      V.check_t5_mlp),
     ("T5 MLP: output bias dropped", "s = p->t5_mlp[64];", "s = 0.0f;", V.check_t5_mlp),
+    # ---- the candidate counters of orc_run_event (the denominator of the near-threshold bar, reading N2) ----
+    ("n_tests[MD] counts accepted candidates only",
+     "ev->n_tests[ORC_ST_MD]++;\n          int acc = orc_md_test(p, endcap, x[a], y[a], z[a], x[b], y[b], z[b], vals, &nr);",
+     "int acc = orc_md_test(p, endcap, x[a], y[a], z[a], x[b], y[b], z[b], vals, &nr);\n          ev->n_tests[ORC_ST_MD] += acc;",
+     lambda O: P.test_bruteforce_all_pairs(O, "dense")),
+    ("n_tests[LS] counted once per map entry, not per candidate",
+     "for (int B = md_first[m2]; B < md_first[m2 + 1]; ++B) {\n          float vals[8];\n          int nr;\n          ev->n_tests[ORC_ST_LS]++;",
+     "ev->n_tests[ORC_ST_LS]++;\n        for (int B = md_first[m2]; B < md_first[m2 + 1]; ++B) {\n          float vals[8];\n          int nr;",
+     lambda O: P.test_bruteforce_all_pairs(O, "dense")),
+    ("n_tests[T3] goes to the LS counter",
+     "ev->n_tests[ORC_ST_T3]++;", "ev->n_tests[ORC_ST_LS]++;", lambda O: P.test_bruteforce_all_pairs(O, "dense")),
+    ("n_tests[T5] counts the first T3s that have a candidate, not the candidates",
+     "ev->n_tests[ORC_ST_T5]++;", "ev->n_tests[ORC_ST_T5] += (t2 == t3_first[C]);",
+     lambda O: P.test_bruteforce_all_pairs(O, "dense")),
+    ("n_tests[pT3] leaves out the accepted candidates",
+     "ev->n[ORC_K_PT3]++;", "ev->n[ORC_K_PT3]++;\n        ev->n_tests[ORC_ST_PT3]--;", lambda O: P.test_bruteforce_all_pairs(O, "dense")),
+    ("n_tests[pT5] goes to the pT3 counter",
+     "ev->n_tests[ORC_ST_PT5]++;", "ev->n_tests[ORC_ST_PT3]++;", lambda O: P.test_bruteforce_all_pairs(O, "dense")),
     ("g: third coefficient", "t = 0.075f + t;", "t = 0.75f + t;", P.test_g_taylor_coefficients),
     ("kappa3: factor 2", "return (2.0f * crs) / ((lpq * lqs) * lps);", "return (1.0f * crs) / ((lpq * lqs) * lps);",
      lambda O: P.test_kappa3_is_textbook_circumradius(O, 100.0, True)),

@@ -336,6 +336,10 @@ def test_bruteforce_all_pairs(oracle_mod, kind):
     hx = np.stack([ev.x, ev.y, ev.z], axis=1)
     n = ev.n_hits
 
+    # candidates visited and near-threshold flags raised per stage (MD, LS, T3, T5, pT3, pT5), counted by this
+    # enumeration: the oracle's n_tests / near counters (CUTS.md section 0) must equal them
+    n_cand, n_near = [0] * 6, [0] * 6
+
     # MD: every ordered hit pair of the whole event, kept only if (lower, upper) of one module
     mds = {}
     for a in range(n):
@@ -344,13 +348,16 @@ def test_bruteforce_all_pairs(oracle_mod, kind):
             if sa % 2 == 0 and sb == sa + 1:
                 m = sa // 2
                 acc, near, v = O.md_test(hx[a], hx[b], bool(geom.subdet[m]), p)
+                n_cand[0] += 1
+                n_near[0] += int(near)
                 if acc:
                     r = np.float32(np.sqrt(ev.x[a] * ev.x[a] + ev.y[a] * ev.y[a]))
                     ecap = bool(geom.subdet[m])
                     mds[(a, b)] = (m, np.array([*hx[a], r, 0 if ecap else v["ux"], 0 if ecap else v["uy"]], np.float32))
     assert sorted(mds) == [tuple(t) for t in c["md"]]
 
-    conn = {m: set(tgt[off[m]:off[m + 1]].tolist()) for m in range(geom.n_modules)}
+    conn = {m: tgt[off[m]:off[m + 1]].tolist() for m in range(geom.n_modules)}
+    assert all(len(set(row)) == len(row) for row in conn.values())  # no module twice in a row of the map
     keys = sorted(mds)
     # LS: every ordered MD pair, kept only if module(B) in conn[module(A)]
     lss = {}
@@ -360,6 +367,8 @@ def test_bruteforce_all_pairs(oracle_mod, kind):
             mB, fB = mds[B]
             if mB in conn[mA]:
                 acc, near, v = O.ls_test(fA, bool(geom.subdet[mA]), fB, bool(geom.subdet[mB]), p)
+                n_cand[1] += 1
+                n_near[1] += int(near)
                 if acc:
                     lss[(A, B)] = v["kappa"]
     assert sorted(a + b for a, b in lss) == [tuple(t) for t in c["ls"]]
@@ -371,6 +380,8 @@ def test_bruteforce_all_pairs(oracle_mod, kind):
             if B2 == B:
                 e = [bool(geom.subdet[mds[k][0]]) for k in (A, B, Cc)]
                 acc, near, v = O.t3_test(mds[A][1], e[0], mds[B][1], e[1], mds[Cc][1], e[2], p)
+                n_cand[2] += 1
+                n_near[2] += int(near)
                 if acc:
                     t3s[(A, B, Cc)] = v["k3"]
     assert sorted(a + b + d for a, b, d in t3s) == [tuple(t) for t in c["t3"]]
@@ -381,6 +392,8 @@ def test_bruteforce_all_pairs(oracle_mod, kind):
         for (C2, D, E), ko in t3s.items():
             if C2 == Cc:
                 acc, near, v = O.t5_test(ki, ko, mds[B][1], mds[Cc][1], mds[D][1], p)
+                n_cand[3] += 1
+                n_near[3] += int(near)
                 if acc:
                     t5s[(A, B, Cc, D, E)] = v["score"]
     assert sorted(sum(k, ()) for k in t5s) == [tuple(t) for t in c["t5"]]
@@ -392,17 +405,28 @@ def test_bruteforce_all_pairs(oracle_mod, kind):
         for ip in range(ev.n_pls):
             pls = [ev.pls[k][ip] for k in ("pt", "q", "x0", "y0", "z0", "x1", "y1", "z1")]
             for (A, B, Cc), k3 in t3s.items():
-                if O.pt_test(pls, mds[A][1], bool(geom.subdet[mds[A][0]]), mds[Cc][1],
-                             bool(geom.subdet[mds[Cc][0]]), [k3], 0.0, p)[0]:
+                t = O.pt_test(pls, mds[A][1], bool(geom.subdet[mds[A][0]]), mds[Cc][1],
+                              bool(geom.subdet[mds[Cc][0]]), [k3], 0.0, p)
+                n_cand[4] += 1
+                n_near[4] += int(t[1])
+                if t[0]:
                     pt3.append((ip,) + A + B + Cc)
             for (A, B, Cc, D, E), sc in t5s.items():
                 kt = [t3s[(A, B, Cc)], t3s[(Cc, D, E)]]
-                if O.pt_test(pls, mds[A][1], bool(geom.subdet[mds[A][0]]), mds[E][1],
-                             bool(geom.subdet[mds[E][0]]), kt, sc, p)[0]:
+                t = O.pt_test(pls, mds[A][1], bool(geom.subdet[mds[A][0]]), mds[E][1],
+                              bool(geom.subdet[mds[E][0]]), kt, sc, p)
+                n_cand[5] += 1
+                n_near[5] += int(t[1])
+                if t[0]:
                     pt5.append((ip,) + A + B + Cc + D + E)
         assert sorted(pt3) == [tuple(t) for t in c["pt3"]]
         assert sorted(pt5) == [tuple(t) for t in c["pt5"]]
         assert len(pt3) > 0 and len(pt5) > 0
+    # every candidate is counted once, accepted or not, and in no other stage's counter
+    assert min(n_cand[:4]) > 0 and (not ev.n_pls or min(n_cand[4:]) > 0)
+    assert [int(v) for v in res["n_tests"][:6]] == n_cand, "candidates per stage"
+    assert [int(v) for v in res["near"][:6]] == n_near, "near-threshold candidates per stage"
+    assert int(res["n_tests"][6]) == 0 and int(res["near"][6]) == 0  # T4 is off in the default stage mask
 
 
 # ------------------------------------------------------------------------------------------------
