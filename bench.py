@@ -15,8 +15,9 @@ T5, pT3, pT5, duplicate removal, track-candidate selection) = SURVEY.md section 
   kernels / kernels_full_grid : per-kernel CUDA-event times (lst_ctx_kernel_times) of L2-flushed batches on one
            stream, in the configuration of the timed region (--blocks-per-sm, default 2: kernels of different
            batches share the SMs) and with every kernel filling the GPU (8 blocks per SM)
-  roofline : the dominant kernel alone on the GPU (full grid); roofline_timed_config: the same in the timed
-           region's configuration
+  roofline : the dominant kernel in the launch configuration of the timed region; roofline_full_grid: the same
+           kernel filling the GPU on its own (8 blocks per SM)
+  step_roofline : the whole timed step against the HBM and the issue-rate rooflines (BASELINE.json's metric)
   cpu_baseline : the oracle (oracle/) on the host cores over a bounded sample of the same events
 
 Multi-GPU (N > 1): replicas only -- every rank runs its own batches (different seeds), no
@@ -62,6 +63,11 @@ def parse_args():
                          "(8 = every kernel fills the GPU; 1-2 let kernels of different batches share the SMs)")
     ap.add_argument("--batches", type=int, default=6, help="distinct input batches rotated through")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stage-mask", type=lambda v: int(v, 0), default=None,
+                    help="diagnostic: run the chain only up to a stage (CUTS.md section 9); written to config, "
+                         "a line produced with it is not a benchmark of the whole path")
+    ap.add_argument("--no-l2-flush", action="store_true",
+                    help="diagnostic: per-kernel times with a warm L2; written to config")
     ap.add_argument("--profile-kernels-only", action="store_true",
                     help="run only the L2-flushed single-stream loop (the command ncu wraps)")
     return ap.parse_args()
@@ -206,16 +212,49 @@ def oracle_params(workload):
     return None
 
 
-def workload_params(lst, workload):
-    """Cut constants of the workload: CUTS.md defaults for C5; C6 opens the r-z windows to the strip length."""
+def workload_params(lst, workload, stage_mask=None):
+    """Cut constants of the workload: CUTS.md defaults for C5; C6 opens the r-z windows to the strip length.
+    stage_mask (--stage-mask, diagnostic only) cuts the chain short; it is recorded in the line's config."""
+    kw = {}
     if workload == "C6":
         from lst_inputs.configs import C6_PARAMS
 
-        return lst.lst_default_params(**C6_PARAMS)
-    mask = os.environ.get("LST_BENCH_STAGE_MASK")  # diagnostic only: cost of the chain up to a stage (CUTS.md section 9)
-    if mask:
-        return lst.lst_default_params(stage_mask=int(mask, 0))
-    return None
+        kw.update(C6_PARAMS)
+    if stage_mask is not None:
+        kw["stage_mask"] = int(stage_mask)
+    return lst.lst_default_params(**kw) if kw else None
+
+
+def step_roofline(kernels, ms_step, hbm_gbs, peak_src, sm_max_mhz, args, E):
+    """BASELINE.json's metric at step level: what the whole timed step reaches of the HBM roofline (sum of the kernels'
+    algorithmic bytes / step time) and of the issue-rate roofline (sum of the executed warp instructions / step
+    time).  Bytes are computed from this run's object counts; instruction counts need a profiler, so they come from the
+    committed ncu capture (profiles/traffic.json) and only when it was taken on this workload."""
+    alg = int(sum(k["alg_bytes"] for k in kernels))
+    gbs = alg / (ms_step * 1e-3) / 1e9
+    out = {"alg_bytes_per_step": alg, "gbs": round(gbs, 1), "hbm_peak_gbs": hbm_gbs, "hbm_frac": round(gbs / hbm_gbs, 4),
+           "hbm_peak_source": peak_src + " copy bandwidth",
+           "alg_bytes_source": "sum over the kernels of bench.algorithmic_work (every input read once, every output "
+                               "written once) for this run's object counts",
+           "ms_per_step": round(ms_step, 5), "warp_inst_per_step": None, "issue_frac": None, "dram_bytes_cold": None,
+           "warp_inst_source": None}
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            cap = json.load(f)
+        key = "kernels" if args.blocks_per_sm not in (0, 8) else "kernels_full_grid"
+        names = [k["name"] for k in kernels]
+        if cap.get("workload") == args.workload and cap.get("pu") == args.pu and cap.get("events") == E \
+                and args.stage_mask is None and all(n in cap.get(key, {}) for n in names):
+            wi = int(sum(cap[key][n].get("warp_inst", 0) for n in names))
+            issue_peak = 148 * 4 * sm_max_mhz * 1e6  # 148 SMs x 4 schedulers x clock (SURVEY.md 8(d))
+            out["warp_inst_per_step"] = wi
+            out["issue_frac"] = round(wi / (ms_step * 1e-3) / issue_peak, 4)
+            out["dram_bytes_cold"] = int(sum(cap[key][n].get("dram_bytes", 0) for n in names))
+            out["warp_inst_source"] = ("ncu capture %s (stored, not measured in this run; dram_bytes_cold = every kernel "
+                                       "alone with caches flushed, an upper bound of the step's HBM traffic)"
+                                       % cap.get("capture", "?"))
+    return out
 
 
 def peaks():
@@ -256,7 +295,7 @@ def run_b200(args):
     batches = make_batches(args.pu, E, NB, rank, world, args.workload)
     gen_s = time.time() - t0
 
-    g = lst.lst_load_geometry(geom.module_table(), off, tgt, workload_params(lst, args.workload))
+    g = lst.lst_load_geometry(geom.module_table(), off, tgt, workload_params(lst, args.workload, args.stage_mask))
     caps = lst.lst_default_caps(max_events=E)
     streams = [torch.cuda.Stream() for _ in range(S)]
     ctxs = [lst.lst_ctx_create(g, caps, st.cuda_stream) for st in streams]
@@ -361,7 +400,7 @@ def run_b200(args):
         for r in range(reps + 2):
             b = r % NB
             with torch.cuda.stream(streams[0]):
-                if not os.environ.get("LST_BENCH_NO_FLUSH"):  # diagnostic only: warm-L2 kernel times
+                if not args.no_l2_flush:
                     flush.zero_()
             lst.lst_ctx_run(ctxs[0], E, dev_in[b][0], dev_in[b][1])
             s_b = lst.lst_ctx_sync(ctxs[0])
@@ -424,20 +463,17 @@ def run_b200(args):
                     roof["warp_inst"] = k["warp_inst"]
         return roof
 
-    # `roofline`: the dominant kernel ALONE ON THE GPU with its full grid (8 blocks per SM) -- what the kernel achieves
-    # of the peak.  With --blocks-per-sm 1..4 (the timed region) a kernel takes only that share of every SM by design
-    # and leaves the rest to the kernels of other batches, so its duration alone in that configuration
-    # (`roofline_timed_config`) measures the share it was given, not its efficiency.
-    cfg = "%d blocks per SM per kernel, kernel alone on one stream, L2 flushed"
+    # `roofline`: the dominant kernel in the LAUNCH CONFIGURATION OF THE TIMED REGION (--blocks-per-sm), timed alone on
+    # one stream.  With 1..4 blocks per SM a kernel takes only that share of every SM by design and leaves the rest to
+    # the kernels of other batches, so this is the kernel as the step runs it, not the most the kernel can reach:
+    # `roofline_full_grid` is the same kernel filling the GPU on its own (8 blocks per SM).
+    cfg = "%d blocks per SM per kernel, kernel alone on one stream, L2 " + ("warm" if args.no_l2_flush else "flushed")
+    roof = make_roof(kernels, "kernels" if args.blocks_per_sm not in (0, 8) else "kernels_full_grid")
+    roof["launch"] = cfg % (args.blocks_per_sm or 8) + " (the configuration of the timed region)"
+    roof_full = None
     if kernels_alone:
-        roof = make_roof(kernels_alone, "kernels_full_grid")
-        roof["launch"] = cfg % 8
-        roof_cfg = make_roof(kernels, "kernels")
-        roof_cfg["launch"] = cfg % args.blocks_per_sm + " (the configuration of the timed region)"
-    else:
-        roof = make_roof(kernels, "kernels" if args.blocks_per_sm not in (0, 8) else "kernels_full_grid")
-        roof["launch"] = cfg % (args.blocks_per_sm or 8)
-        roof_cfg = None
+        roof_full = make_roof(kernels_alone, "kernels_full_grid")
+        roof_full["launch"] = cfg % 8
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -448,6 +484,35 @@ def run_b200(args):
             lst.lst_free(c)
         lst.lst_free(g)
         return
+
+    # ---- PCIe: what a pinned host -> device copy of one step's input reaches on this box, next to what e2e moved ----
+    nbytes = int(np.mean(in_bytes))
+    src = [torch.zeros(nbytes, dtype=torch.uint8).pin_memory() for _ in range(S)]
+    dst = [torch.empty(nbytes, dtype=torch.uint8, device="cuda") for _ in range(S)]
+
+    def h2d_rate(n_streams, reps):
+        """GB/s of `reps` pinned host -> device copies of one step's input per stream, n_streams streams at once."""
+        t0 = torch.cuda.Event(enable_timing=True)
+        t1 = [torch.cuda.Event(enable_timing=True) for _ in range(n_streams)]
+        torch.cuda.synchronize()
+        t0.record(streams[0])
+        for k in range(n_streams):
+            streams[k].wait_event(t0)
+            with torch.cuda.stream(streams[k]):
+                for r in range(reps):
+                    dst[k].copy_(src[k], non_blocking=True)
+            t1[k].record(streams[k])
+        torch.cuda.synchronize()
+        return n_streams * reps * nbytes / (max(t0.elapsed_time(e) for e in t1) * 1e-3) / 1e9
+
+    h2d_rate(S, 2)
+    h2d_one, h2d_peak = h2d_rate(1, 20), h2d_rate(S, 10)
+    e2e_gbs = (nbytes + d2h / args.steps) / (ms_e2e / args.steps * 1e-3) / 1e9
+    pcie = {"pcie_h2d_peak_gbs": round(h2d_peak, 1), "pcie_h2d_one_stream_gbs": round(h2d_one, 1),
+            "pcie_gbs": round(e2e_gbs, 1), "pcie_frac": round(e2e_gbs / max(h2d_peak, h2d_one), 3),
+            "pcie_note": "peak = pinned cudaMemcpyAsync host -> device of one step's input size, 10 copies on each of "
+                         "the %d streams at once (one stream alone: 20 copies), measured in this run; pcie_gbs = (H2D + "
+                         "D2H bytes per step) / e2e ms per step; pcie_frac = pcie_gbs / the larger of the two" % S}
 
     # ---- CPU baseline (rank 0, N = 1 only) -------------------------------------------------------
     cpu = None
@@ -476,16 +541,19 @@ def run_b200(args):
             "near_frac_of_objects": {k: (round(n / ksum["n_" + k], 9) if ksum["n_" + k] else None) for k, n in
                                      zip(("md", "ls", "t3", "t5", "pt3", "pt5"), ksum["near"])},
             "generation_s": round(gen_s, 1),
+            "stage_mask": hex(args.stage_mask) if args.stage_mask is not None else "default (0x3f, whole chain)",
+            "l2_flush_per_kernel_pass": not args.no_l2_flush,
         },
         "e2e": {"value": round(world * args.steps * E / (ms_e2e * 1e-3), 1), "unit": UNIT,
                 "h2d_bytes_per_step": int(np.mean(in_bytes)), "d2h_bytes_per_step": int(d2h / args.steps),
                 "input_format": "x, y, z float32 + sensor %s per hit; 8 x 4 bytes per seed" % ("uint16" if u16 else "int32"),
-                "ms_per_step": round(ms_e2e / args.steps, 5)},
+                "ms_per_step": round(ms_e2e / args.steps, 5), **pcie},
         "gpu_launches": launches,
         "clocks": sampler.summary(),
         "roofline": roof,
+        "step_roofline": step_roofline(kernels, ms / args.steps, hbm_gbs, peak_src, sm_max_mhz, args, E),
         "kernels": kernels,
-        "roofline_timed_config": roof_cfg,
+        "roofline_full_grid": roof_full,
         "kernels_full_grid": kernels_alone,
         "objects_per_s": {k: round(ksum["n_" + k] / (ms / args.steps * 1e-3), 1)
                           for k in ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")},

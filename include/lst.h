@@ -59,7 +59,8 @@ typedef struct lst_params {
   float t3_kappa_max, t3_z_tol0, t3_z_tol1;
   float t5_tol0, t5_tol1;
   float pt_gate_tol, pt_k_tol0, pt_k_tol1, pt_z_tol;
-  float near_rel;
+  float near_rel; /* NEAR_REL of CUTS.md section 0; 0 <= near_rel <= 1e-5 (the default), else lst_load_geometry
+                     returns LST_ERR_ARG: the kernels' pre-filters are sized for a near window of at most 1e-5 */
   int32_t stage_mask; /* bit0 MD, 1 LS, 2 T3, 3 T5, 4 pT3/pT5, 5 duplicate removal + TC, 6 T4, 7 learned T5 */
   /* extensions of CUTS.md sections 10 and 11, used only with stage_mask bits 6 / 7 */
   float t4_tol0, t4_tol1;
@@ -204,8 +205,14 @@ int lst_ctx_fetch_tc(lst_ctx* ctx, int32_t* tc, int32_t cap_tc, int32_t* tc_even
  * changes no result, only who shares the SMs: with several contexts in flight on different streams
  * (PAPER.md:79 ran 2 streams; BASELINE.json configs[4] "pipelined over CUDA streams") kernels of different
  * batches co-reside and hide each other's latency when each takes 1-2 blocks per SM.  May be called
- * between batches (the captured launch sequence is rebuilt).  Returns LST_ERR_ARG for blocks outside 0..8. */
+ * between batches (the captured launch sequence is rebuilt; a batch still in flight is waited for first).  Returns LST_ERR_ARG for blocks outside 0..8. */
 int lst_ctx_set_blocks_per_sm(lst_ctx* ctx, int32_t blocks);
+
+/* How lst_ctx_run launches the chain.  enable != 0 (the default for a context on a stream of the caller's): the
+ * launch sequence is captured once as a CUDA graph and replayed per batch; enable == 0: the kernels are launched
+ * one by one (what a context on the legacy default stream, which cannot be captured, always does).  Same
+ * kernels, same results.  Returns LST_ERR_ARG for enable != 0 on a context of the legacy default stream. */
+int lst_ctx_set_graph(lst_ctx* ctx, int32_t enable);
 
 /* Per-kernel device times of the last batch, measured with CUDA events on the context's stream.
  * enable != 0 switches the recording on for the following lst_ctx_run calls. */

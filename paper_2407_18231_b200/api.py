@@ -170,6 +170,11 @@ def lst_ctx_set_blocks_per_sm(ctx, blocks: int) -> None:
     _check(_lib().lst_ctx_set_blocks_per_sm(ctx, int(blocks)), "lst_ctx_set_blocks_per_sm")
 
 
+def lst_ctx_set_graph(ctx, enable: bool) -> None:
+    """Replay the captured CUDA graph per batch (default on a caller's stream) or launch kernel by kernel."""
+    _check(_lib().lst_ctx_set_graph(ctx, int(bool(enable))), "lst_ctx_set_graph")
+
+
 def lst_ctx_set_timing(ctx, enable: bool) -> None:
     _check(_lib().lst_ctx_set_timing(ctx, int(bool(enable))), "lst_ctx_set_timing")
 

@@ -91,7 +91,7 @@ class lst_batch_summary(C.Structure):
 ABI_SYMBOLS = (
     "lst_strerror", "lst_default_params", "lst_default_caps", "lst_workspace_bytes", "lst_load_geometry",
     "lst_run_event", "lst_free", "lst_ctx_create", "lst_ctx_run", "lst_ctx_sync", "lst_ctx_fetch_event",
-    "lst_ctx_fetch_tc", "lst_ctx_set_blocks_per_sm", "lst_ctx_set_timing", "lst_ctx_kernel_times", "lst_ctx_launch_count", "lst_ctx_stat",
+    "lst_ctx_fetch_tc", "lst_ctx_set_blocks_per_sm", "lst_ctx_set_graph", "lst_ctx_set_timing", "lst_ctx_kernel_times", "lst_ctx_launch_count", "lst_ctx_stat",
     "lst_scan_counts", "lst_scan_counts_static",
 )
 
@@ -131,6 +131,7 @@ def _lib():
     L.lst_ctx_fetch_tc.argtypes = [vp, _ip, C.c_int32, _ip]
     L.lst_ctx_set_timing.argtypes = [vp, C.c_int32]
     L.lst_ctx_set_blocks_per_sm.argtypes = [vp, C.c_int32]
+    L.lst_ctx_set_graph.argtypes = [vp, C.c_int32]
     L.lst_ctx_kernel_times.argtypes = [vp, _fp, C.POINTER(C.c_char_p), C.c_int32]
     L.lst_ctx_launch_count.argtypes = [vp]
     L.lst_ctx_stat.argtypes = [vp, C.c_int32]

@@ -148,6 +148,10 @@ extern "C" int lst_load_geometry(const lst_module* modules, int32_t n_modules, c
   if (!out) return LST_ERR_ARG;
   *out = nullptr;
   if (!modules || n_modules <= 0 || !conn_offsets) return LST_ERR_ARG;
+  // The approximate pre-filters in front of the exact cuts (lst_cuts.cuh, lst_cuts_pt.cuh, lst_ls.cuh, lst_pt.cuh)
+  // leave every candidate within NEAR_REL = 1e-5 of a threshold to the exact cut; their bands are constants sized
+  // for that value.  A wider near window would be classified by them and never counted: refused, not mis-counted.
+  if (params && !(params->near_rel >= 0.0f && params->near_rel <= 1e-5f)) return LST_ERR_ARG;
   if (conn_offsets[0] != 0) return LST_ERR_GEOMETRY;
   for (int m = 0; m < n_modules; ++m) {
     if (conn_offsets[m + 1] < conn_offsets[m]) return LST_ERR_GEOMETRY;
@@ -398,7 +402,7 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
   ctx->timing = false;
   ctx->graph = nullptr;
   ctx->owned_stream = nullptr;
-  ctx->use_graph = getenv("LST_NO_GRAPH") == nullptr && cuda_stream != nullptr;  // the legacy default stream cannot be captured
+  ctx->use_graph = cuda_stream != nullptr;  // lst_ctx_set_graph;  // the legacy default stream cannot be captured
   ctx->n_kernels = 0;
   ctx->last_n_events = 0;
   ctx->synced = true;

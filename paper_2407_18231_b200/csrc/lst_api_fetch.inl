@@ -83,10 +83,25 @@ extern "C" int lst_ctx_fetch_event(lst_ctx* ctx, int32_t ev, lst_event_out** out
   o->t4_t3 = halloc<int32_t>(2 * (size_t)o->n_t4);
   o->t4_md = halloc<int32_t>(4 * (size_t)o->n_t4);
   o->t4_score = halloc<float>(o->n_t4);
-  std::vector<int> info(n_md);
-  std::vector<float4> a(n_md);
-  std::vector<float2> u(n_md);
-  std::vector<int4> m3(n_t3);
+  // host memory: a failed allocation is an error code, never a NULL destination or an exception across the ABI
+  const void* const bufs[] = {o->md_hits, o->md_module, o->md_f, o->ls_md, o->ls_kappa, o->t3_ls, o->t3_md, o->t3_k,
+                              o->t5_t3, o->t5_md, o->t5_score, o->pt3, o->pt3_score, o->pt5, o->pt5_score, o->tc,
+                              o->t4_t3, o->t4_md, o->t4_score};
+  bool have = true;
+  for (const void* b : bufs) have = have && b != nullptr;
+  std::vector<int> info;
+  std::vector<float4> a;
+  std::vector<float2> u;
+  std::vector<int4> m3;
+  try {
+    info.resize(n_md);  a.resize(n_md);  u.resize(n_md);  m3.resize(n_t3);
+  } catch (const std::bad_alloc&) {
+    have = false;
+  }
+  if (!have) {
+    out_destroy(o);
+    return LST_ERR_CUDA;
+  }
   // every copy goes to the context's stream; one synchronisation, then the index shifts on the host
   bool ok = d2h(reinterpret_cast<int2*>(o->md_hits), d.md_hit, f_md, n_md) &&
             d2h(info.data(), d.md_info, f_md, n_md) && d2h(a.data(), d.md_a, f_md, n_md) &&

@@ -255,10 +255,18 @@ extern "C" int lst_ctx_set_blocks_per_sm(lst_ctx* ctx, int32_t blocks) {
   if (!ctx || ctx->magic != MAGIC_CTX || blocks < 0 || blocks > 8) return LST_ERR_ARG;
   const int b = blocks == 0 ? 8 : blocks;
   if (b != ctx->blocks_per_sm && ctx->graph) {  // the captured launch sequence holds the old grids
+    if (!ctx->synced) CK(cudaStreamSynchronize(ctx->stream));  // a batch still in flight finishes on the old grids first
     cudaGraphExecDestroy(ctx->graph);
     ctx->graph = nullptr;
   }
   ctx->blocks_per_sm = b;
+  return LST_OK;
+}
+
+extern "C" int lst_ctx_set_graph(lst_ctx* ctx, int32_t enable) {
+  if (!ctx || ctx->magic != MAGIC_CTX) return LST_ERR_ARG;
+  if (enable && !ctx->stream) return LST_ERR_ARG;  // the legacy default stream cannot be captured
+  ctx->use_graph = enable != 0;
   return LST_OK;
 }
 

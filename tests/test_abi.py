@@ -89,6 +89,10 @@ def test_argument_errors_are_reported_before_any_cuda_call(lst):
     with pytest.raises(lst.LstError) as e:
         lst.lst_load_geometry(mods, [0, 2, 1, 1], [0, 1])  # decreasing offsets
     assert e.value.status == lst.LST_ERR_GEOMETRY
+    for bad_rel in (1e-4, 1.1e-5, -1e-6, float("nan")):  # the near window the pre-filters are sized for: [0, 1e-5]
+        with pytest.raises(lst.LstError) as e:
+            lst.lst_load_geometry(mods, [0, 0, 0, 0], [], lst.lst_default_params(near_rel=bad_rel))
+        assert e.value.status == lst.LST_ERR_ARG
     lst.lst_free(None)  # NULL is a no-op
 
 

@@ -127,6 +127,35 @@ def test_cut_constants_tuned_onto_candidates(lst, oracle_mod):
     assert flagged == {0, 1, 2, 3, 4, 5}
 
 
+def test_narrower_near_windows(lst, oracle_mod):
+    """near_rel is an input (lst_params, CUTS.md section 0).  The kernels' pre-filters hand every candidate within
+    1e-5 of a threshold to the exact cut, so any window up to that is counted exactly as the oracle counts it --
+    here 0 (only v == t is flagged) and 2.5e-6, with a constant tuned onto a candidate and one ulp to either side;
+    a wider window is refused (LST_ERR_ARG, include/lst.h)."""
+    O = oracle_mod
+    geom, off, tgt = make_config_geometry("C4")
+    ev = make_config_event("C4")
+    base = O.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+    seen = np.zeros((2, 7), np.int64)
+    for stage, name, value in tuned_constants(O, geom, ev, base):
+        for j, rel in enumerate((0.0, 2.5e-6)):
+            for du in (-1, 0, 1):
+                kw = {name: _ulps(value, du), "near_rel": rel}
+                want = O.run_event(geom.subdet, off, tgt, ev.x, ev.y, ev.z, ev.sensor, ev.pls, O.default_params(**kw))
+                g = lst.lst_load_geometry(geom.module_table(), off, tgt, lst.lst_default_params(**kw))
+                try:
+                    got = lst.lst_run_event(g, ev.x, ev.y, ev.z, ev.sensor, ev.pls)
+                finally:
+                    lst.lst_free(g)
+                assert_same(canon(got), canon(want), f"near_rel = {rel}, {name} {du:+d} ulp: ")
+                seen[j] += want["near"]
+    assert np.all(seen[1][:6] > 0), seen          # the narrow window still flags the tuned candidates
+    assert np.all(seen[0] <= seen[1]) and seen[0].sum() > 0, seen   # v == t exactly happens at 0 ulp
+    with pytest.raises(lst.LstError) as e:
+        lst.lst_load_geometry(geom.module_table(), off, tgt, lst.lst_default_params(near_rel=1e-4))
+    assert e.value.status == lst.LST_ERR_ARG
+
+
 def straight_dense_event(n_trk=90, seed=11):
     """Near-parallel straight tracks through a chain of five barrel modules (thousands of T3s / T5s whose
     circle through a seed has |kx| ~ 1e-6 ... 1e-5), with 40 seeds per track direction whose pT scans
