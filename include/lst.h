@@ -230,6 +230,29 @@ int lst_ctx_launch_count(lst_ctx* ctx);
 enum { LST_STAT_PT_QUEUE = 0, LST_STAT_WORKSPACE_MB = 1 };
 int64_t lst_ctx_stat(lst_ctx* ctx, int32_t which);
 
+/* ---- audit of the approximate cut cascades ------------------------------------------------------ */
+
+/* MD, LS and the seed linking decide most candidates with cheaper arithmetic than CUTS.md's (approximate
+ * reciprocal square roots and divisions, bounding circles) inside error bands; only what falls inside a band is
+ * given to the exact cuts.  lst_ctx_audit checks, on the batch the context has just run
+ * (after lst_ctx_sync, before the next lst_ctx_run), that none of those decisions was wrong: it re-evaluates EVERY
+ * candidate of the three stages with the exact cuts only -- all hit pairs of a module (CUTS.md 3), all MD pairs along
+ * the connection map (4), all (seed, T3) and (seed, T5) pairs of an event (7) -- and compares, per stage, the
+ * number of candidates, of accepted and of near-threshold candidates and a 64-bit order-independent hash of the
+ * accepted candidates' identities with what the chain counted and stored.  Index 0 MD, 1 LS, 2 pT3, 3 pT5; a
+ * stage that the stage mask switches off (or pT without seeds) stays 0.  mismatches = how many of those
+ * comparisons differ: 0 means every pre-filter decision of the batch agreed with the exact cuts and hid no
+ * near-threshold candidate.  A debugging call: allocates a few hundred bytes, synchronises the stream, takes
+ * milliseconds; never used by lst_ctx_run.  rep: host.  Errors: LST_ERR_ARG (no synchronised batch), the
+ * batch's own error, LST_ERR_CUDA. */
+typedef struct lst_audit_report {
+  int64_t candidates[4], accepted[4], near[4];                   /* by the exact cuts on every candidate */
+  int64_t chain_candidates[4], chain_objects[4], chain_near[4];  /* what the chain counted and stored */
+  uint64_t hash_exact[4], hash_chain[4];
+  int64_t mismatches;
+} lst_audit_report;
+int lst_ctx_audit(lst_ctx* ctx, lst_audit_report* rep);
+
 /* ---- slot offsets from per-owner counts, stand-alone ------------------------------------------- */
 
 /* Every stage of the chain is "owner -> a variable number of accepted objects" (an MD owns its

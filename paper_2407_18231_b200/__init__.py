@@ -10,4 +10,4 @@ from .binding import (ABI_SYMBOLS, LST_ERR_ARG, LST_ERR_CAPACITY, LST_ERR_CUDA, 
 from .api import (event_out_to_dict, lst_ctx_create, lst_ctx_fetch_event, lst_ctx_fetch_tc,  # noqa: F401
                   lst_ctx_kernel_times, lst_ctx_launch_count, lst_ctx_run, lst_ctx_set_blocks_per_sm, lst_ctx_set_graph, lst_ctx_set_timing, lst_ctx_sync,
                   lst_run_event, make_hits, make_pls, lst_ctx_stat, LST_STAT_PT_QUEUE, LST_STAT_WORKSPACE_MB,
-                  lst_scan_counts, lst_scan_counts_static)
+                  lst_scan_counts, lst_scan_counts_static, lst_ctx_audit, AUDIT_STAGES)

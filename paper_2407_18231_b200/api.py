@@ -9,7 +9,7 @@ import ctypes as C
 
 import numpy as np
 
-from .binding import (LST_OK, N_STAGES, LstError, _check, _fp, _ip, _lib, lst_batch_summary, lst_caps,
+from .binding import (LST_OK, N_STAGES, LstError, _check, _fp, _ip, _lib, lst_audit_report, lst_batch_summary, lst_caps,
                       lst_event_out, lst_hits, lst_pls)
 
 _PLS_F = ("pt", "x0", "y0", "z0", "x1", "y1", "z1")
@@ -232,3 +232,14 @@ def lst_scan_counts_static(counts, offsets, cuda_stream: int | None = None) -> N
     c, n, o = _scan_args(counts, offsets, "lst_scan_counts_static")
     _check(_lib().lst_scan_counts_static(c, n, o, C.c_void_p(cuda_stream) if cuda_stream else None),
            "lst_scan_counts_static")
+
+
+AUDIT_STAGES = ("md", "ls", "pt3", "pt5")
+
+
+def lst_ctx_audit(ctx) -> dict:
+    """Re-evaluates every MD, LS, pT3 and pT5 candidate of the last synchronised batch with the exact cuts on the GPU
+    and compares counts, near flags and a hash of the accepted set with what the chain produced (include/lst.h)."""
+    rep = lst_audit_report()
+    _check(_lib().lst_ctx_audit(ctx, C.byref(rep)), "lst_ctx_audit")
+    return rep.as_dict()

@@ -87,12 +87,23 @@ class lst_batch_summary(C.Structure):
         return d
 
 
+class lst_audit_report(C.Structure):
+    _fields_ = [(f, C.c_int64 * 4) for f in ("candidates", "accepted", "near", "chain_candidates", "chain_objects",
+                                              "chain_near")] + \
+        [("hash_exact", C.c_uint64 * 4), ("hash_chain", C.c_uint64 * 4), ("mismatches", C.c_int64)]
+
+    def as_dict(self):
+        d = {f: [int(v) for v in getattr(self, f)] for f, _ in self._fields_[:8]}
+        d["mismatches"] = int(self.mismatches)
+        return d
+
+
 # every symbol include/lst.h declares (tests check the library exports all of them)
 ABI_SYMBOLS = (
     "lst_strerror", "lst_default_params", "lst_default_caps", "lst_workspace_bytes", "lst_load_geometry",
     "lst_run_event", "lst_free", "lst_ctx_create", "lst_ctx_run", "lst_ctx_sync", "lst_ctx_fetch_event",
     "lst_ctx_fetch_tc", "lst_ctx_set_blocks_per_sm", "lst_ctx_set_graph", "lst_ctx_set_timing", "lst_ctx_kernel_times", "lst_ctx_launch_count", "lst_ctx_stat",
-    "lst_scan_counts", "lst_scan_counts_static",
+    "lst_scan_counts", "lst_scan_counts_static", "lst_ctx_audit",
 )
 
 _LIB = None
@@ -137,6 +148,7 @@ def _lib():
     L.lst_ctx_stat.argtypes = [vp, C.c_int32]
     L.lst_ctx_stat.restype = C.c_int64
     L.lst_scan_counts.argtypes = [vp, C.c_int32, vp, vp]
+    L.lst_ctx_audit.argtypes = [vp, C.POINTER(lst_audit_report)]
     L.lst_scan_counts_static.argtypes = [vp, C.c_int32, vp, vp]
     _LIB = L
     return L

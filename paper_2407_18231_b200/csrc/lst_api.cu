@@ -12,6 +12,7 @@
 
 #include "../../include/lst.h"
 #include "lst_select.cuh"
+#include "lst_audit.cuh"
 
 using namespace lst;
 
@@ -457,3 +458,4 @@ extern "C" int lst_ctx_create(lst_geometry* g, const lst_caps* caps, void* cuda_
 #include "lst_api_run.inl"
 #include "lst_api_fetch.inl"
 #include "lst_api_static.inl"
+#include "lst_api_audit.inl"
