@@ -29,15 +29,29 @@ def sources():
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(SO) and os.path.getmtime(SO) >= max(os.path.getmtime(s) for s in sources()):
         return SO
+    return _compile(SO, [], verbose)
+
+
+def _compile(out: str, defines, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = SO + f".tmp{os.getpid()}"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    tmp = out + f".tmp{os.getpid()}"
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [f"-D{d}" for d in defines] + \
           ["-I", INCLUDE, "-o", tmp, os.path.join(CSRC, "lst_api.cu")]
     subprocess.run(cmd, check=True)
-    os.replace(tmp, SO)
-    return SO
+    os.replace(tmp, out)
+    return out
+
+
+def build_variant(out: str, defines) -> str:
+    """A debugging build next to the product (never loaded by the package): the same sources with extra -D macros,
+    e.g. LST_DEBUG_SYNC (waits and prints before every kernel) or the reproducer of profiles/r03_rule3_fault.md."""
+    return _compile(os.path.abspath(out), list(defines))
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    if "--variant" in sys.argv:  # python -m paper_2407_18231_b200.build --variant OUT.so MACRO [MACRO ...]
+        i = sys.argv.index("--variant")
+        print(build_variant(sys.argv[i + 1], sys.argv[i + 2:]))
+    else:
+        print(build(force=True, verbose="-v" in sys.argv))

@@ -218,6 +218,9 @@ struct Bump {
 inline int tiles_of(long long n, int tile) { return (int)((n + tile - 1) / tile) + 2; }
 
 // Fills the pointer table of `dev` (pointers are offsets from `base`; base == nullptr only sizes).
+// Rule: everything a kernel reads before a kernel of the SAME batch has written it -- counters, cursors, tickets,
+// status words, flags that are only ever set (linked) -- lives in the leading region that is cleared per batch.
+// An array outside it still holds the previous batch of this context.
 // Returns total bytes; *zero_bytes = size of the leading region that is memset per batch.
 size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, size_t* zero_bytes) {
   Bump b{base, 0};
@@ -244,6 +247,9 @@ size_t layout(const lst_caps& c, int n_mod, char* base, Dev& d, lst_ctx* ctx, si
   d.tc_cnt = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
   d.tc_cur = b.take<int>(kTcClasses * (size_t)c.max_events + 1);
   d.linked = b.take<unsigned char>(c.max_pls);
+#ifdef LST_RULE3_SKIP_COVERED
+  d.t5_cov = b.take<unsigned char>(c.max_t5);
+#endif
   d.ls_cnt = b.take<int>(c.max_md);
   d.ls_cur = b.take<int>(c.max_md);
   b.off = (b.off + 255) & ~size_t(255);

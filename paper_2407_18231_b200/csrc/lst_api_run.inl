@@ -15,6 +15,12 @@ struct Launcher {
   int k = 0;
   bool capturing = false;
   void mark(const char* name) {
+#ifdef LST_DEBUG_SYNC  // debugging build only: wait for everything launched so far and say which kernel comes next
+    if (!capturing) {
+      const cudaError_t e = cudaStreamSynchronize(ctx->stream);
+      fprintf(stderr, "[lst] before %s: %s\n", name, cudaGetErrorString(e));
+    }
+#endif
     if (ctx->timing && !capturing && k < kMaxKernels) {
       cudaEventRecord(ctx->ev[k], ctx->stream);
       ctx->kname[k] = name;

@@ -192,6 +192,9 @@ __global__ void __launch_bounds__(kBlock) k_rule1(Dev d) {
       d.keep5[X] = keep;
       if (keep) {
         d.linked[x.x] = 1;  // one writer per value; rule 4 (k_rule3) completes it with the surviving pT3s
+#ifdef LST_RULE3_SKIP_COVERED
+        d.t5_cov[x.y] = 1;
+#endif
         atomicAdd(d.tc_cnt + kTcClasses * d.pls_event[x.x] + 0, 1);
       }
     }
@@ -305,15 +308,35 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
   const int n_groups = stride / kRuleLanes, g0 = i0 / kRuleLanes;
   for (int X0 = 0; X0 < n; X0 += n_groups) {
     const int X = X0 + g0;
+#ifdef LST_RULE3_SKIP_COVERED
+    // NOT part of the product: the variant that faults (profiles/r03_rule3_fault.md).  A T5 with a surviving pT5 built
+    // on it (rule 3b, all five MDs shared) skips its lists.  Same results by the spec; built with this macro the
+    // kernel gives wrong survivor sets within a few batches and then hangs or faults -- unless the MD of a lane's
+    // list is picked by selects (LST_RULE3_SELECT) instead of mX[2 * task] / mX[task - 3] / mX[task - 7].
+    bool rem = X < n && d.t5_cov[X] != 0;
+#else
     bool rem = false;
+#endif
     int md0 = 0;
-    if (X < n && task < 11) {
+    if (X < n && task < 11 && !rem) {
       const float sX = d.t5_score[X];
       int mX[5], mY[5];
       load_t5_md(d, X, mX);
       md0 = mX[0];
+#ifdef LST_RULE3_SELECT
+      const int t4 = task < 7 ? task - 3 : task - 7;
+      const int md_a = task == 0 ? mX[0] : (task == 1 ? mX[2] : mX[4]);
+      const int md_b = t4 == 0 ? mX[0] : (t4 == 1 ? mX[1] : (t4 == 2 ? mX[2] : mX[3]));
+#define LST_MD_A md_a
+#define LST_MD_B md_b
+#define LST_MD_C md_b
+#else
+#define LST_MD_A mX[2 * task]
+#define LST_MD_B mX[task - 3]
+#define LST_MD_C mX[task - 7]
+#endif
       if (task < 3) {
-        for (IdxIt it(d, n_md, 0, mX[2 * task]); it.obj >= 0 && !rem; it.advance()) {
+        for (IdxIt it(d, n_md, 0, LST_MD_A); it.obj >= 0 && !rem; it.advance()) {
           const int Y = it.obj;
           if (Y == X) continue;
           load_t5_md(d, Y, mY);
@@ -321,14 +344,14 @@ __global__ void __launch_bounds__(kBlock) k_rule3(Dev d) {
         }
       } else if (task < 7) {
         if (n_pt5 > 0)
-          for (IdxIt it(d, n_md, 1, mX[task - 3]); it.obj >= 0 && !rem; it.advance()) {
+          for (IdxIt it(d, n_md, 1, LST_MD_B); it.obj >= 0 && !rem; it.advance()) {
             const int Z = it.obj;
             if (!d.keep5[Z]) continue;
             load_t5_md(d, d.pt5[Z].y, mY);
             rem = share(mX, 5, mY, 5) >= 2;
           }
       } else if (n_pt3 > 0) {
-        for (IdxIt it(d, n_md, 2, mX[task - 7]); it.obj >= 0 && !rem; it.advance()) {
+        for (IdxIt it(d, n_md, 2, LST_MD_C); it.obj >= 0 && !rem; it.advance()) {
           const int Z = it.obj;
           if (!d.keep3[Z]) continue;
           load_t3_md(d, d.pt3[Z].y, mY);

@@ -135,6 +135,9 @@ struct Dev {
   int* idx_head;   // [4 * n_md] objects containing MD m, as linked lists: kind 0 T5, 1 pT5, 2 pT3, 3 T4; 0 = end, else node + 1
   int* idx_next;   // [5 * cap T5 | 5 * cap pT5 | 3 * cap pT3 | 4 * cap T4] node = object * (5, 3 or 4) + position of the MD in it
   unsigned char *keep5, *keep3, *keepT, *keep4, *linked;
+#ifdef LST_RULE3_SKIP_COVERED  // reproducer of profiles/r03_rule3_fault.md only
+  unsigned char* t5_cov;  // [n_t5] a surviving pT5 is built on this T5 (set by k_rule1; zeroed per batch)
+#endif
   int* tc_cnt;    // [n_events * 5 + 1] survivors per (event, class) (zeroed per batch)
   int* tc_begin;  // [n_events * 5 + 1]
   int* tc_cur;    // [n_events * 5] (zeroed per batch)
